@@ -1,0 +1,209 @@
+/* fstc — weighted FST composition M1∘M2 on one NVIDIA B200 (sm_100a).  C ABI.
+ *
+ * The operation is the one "Composing Finite State Transducers on GPUs" (arXiv 1805.06383;
+ * citations below are /root/reference/PAPER.md line numbers) states:
+ *
+ *   M1 = (Q1, Σ, Γ, s1, F1, δ1),  M2 = (Q2, Γ, Δ, s2, F2, δ2)                          (:39-45)
+ *   M1∘M2 = (Q1×Q2, Σ, Δ, s1s2, F1×F2, δ),
+ *   δ(q1q2, a, b, r1r2) = Σ_{c∈Γ} δ1(q1,a,c,r1)·δ2(q2,c,b,r2)                           (:47-53)
+ *   "Transitions with the same source, target, input, and output symbols are merged,
+ *    adding their weights."                                                             (:65)
+ *
+ * restricted to the state pairs accessible from s1s2, found by a breadth-first search over
+ * the product graph (:77, :100, Algorithms 1-2 :106-131/:157-215).  No epsilon transitions
+ * (:37); real weights, sum-of-products semiring; weights are fp32, products and sums fp32.
+ *
+ * Every step (packing, expansion, visited-set, merging, assembly) runs in CUDA kernels of this
+ * library; there is no CPU fallback.  Nothing here depends on PyTorch.
+ *
+ * Memory spaces.  Every array pointer inside fstc_fst_t lives in the space named by its
+ * `mem` field: FSTC_MEM_DEVICE (CUDA device memory of the current device) or FSTC_MEM_HOST
+ * (ordinary or pinned host memory; the library stages it to the device itself).  All arrays of
+ * fstc_result_t are DEVICE memory owned by the library.  Struct pointers themselves
+ * (fstc_fst_t*, fstc_opts_t*, fstc_stats_t*, fstc_host_result_t*) are host pointers.
+ *
+ * Threading / streams.  All work of a call is enqueued on `cuda_stream` (a cudaStream_t; NULL =
+ * the legacy default stream).  Calls synchronise that stream internally where a size has to be
+ * known on the host (once or twice per BFS level) and before returning.  Inputs are never
+ * modified and may be released as soon as the call returns.
+ *
+ * Errors.  Every int-returning call returns FSTC_OK (0) or a negative FSTC_ERR_* code; on error
+ * the output pointer is set to NULL, nothing is leaked, and fstc_last_error() (thread-local)
+ * holds a one-line description.
+ */
+#ifndef FSTC_H_
+#define FSTC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FSTC_VERSION 1
+
+#if defined(__GNUC__)
+#define FSTC_API __attribute__((visibility("default")))
+#else
+#define FSTC_API
+#endif
+
+enum {
+  FSTC_OK = 0,
+  FSTC_ERR_ARG = -1,      /* null pointer, negative size, start out of range, inner alphabets differ (:45) */
+  FSTC_ERR_INPUT = -2,    /* a state or symbol id out of range (found by a device validation pass)        */
+  FSTC_ERR_OOM = -3,      /* device (or pinned host) allocation failed                                     */
+  FSTC_ERR_CAPACITY = -4, /* an internal limit was exceeded (see fstc_opts_t and DESIGN.md "limits")       */
+  FSTC_ERR_CUDA = -5      /* any other CUDA runtime error                                                  */
+};
+
+enum { FSTC_MEM_DEVICE = 0, FSTC_MEM_HOST = 1 };
+
+/* A weighted FST (:25-35).  Borrowed; never modified; must stay valid until the call returns.
+ * States are 0..n_states-1 and symbols 0..n-1; symbol 0 is an ordinary symbol (there is no
+ * epsilon, :37).  Arcs may come in any order; parallel duplicates (same src,ilabel,olabel,tgt)
+ * are allowed and each contributes to the sum.  Every stored arc exists, whatever its weight. */
+typedef struct fstc_fst_t {
+  int32_t n_states;         /* |Q| >= 1                                                          */
+  int32_t n_isyms;          /* input alphabet size  (M1: |Σ|, M2: |Γ|)                           */
+  int32_t n_osyms;          /* output alphabet size (M1: |Γ|, M2: |Δ|)                           */
+  int32_t start;            /* s, 0 <= start < n_states                                          */
+  int64_t n_arcs;           /* 0 <= n_arcs < 2^31                                                */
+  const int32_t *src;       /* [n_arcs] source state                                             */
+  const int32_t *ilabel;    /* [n_arcs] input symbol                                             */
+  const int32_t *olabel;    /* [n_arcs] output symbol                                            */
+  const int32_t *tgt;       /* [n_arcs] target state                                             */
+  const float *weight;      /* [n_arcs] fp32 weight                                              */
+  int32_t n_accept;         /* |F|                                                               */
+  const int32_t *accept;    /* [n_accept] accept state ids (duplicates tolerated)                */
+  int32_t mem;              /* FSTC_MEM_DEVICE or FSTC_MEM_HOST: where the seven arrays live     */
+} fstc_fst_t;
+
+enum {
+  FSTC_MERGE_AUTO = 0,      /* default: identical (src,tgt,a,b) arcs are summed (:65).  Only the sources
+                               that CAN hold duplicates (exact test, N10, replacing the lossy
+                               table H of :243) go through sort + reduce; their arcs come out sorted by
+                               (tgt,a,b), the other sources' arcs in generation order.                 */
+  FSTC_MERGE_OFF = 1,       /* "without performing any reductions" (:289): one arc per (e1,e2) match */
+  FSTC_MERGE_SORT_ALL = 2   /* every source goes through sort + reduce: arcs sorted by (src,tgt,a,b) */
+};
+
+/* Options; NULL or all-zero = defaults. */
+typedef struct fstc_opts_t {
+  int32_t merge_mode;       /* FSTC_MERGE_*                                                           */
+  int32_t max_levels;       /* stop before expanding BFS level max_levels (0 = unlimited)             */
+  int64_t max_raw_arcs;     /* output budget in RAW composed arcs, rule T below (0 = unlimited)       */
+  int64_t arc_capacity_hint;   /* expected number of output arcs (0 = none): avoids regrowing        */
+  int64_t state_capacity_hint; /* expected number of output states (0 = none)                        */
+  int32_t profile;          /* 1: time every stage with CUDA events on the stream (fills stats ms)    */
+  int32_t reserved;
+} fstc_opts_t;
+
+/* Rule T (the paper only notes that the result may not fit the device, :153).  BFS levels are
+ * expanded whole while the running total of raw composed arcs stays <= max_raw_arcs.  The first
+ * level that would exceed it is ordered by ascending pair key k = q1*|Q2|+q2 and its longest
+ * prefix that still fits is expanded; then the search stops with truncated = 1.  States created
+ * but not expanded stay in the result with expanded[i] = 0 and no outgoing arcs.  The rule only
+ * depends on the frontier SET, so the result does not depend on thread scheduling. */
+
+#define FSTC_MAX_LEVEL_STATS 64
+enum {                      /* indices into fstc_stats_t.ms[] (filled when opts.profile = 1)         */
+  FSTC_T_COUNT = 0,         /* per-pair inner-symbol intersection + raw counts                       */
+  FSTC_T_SCAN = 1,          /* exclusive scans and the budget cut                                    */
+  FSTC_T_MATCH = 2,         /* match work-list construction                                          */
+  FSTC_T_EMIT = 3,          /* load-balanced product-arc emission fused with visited-set find-or-insert */
+  FSTC_T_SORT = 4,          /* radix sort of the arcs that may merge                                 */
+  FSTC_T_REDUCE = 5,        /* segmented reduction + placement of merged arcs                        */
+  FSTC_T_TABLE = 6,         /* visited table clear / grow + rehash                                   */
+  FSTC_T_ASSEMBLE = 7,      /* accept list, expanded flags, output growth copies                     */
+  FSTC_T_NSTAGES = 8
+};
+
+typedef struct fstc_stats_t {
+  int64_t n_states, n_arcs, n_raw_arcs, n_expanded;
+  int32_t n_levels, truncated;
+  /* terms of the algorithmic-bytes model */
+  int64_t n_seg_visited;    /* Σ over expanded pairs of (distinct inner symbols of q1 + of q2)        */
+  int64_t n_matches;        /* number of (pair, inner symbol) matches                                 */
+  int64_t n_match_arcs;     /* Σ over matches of (n1 + n2) input arcs read                            */
+  int64_t n_raw_sorted;     /* raw arcs that went through sort + reduce                               */
+  int64_t table_capacity;   /* final number of visited-table slots                                    */
+  int32_t n_rehash, n_grow; /* table rebuilds, output regrow copies                                   */
+  int32_t n_emit_launches, n_kernel_launches;
+  double ms[FSTC_T_NSTAGES];/* device time per stage (CUDA events), only when opts.profile = 1       */
+  double ms_total;          /* device time of the whole call (CUDA events), always                    */
+  int64_t level_frontier[FSTC_MAX_LEVEL_STATS];  /* |F_l|                                             */
+  int64_t level_raw[FSTC_MAX_LEVEL_STATS];       /* raw arcs composed in level l                      */
+  int64_t level_new_states[FSTC_MAX_LEVEL_STATS];
+} fstc_stats_t;
+
+/* The composed transducer.  Owned by the library; release with fstc_result_free.
+ * State i is the pair (pair[2i], pair[2i+1]) = (q1, q2); state 0 is the start pair s1s2 (:49).
+ * Other state numbers are implementation-defined (:239 numbers them in discovery order, which is
+ * racy on a GPU); compare results in pair coordinates. */
+typedef struct fstc_result_t {
+  int64_t n_states, n_arcs, n_raw_arcs, n_accept, n_expanded;
+  int32_t n_levels;         /* BFS levels at least partly expanded                                    */
+  int32_t truncated;        /* 1 iff max_raw_arcs / max_levels stopped the search                     */
+  int32_t *pair;            /* device [2*n_states]  interleaved (q1, q2)                              */
+  int32_t *src;             /* device [n_arcs] source state id, ASCENDING                             */
+  int32_t *ilabel;          /* device [n_arcs] a ∈ Σ                                                  */
+  int32_t *olabel;          /* device [n_arcs] b ∈ Δ                                                  */
+  int32_t *tgt;             /* device [n_arcs] target state id                                        */
+  float *weight;            /* device [n_arcs]                                                        */
+  int32_t *accept;          /* device [n_accept] ascending ids with q1 ∈ F1 and q2 ∈ F2 (:49,:131)    */
+  uint8_t *expanded;        /* device [n_states] 1 iff the state's outgoing arcs are present          */
+  void *impl;               /* private                                                                */
+} fstc_result_t;
+
+/* Caller-allocated HOST arrays that receive a copy of a result (sizes from fstc_result_t). */
+typedef struct fstc_host_result_t {
+  int32_t *pair, *src, *ilabel, *olabel, *tgt;
+  float *weight;
+  int32_t *accept;
+  uint8_t *expanded;        /* any pointer may be NULL = skip that array                              */
+} fstc_host_result_t;
+
+/* A transducer in the layout the kernels read (§3.3 :141-149, adapted): arcs sorted by
+ * (source, inner symbol, outer symbol, target), a per-state index of its distinct inner symbols,
+ * an accept bitmap and the per-state duplicate flags of DESIGN.md N10.  Opaque, device-resident,
+ * reusable across any number of compositions; release with fstc_packed_free. */
+typedef struct fstc_packed_t fstc_packed_t;
+
+/* side 1: the inner alphabet is the OUTPUT side (left operand M1); side 2: the INPUT side (M2). */
+FSTC_API int fstc_pack(const fstc_fst_t *m, int side, void *cuda_stream, fstc_packed_t **out);
+FSTC_API void fstc_packed_free(fstc_packed_t *p);
+/* info[0..5] = n_states, n_arcs, n_segments (distinct (state, inner symbol)), n_inner, n_outer, side */
+FSTC_API int fstc_packed_info(const fstc_packed_t *p, int64_t *info);
+/* Debug/test access: copies the packed arrays to HOST buffers (any may be NULL).
+ * arcs4: [4*n_arcs] uint32 (tgt, outer, weight bits, inner); segs2: [2*(n_segments+1)] (symbol, arc offset);
+ * seg_ptr: [n_states+1]; flags: [n_states] bit0 = D (two arcs share (outer,tgt)), bit1 = X (two arcs share
+ * (inner,outer,tgt)); accept_bits: [(n_states+31)/32]. */
+FSTC_API int fstc_packed_to_host(const fstc_packed_t *p, void *cuda_stream, uint32_t *arcs4, uint32_t *segs2,
+                        uint32_t *seg_ptr, uint8_t *flags, uint32_t *accept_bits);
+
+/* M1∘M2 from packed operands (m1 packed with side 1, m2 with side 2; inner alphabets must agree, :45). */
+FSTC_API int fstc_compose_packed(const fstc_packed_t *m1, const fstc_packed_t *m2, const fstc_opts_t *opts,
+                        void *cuda_stream, fstc_result_t **out, fstc_stats_t *stats /* nullable */);
+
+/* fst_compose(M1, M2) -> M1∘M2: packs both operands, composes, frees the packed forms. */
+FSTC_API int fstc_compose(const fstc_fst_t *m1, const fstc_fst_t *m2, const fstc_opts_t *opts, void *cuda_stream,
+                 fstc_result_t **out, fstc_stats_t *stats /* nullable */);
+
+/* Copies the result arrays to caller-allocated host memory (pinned memory makes it asynchronous
+ * until the final stream synchronisation, which this call performs). */
+FSTC_API int fstc_result_to_host(const fstc_result_t *r, void *cuda_stream, const fstc_host_result_t *dst);
+FSTC_API void fstc_result_free(fstc_result_t *r);
+
+/* Releases the cached device memory of the library's pool back to the driver. */
+FSTC_API int fstc_trim_pool(void);
+
+FSTC_API const char *fstc_strerror(int code);
+FSTC_API const char *fstc_last_error(void);
+FSTC_API int fstc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FSTC_H_ */

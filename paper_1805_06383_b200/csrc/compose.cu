@@ -1,0 +1,941 @@
+// Weighted FST composition as a level-synchronous search over the product graph
+// (§3.2-3.4, Algorithms 1-2; DESIGN.md steps 2-9).  Everything runs on the device; the host
+// only reads a few scalars per BFS level.
+//
+//   count    per frontier pair (q1,q2): intersect the inner-symbol lists, raw = Σ_c n1(c)·n2(c)   (step 3)
+//   scan     exclusive scans of the raw counts / match counts, budget rule T                      (step 4)
+//   match    work-list of (pair, inner symbol) matches with the running arc rank                  (step 3b)
+//   emit     one thread per 4 consecutive output ranks (load-balanced over matches, so a match of
+//            10^9 arcs is spread over many blocks): read e1,e2, w = p1·p2, find-or-insert the
+//            target pair in the visited hash table (64-bit key q1·|Q2|+q2, atomicCAS), new ids are
+//            the next frontier                                                                     (steps 5-6)
+//   merge    sources that can hold duplicate (tgt,a,b) go through radix sort + segmented sum      (step 7)
+//   assemble accept list, expanded flags                                                           (step 8)
+//
+// What differs from the paper's own kernel design (one launch per inner symbol per popped pair, 32-thread
+// blocks, host-side queue, dense |Q1||Q2| visited table, lossy table H — PAPER.md:219-243) is listed in
+// DESIGN.md "differences".
+#include <algorithm>
+#include <cstring>
+
+#include "internal.h"
+#include "scan.cuh"
+
+namespace fstc {
+
+namespace {
+
+constexpr unsigned long long EMPTY_KEY = ~0ull;
+constexpr uint32_t PENDING_ID = 0xFFFFFFFFu;
+constexpr int CT_THREADS = 256;
+
+struct MachineView {
+    const uint4 *arcs;
+    const uint2 *segs;
+    const uint32_t *seg_ptr;
+    const uint8_t *flags;
+};
+
+inline MachineView view_of(const fstc_packed_t &p) { return MachineView{p.arcs, p.segs, p.seg_ptr, p.flags}; }
+
+// ------------------------------------------------------------------------------------------ hash table
+// Open addressing, linear probing, 16-byte slots {key lo, key hi, id, unused}; a slot never straddles a
+// 32-byte sector, so one probe is one sector.  Empty = all ones (a cudaMemset of 0xFF clears it).
+__device__ __forceinline__ uint64_t mix64(uint64_t k) {
+    k ^= k >> 33; k *= 0xff51afd7ed558ccdULL;
+    k ^= k >> 33; k *= 0xc4ceb9fe1a85ec53ULL;
+    k ^= k >> 33;
+    return k;
+}
+__device__ __forceinline__ uint64_t home_slot(uint64_t key, uint64_t cap) { return __umul64hi(mix64(key), cap); }
+
+__global__ void tb_insert_ids(const int2 *__restrict__ pair, int64_t n, uint64_t nq2, uint4 *table, uint64_t cap) {
+    // rebuild after growth: keys are distinct, ids known -> plain CAS claim, then store the id
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int2 p = pair[i];
+    unsigned long long key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
+    uint64_t s = home_slot(key, cap);
+    while (true) {
+        unsigned long long old = atomicCAS(reinterpret_cast<unsigned long long *>(table + s), EMPTY_KEY, key);
+        if (old == EMPTY_KEY) break;
+        s = (s + 1 == cap) ? 0 : s + 1;
+    }
+    reinterpret_cast<uint32_t *>(table + s)[2] = static_cast<uint32_t>(i);
+}
+
+// ------------------------------------------------------------------------------------------ count / match
+// Intersection of the two states' sorted inner-symbol lists.  F is called for every shared symbol with
+// (first arc of q1's segment, n1, first arc of q2's segment, n2).
+template <typename F>
+__device__ __forceinline__ void intersect(const MachineView &A, const MachineView &B, int q1, int q2, F &&on_match) {
+    uint32_t s1 = A.seg_ptr[q1], e1 = A.seg_ptr[q1 + 1];
+    uint32_t s2 = B.seg_ptr[q2], e2 = B.seg_ptr[q2 + 1];
+    if (s1 == e1 || s2 == e2) return;
+    uint2 a = A.segs[s1], an = A.segs[s1 + 1];
+    uint2 b = B.segs[s2], bn = B.segs[s2 + 1];
+    while (true) {
+        if (a.x == b.x) {
+            on_match(a.y, an.y - a.y, b.y, bn.y - b.y);
+            if (++s1 == e1 || ++s2 == e2) break;
+            a = an; an = A.segs[s1 + 1];
+            b = bn; bn = B.segs[s2 + 1];
+        } else if (a.x < b.x) {
+            if (++s1 == e1) break;
+            a = an; an = A.segs[s1 + 1];
+        } else {
+            if (++s2 == e2) break;
+            b = bn; bn = B.segs[s2 + 1];
+        }
+    }
+}
+
+// class U = arcs go straight to the output; class F = arcs go through sort + reduce first
+__global__ void __launch_bounds__(CT_THREADS)
+k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, int merge_mode,
+        int64_t *__restrict__ rawU, int64_t *__restrict__ rawF, uint32_t *__restrict__ nmU, uint32_t *__restrict__ nmF,
+        unsigned long long *__restrict__ counters /* [0] Σ segments visited, [1] Σ (n1+n2) over matches */) {
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    unsigned long long segs = 0, marcs = 0;
+    if (i < nf) {
+        int2 p = pair[f_lo + i];
+        int64_t raw = 0;
+        uint32_t nm = 0;
+        intersect(A, B, p.x, p.y, [&](uint32_t, uint32_t n1, uint32_t, uint32_t n2) {
+            raw += static_cast<int64_t>(n1) * n2;
+            nm += 1;
+            marcs += n1 + n2;
+        });
+        segs = (A.seg_ptr[p.x + 1] - A.seg_ptr[p.x]) + (B.seg_ptr[p.y + 1] - B.seg_ptr[p.y]);
+        bool f = false;
+        if (merge_mode == FSTC_MERGE_SORT_ALL) f = true;
+        else if (merge_mode == FSTC_MERGE_AUTO) {
+            uint8_t fa = A.flags[p.x], fb = B.flags[p.y];
+            f = ((fa & FLAG_D) && (fb & FLAG_D)) || (fa & FLAG_X) || (fb & FLAG_X);
+        }
+        rawU[i] = f ? 0 : raw; rawF[i] = f ? raw : 0;
+        nmU[i] = f ? 0 : nm;   nmF[i] = f ? nm : 0;
+    }
+    // block-level totals for the statistics
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        segs += __shfl_xor_sync(0xffffffffu, segs, d);
+        marcs += __shfl_xor_sync(0xffffffffu, marcs, d);
+    }
+    if ((threadIdx.x & 31) == 0 && (segs | marcs)) {
+        atomicAdd(&counters[0], segs);
+        atomicAdd(&counters[1], marcs);
+    }
+}
+
+// Budget rule T, radix select: weighted histogram of one 8-bit key digit over the pairs whose higher key bits
+// equal `prefix`.
+__global__ void __launch_bounds__(CT_THREADS)
+k_cut_hist(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, uint64_t nq2, const int64_t *__restrict__ rawU,
+           const int64_t *__restrict__ rawF, uint64_t prefix, int shift, unsigned long long *__restrict__ hist) {
+    __shared__ unsigned long long h[256];
+    h[threadIdx.x] = 0;
+    __syncthreads();
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i < nf) {
+        int2 p = pair[f_lo + i];
+        uint64_t key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
+        uint64_t hi = (shift + 8 >= 64) ? 0 : (key >> (shift + 8));
+        int64_t r = rawU[i] + rawF[i];
+        if (hi == prefix && r > 0) atomicAdd(&h[(key >> shift) & 255], static_cast<unsigned long long>(r));
+    }
+    __syncthreads();
+    if (h[threadIdx.x]) atomicAdd(&hist[threadIdx.x], h[threadIdx.x]);
+}
+
+// pairs with key >= cut are not expanded in this (last) level
+__global__ void k_apply_cut(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, uint64_t nq2, uint64_t cut,
+                            int64_t *__restrict__ rawU, int64_t *__restrict__ rawF, uint32_t *__restrict__ nmU,
+                            uint32_t *__restrict__ nmF, unsigned long long *__restrict__ n_selected) {
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    bool sel = false;
+    if (i < nf) {
+        int2 p = pair[f_lo + i];
+        uint64_t key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
+        sel = key < cut;
+        if (!sel) { rawU[i] = 0; rawF[i] = 0; nmU[i] = 0; nmF[i] = 0; }
+    }
+    unsigned b = __ballot_sync(0xffffffffu, sel);
+    if ((threadIdx.x & 31) == 0 && b) atomicAdd(n_selected, static_cast<unsigned long long>(__popc(b)));
+}
+
+struct MatchList {           // SoA work-list of one class
+    int64_t *cum;            // [n+1] rank of the match's first arc; cum[n] = total
+    uint4 *rec;              // [n] {first arc in M1, first arc in M2, n1, n2}
+    uint32_t *pl;            // [n] pair index inside the level
+};
+
+__global__ void __launch_bounds__(CT_THREADS)
+k_match(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_lo, int64_t nf,
+        const uint32_t *__restrict__ nmU, const uint32_t *__restrict__ nmF, const int64_t *__restrict__ moffU,
+        const int64_t *__restrict__ moffF, const int64_t *__restrict__ roffU, const int64_t *__restrict__ roffF,
+        MatchList U, MatchList F) {
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= nf) return;
+    const bool isF = nmF[i] != 0;
+    if (!isF && nmU[i] == 0) return;
+    int2 p = pair[f_lo + i];
+    MatchList L = isF ? F : U;
+    int64_t m = isF ? moffF[i] : moffU[i];
+    int64_t run = isF ? roffF[i] : roffU[i];
+    intersect(A, B, p.x, p.y, [&](uint32_t o1, uint32_t n1, uint32_t o2, uint32_t n2) {
+        L.cum[m] = run;
+        L.rec[m] = make_uint4(o1, o2, n1, n2);
+        L.pl[m] = static_cast<uint32_t>(i);
+        run += static_cast<int64_t>(n1) * n2;
+        ++m;
+    });
+}
+
+// ------------------------------------------------------------------------------------------ emit
+constexpr int EM_THREADS = 256;
+constexpr int EM_IPT = 4;                          // consecutive output ranks per thread
+constexpr int EM_TILE = EM_THREADS * EM_IPT;       // 1024 arcs per block
+
+enum { EMIT_DIRECT = 0, EMIT_INDIRECT = 1, EMIT_SORTREC = 2 };
+
+struct EmitArgs {
+    MachineView A, B;
+    MatchList L;
+    int64_t n_matches;
+    int64_t R;               // ranks [0, R)
+    int64_t pos_base;        // DIRECT: output position of rank 0 (tiles are aligned on absolute positions)
+    int64_t f_lo;            // source id = f_lo + pair index
+    const int64_t *foff;     // INDIRECT: final position of the pair's first arc (relative to arc_base)
+    const int64_t *roff;     // INDIRECT: rank of the pair's first arc
+    int64_t arc_base;        // INDIRECT
+    uint64_t nq2;
+    uint4 *table;
+    uint64_t cap;
+    unsigned long long *n_states;
+    int2 *pair;
+    int32_t *o_src, *o_il, *o_ol, *o_tgt;
+    float *o_w;
+    uint4 *sortrec;          // SORTREC: {key lo, key hi, pair index, weight}, key = tgt id << shift_t | a << bits_b | b
+    int shift_t, bits_b;
+    const int64_t *tile_m;   // [n_tiles+1] match index holding the first rank of every tile
+};
+
+// tile_m[t] = last match whose first rank <= first rank of tile t
+__global__ void k_partition(const int64_t *__restrict__ cum, int64_t n_matches, int64_t R, int64_t pos_base,
+                            int64_t n_tiles, int64_t *__restrict__ tile_m) {
+    int64_t t = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (t > n_tiles) return;
+    int64_t tile0 = (pos_base / EM_TILE) * EM_TILE;
+    int64_t rank = tile0 + t * EM_TILE - pos_base;
+    if (rank < 0) rank = 0;
+    if (rank >= R) { tile_m[t] = n_matches; return; }   // only t == n_tiles (or beyond the data)
+    int64_t lo = 0, hi = n_matches;                      // first m with cum[m] > rank
+    while (lo < hi) {
+        int64_t mid = (lo + hi) >> 1;
+        if (cum[mid] <= rank) lo = mid + 1; else hi = mid;
+    }
+    tile_m[t] = lo - 1;
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(EM_THREADS) k_emit(EmitArgs g) {
+    __shared__ uint32_t relcum[EM_TILE + 1];
+    __shared__ int64_t s_first_cum;
+    __shared__ uint32_t s_warp[EM_THREADS / 32];
+    __shared__ unsigned long long s_base;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t tile0 = (g.pos_base / EM_TILE) * EM_TILE;
+    const int64_t tile_pos = tile0 + static_cast<int64_t>(blockIdx.x) * EM_TILE;   // absolute position of the tile
+    int64_t rank_lo = tile_pos - g.pos_base;                 // first rank of the tile (may be < 0 in tile 0)
+    int64_t rank_hi = rank_lo + EM_TILE;
+    if (rank_lo < 0) rank_lo = 0;
+    if (rank_hi > g.R) rank_hi = g.R;
+
+    const int64_t m_lo = g.tile_m[blockIdx.x];
+    int64_t m_hi = g.tile_m[blockIdx.x + 1];                 // inclusive, last match that can start inside the tile
+    if (m_hi >= g.n_matches) m_hi = g.n_matches - 1;
+    const int nm = static_cast<int>(m_hi - m_lo + 1);        // <= EM_TILE + 1
+    for (int j = tid; j < nm; j += EM_THREADS) {
+        int64_t c = g.L.cum[m_lo + j] - rank_lo;
+        relcum[j] = c < 0 ? 0u : static_cast<uint32_t>(c > EM_TILE ? EM_TILE : c);
+    }
+    if (tid == 0) s_first_cum = g.L.cum[m_lo];
+    __syncthreads();
+
+    // ---- locate this thread's first rank
+    const int64_t my_pos = tile_pos + tid * EM_IPT;
+    int64_t rank0 = my_pos - g.pos_base;
+    int n_valid = 0;                                          // ranks rank0+skip .. rank0+skip+n_valid-1
+    int skip = 0;
+    {
+        int64_t a = rank0 < rank_lo ? rank_lo : rank0;
+        int64_t b = rank0 + EM_IPT < rank_hi ? rank0 + EM_IPT : rank_hi;
+        if (b > a) { n_valid = static_cast<int>(b - a); skip = static_cast<int>(a - rank0); }
+    }
+    uint32_t idx1[EM_IPT], idx2[EM_IPT], pl[EM_IPT];
+    if (n_valid > 0) {
+        const int64_t first = rank0 + skip;
+        const uint32_t rr = static_cast<uint32_t>(first - rank_lo);
+        int lo = 0, hi = nm;                                  // first j with relcum[j] > rr
+        while (lo < hi) {
+            int mid = (lo + hi) >> 1;
+            if (relcum[mid] <= rr) lo = mid + 1; else hi = mid;
+        }
+        int j = lo - 1;
+        int64_t m = m_lo + j;
+        uint64_t r = (j == 0) ? static_cast<uint64_t>(first - s_first_cum) : static_cast<uint64_t>(rr - relcum[j]);
+        uint4 rec = g.L.rec[m];
+        uint32_t p = g.L.pl[m];
+        uint32_t i1, i2;
+        if (r < 0xFFFFFFFFull) { i1 = static_cast<uint32_t>(r) / rec.w; i2 = static_cast<uint32_t>(r) - i1 * rec.w; }
+        else { i1 = static_cast<uint32_t>(r / rec.w); i2 = static_cast<uint32_t>(r - static_cast<uint64_t>(i1) * rec.w); }
+#pragma unroll
+        for (int u = 0; u < EM_IPT; ++u) {
+            if (u >= skip && u < skip + n_valid) {
+                idx1[u] = rec.x + i1; idx2[u] = rec.y + i2; pl[u] = p;
+                if (++i2 == rec.w) {
+                    i2 = 0;
+                    if (++i1 == rec.z) {
+                        i1 = 0; ++m;
+                        if (m <= m_hi) { rec = g.L.rec[m]; p = g.L.pl[m]; }
+                    }
+                }
+            }
+        }
+    }
+
+    // ---- read the two input arcs of every rank, form the composed arc
+    uint32_t a_sym[EM_IPT], b_sym[EM_IPT];
+    float w[EM_IPT];
+    unsigned long long key[EM_IPT];
+    int2 tgt_pair[EM_IPT];
+#pragma unroll
+    for (int u = 0; u < EM_IPT; ++u) {
+        if (u >= skip && u < skip + n_valid) {
+            uint4 e1 = __ldg(g.A.arcs + idx1[u]);             // {tgt, outer, weight, inner}
+            uint4 e2 = __ldg(g.B.arcs + idx2[u]);
+            a_sym[u] = e1.y; b_sym[u] = e2.y;
+            w[u] = __uint_as_float(e1.z) * __uint_as_float(e2.z);
+            tgt_pair[u] = make_int2(static_cast<int>(e1.x), static_cast<int>(e2.x));
+            key[u] = static_cast<uint64_t>(e1.x) * g.nq2 + e2.x;
+        }
+    }
+
+    // ---- visited set: find or insert, all first probes in flight together
+    uint64_t slot[EM_IPT];
+    uint4 probe[EM_IPT];
+    uint32_t id[EM_IPT];
+    bool won[EM_IPT];
+#pragma unroll
+    for (int u = 0; u < EM_IPT; ++u) {
+        won[u] = false; id[u] = 0;
+        if (u >= skip && u < skip + n_valid) {
+            slot[u] = home_slot(key[u], g.cap);
+            probe[u] = __ldcg(g.table + slot[u]);
+        }
+    }
+    uint32_t n_won = 0;
+#pragma unroll
+    for (int u = 0; u < EM_IPT; ++u) {
+        if (u >= skip && u < skip + n_valid) {
+            uint4 v = probe[u];
+            uint64_t s = slot[u];
+            while (true) {
+                unsigned long long k = (static_cast<unsigned long long>(v.y) << 32) | v.x;
+                if (k == key[u]) { id[u] = v.z; break; }
+                if (k == EMPTY_KEY) {
+                    unsigned long long old =
+                        atomicCAS(reinterpret_cast<unsigned long long *>(g.table + s), EMPTY_KEY, key[u]);
+                    if (old == EMPTY_KEY) { won[u] = true; ++n_won; break; }
+                    if (old == key[u]) { id[u] = PENDING_ID; break; }
+                }
+                s = (s + 1 == g.cap) ? 0 : s + 1;
+                v = __ldcg(g.table + s);
+            }
+            slot[u] = s;
+        }
+    }
+
+    // ---- new state ids: one atomicAdd per block; the new ids of a level are the next frontier
+    uint32_t incl = n_won;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += t;
+    }
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t tot = 0;
+#pragma unroll
+        for (int wv = 0; wv < EM_THREADS / 32; ++wv) { uint32_t c = s_warp[wv]; s_warp[wv] = tot; tot += c; }
+        s_base = tot ? atomicAdd(g.n_states, static_cast<unsigned long long>(tot)) : 0ull;
+    }
+    __syncthreads();
+    uint32_t next_id = static_cast<uint32_t>(s_base) + s_warp[warp] + (incl - n_won);
+#pragma unroll
+    for (int u = 0; u < EM_IPT; ++u) {
+        if (won[u]) {
+            id[u] = next_id++;
+            __stcg(reinterpret_cast<uint32_t *>(g.table + slot[u]) + 2, id[u]);   // publish
+            g.pair[id[u]] = tgt_pair[u];
+        }
+    }
+    // ---- targets inserted concurrently by another thread: wait for their id to be published
+#pragma unroll
+    for (int u = 0; u < EM_IPT; ++u) {
+        if (u >= skip && u < skip + n_valid && !won[u] && id[u] == PENDING_ID) {
+            const uint32_t *pid = reinterpret_cast<const uint32_t *>(g.table + slot[u]) + 2;
+            uint32_t v;
+            while ((v = __ldcg(pid)) == PENDING_ID) __nanosleep(20);
+            id[u] = v;
+        }
+    }
+
+    // ---- write the composed arcs
+    if (MODE == EMIT_DIRECT) {
+        if (n_valid == EM_IPT) {                               // whole aligned group: 16-byte stores
+            const int64_t q = my_pos;
+            *reinterpret_cast<int4 *>(g.o_src + q) = make_int4(static_cast<int>(g.f_lo + pl[0]), static_cast<int>(g.f_lo + pl[1]),
+                                                               static_cast<int>(g.f_lo + pl[2]), static_cast<int>(g.f_lo + pl[3]));
+            *reinterpret_cast<uint4 *>(g.o_il + q) = make_uint4(a_sym[0], a_sym[1], a_sym[2], a_sym[3]);
+            *reinterpret_cast<uint4 *>(g.o_ol + q) = make_uint4(b_sym[0], b_sym[1], b_sym[2], b_sym[3]);
+            *reinterpret_cast<uint4 *>(g.o_tgt + q) = make_uint4(id[0], id[1], id[2], id[3]);
+            *reinterpret_cast<float4 *>(g.o_w + q) = make_float4(w[0], w[1], w[2], w[3]);
+        } else {
+#pragma unroll
+            for (int u = 0; u < EM_IPT; ++u) {
+                if (u >= skip && u < skip + n_valid) {
+                    const int64_t q = my_pos + u;
+                    g.o_src[q] = static_cast<int>(g.f_lo + pl[u]);
+                    g.o_il[q] = a_sym[u]; g.o_ol[q] = b_sym[u]; g.o_tgt[q] = id[u]; g.o_w[q] = w[u];
+                }
+            }
+        }
+    } else if (MODE == EMIT_INDIRECT) {
+#pragma unroll
+        for (int u = 0; u < EM_IPT; ++u) {
+            if (u >= skip && u < skip + n_valid) {
+                const int64_t rank = rank0 + u;
+                const int64_t q = g.arc_base + g.foff[pl[u]] + (rank - g.roff[pl[u]]);
+                g.o_src[q] = static_cast<int>(g.f_lo + pl[u]);
+                g.o_il[q] = a_sym[u]; g.o_ol[q] = b_sym[u]; g.o_tgt[q] = id[u]; g.o_w[q] = w[u];
+            }
+        }
+    } else {
+#pragma unroll
+        for (int u = 0; u < EM_IPT; ++u) {
+            if (u >= skip && u < skip + n_valid) {
+                unsigned long long k = (static_cast<unsigned long long>(id[u]) << g.shift_t) |
+                                       (static_cast<unsigned long long>(a_sym[u]) << g.bits_b) | b_sym[u];
+                g.sortrec[rank0 + u] = make_uint4(static_cast<uint32_t>(k), static_cast<uint32_t>(k >> 32), pl[u],
+                                                  __float_as_uint(w[u]));
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------ merge (reduce by key)
+__global__ void k_heads(const uint4 *__restrict__ rec, int64_t n, uint8_t *__restrict__ head) {
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint8_t h = 1;
+    if (i > 0) {
+        uint4 r = rec[i], p = rec[i - 1];
+        h = (r.x != p.x) || (r.y != p.y) || (r.z != p.z);
+    }
+    head[i] = h;
+}
+
+// Segment id of record i = hidx[i] + head[i] - 1.  Weights of a segment are summed as a shuffle tree inside
+// each warp; the per-warp pieces are combined with one float atomicAdd per (warp, segment).
+__global__ void __launch_bounds__(CT_THREADS)
+k_reduce(const uint4 *__restrict__ rec, const uint8_t *__restrict__ head, const int64_t *__restrict__ hidx, int64_t n,
+         unsigned long long *__restrict__ mkey, uint32_t *__restrict__ msrc, float *__restrict__ mw) {
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    int64_t seg = -1 - lane;                                   // distinct sentinels for out-of-range lanes
+    float w = 0.f;
+    if (i < n) {
+        uint4 r = rec[i];
+        uint8_t h = head[i];
+        seg = hidx[i] + h - 1;
+        w = __uint_as_float(r.w);
+        if (h) {
+            mkey[seg] = (static_cast<unsigned long long>(r.y) << 32) | r.x;
+            msrc[seg] = r.z;
+        }
+    }
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        float t = __shfl_down_sync(0xffffffffu, w, d);
+        int64_t s = __shfl_down_sync(0xffffffffu, seg, d);
+        if (lane + d < 32 && s == seg) w += t;
+    }
+    int64_t sp = __shfl_up_sync(0xffffffffu, seg, 1);
+    if (i < n && (lane == 0 || sp != seg)) atomicAdd(&mw[seg], w);
+}
+
+// mstart[p] = first merged arc whose pair index >= p  (p = 0..nf)
+__global__ void k_mstart(const uint32_t *__restrict__ msrc, int64_t n_merged, int64_t nf, int64_t *__restrict__ mstart) {
+    int64_t p = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (p > nf) return;
+    int64_t lo = 0, hi = n_merged;
+    while (lo < hi) {
+        int64_t mid = (lo + hi) >> 1;
+        if (msrc[mid] < static_cast<uint32_t>(p)) lo = mid + 1; else hi = mid;
+    }
+    mstart[p] = lo;
+}
+
+__global__ void k_final_counts(const int64_t *__restrict__ rawU, const int64_t *__restrict__ mstart, int64_t nf,
+                               int64_t *__restrict__ fc) {
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i < nf) fc[i] = rawU[i] + (mstart[i + 1] - mstart[i]);
+}
+
+__global__ void k_place_merged(const unsigned long long *__restrict__ mkey, const uint32_t *__restrict__ msrc,
+                               const float *__restrict__ mw, int64_t n_merged, const int64_t *__restrict__ mstart,
+                               const int64_t *__restrict__ foff, int64_t arc_base, int64_t f_lo, int shift_t, int bits_b,
+                               int32_t *__restrict__ o_src, int32_t *__restrict__ o_il, int32_t *__restrict__ o_ol,
+                               int32_t *__restrict__ o_tgt, float *__restrict__ o_w) {
+    int64_t j = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (j >= n_merged) return;
+    uint32_t p = msrc[j];
+    unsigned long long k = mkey[j];
+    int64_t q = arc_base + foff[p] + (j - mstart[p]);
+    o_src[q] = static_cast<int>(f_lo + p);
+    o_tgt[q] = static_cast<int>(k >> shift_t);
+    o_il[q] = static_cast<int>((k & ((1ull << shift_t) - 1)) >> bits_b);
+    o_ol[q] = static_cast<int>(k & ((1ull << bits_b) - 1));
+    o_w[q] = mw[j];
+}
+
+// ------------------------------------------------------------------------------------------ assembly
+__global__ void k_accept_flags(const int2 *__restrict__ pair, int64_t n, const uint32_t *__restrict__ acc1,
+                               const uint32_t *__restrict__ acc2, uint8_t *__restrict__ flag) {
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int2 p = pair[i];
+    flag[i] = ((acc1[p.x >> 5] >> (p.x & 31)) & 1u) & ((acc2[p.y >> 5] >> (p.y & 31)) & 1u);
+}
+
+__global__ void k_accept_scatter(const uint8_t *__restrict__ flag, const int64_t *__restrict__ idx, int64_t n,
+                                 int32_t *__restrict__ out) {
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i < n && flag[i]) out[idx[i]] = static_cast<int32_t>(i);
+}
+
+// expanded[i] = 1 for every state before the last frontier [last_lo, last_hi); inside it, 1 iff it was
+// selected; states created while expanding a frontier that stopped the search are never expanded
+__global__ void k_expanded(const int2 *__restrict__ pair, int64_t n, int64_t last_lo, int64_t last_hi,
+                           int last_mode /*0 none,1 all,2 cut*/, uint64_t nq2, uint64_t cut,
+                           uint8_t *__restrict__ expanded) {
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint8_t e = 1;
+    if (i >= last_hi) e = 0;
+    else if (i >= last_lo) {
+        if (last_mode == 0) e = 0;
+        else if (last_mode == 2) {
+            int2 p = pair[i];
+            uint64_t key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
+            e = key < cut;
+        }
+    }
+    expanded[i] = e;
+}
+
+inline unsigned nblk(int64_t n, int threads = CT_THREADS) { return static_cast<unsigned>(ceil_div(n > 0 ? n : 1, threads)); }
+
+// ------------------------------------------------------------------------------------------ host side
+struct StageTimer {
+    Ctx &c;
+    bool on;
+    struct Span { int stage; cudaEvent_t a, b; };
+    std::vector<Span> spans;
+    StageTimer(Ctx &ctx, bool enable) : c(ctx), on(enable) {}
+    ~StageTimer() { for (auto &s : spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); } }
+    int begin(int stage) {
+        if (!on) return -1;
+        Span s; s.stage = stage;
+        cudaEventCreate(&s.a); cudaEventCreate(&s.b);
+        cudaEventRecord(s.a, c.stream);
+        spans.push_back(s);
+        return static_cast<int>(spans.size()) - 1;
+    }
+    void end(int h) { if (h >= 0) cudaEventRecord(spans[h].b, c.stream); }
+    void collect(double *ms) {
+        for (auto &s : spans) {
+            float t = 0.f;
+            if (cudaEventElapsedTime(&t, s.a, s.b) == cudaSuccess) ms[s.stage] += t;
+        }
+    }
+};
+
+struct ResultImpl {           // owns the device arrays of a result
+    void *bufs[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+};
+
+struct Composer {
+    Ctx &c;
+    const fstc_packed_t &m1, &m2;
+    fstc_opts_t o;
+    fstc_stats_t st;
+    StageTimer tm;
+    uint64_t nq2;
+    // growing outputs
+    DBuf<int2> pair; int64_t pair_cap = 0;
+    DBuf<int32_t> a_src, a_il, a_ol, a_tgt; DBuf<float> a_w; int64_t arc_cap = 0;
+    int64_t n_arcs = 0, n_states = 0;
+    // visited table
+    DBuf<uint4> table; uint64_t cap = 0;
+    DBuf<unsigned long long> d_counters;   // [0] n_states, [1] seg visited, [2] match arcs, [3] n_selected, [4..259] hist
+
+    Composer(Ctx &ctx, const fstc_packed_t &a, const fstc_packed_t &b, const fstc_opts_t &opts)
+        : c(ctx), m1(a), m2(b), o(opts), tm(ctx, opts.profile != 0), nq2(static_cast<uint64_t>(b.n_states)) {
+        std::memset(&st, 0, sizeof st);
+    }
+
+    void ensure_pairs(int64_t need) {
+        if (need <= pair_cap) return;
+        int64_t nc = std::max<int64_t>(need, pair_cap * 2);
+        DBuf<int2> np(c, nc);
+        if (n_states > 0)
+            FSTC_CUDA(cudaMemcpyAsync(np.p, pair.p, sizeof(int2) * n_states, cudaMemcpyDeviceToDevice, c.stream));
+        pair = std::move(np);
+        pair_cap = nc;
+        if (n_states > 0) st.n_grow += 1;
+    }
+
+    template <typename T>
+    void regrow(DBuf<T> &b, int64_t nc) {
+        DBuf<T> nb(c, nc);
+        if (n_arcs > 0) FSTC_CUDA(cudaMemcpyAsync(nb.p, b.p, sizeof(T) * n_arcs, cudaMemcpyDeviceToDevice, c.stream));
+        b = std::move(nb);
+    }
+    void ensure_arcs(int64_t need) {
+        if (need <= arc_cap) return;
+        int h = tm.begin(FSTC_T_ASSEMBLE);
+        int64_t nc = std::max<int64_t>(need, arc_cap + arc_cap / 2);
+        nc = (nc + 3) & ~int64_t(3);
+        regrow(a_src, nc); regrow(a_il, nc); regrow(a_ol, nc); regrow(a_tgt, nc); regrow(a_w, nc);
+        arc_cap = nc;
+        if (n_arcs > 0) st.n_grow += 1;
+        tm.end(h);
+    }
+
+    // table able to hold `bound` states at load <= 0.6
+    void ensure_table(int64_t bound) {
+        uint64_t need = static_cast<uint64_t>(bound + bound / 2 + bound / 6) + 64;   // bound / 0.6
+        if (need <= cap) return;
+        int h = tm.begin(FSTC_T_TABLE);
+        uint64_t nc = std::max<uint64_t>(need, 4096);
+        DBuf<uint4> nt(c, static_cast<int64_t>(nc));
+        FSTC_CUDA(cudaMemsetAsync(nt.p, 0xFF, sizeof(uint4) * nc, c.stream));
+        if (n_states > 0) {
+            tb_insert_ids<<<nblk(n_states), CT_THREADS, 0, c.stream>>>(pair.p, n_states, nq2, nt.p, nc);
+            FSTC_LAUNCH_CHECK();
+            c.n_launch += 1;
+            if (cap) st.n_rehash += 1;
+        }
+        table = std::move(nt);
+        cap = nc;
+        tm.end(h);
+    }
+
+    void launch_emit(int mode, const MatchList &L, int64_t n_matches, int64_t R, int64_t pos_base, int64_t f_lo,
+                     const int64_t *foff, const int64_t *roff, int64_t arc_base, uint4 *sortrec, int shift_t, int bits_b) {
+        if (R <= 0) return;
+        const int64_t tile0 = (pos_base / EM_TILE) * EM_TILE;
+        const int64_t n_tiles = ceil_div(pos_base + R - tile0, EM_TILE);
+        DBuf<int64_t> tile_m(c, n_tiles + 1);
+        k_partition<<<nblk(n_tiles + 1), CT_THREADS, 0, c.stream>>>(L.cum, n_matches, R, pos_base, n_tiles, tile_m.p);
+        FSTC_LAUNCH_CHECK();
+        EmitArgs g;
+        g.A = view_of(m1); g.B = view_of(m2);
+        g.L = L; g.n_matches = n_matches; g.R = R; g.pos_base = pos_base; g.f_lo = f_lo;
+        g.foff = foff; g.roff = roff; g.arc_base = arc_base; g.nq2 = nq2;
+        g.table = table.p; g.cap = cap; g.n_states = d_counters.p; g.pair = pair.p;
+        g.o_src = a_src.p; g.o_il = a_il.p; g.o_ol = a_ol.p; g.o_tgt = a_tgt.p; g.o_w = a_w.p;
+        g.sortrec = sortrec; g.shift_t = shift_t; g.bits_b = bits_b; g.tile_m = tile_m.p;
+        const unsigned grid = static_cast<unsigned>(n_tiles);
+        if (mode == EMIT_DIRECT) k_emit<EMIT_DIRECT><<<grid, EM_THREADS, 0, c.stream>>>(g);
+        else if (mode == EMIT_INDIRECT) k_emit<EMIT_INDIRECT><<<grid, EM_THREADS, 0, c.stream>>>(g);
+        else k_emit<EMIT_SORTREC><<<grid, EM_THREADS, 0, c.stream>>>(g);
+        FSTC_LAUNCH_CHECK();
+        c.n_launch += 2;
+        st.n_emit_launches += 1;
+    }
+
+    fstc_result_t *run();
+};
+
+fstc_result_t *Composer::run() {
+    if (m1.side != 1 || m2.side != 2) fail(FSTC_ERR_ARG, "operands must be packed with side 1 (left) and side 2 (right)");
+    if (m1.n_inner != m2.n_inner)
+        fail(FSTC_ERR_ARG, "inner alphabets differ: |Γ| = %d vs %d (PAPER.md:45)", m1.n_inner, m2.n_inner);
+    if (o.merge_mode < 0 || o.merge_mode > 2 || o.max_levels < 0 || o.max_raw_arcs < 0)
+        fail(FSTC_ERR_ARG, "bad options");
+    const int bits_a = bits_for(m1.n_outer > 0 ? m1.n_outer - 1 : 0), bits_b = bits_for(m2.n_outer > 0 ? m2.n_outer - 1 : 0);
+    const int shift_t = bits_a + bits_b;
+    const uint64_t n_pairs_total = static_cast<uint64_t>(m1.n_states) * nq2;
+    const int key_bits = bits_for(n_pairs_total - 1);
+
+    cudaEvent_t ev0, ev1;
+    FSTC_CUDA(cudaEventCreate(&ev0));
+    FSTC_CUDA(cudaEventCreate(&ev1));
+    FSTC_CUDA(cudaEventRecord(ev0, c.stream));
+
+    d_counters.alloc(c, 4 + 256);
+    FSTC_CUDA(cudaMemsetAsync(d_counters.p, 0, sizeof(unsigned long long) * (4 + 256), c.stream));
+
+    // ---- init (Alg. 2 lines 1-3): state 0 = (s1, s2)
+    ensure_pairs(std::max<int64_t>(o.state_capacity_hint, 1024));
+    ensure_arcs(std::max<int64_t>(o.arc_capacity_hint, 1024));
+    {
+        int2 s = make_int2(m1.start, m2.start);
+        FSTC_CUDA(cudaMemcpyAsync(pair.p, &s, sizeof s, cudaMemcpyHostToDevice, c.stream));
+        unsigned long long one = 1;
+        FSTC_CUDA(cudaMemcpyAsync(d_counters.p, &one, sizeof one, cudaMemcpyHostToDevice, c.stream));
+        n_states = 1;
+        ensure_table(std::max<int64_t>(o.state_capacity_hint, 1));
+    }
+
+    int64_t f_lo = 0, f_hi = 1, cum_raw = 0;
+    int last_mode = 1;           // how the last frontier [f_lo, f_hi) was treated: 0 not expanded, 1 all, 2 cut
+    uint64_t cut_key = 0;
+    int64_t last_lo = 0, last_hi = 1;
+    int lvl = 0;
+    MachineView A = view_of(m1), B = view_of(m2);
+
+    for (;; ++lvl) {
+        const int64_t nf = f_hi - f_lo;
+        if (nf == 0) break;
+        last_lo = f_lo; last_hi = f_hi;
+        if (o.max_levels > 0 && lvl == o.max_levels) { st.truncated = 1; last_mode = 0; break; }
+        last_mode = 1;
+
+        // ---- count
+        DBuf<int64_t> rawU(c, nf), rawF(c, nf);
+        DBuf<uint32_t> nmU(c, nf), nmF(c, nf);
+        int h = tm.begin(FSTC_T_COUNT);
+        k_count<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, o.merge_mode, rawU.p, rawF.p, nmU.p, nmF.p,
+                                                       d_counters.p + 1);
+        FSTC_LAUNCH_CHECK();
+        c.n_launch += 1;
+        tm.end(h);
+
+        // ---- scan + budget
+        h = tm.begin(FSTC_T_SCAN);
+        DBuf<int64_t> roffU(c, nf + 1), roffF(c, nf + 1), moffU(c, nf + 1), moffF(c, nf + 1);
+        exclusive_scan<int64_t>(c, rawU.p, nf, roffU.p);
+        exclusive_scan<int64_t>(c, rawF.p, nf, roffF.p);
+        int64_t RU = read_scalar(c, roffU.p + nf), RF = read_scalar(c, roffF.p + nf);
+        bool stop_after = false;
+        int64_t n_sel = nf;
+        if (o.max_raw_arcs > 0 && cum_raw + RU + RF > o.max_raw_arcs) {
+            // rule T: find the key of the first pair (ascending key order) whose arcs no longer fit
+            const uint64_t remaining = static_cast<uint64_t>(o.max_raw_arcs - cum_raw);
+            uint64_t prefix = 0, before = 0;
+            const int top = ((key_bits + 7) / 8) * 8;
+            for (int shift = top - 8; shift >= 0; shift -= 8) {
+                FSTC_CUDA(cudaMemsetAsync(d_counters.p + 4, 0, sizeof(unsigned long long) * 256, c.stream));
+                k_cut_hist<<<nblk(nf), CT_THREADS, 0, c.stream>>>(pair.p, f_lo, nf, nq2, rawU.p, rawF.p, prefix, shift,
+                                                                  d_counters.p + 4);
+                FSTC_LAUNCH_CHECK();
+                c.n_launch += 1;
+                unsigned long long hist[256];
+                FSTC_CUDA(cudaMemcpyAsync(hist, d_counters.p + 4, sizeof hist, cudaMemcpyDeviceToHost, c.stream));
+                c.sync();
+                int d = 0;
+                for (; d < 256; ++d) {
+                    if (before + hist[d] > remaining) break;
+                    before += hist[d];
+                }
+                if (d == 256) fail(FSTC_ERR_CUDA, "internal: budget cut not found");
+                prefix = (prefix << 8) | static_cast<uint64_t>(d);
+            }
+            cut_key = prefix;
+            FSTC_CUDA(cudaMemsetAsync(d_counters.p + 3, 0, sizeof(unsigned long long), c.stream));
+            k_apply_cut<<<nblk(nf), CT_THREADS, 0, c.stream>>>(pair.p, f_lo, nf, nq2, cut_key, rawU.p, rawF.p, nmU.p, nmF.p,
+                                                               d_counters.p + 3);
+            FSTC_LAUNCH_CHECK();
+            c.n_launch += 1;
+            exclusive_scan<int64_t>(c, rawU.p, nf, roffU.p);
+            exclusive_scan<int64_t>(c, rawF.p, nf, roffF.p);
+            RU = read_scalar(c, roffU.p + nf);
+            RF = read_scalar(c, roffF.p + nf);
+            n_sel = static_cast<int64_t>(read_scalar(c, d_counters.p + 3));
+            st.truncated = 1;
+            stop_after = true;
+            last_mode = 2;
+        }
+        exclusive_scan<uint32_t>(c, nmU.p, nf, moffU.p);
+        exclusive_scan<uint32_t>(c, nmF.p, nf, moffF.p);
+        const int64_t MU = read_scalar(c, moffU.p + nf), MF = read_scalar(c, moffF.p + nf);
+        tm.end(h);
+
+        const int64_t R = RU + RF;
+        // ---- capacities for this level
+        const uint64_t remaining_pairs = n_pairs_total - static_cast<uint64_t>(n_states);
+        const int64_t new_bound = static_cast<int64_t>(std::min<uint64_t>(static_cast<uint64_t>(R), remaining_pairs));
+        if (n_states + new_bound >= 0x7FFFFFFFll) fail(FSTC_ERR_CAPACITY, "more than 2^31-1 states");
+        ensure_pairs(n_states + new_bound);
+        ensure_table(n_states + new_bound);
+        ensure_arcs(n_arcs + R);
+
+        // ---- match work-lists
+        MatchList LU{nullptr, nullptr, nullptr}, LF{nullptr, nullptr, nullptr};
+        DBuf<int64_t> cumU(c, MU + 1), cumF(c, MF + 1);
+        DBuf<uint4> recU(c, MU), recF(c, MF);
+        DBuf<uint32_t> plU(c, MU), plF(c, MF);
+        LU = MatchList{cumU.p, recU.p, plU.p};
+        LF = MatchList{cumF.p, recF.p, plF.p};
+        if (MU + MF > 0) {
+            h = tm.begin(FSTC_T_MATCH);
+            k_match<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, nmU.p, nmF.p, moffU.p, moffF.p, roffU.p,
+                                                           roffF.p, LU, LF);
+            FSTC_LAUNCH_CHECK();
+            c.n_launch += 1;
+            tm.end(h);
+        }
+
+        const int64_t arc_base = n_arcs;
+        if (RF == 0) {
+            // no source of this level can hold duplicates: arcs go straight to their final place
+            h = tm.begin(FSTC_T_EMIT);
+            launch_emit(EMIT_DIRECT, LU, MU, RU, arc_base, f_lo, nullptr, nullptr, 0, nullptr, 0, 0);
+            tm.end(h);
+            n_arcs += RU;
+        } else {
+            if (shift_t > 32) fail(FSTC_ERR_CAPACITY, "bits(|Σ|)+bits(|Δ|) = %d > 32: merge key does not fit 64 bits", shift_t);
+            DBuf<uint4> sa(c, RF), sb(c, RF);
+            h = tm.begin(FSTC_T_EMIT);
+            launch_emit(EMIT_SORTREC, LF, MF, RF, 0, f_lo, nullptr, nullptr, 0, sa.p, shift_t, bits_b);
+            tm.end(h);
+            // target ids are now known: n_states bounds them
+            const int64_t ns_now = static_cast<int64_t>(read_scalar(c, d_counters.p));
+            const int tgt_bits = bits_for(static_cast<uint64_t>(ns_now - 1));
+            h = tm.begin(FSTC_T_SORT);
+            uint4 *sorted = radix_sort_records(c, sa.p, sb.p, RF, make_sort_passes(shift_t + tgt_bits, bits_for(static_cast<uint64_t>(nf - 1))));
+            tm.end(h);
+            h = tm.begin(FSTC_T_REDUCE);
+            DBuf<uint8_t> head(c, RF);
+            DBuf<int64_t> hidx(c, RF + 1);
+            k_heads<<<nblk(RF), CT_THREADS, 0, c.stream>>>(sorted, RF, head.p);
+            FSTC_LAUNCH_CHECK();
+            exclusive_scan<uint8_t>(c, head.p, RF, hidx.p);
+            const int64_t M = read_scalar(c, hidx.p + RF);
+            DBuf<unsigned long long> mkey(c, M);
+            DBuf<uint32_t> msrc(c, M);
+            DBuf<float> mw(c, M);
+            FSTC_CUDA(cudaMemsetAsync(mw.p, 0, sizeof(float) * M, c.stream));
+            k_reduce<<<nblk(RF), CT_THREADS, 0, c.stream>>>(sorted, head.p, hidx.p, RF, mkey.p, msrc.p, mw.p);
+            FSTC_LAUNCH_CHECK();
+            DBuf<int64_t> mstart(c, nf + 1), fc(c, nf), foff(c, nf + 1);
+            k_mstart<<<nblk(nf + 1), CT_THREADS, 0, c.stream>>>(msrc.p, M, nf, mstart.p);
+            FSTC_LAUNCH_CHECK();
+            k_final_counts<<<nblk(nf), CT_THREADS, 0, c.stream>>>(rawU.p, mstart.p, nf, fc.p);
+            FSTC_LAUNCH_CHECK();
+            exclusive_scan<int64_t>(c, fc.p, nf, foff.p);
+            k_place_merged<<<nblk(M), CT_THREADS, 0, c.stream>>>(mkey.p, msrc.p, mw.p, M, mstart.p, foff.p, arc_base, f_lo,
+                                                                 shift_t, bits_b, a_src.p, a_il.p, a_ol.p, a_tgt.p, a_w.p);
+            FSTC_LAUNCH_CHECK();
+            c.n_launch += 5;
+            tm.end(h);
+            h = tm.begin(FSTC_T_EMIT);
+            launch_emit(EMIT_INDIRECT, LU, MU, RU, 0, f_lo, foff.p, roffU.p, arc_base, nullptr, 0, 0);
+            tm.end(h);
+            n_arcs += RU + M;
+            st.n_raw_sorted += RF;
+            c.sync();   // the level's temporaries go out of scope below
+        }
+
+        const int64_t ns_after = static_cast<int64_t>(read_scalar(c, d_counters.p));
+        if (lvl < FSTC_MAX_LEVEL_STATS) {
+            st.level_frontier[lvl] = nf;
+            st.level_raw[lvl] = R;
+            st.level_new_states[lvl] = ns_after - n_states;
+        }
+        st.n_matches += MU + MF;
+        st.n_expanded += n_sel;
+        cum_raw += R;
+        n_states = ns_after;
+        f_lo = f_hi;
+        f_hi = n_states;
+        st.n_levels = lvl + 1;
+        if (stop_after) break;
+    }
+
+    // ---- assemble
+    int h = tm.begin(FSTC_T_ASSEMBLE);
+    DBuf<uint8_t> accf(c, n_states), expanded(c, n_states);
+    DBuf<int64_t> accidx(c, n_states + 1);
+    k_accept_flags<<<nblk(n_states), CT_THREADS, 0, c.stream>>>(pair.p, n_states, m1.accept_bits, m2.accept_bits, accf.p);
+    FSTC_LAUNCH_CHECK();
+    exclusive_scan<uint8_t>(c, accf.p, n_states, accidx.p);
+    const int64_t n_accept = read_scalar(c, accidx.p + n_states);
+    DBuf<int32_t> accept(c, n_accept);
+    k_accept_scatter<<<nblk(n_states), CT_THREADS, 0, c.stream>>>(accf.p, accidx.p, n_states, accept.p);
+    FSTC_LAUNCH_CHECK();
+    k_expanded<<<nblk(n_states), CT_THREADS, 0, c.stream>>>(pair.p, n_states, last_lo, last_hi, last_mode, nq2, cut_key,
+                                                          expanded.p);
+    FSTC_LAUNCH_CHECK();
+    c.n_launch += 3;
+    tm.end(h);
+
+    unsigned long long cnt[3];
+    FSTC_CUDA(cudaMemcpyAsync(cnt, d_counters.p, sizeof cnt, cudaMemcpyDeviceToHost, c.stream));
+    FSTC_CUDA(cudaEventRecord(ev1, c.stream));
+    c.sync();
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, ev0, ev1);
+    cudaEventDestroy(ev0);
+    cudaEventDestroy(ev1);
+    tm.collect(st.ms);
+
+    st.ms_total = ms;
+    st.n_states = n_states; st.n_arcs = n_arcs; st.n_raw_arcs = cum_raw;
+    st.n_seg_visited = static_cast<int64_t>(cnt[1]);
+    st.n_match_arcs = static_cast<int64_t>(cnt[2]);
+    st.table_capacity = static_cast<int64_t>(cap);
+    st.n_kernel_launches = static_cast<int32_t>(c.n_launch);
+
+    fstc_result_t *r = new fstc_result_t();
+    ResultImpl *impl = new ResultImpl();
+    r->n_states = n_states; r->n_arcs = n_arcs; r->n_raw_arcs = cum_raw; r->n_accept = n_accept;
+    r->n_expanded = st.n_expanded; r->n_levels = st.n_levels; r->truncated = st.truncated;
+    r->pair = reinterpret_cast<int32_t *>(pair.take());
+    r->src = a_src.take(); r->ilabel = a_il.take(); r->olabel = a_ol.take(); r->tgt = a_tgt.take();
+    r->weight = a_w.take(); r->accept = accept.take(); r->expanded = expanded.take();
+    impl->bufs[0] = r->pair; impl->bufs[1] = r->src; impl->bufs[2] = r->ilabel; impl->bufs[3] = r->olabel;
+    impl->bufs[4] = r->tgt; impl->bufs[5] = r->weight; impl->bufs[6] = r->accept; impl->bufs[7] = r->expanded;
+    r->impl = impl;
+    return r;
+}
+
+}  // namespace
+
+fstc_result_t *compose_packed(Ctx &c, const fstc_packed_t &m1, const fstc_packed_t &m2, const fstc_opts_t &opts,
+                              fstc_stats_t *stats) {
+    Composer k(c, m1, m2, opts);
+    fstc_result_t *r = k.run();
+    if (stats) *stats = k.st;
+    return r;
+}
+
+void free_result(fstc_result_t *r) {
+    if (!r) return;
+    ResultImpl *impl = static_cast<ResultImpl *>(r->impl);
+    if (impl) {
+        for (void *p : impl->bufs)
+            if (p) (void)cudaFreeAsync(p, nullptr);
+        delete impl;
+    }
+    delete r;
+}
+
+}  // namespace fstc

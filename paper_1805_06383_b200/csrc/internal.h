@@ -1,0 +1,53 @@
+// Internal interfaces between the translation units of libfstc.  Not part of the C ABI.
+#pragma once
+
+#include <vector>
+
+#include "common.cuh"
+
+namespace fstc {
+
+// ---------------------------------------------------------------- radix sort (radix_sort.cu)
+// Records are 16 bytes: {x,y} = 64-bit key (x low word), z = 32-bit high key ("src"), w = payload.
+// The sort order is (z, key64) ascending, restricted to the bits the passes name; it is a stable
+// least-significant-digit radix sort with digits of up to 8 bits.
+struct SortPass {
+    int word;   // 0: digit taken from the 64-bit key; 1: from z
+    int shift;  // bit offset inside that word
+    int bits;   // 1..8
+};
+// LSD pass list covering key bits [0, key_bits) then z bits [0, z_bits).
+std::vector<SortPass> make_sort_passes(int key_bits, int z_bits);
+// Sorts n records.  `a` holds the input; `b` is scratch of the same size.  Returns the buffer
+// (a or b) that holds the sorted records.
+uint4 *radix_sort_records(Ctx &c, uint4 *a, uint4 *b, int64_t n, const std::vector<SortPass> &passes);
+
+// ---------------------------------------------------------------- packed transducer (pack.cu)
+enum : uint8_t { FLAG_D = 1, FLAG_X = 2 };
+
+}  // namespace fstc
+
+// The opaque type of include/fstc.h.  All arrays are device memory from the library pool.
+struct fstc_packed_t {
+    int side = 0;                 // 1: inner = olabel (left operand), 2: inner = ilabel (right operand)
+    int32_t n_states = 0, n_inner = 0, n_outer = 0, start = 0;
+    int64_t n_arcs = 0, n_segs = 0;
+    uint4 *arcs = nullptr;        // [n_arcs]   {tgt, outer, weight bits, inner}, sorted by (src, inner, outer, tgt)
+    uint2 *segs = nullptr;        // [n_segs+1] {inner symbol, first arc}; sentinel {0xFFFFFFFF, n_arcs}
+    uint32_t *seg_ptr = nullptr;  // [n_states+1] first segment of each state
+    uint8_t *flags = nullptr;     // [n_states] FLAG_D | FLAG_X
+    uint32_t *accept_bits = nullptr;  // [(n_states+31)/32]
+    int device = 0;
+};
+
+namespace fstc {
+
+fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side);
+void free_packed(fstc_packed_t *p);
+
+// ---------------------------------------------------------------- composition (compose.cu)
+fstc_result_t *compose_packed(Ctx &c, const fstc_packed_t &m1, const fstc_packed_t &m2, const fstc_opts_t &opts,
+                              fstc_stats_t *stats);
+void free_result(fstc_result_t *r);
+
+}  // namespace fstc

@@ -1,0 +1,349 @@
+"""Thin Python binding of libfstc.so (include/fstc.h): argument marshalling only.
+
+Every step of the composition runs in the library's CUDA kernels.  PyTorch is used for
+device memory (inputs as CUDA tensors, outputs wrapped zero-copy as CUDA tensors) and for
+the current stream.  There is NO CPU fallback: if libfstc.so is missing, importing any
+compute entry point raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfstc.so")
+
+FSTC_MEM_DEVICE, FSTC_MEM_HOST = 0, 1
+MERGE_AUTO, MERGE_OFF, MERGE_SORT_ALL = 0, 1, 2
+MAX_LEVEL_STATS = 64
+STAGES = ("count", "scan", "match", "emit", "sort", "reduce", "table", "assemble")
+
+EXPORTS = (
+    "fstc_pack", "fstc_packed_free", "fstc_packed_info", "fstc_packed_to_host", "fstc_compose_packed",
+    "fstc_compose", "fstc_result_to_host", "fstc_result_free", "fstc_trim_pool", "fstc_strerror",
+    "fstc_last_error", "fstc_version",
+)
+
+
+class FstcError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"fstc error {code}: {msg}")
+        self.code = code
+
+
+class _Fst(ctypes.Structure):
+    _fields_ = [
+        ("n_states", ctypes.c_int32), ("n_isyms", ctypes.c_int32), ("n_osyms", ctypes.c_int32),
+        ("start", ctypes.c_int32), ("n_arcs", ctypes.c_int64),
+        ("src", ctypes.c_void_p), ("ilabel", ctypes.c_void_p), ("olabel", ctypes.c_void_p),
+        ("tgt", ctypes.c_void_p), ("weight", ctypes.c_void_p),
+        ("n_accept", ctypes.c_int32), ("accept", ctypes.c_void_p), ("mem", ctypes.c_int32),
+    ]
+
+
+class _Opts(ctypes.Structure):
+    _fields_ = [
+        ("merge_mode", ctypes.c_int32), ("max_levels", ctypes.c_int32), ("max_raw_arcs", ctypes.c_int64),
+        ("arc_capacity_hint", ctypes.c_int64), ("state_capacity_hint", ctypes.c_int64),
+        ("profile", ctypes.c_int32), ("reserved", ctypes.c_int32),
+    ]
+
+
+class _Stats(ctypes.Structure):
+    _fields_ = [
+        ("n_states", ctypes.c_int64), ("n_arcs", ctypes.c_int64), ("n_raw_arcs", ctypes.c_int64),
+        ("n_expanded", ctypes.c_int64), ("n_levels", ctypes.c_int32), ("truncated", ctypes.c_int32),
+        ("n_seg_visited", ctypes.c_int64), ("n_matches", ctypes.c_int64), ("n_match_arcs", ctypes.c_int64),
+        ("n_raw_sorted", ctypes.c_int64), ("table_capacity", ctypes.c_int64),
+        ("n_rehash", ctypes.c_int32), ("n_grow", ctypes.c_int32),
+        ("n_emit_launches", ctypes.c_int32), ("n_kernel_launches", ctypes.c_int32),
+        ("ms", ctypes.c_double * len(STAGES)), ("ms_total", ctypes.c_double),
+        ("level_frontier", ctypes.c_int64 * MAX_LEVEL_STATS), ("level_raw", ctypes.c_int64 * MAX_LEVEL_STATS),
+        ("level_new_states", ctypes.c_int64 * MAX_LEVEL_STATS),
+    ]
+
+
+class _Result(ctypes.Structure):
+    _fields_ = [
+        ("n_states", ctypes.c_int64), ("n_arcs", ctypes.c_int64), ("n_raw_arcs", ctypes.c_int64),
+        ("n_accept", ctypes.c_int64), ("n_expanded", ctypes.c_int64),
+        ("n_levels", ctypes.c_int32), ("truncated", ctypes.c_int32),
+        ("pair", ctypes.c_void_p), ("src", ctypes.c_void_p), ("ilabel", ctypes.c_void_p),
+        ("olabel", ctypes.c_void_p), ("tgt", ctypes.c_void_p), ("weight", ctypes.c_void_p),
+        ("accept", ctypes.c_void_p), ("expanded", ctypes.c_void_p), ("impl", ctypes.c_void_p),
+    ]
+
+
+class _HostResult(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_void_p) for n in
+                ("pair", "src", "ilabel", "olabel", "tgt", "weight", "accept", "expanded")]
+
+
+_lib = None
+
+
+def lib():
+    """The loaded C-ABI library; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1805_06383_b200.build` "
+                              "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        P, I = ctypes.c_void_p, ctypes.c_int
+        L.fstc_pack.argtypes = [P, I, P, ctypes.POINTER(P)]
+        L.fstc_packed_free.argtypes = [P]
+        L.fstc_packed_free.restype = None
+        L.fstc_packed_info.argtypes = [P, P]
+        L.fstc_packed_to_host.argtypes = [P, P, P, P, P, P, P]
+        L.fstc_compose_packed.argtypes = [P, P, P, P, ctypes.POINTER(ctypes.POINTER(_Result)), P]
+        L.fstc_compose.argtypes = [P, P, P, P, ctypes.POINTER(ctypes.POINTER(_Result)), P]
+        L.fstc_result_to_host.argtypes = [ctypes.POINTER(_Result), P, P]
+        L.fstc_result_free.argtypes = [ctypes.POINTER(_Result)]
+        L.fstc_result_free.restype = None
+        L.fstc_trim_pool.argtypes = []
+        L.fstc_strerror.argtypes = [I]
+        L.fstc_strerror.restype = ctypes.c_char_p
+        L.fstc_last_error.restype = ctypes.c_char_p
+        L.fstc_version.restype = I
+        _lib = L
+    return _lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        L = lib()
+        msg = L.fstc_last_error().decode() or L.fstc_strerror(rc).decode()
+        raise FstcError(rc, msg)
+
+
+def _stream_ptr(stream=None) -> int:
+    import torch
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return int(s.cuda_stream)
+
+
+# ------------------------------------------------------------------------------------------------ inputs
+@dataclass
+class DeviceFst:
+    """A transducer whose arrays are CUDA tensors (int32 / float32, contiguous)."""
+    n_states: int
+    n_isyms: int
+    n_osyms: int
+    start: int
+    src: "object"
+    ilabel: "object"
+    olabel: "object"
+    tgt: "object"
+    weight: "object"
+    accept: "object"
+
+    @staticmethod
+    def from_host(f, device="cuda") -> "DeviceFst":
+        import torch
+        t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(device)   # noqa: E731
+        return DeviceFst(int(f.n_states), int(f.n_isyms), int(f.n_osyms), int(f.start), t(f.src), t(f.ilabel),
+                         t(f.olabel), t(f.tgt), t(f.weight), t(f.accept))
+
+
+def _marshal(f):
+    """-> (_Fst, keepalive).  Accepts DeviceFst (CUDA tensors) or any object with numpy arrays (host)."""
+    keep = []
+    s = _Fst()
+    s.n_states, s.n_isyms, s.n_osyms, s.start = int(f.n_states), int(f.n_isyms), int(f.n_osyms), int(f.start)
+    is_dev = hasattr(f.src, "data_ptr")
+    names = (("src", np.int32), ("ilabel", np.int32), ("olabel", np.int32), ("tgt", np.int32),
+             ("weight", np.float32), ("accept", np.int32))
+    if is_dev:
+        import torch
+        want = {np.int32: torch.int32, np.float32: torch.float32}
+        for n, dt in names:
+            t = getattr(f, n)
+            if not t.is_cuda and not t.is_pinned():
+                raise ValueError(f"{n}: expected a CUDA (or pinned host) tensor")
+            if t.dtype != want[dt] or not t.is_contiguous():
+                raise ValueError(f"{n}: expected contiguous {want[dt]}")
+            keep.append(t)
+            setattr(s, n, t.data_ptr())
+        s.mem = FSTC_MEM_DEVICE if f.src.is_cuda else FSTC_MEM_HOST
+        s.n_arcs, s.n_accept = int(f.src.numel()), int(f.accept.numel())
+    else:
+        for n, dt in names:
+            a = np.ascontiguousarray(np.asarray(getattr(f, n)), dtype=dt)
+            keep.append(a)
+            setattr(s, n, a.ctypes.data)
+        s.mem = FSTC_MEM_HOST
+        s.n_arcs, s.n_accept = int(keep[0].shape[0]), int(keep[5].shape[0])
+    return s, keep
+
+
+# ------------------------------------------------------------------------------------------------ outputs
+class _DevView:
+    """Zero-copy __cuda_array_interface__ view of library-owned device memory."""
+
+    def __init__(self, ptr: int, shape, typestr: str, owner):
+        self.__cuda_array_interface__ = {"shape": tuple(shape), "typestr": typestr, "data": (int(ptr), False),
+                                         "version": 3, "strides": None}
+        self._owner = owner
+
+
+def _tensor(ptr, shape, typestr, owner):
+    import torch
+    n = int(np.prod(shape))
+    dt = {"<i4": torch.int32, "<f4": torch.float32, "|u1": torch.uint8}[typestr]
+    if n == 0 or not ptr:
+        return torch.empty(tuple(shape), dtype=dt, device="cuda")
+    return torch.as_tensor(_DevView(ptr, shape, typestr, owner), device="cuda")
+
+
+class _ResultHandle:
+    def __init__(self, ptr):
+        self.ptr = ptr
+
+    def __del__(self):
+        if self.ptr:
+            try:
+                lib().fstc_result_free(self.ptr)
+            except Exception:
+                pass
+            self.ptr = None
+
+
+class ComposeResult:
+    """M1∘M2 on the device.  State i is the pair (pair[i,0], pair[i,1]) = (q1,q2); state 0 = (s1,s2).
+    Arcs are sorted by source id; tensors are views of library memory kept alive by this object."""
+
+    def __init__(self, rptr, stats: Optional[_Stats]):
+        self._h = _ResultHandle(rptr)
+        r = rptr.contents
+        self.n_states, self.n_arcs, self.n_raw_arcs = int(r.n_states), int(r.n_arcs), int(r.n_raw_arcs)
+        self.n_accept, self.n_expanded = int(r.n_accept), int(r.n_expanded)
+        self.n_levels, self.truncated = int(r.n_levels), int(r.truncated)
+        h = self._h
+        self.pair = _tensor(r.pair, (self.n_states, 2), "<i4", h)
+        self.src = _tensor(r.src, (self.n_arcs,), "<i4", h)
+        self.ilabel = _tensor(r.ilabel, (self.n_arcs,), "<i4", h)
+        self.olabel = _tensor(r.olabel, (self.n_arcs,), "<i4", h)
+        self.tgt = _tensor(r.tgt, (self.n_arcs,), "<i4", h)
+        self.weight = _tensor(r.weight, (self.n_arcs,), "<f4", h)
+        self.accept = _tensor(r.accept, (self.n_accept,), "<i4", h)
+        self.expanded = _tensor(r.expanded, (self.n_states,), "|u1", h)
+        self.stats = stats_dict(stats) if stats is not None else None
+
+    def to_host(self, out: Optional[dict] = None, stream=None) -> dict:
+        """Copies every array to host memory through fstc_result_to_host.  `out` may hold preallocated
+        (pinned) torch CPU tensors named like the fields, each at least as long as needed."""
+        import torch
+        spec = {"pair": ((self.n_states, 2), torch.int32), "src": ((self.n_arcs,), torch.int32),
+                "ilabel": ((self.n_arcs,), torch.int32), "olabel": ((self.n_arcs,), torch.int32),
+                "tgt": ((self.n_arcs,), torch.int32), "weight": ((self.n_arcs,), torch.float32),
+                "accept": ((self.n_accept,), torch.int32), "expanded": ((self.n_states,), torch.uint8)}
+        hr = _HostResult()
+        res = {}
+        for name, (shape, dt) in spec.items():
+            n = int(np.prod(shape))
+            if out is not None and name in out:
+                buf = out[name]
+                assert buf.dtype == dt and buf.numel() >= n and buf.is_contiguous()
+            else:
+                buf = torch.empty(n, dtype=dt)
+            setattr(hr, name, buf.data_ptr() if n else None)
+            res[name] = buf.view(-1)[:n].view(*shape)
+        _check(lib().fstc_result_to_host(self._h.ptr, _stream_ptr(stream), ctypes.addressof(hr)))
+        return res
+
+
+def stats_dict(s: _Stats) -> dict:
+    nl = min(int(s.n_levels), MAX_LEVEL_STATS)
+    return {
+        "n_states": int(s.n_states), "n_arcs": int(s.n_arcs), "n_raw_arcs": int(s.n_raw_arcs),
+        "n_expanded": int(s.n_expanded), "n_levels": int(s.n_levels), "truncated": int(s.truncated),
+        "n_seg_visited": int(s.n_seg_visited), "n_matches": int(s.n_matches), "n_match_arcs": int(s.n_match_arcs),
+        "n_raw_sorted": int(s.n_raw_sorted), "table_capacity": int(s.table_capacity),
+        "n_rehash": int(s.n_rehash), "n_grow": int(s.n_grow), "n_emit_launches": int(s.n_emit_launches),
+        "n_kernel_launches": int(s.n_kernel_launches),
+        "ms": {k: float(s.ms[i]) for i, k in enumerate(STAGES)}, "ms_total": float(s.ms_total),
+        "level_frontier": [int(s.level_frontier[i]) for i in range(nl)],
+        "level_raw": [int(s.level_raw[i]) for i in range(nl)],
+        "level_new_states": [int(s.level_new_states[i]) for i in range(nl)],
+    }
+
+
+def _opts(merge_mode=MERGE_AUTO, max_raw_arcs=0, max_levels=0, arc_capacity_hint=0, state_capacity_hint=0,
+          profile=False) -> _Opts:
+    o = _Opts()
+    o.merge_mode, o.max_levels, o.max_raw_arcs = int(merge_mode), int(max_levels), int(max_raw_arcs)
+    o.arc_capacity_hint, o.state_capacity_hint, o.profile = int(arc_capacity_hint), int(state_capacity_hint), int(bool(profile))
+    return o
+
+
+class Packed:
+    """fstc_packed_t handle (device-resident, reusable)."""
+
+    def __init__(self, ptr):
+        self.ptr = ptr
+
+    def info(self) -> dict:
+        a = (ctypes.c_int64 * 6)()
+        _check(lib().fstc_packed_info(self.ptr, ctypes.addressof(a)))
+        return dict(zip(("n_states", "n_arcs", "n_segments", "n_inner", "n_outer", "side"), (int(x) for x in a)))
+
+    def to_host(self, stream=None) -> dict:
+        i = self.info()
+        arcs = np.empty((i["n_arcs"], 4), np.uint32)
+        segs = np.empty((i["n_segments"] + 1, 2), np.uint32)
+        seg_ptr = np.empty(i["n_states"] + 1, np.uint32)
+        flags = np.empty(i["n_states"], np.uint8)
+        acc = np.empty((i["n_states"] + 31) // 32, np.uint32)
+        _check(lib().fstc_packed_to_host(self.ptr, _stream_ptr(stream), arcs.ctypes.data, segs.ctypes.data,
+                                         seg_ptr.ctypes.data, flags.ctypes.data, acc.ctypes.data))
+        return {"arcs": arcs, "segs": segs, "seg_ptr": seg_ptr, "flags": flags, "accept_bits": acc, **i}
+
+    def free(self):
+        if self.ptr:
+            lib().fstc_packed_free(self.ptr)
+            self.ptr = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+def fstc_pack(m, side: int, stream=None) -> Packed:
+    s, keep = _marshal(m)
+    out = ctypes.c_void_p()
+    _check(lib().fstc_pack(ctypes.addressof(s), int(side), _stream_ptr(stream), ctypes.byref(out)))
+    del keep
+    return Packed(out)
+
+
+def fstc_compose_packed(p1: Packed, p2: Packed, *, stream=None, with_stats=True, **opts) -> ComposeResult:
+    o = _opts(**opts)
+    st = _Stats() if with_stats else None
+    out = ctypes.POINTER(_Result)()
+    _check(lib().fstc_compose_packed(p1.ptr, p2.ptr, ctypes.addressof(o), _stream_ptr(stream), ctypes.byref(out),
+                                     ctypes.addressof(st) if st is not None else None))
+    return ComposeResult(out, st)
+
+
+def fstc_compose(m1, m2, *, stream=None, with_stats=True, **opts) -> ComposeResult:
+    """fst_compose(M1, M2) -> M1∘M2.  m1/m2: DeviceFst (CUDA tensors) or host arrays."""
+    s1, k1 = _marshal(m1)
+    s2, k2 = _marshal(m2)
+    o = _opts(**opts)
+    st = _Stats() if with_stats else None
+    out = ctypes.POINTER(_Result)()
+    _check(lib().fstc_compose(ctypes.addressof(s1), ctypes.addressof(s2), ctypes.addressof(o), _stream_ptr(stream),
+                              ctypes.byref(out), ctypes.addressof(st) if st is not None else None))
+    del k1, k2
+    return ComposeResult(out, st)
+
+
+def fstc_trim_pool():
+    _check(lib().fstc_trim_pool())
