@@ -1,0 +1,344 @@
+#!/usr/bin/env python
+"""Benchmark of the composition hot path (pack -> compose) on BASELINE.json's workloads.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload large|medium|skewed|nlp|tiny]
+                    [--impl ours|reference] [--no-e2e] [--no-cpu-baseline]
+
+One "step" = one pass of the whole hot path over one pair of synthetic transducers: pack(M1),
+pack(M2), compose_packed (count, scan, match, emit + visited set, merge, assembly).  Inputs are resident
+in HBM when the timed region of `value` starts; `e2e` repeats the step through the C ABI with HOST
+buffers (H2D of the inputs and D2H of the whole result inside the timed region).
+
+N > 1 (torchrun): the path shards by independent problems — every rank composes its own seeded pair of
+the same shape, no data-path collective ("scaling": "weak"); time = max over ranks, value = Σ arcs / time.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands, 1 core) on a bounded sample of the same
+workload; it is a deliberately slow baseline, not a target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "composed_raw_arcs_per_sec"
+UNIT = "arcs/s"
+# bounded oracle samples (raw-arc budget) sized for roughly 10-30 s of one host core
+ORACLE_SAMPLE_BUDGET = {"large": 20_000_000, "medium": 60_000_000, "skewed": 60_000_000, "nlp": 0, "tiny": 0}
+WORKLOAD_DESC = {
+    "large": "large random (BASELINE.json configs[3]): |Q1|=|Q2|=1e5, |Σ|=|Δ|=2e4, |Γ|=5e3 Zipf 1.1, 5e6 arcs each, "
+             "max_raw_arcs=1e9 (rule T)",
+    "medium": "medium random (configs[1]): |Q1|=|Q2|=1e4, |Σ|=|Δ|=1e3, |Γ|=1e3 Zipf 1.0, 2e5 arcs each, complete",
+    "skewed": "skewed/high-merge (configs[4]): |Q|=2e3, |Σ|=|Δ|=10, |Γ|=50 Zipf 1.5, 1e6 arcs each, power-law degree, "
+              "max_raw_arcs=1e9",
+    "nlp": "NLP-shaped (configs[2]): 50x8 lattice ∘ 30k-state bigram (3e6 arcs), complete",
+    "tiny": "tiny random (configs[0])",
+}
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx = float(r[1])
+            except ValueError:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        # clocks under load: the upper half of the samples (idle gaps between steps pull the median down)
+        load = sm[len(sm) // 2:] if sm else []
+        return {"sm_mhz": load[len(load) // 2] if load else None, "sm_max_mhz": mx, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def alg_bytes(st: dict, n_new_states: int) -> dict:
+    """Algorithmic bytes of one composition, from exact device-side counts."""
+    E, R, S, M = st["n_expanded"], st["n_raw_arcs"], st["n_states"], st["n_arcs"]
+    Rm = st["n_raw_sorted"]
+    path = (16 * E + 8 * st["n_seg_visited"] + 12 * st["n_match_arcs"] + 12 * R + 12 * S + 20 * M + 9 * S + 40 * Rm)
+    emit = 12 * st["n_match_arcs"] + 12 * R + 12 * n_new_states + 8 * n_new_states + 20 * (R - Rm) + 16 * Rm
+    return {"path": path, "emit": emit}
+
+
+def run_reference(args, rank, world):
+    """The CPU oracle, as it stands, on a bounded sample of the workload (rank 0 only)."""
+    if rank != 0:
+        return
+    import oracle
+    from paper_1805_06383_b200 import workloads
+    m1, m2 = workloads.make_config(args.workload)
+    full_budget = int(workloads.CONFIGS[args.workload]["max_raw_arcs"])
+    sample = ORACLE_SAMPLE_BUDGET[args.workload] or full_budget
+    if full_budget:
+        sample = min(sample, full_budget) if sample else full_budget
+    secs, arcs = [], 0
+    for i in range(args.warmup + args.steps):
+        r = oracle.compose(m1, m2, max_raw_arcs=sample, keep_arcs=False)
+        if i >= args.warmup:
+            secs.append(r.seconds)
+            arcs = r.n_raw_arcs
+        if sum(secs) > 240:      # keep the whole run within a few minutes
+            break
+    steps = len(secs)
+    t = sum(secs)
+    value = arcs * steps / t
+    desc = f"oracle.compose on the same inputs with max_raw_arcs={sample} ({arcs} raw arcs per step), 1 thread"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t / steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD_DESC[args.workload], "sample": desc},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="large", choices=sorted(WORKLOAD_DESC))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--merge-mode", type=int, default=0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1805_06383_b200 import fstc, workloads
+    fstc.lib()                                   # no CUDA library, no benchmark (there is no fallback)
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device"
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # every rank composes its own seeded pair of the same shape (independent problems, no collective)
+    s1, s2 = workloads.CONFIGS[args.workload]["seeds"]
+    m1, m2 = workloads.make_config(args.workload, seeds=(s1 + 1000 * rank, s2 + 1000 * rank))
+    budget = int(workloads.CONFIGS[args.workload]["max_raw_arcs"])
+    d1, d2 = fstc.DeviceFst.from_host(m1), fstc.DeviceFst.from_host(m2)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+    hints = {"arc": 0, "state": 0}
+
+    def step(profile=True):
+        """pack + compose on device-resident inputs; returns (ms, stats, pack_launches)."""
+        flush.fill_(1)                                                   # L2 flush, outside the timed region
+        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        torch.cuda.synchronize()
+        e0.record()
+        p1 = fstc.fstc_pack(d1, 1)
+        p2 = fstc.fstc_pack(d2, 2)
+        e1.record()
+        r = fstc.fstc_compose_packed(p1, p2, merge_mode=args.merge_mode, max_raw_arcs=budget, profile=profile,
+                                     arc_capacity_hint=hints["arc"], state_capacity_hint=hints["state"])
+        e2.record()
+        torch.cuda.synchronize()
+        st = r.stats
+        st["pack_ms"], st["compose_ms"] = e0.elapsed_time(e1), e1.elapsed_time(e2)
+        launches = st["n_kernel_launches"] + p1.info().get("n_kernel_launches", 0) + p2.info().get("n_kernel_launches", 0)
+        del r
+        p1.free(); p2.free()
+        return e0.elapsed_time(e2), st, launches
+
+    for _ in range(max(args.warmup, 3)):
+        _, st, _ = step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    barrier()
+    ms_steps, stats, launches = [], [], 0
+    for _ in range(args.steps):
+        ms, st, nl = step()
+        ms_steps.append(ms); stats.append(st); launches += nl
+    barrier()
+    clocks = sampler.stop()
+
+    t_ms = sum(ms_steps)
+    arcs = sum(s["n_raw_arcs"] for s in stats)
+    t = torch.tensor([t_ms, float(arcs), float(launches)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        t_ms, arcs, launches = float(tmax[0]), float(tsum[1]), int(tsum[2])
+    value = arcs / (t_ms * 1e-3)
+
+    st = stats[-1]
+    peak, peak_src = _peaks()
+    new_states = st["n_states"] - 1
+    ab = alg_bytes(st, new_states)
+    emit_ms = sum(s["ms"]["emit"] for s in stats) / max(1, sum(s["n_emit_launches"] for s in stats))
+    emit_bytes_per_launch = ab["emit"] / max(1, st["n_emit_launches"])
+    emit_gbs = emit_bytes_per_launch / (emit_ms * 1e-3) / 1e9 if emit_ms > 0 else 0.0
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", f"emit_traffic_{args.workload}.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
+        except Exception:
+            traffic = None
+    compose_ms = sum(s["compose_ms"] for s in stats) / len(stats)
+    pack_ms = sum(s["pack_ms"] for s in stats) / len(stats)
+    path_gbs = ab["path"] / (compose_ms * 1e-3) / 1e9
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": t_ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": WORKLOAD_DESC[args.workload], "name": args.workload, "seeds": [s1, s2],
+                   "max_raw_arcs": budget, "merge_mode": args.merge_mode, "parallelism": f"replicas x{world}",
+                   "cache": "L2 flushed (256 MiB write) before every step; working set >> L2"},
+        "result": {"n_states": st["n_states"], "n_arcs": st["n_arcs"], "n_raw_arcs": st["n_raw_arcs"],
+                   "n_levels": st["n_levels"], "truncated": st["truncated"], "n_expanded": st["n_expanded"],
+                   "merged_arcs_per_sec": st["n_arcs"] * world / (t_ms / args.steps * 1e-3)},
+        "timing_ms": {"pack": pack_ms, "compose_packed": compose_ms,
+                      "stages": {k: sum(s["ms"][k] for s in stats) / len(stats) for k in fstc.STAGES},
+                      "compose_raw_arcs_per_sec": st["n_raw_arcs"] / (compose_ms * 1e-3)},
+        "roofline": {"bound": "hbm", "kernel": "k_emit (emit + visited-set find-or-insert)", "achieved": emit_gbs,
+                     "peak": peak, "unit": "GB/s", "frac": emit_gbs / peak, "peak_source": peak_src,
+                     "traffic": traffic, "alg_bytes_per_launch": emit_bytes_per_launch, "ms_per_launch": emit_ms,
+                     "launches_per_step": st["n_emit_launches"], "frac_of_8TBs_nominal": emit_gbs / 8000.0},
+        "roofline_path": {"alg_bytes": ab["path"], "achieved": path_gbs, "frac": path_gbs / peak,
+                          "frac_of_8TBs_nominal": path_gbs / 8000.0,
+                          "alg_bytes_per_raw_arc": ab["path"] / max(1, st["n_raw_arcs"])},
+        "clocks": clocks, "gpu_launches": int(launches),
+        "host": {"nproc": os.cpu_count()},
+    }
+
+    # ---- end to end through the C ABI with host buffers (rank-local, then max over ranks)
+    if not args.no_e2e:
+        pin = lambda a: torch.from_numpy(a).pin_memory()     # noqa: E731
+        class HostFst:                                        # pinned host tensors: mem = FSTC_MEM_HOST
+            pass
+        hs = []
+        for m in (m1, m2):
+            h = HostFst()
+            h.n_states, h.n_isyms, h.n_osyms, h.start = m.n_states, m.n_isyms, m.n_osyms, m.start
+            for n in ("src", "ilabel", "olabel", "tgt", "weight", "accept"):
+                setattr(h, n, pin(getattr(m, n)))
+            hs.append(h)
+        na, ns = st["n_arcs"], st["n_states"]
+        out = {"pair": torch.empty(2 * ns, dtype=torch.int32).pin_memory(),
+               "expanded": torch.empty(ns, dtype=torch.uint8).pin_memory(),
+               "accept": torch.empty(max(1, ns), dtype=torch.int32).pin_memory()}
+        for n in ("src", "ilabel", "olabel", "tgt"):
+            out[n] = torch.empty(na, dtype=torch.int32).pin_memory()
+        out["weight"] = torch.empty(na, dtype=torch.float32).pin_memory()
+        h2d = sum(int(getattr(h, n).numel()) * 4 for h in hs for n in ("src", "ilabel", "olabel", "tgt", "weight", "accept"))
+        e2e_ms, e2e_arcs, d2h = 0.0, 0, 0
+        n_e2e = max(1, min(args.e2e_steps, args.steps))
+        for i in range(1 + n_e2e):
+            flush.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            barrier()
+            a.record()
+            r = fstc.fstc_compose(hs[0], hs[1], merge_mode=args.merge_mode, max_raw_arcs=budget,
+                                  arc_capacity_hint=hints["arc"], state_capacity_hint=hints["state"])
+            r.to_host(out)
+            b.record()
+            torch.cuda.synchronize()
+            if i > 0:
+                e2e_ms += a.elapsed_time(b)
+                e2e_arcs += r.n_raw_arcs
+            d2h = 8 * r.n_states + r.n_states + 4 * r.n_accept + 20 * r.n_arcs
+            del r
+        t = torch.tensor([e2e_ms, float(e2e_arcs)], dtype=torch.float64, device="cuda")
+        if world > 1:
+            tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+            tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+            e2e_ms, e2e_arcs = float(tmax[0]), float(tsum[1])
+        line["e2e"] = {"value": e2e_arcs / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                       "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / n_e2e, "steps": n_e2e,
+                       "api": "fstc_compose(host arrays) + fstc_result_to_host(pinned buffers)"}
+        del out
+
+    # ---- the oracle, as it stands, on this box's host cores (rank 0, N = 1 only)
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        sample = ORACLE_SAMPLE_BUDGET[args.workload] or budget
+        if budget:
+            sample = min(sample, budget) if sample else budget
+        r = oracle.compose(m1, m2, max_raw_arcs=sample, keep_arcs=False)
+        line["cpu_baseline"] = {
+            "value": r.n_raw_arcs / r.seconds, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"oracle.compose (serial C++, fp64, Algorithm 1) on the same inputs with max_raw_arcs={sample}: "
+                      f"{r.n_raw_arcs} raw arcs in {r.seconds:.2f} s on 1 of {os.cpu_count()} cores"}
+
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -174,7 +174,8 @@ typedef struct fstc_packed_t fstc_packed_t;
 /* side 1: the inner alphabet is the OUTPUT side (left operand M1); side 2: the INPUT side (M2). */
 FSTC_API int fstc_pack(const fstc_fst_t *m, int side, void *cuda_stream, fstc_packed_t **out);
 FSTC_API void fstc_packed_free(fstc_packed_t *p);
-/* info[0..5] = n_states, n_arcs, n_segments (distinct (state, inner symbol)), n_inner, n_outer, side */
+/* info[0..6] = n_states, n_arcs, n_segments (distinct (state, inner symbol)), n_inner, n_outer, side,
+ *               kernel launches the pack took */
 FSTC_API int fstc_packed_info(const fstc_packed_t *p, int64_t *info);
 /* Debug/test access: copies the packed arrays to HOST buffers (any may be NULL).
  * arcs4: [4*n_arcs] uint32 (tgt, outer, weight bits, inner); segs2: [2*(n_segments+1)] (symbol, arc offset);

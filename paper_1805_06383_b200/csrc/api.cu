@@ -104,7 +104,7 @@ int fstc_packed_info(const fstc_packed_t *p, int64_t *info) {
     return guarded([&] {
         if (!p || !info) fail(FSTC_ERR_ARG, "null argument");
         info[0] = p->n_states; info[1] = p->n_arcs; info[2] = p->n_segs;
-        info[3] = p->n_inner; info[4] = p->n_outer; info[5] = p->side;
+        info[3] = p->n_inner; info[4] = p->n_outer; info[5] = p->side; info[6] = p->n_launch;
     });
 }
 

@@ -38,6 +38,7 @@ struct fstc_packed_t {
     uint8_t *flags = nullptr;     // [n_states] FLAG_D | FLAG_X
     uint32_t *accept_bits = nullptr;  // [(n_states+31)/32]
     int device = 0;
+    int64_t n_launch = 0;         // kernel launches fstc_pack took
 };
 
 namespace fstc {

@@ -155,6 +155,7 @@ void free_packed(fstc_packed_t *p) {
 }
 
 fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side) {
+    const int64_t launch0 = c.n_launch;
     if (side != 1 && side != 2) fail(FSTC_ERR_ARG, "side must be 1 or 2");
     if (m.n_states < 1 || m.n_isyms < 0 || m.n_osyms < 0 || m.n_arcs < 0 || m.n_accept < 0)
         fail(FSTC_ERR_ARG, "negative size or no states");
@@ -254,6 +255,7 @@ fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side) {
     p->arcs = arcs.take(); p->segs = segs.take(); p->seg_ptr = seg_ptr.take();
     p->flags = flags.take(); p->accept_bits = accept_bits.take();
     FSTC_CUDA(cudaGetDevice(&p->device));
+    p->n_launch = c.n_launch - launch0;
     return p;
 }
 

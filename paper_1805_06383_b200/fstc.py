@@ -288,9 +288,9 @@ class Packed:
         self.ptr = ptr
 
     def info(self) -> dict:
-        a = (ctypes.c_int64 * 6)()
+        a = (ctypes.c_int64 * 7)()
         _check(lib().fstc_packed_info(self.ptr, ctypes.addressof(a)))
-        return dict(zip(("n_states", "n_arcs", "n_segments", "n_inner", "n_outer", "side"), (int(x) for x in a)))
+        return dict(zip(("n_states", "n_arcs", "n_segments", "n_inner", "n_outer", "side", "n_kernel_launches"), (int(x) for x in a)))
 
     def to_host(self, stream=None) -> dict:
         i = self.info()
