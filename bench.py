@@ -115,6 +115,24 @@ def alg_bytes(st: dict, n_new_states: int) -> dict:
     return {"path": path, "emit": emit}
 
 
+def rank_seeds(workload: str, rank: int):
+    """Every rank composes its own pair of the same shape: independent problems, no data-path collective."""
+    from paper_1805_06383_b200 import workloads
+    s1, s2 = workloads.CONFIGS[workload]["seeds"]
+    return s1 + 1000 * rank, s2 + 1000 * rank
+
+
+def reduce_over_ranks(dist, world: int, time_like, sum_like, device):
+    """(max over ranks of each time-like value, sum over ranks of each additive value)."""
+    import torch
+    tm = torch.tensor([float(x) for x in time_like], dtype=torch.float64, device=device)
+    ts = torch.tensor([float(x) for x in sum_like], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+        dist.all_reduce(ts, op=dist.ReduceOp.SUM)
+    return [float(x) for x in tm], [float(x) for x in ts]
+
+
 def run_reference(args, rank, world):
     """The CPU oracle, as it stands, on a bounded sample of the workload (rank 0 only)."""
     if rank != 0:
@@ -185,7 +203,7 @@ def main():
 
     # every rank composes its own seeded pair of the same shape (independent problems, no collective)
     s1, s2 = workloads.CONFIGS[args.workload]["seeds"]
-    m1, m2 = workloads.make_config(args.workload, seeds=(s1 + 1000 * rank, s2 + 1000 * rank))
+    m1, m2 = workloads.make_config(args.workload, seeds=rank_seeds(args.workload, rank))
     budget = int(workloads.CONFIGS[args.workload]["max_raw_arcs"])
     d1, d2 = fstc.DeviceFst.from_host(m1), fstc.DeviceFst.from_host(m2)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
@@ -226,11 +244,7 @@ def main():
 
     t_ms = sum(ms_steps)
     arcs = sum(s["n_raw_arcs"] for s in stats)
-    t = torch.tensor([t_ms, float(arcs), float(launches)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        t_ms, arcs, launches = float(tmax[0]), float(tsum[1]), int(tsum[2])
+    (t_ms,), (arcs, launches) = reduce_over_ranks(dist, world, [t_ms], [arcs, launches], "cuda")
     value = arcs / (t_ms * 1e-3)
 
     st = stats[-1]
@@ -244,7 +258,8 @@ def main():
     tpath = os.path.join(ROOT, "profiles", f"emit_traffic_{args.workload}.json")
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
+            # measured DRAM bytes per raw arc of the captured launch x arcs per launch (average, like `achieved`)
+            traffic = json.load(open(tpath))["dram_bytes_per_raw_arc"] * st["n_raw_arcs"] / max(1, st["n_emit_launches"])
         except Exception:
             traffic = None
     compose_ms = sum(s["compose_ms"] for s in stats) / len(stats)
@@ -312,11 +327,7 @@ def main():
                 e2e_arcs += r.n_raw_arcs
             d2h = 8 * r.n_states + r.n_states + 4 * r.n_accept + 20 * r.n_arcs
             del r
-        t = torch.tensor([e2e_ms, float(e2e_arcs)], dtype=torch.float64, device="cuda")
-        if world > 1:
-            tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-            tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-            e2e_ms, e2e_arcs = float(tmax[0]), float(tsum[1])
+        (e2e_ms,), (e2e_arcs,) = reduce_over_ranks(dist, world, [e2e_ms], [e2e_arcs], "cuda")
         line["e2e"] = {"value": e2e_arcs / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                        "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / n_e2e, "steps": n_e2e,
                        "api": "fstc_compose(host arrays) + fstc_result_to_host(pinned buffers)"}

@@ -93,10 +93,8 @@ __device__ __forceinline__ void intersect(const MachineView &A, const MachineVie
 // class U = arcs go straight to the output; class F = arcs go through sort + reduce first
 __global__ void __launch_bounds__(CT_THREADS)
 k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, int merge_mode,
-        int64_t *__restrict__ rawU, int64_t *__restrict__ rawF, uint32_t *__restrict__ nmU, uint32_t *__restrict__ nmF,
-        unsigned long long *__restrict__ counters /* [0] Σ segments visited, [1] Σ (n1+n2) over matches */) {
+        int64_t *__restrict__ rawU, int64_t *__restrict__ rawF, uint32_t *__restrict__ nmU, uint32_t *__restrict__ nmF) {
     int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    unsigned long long segs = 0, marcs = 0;
     if (i < nf) {
         int2 p = pair[f_lo + i];
         int64_t raw = 0;
@@ -104,9 +102,7 @@ k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_l
         intersect(A, B, p.x, p.y, [&](uint32_t, uint32_t n1, uint32_t, uint32_t n2) {
             raw += static_cast<int64_t>(n1) * n2;
             nm += 1;
-            marcs += n1 + n2;
         });
-        segs = (A.seg_ptr[p.x + 1] - A.seg_ptr[p.x]) + (B.seg_ptr[p.y + 1] - B.seg_ptr[p.y]);
         bool f = false;
         if (merge_mode == FSTC_MERGE_SORT_ALL) f = true;
         else if (merge_mode == FSTC_MERGE_AUTO) {
@@ -115,16 +111,6 @@ k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_l
         }
         rawU[i] = f ? 0 : raw; rawF[i] = f ? raw : 0;
         nmU[i] = f ? 0 : nm;   nmF[i] = f ? nm : 0;
-    }
-    // block-level totals for the statistics
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) {
-        segs += __shfl_xor_sync(0xffffffffu, segs, d);
-        marcs += __shfl_xor_sync(0xffffffffu, marcs, d);
-    }
-    if ((threadIdx.x & 31) == 0 && (segs | marcs)) {
-        atomicAdd(&counters[0], segs);
-        atomicAdd(&counters[1], marcs);
     }
 }
 
@@ -174,22 +160,36 @@ __global__ void __launch_bounds__(CT_THREADS)
 k_match(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_lo, int64_t nf,
         const uint32_t *__restrict__ nmU, const uint32_t *__restrict__ nmF, const int64_t *__restrict__ moffU,
         const int64_t *__restrict__ moffF, const int64_t *__restrict__ roffU, const int64_t *__restrict__ roffF,
-        MatchList U, MatchList F) {
+        MatchList U, MatchList F,
+        unsigned long long *__restrict__ counters /* [0] Σ segments visited, [1] Σ (n1+n2) over matches */) {
     int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i >= nf) return;
-    const bool isF = nmF[i] != 0;
-    if (!isF && nmU[i] == 0) return;
-    int2 p = pair[f_lo + i];
-    MatchList L = isF ? F : U;
-    int64_t m = isF ? moffF[i] : moffU[i];
-    int64_t run = isF ? roffF[i] : roffU[i];
-    intersect(A, B, p.x, p.y, [&](uint32_t o1, uint32_t n1, uint32_t o2, uint32_t n2) {
-        L.cum[m] = run;
-        L.rec[m] = make_uint4(o1, o2, n1, n2);
-        L.pl[m] = static_cast<uint32_t>(i);
-        run += static_cast<int64_t>(n1) * n2;
-        ++m;
-    });
+    unsigned long long segs = 0, marcs = 0;
+    const bool isF = i < nf && nmF[i] != 0;
+    if (i < nf && (isF || nmU[i] != 0)) {
+        int2 p = pair[f_lo + i];
+        MatchList L = isF ? F : U;
+        int64_t m = isF ? moffF[i] : moffU[i];
+        int64_t run = isF ? roffF[i] : roffU[i];
+        intersect(A, B, p.x, p.y, [&](uint32_t o1, uint32_t n1, uint32_t o2, uint32_t n2) {
+            L.cum[m] = run;
+            L.rec[m] = make_uint4(o1, o2, n1, n2);
+            L.pl[m] = static_cast<uint32_t>(i);
+            run += static_cast<int64_t>(n1) * n2;
+            marcs += n1 + n2;
+            ++m;
+        });
+        segs = (A.seg_ptr[p.x + 1] - A.seg_ptr[p.x]) + (B.seg_ptr[p.y + 1] - B.seg_ptr[p.y]);
+    }
+    // statistics for the algorithmic-bytes model: only pairs that are expanded and have a match are charged
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        segs += __shfl_xor_sync(0xffffffffu, segs, d);
+        marcs += __shfl_xor_sync(0xffffffffu, marcs, d);
+    }
+    if ((threadIdx.x & 31) == 0 && (segs | marcs)) {
+        atomicAdd(&counters[0], segs);
+        atomicAdd(&counters[1], marcs);
+    }
 }
 
 // ------------------------------------------------------------------------------------------ emit
@@ -722,8 +722,7 @@ fstc_result_t *Composer::run() {
         DBuf<int64_t> rawU(c, nf), rawF(c, nf);
         DBuf<uint32_t> nmU(c, nf), nmF(c, nf);
         int h = tm.begin(FSTC_T_COUNT);
-        k_count<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, o.merge_mode, rawU.p, rawF.p, nmU.p, nmF.p,
-                                                       d_counters.p + 1);
+        k_count<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, o.merge_mode, rawU.p, rawF.p, nmU.p, nmF.p);
         FSTC_LAUNCH_CHECK();
         c.n_launch += 1;
         tm.end(h);
@@ -797,7 +796,7 @@ fstc_result_t *Composer::run() {
         if (MU + MF > 0) {
             h = tm.begin(FSTC_T_MATCH);
             k_match<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, nmU.p, nmF.p, moffU.p, moffF.p, roffU.p,
-                                                           roffF.p, LU, LF);
+                                                           roffF.p, LU, LF, d_counters.p + 1);
             FSTC_LAUNCH_CHECK();
             c.n_launch += 1;
             tm.end(h);
