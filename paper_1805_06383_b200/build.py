@@ -29,7 +29,15 @@ def _stale(target: str, deps: list[str]) -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, defs: list[str] | None = None, out: str | None = None) -> str:
+    """`defs`/`out` build an experiment variant (extra -D flags) into another file; the product build uses neither."""
+    global OBJ, LIB
+    if defs or out:
+        tag = "_".join(d.replace("-D", "").replace("=", "") for d in (defs or [])) or "variant"
+        OBJ = os.path.join(HERE, "build", tag)
+        LIB = out or os.path.join(HERE, "build", f"libfstc_{tag}.so")
+        FLAGS.extend(defs or [])
+        force = True
     os.makedirs(OBJ, exist_ok=True)
     hdrs = [os.path.join(CSRC, h) for h in HEADERS] + [os.path.abspath(__file__)]
     jobs = []
@@ -65,4 +73,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    _defs = [a for a in sys.argv[1:] if a.startswith("-D")]
+    _out = next((a.split("=", 1)[1] for a in sys.argv[1:] if a.startswith("--out=")), None)
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, defs=_defs or None, out=_out))

@@ -16,6 +16,7 @@
 // blocks, host-side queue, dense |Q1||Q2| visited table, lossy table H — PAPER.md:219-243) is listed in
 // DESIGN.md "differences".
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
 
 #include "internal.h"
@@ -29,6 +30,8 @@ constexpr unsigned long long EMPTY_KEY = ~0ull;
 constexpr uint32_t PENDING_ID = 0xFFFFFFFFu;
 constexpr int CT_THREADS = 256;
 
+__device__ __forceinline__ int64_t ceil_div_dev(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
 struct MachineView {
     const uint4 *arcs;
     const uint2 *segs;
@@ -39,23 +42,39 @@ struct MachineView {
 inline MachineView view_of(const fstc_packed_t &p) { return MachineView{p.arcs, p.segs, p.seg_ptr, p.flags}; }
 
 // ------------------------------------------------------------------------------------------ hash table
-// Open addressing, linear probing, 16-byte slots {key lo, key hi, id, unused}; a slot never straddles a
-// 32-byte sector, so one probe is one sector.  Empty = all ones (a cudaMemset of 0xFF clears it).
+// Open addressing over 32-byte BUCKETS of two 16-byte slots {key lo, key hi, id, unused}: a bucket is exactly
+// one DRAM sector, read with a single 256-bit load.  A key lives in the first free slot on its probe path
+// (home bucket, then the following buckets); slots are never freed, so a lookup that walks the same path
+// finds the key before it meets an empty slot.  Empty = all ones (a cudaMemset of 0xFF clears the table).
+struct Bucket { uint4 s0, s1; };
+
 __device__ __forceinline__ uint64_t mix64(uint64_t k) {
     k ^= k >> 33; k *= 0xff51afd7ed558ccdULL;
     k ^= k >> 33; k *= 0xc4ceb9fe1a85ec53ULL;
     k ^= k >> 33;
     return k;
 }
-__device__ __forceinline__ uint64_t home_slot(uint64_t key, uint64_t cap) { return __umul64hi(mix64(key), cap); }
+// cap = number of slots (even); returns the home BUCKET
+__device__ __forceinline__ uint64_t home_bucket(uint64_t key, uint64_t cap) { return __umul64hi(mix64(key), cap >> 1); }
+
+__device__ __forceinline__ Bucket ld_bucket(const uint4 *table, uint64_t bucket) {
+    Bucket b;
+    asm volatile("ld.global.cg.v8.u32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(b.s0.x), "=r"(b.s0.y), "=r"(b.s0.z), "=r"(b.s0.w), "=r"(b.s1.x), "=r"(b.s1.y), "=r"(b.s1.z), "=r"(b.s1.w)
+                 : "l"(table + 2 * bucket));
+    return b;
+}
+__device__ __forceinline__ unsigned long long slot_key(const uint4 &v) {
+    return (static_cast<unsigned long long>(v.y) << 32) | v.x;
+}
 
 __global__ void tb_insert_ids(const int2 *__restrict__ pair, int64_t n, uint64_t nq2, uint4 *table, uint64_t cap) {
-    // rebuild after growth: keys are distinct, ids known -> plain CAS claim, then store the id
+    // rebuild after growth: keys are distinct and their ids known -> claim the first free slot, store the id
     int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (i >= n) return;
     int2 p = pair[i];
     unsigned long long key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
-    uint64_t s = home_slot(key, cap);
+    uint64_t s = 2 * home_bucket(key, cap);
     while (true) {
         unsigned long long old = atomicCAS(reinterpret_cast<unsigned long long *>(table + s), EMPTY_KEY, key);
         if (old == EMPTY_KEY) break;
@@ -93,16 +112,19 @@ __device__ __forceinline__ void intersect(const MachineView &A, const MachineVie
 // class U = arcs go straight to the output; class F = arcs go through sort + reduce first
 __global__ void __launch_bounds__(CT_THREADS)
 k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, int merge_mode,
+        uint64_t nq2, uint64_t key_limit /* pairs with key >= key_limit are left uncounted (raw = 0) */,
         int64_t *__restrict__ rawU, int64_t *__restrict__ rawF, uint32_t *__restrict__ nmU, uint32_t *__restrict__ nmF) {
     int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (i < nf) {
         int2 p = pair[f_lo + i];
         int64_t raw = 0;
         uint32_t nm = 0;
-        intersect(A, B, p.x, p.y, [&](uint32_t, uint32_t n1, uint32_t, uint32_t n2) {
-            raw += static_cast<int64_t>(n1) * n2;
-            nm += 1;
-        });
+        const uint64_t key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
+        if (key < key_limit)
+            intersect(A, B, p.x, p.y, [&](uint32_t, uint32_t n1, uint32_t, uint32_t n2) {
+                raw += static_cast<int64_t>(n1) * n2;
+                nm += 1;
+            });
         bool f = false;
         if (merge_mode == FSTC_MERGE_SORT_ALL) f = true;
         else if (merge_mode == FSTC_MERGE_AUTO) {
@@ -115,20 +137,35 @@ k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_l
 }
 
 // Budget rule T, radix select: weighted histogram of one 8-bit key digit over the pairs whose higher key bits
-// equal `prefix`.
+// equal `prefix`.  Lanes of a warp that share a digit are summed with match-any + reduce-add (three 22-bit limbs,
+// so 32 lanes cannot overflow 32 bits) and issue ONE shared-memory atomic: the top digits, which are nearly
+// constant over the frontier, no longer serialise.
 __global__ void __launch_bounds__(CT_THREADS)
 k_cut_hist(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, uint64_t nq2, const int64_t *__restrict__ rawU,
            const int64_t *__restrict__ rawF, uint64_t prefix, int shift, unsigned long long *__restrict__ hist) {
     __shared__ unsigned long long h[256];
     h[threadIdx.x] = 0;
     __syncthreads();
-    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i < nf) {
-        int2 p = pair[f_lo + i];
-        uint64_t key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
-        uint64_t hi = (shift + 8 >= 64) ? 0 : (key >> (shift + 8));
-        int64_t r = rawU[i] + rawF[i];
-        if (hi == prefix && r > 0) atomicAdd(&h[(key >> shift) & 255], static_cast<unsigned long long>(r));
+    const int64_t stride = static_cast<int64_t>(gridDim.x) * blockDim.x;
+    const int64_t n_round = ceil_div_dev(nf, stride) * stride;
+    const int lane = threadIdx.x & 31;
+    for (int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x; i < n_round; i += stride) {
+        uint32_t digit = 0xFFFFu;                            // lanes without a contribution
+        uint64_t r = 0;
+        if (i < nf) {
+            int2 p = pair[f_lo + i];
+            uint64_t key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
+            uint64_t hi = (shift + 8 >= 64) ? 0 : (key >> (shift + 8));
+            r = static_cast<uint64_t>(rawU[i] + rawF[i]);
+            if (hi == prefix && r > 0) digit = static_cast<uint32_t>(key >> shift) & 255u;
+        }
+        const uint32_t peers = __match_any_sync(0xffffffffu, digit);
+        const uint32_t l0 = __reduce_add_sync(peers, static_cast<uint32_t>(r & 0x3FFFFFu));
+        const uint32_t l1 = __reduce_add_sync(peers, static_cast<uint32_t>((r >> 22) & 0x3FFFFFu));
+        const uint32_t l2 = __reduce_add_sync(peers, static_cast<uint32_t>(r >> 44));
+        if (digit != 0xFFFFu && lane == __ffs(peers) - 1)
+            atomicAdd(&h[digit], static_cast<unsigned long long>(l0) + (static_cast<unsigned long long>(l1) << 22) +
+                                     (static_cast<unsigned long long>(l2) << 44));
     }
     __syncthreads();
     if (h[threadIdx.x]) atomicAdd(&hist[threadIdx.x], h[threadIdx.x]);
@@ -193,9 +230,40 @@ k_match(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_l
 }
 
 // ------------------------------------------------------------------------------------------ emit
-constexpr int EM_THREADS = 256;
+// L2 residency hints: the packed operands are small and re-read for the whole level (evict-last); the
+// output arcs are written once (streaming stores) so that they do not push the operands out of L2.
+__device__ __forceinline__ uint64_t l2_evict_last_policy() {
+    uint64_t p;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint4 ld_keep(const uint4 *ptr, uint64_t policy) {
+#if FSTC_EM_HINTS
+    uint4 r;
+    asm("ld.global.nc.L2::cache_hint.v4.u32 {%0, %1, %2, %3}, [%4], %5;"
+        : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(ptr), "l"(policy));
+    return r;
+#else
+    (void)policy;
+    return __ldg(ptr);
+#endif
+}
+
+#ifndef FSTC_EM_THREADS
+#define FSTC_EM_THREADS 128
+#endif
+#ifndef FSTC_EM_MINB
+#define FSTC_EM_MINB 5
+#endif
+#ifndef FSTC_EM_HINTS
+#define FSTC_EM_HINTS 1
+#endif
+#ifndef FSTC_TABLE_LOAD_PCT
+#define FSTC_TABLE_LOAD_PCT 40
+#endif
+constexpr int EM_THREADS = FSTC_EM_THREADS;
 constexpr int EM_IPT = 4;                          // consecutive output ranks per thread
-constexpr int EM_TILE = EM_THREADS * EM_IPT;       // 1024 arcs per block
+constexpr int EM_TILE = EM_THREADS * EM_IPT;       // 512 arcs per block
 
 enum { EMIT_DIRECT = 0, EMIT_INDIRECT = 1, EMIT_SORTREC = 2 };
 
@@ -239,7 +307,7 @@ __global__ void k_partition(const int64_t *__restrict__ cum, int64_t n_matches, 
 }
 
 template <int MODE>
-__global__ void __launch_bounds__(EM_THREADS) k_emit(EmitArgs g) {
+__global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
     __shared__ uint32_t relcum[EM_TILE + 1];
     __shared__ int64_t s_first_cum;
     __shared__ uint32_t s_warp[EM_THREADS / 32];
@@ -307,56 +375,69 @@ __global__ void __launch_bounds__(EM_THREADS) k_emit(EmitArgs g) {
     }
 
     // ---- read the two input arcs of every rank, form the composed arc
+    const uint64_t keep_policy = l2_evict_last_policy();     // operands are re-read all level long: keep them in L2
     uint32_t a_sym[EM_IPT], b_sym[EM_IPT];
     float w[EM_IPT];
     unsigned long long key[EM_IPT];
     int2 tgt_pair[EM_IPT];
+    uint32_t todo = 0;                                        // bit u: rank u still has to be resolved in the table
 #pragma unroll
     for (int u = 0; u < EM_IPT; ++u) {
         if (u >= skip && u < skip + n_valid) {
-            uint4 e1 = __ldg(g.A.arcs + idx1[u]);             // {tgt, outer, weight, inner}
-            uint4 e2 = __ldg(g.B.arcs + idx2[u]);
+            uint4 e1 = ld_keep(g.A.arcs + idx1[u], keep_policy);   // {tgt, outer, weight, inner}
+            uint4 e2 = ld_keep(g.B.arcs + idx2[u], keep_policy);
             a_sym[u] = e1.y; b_sym[u] = e2.y;
             w[u] = __uint_as_float(e1.z) * __uint_as_float(e2.z);
             tgt_pair[u] = make_int2(static_cast<int>(e1.x), static_cast<int>(e2.x));
             key[u] = static_cast<uint64_t>(e1.x) * g.nq2 + e2.x;
+            todo |= 1u << u;
         }
     }
 
-    // ---- visited set: find or insert, all first probes in flight together
-    uint64_t slot[EM_IPT];
-    uint4 probe[EM_IPT];
+    // ---- visited set: find or insert.  Rounds of: all pending bucket reads in flight
+    // together, then all pending CAS in flight together; a rank leaves when it finds its key or wins a slot.
+    uint64_t slot[EM_IPT];                                    // bucket while searching, then the key's slot
     uint32_t id[EM_IPT];
-    bool won[EM_IPT];
+    uint32_t won = 0;                                         // bit u: this thread inserted the key (new state)
+    const uint64_t n_buckets = g.cap >> 1;
 #pragma unroll
     for (int u = 0; u < EM_IPT; ++u) {
-        won[u] = false; id[u] = 0;
-        if (u >= skip && u < skip + n_valid) {
-            slot[u] = home_slot(key[u], g.cap);
-            probe[u] = __ldcg(g.table + slot[u]);
-        }
+        id[u] = 0;
+        slot[u] = (todo >> u & 1u) ? home_bucket(key[u], g.cap) : 0;
     }
-    uint32_t n_won = 0;
+    while (todo) {
+        Bucket v[EM_IPT];
+        unsigned long long old[EM_IPT];
+        uint32_t cas = 0, second = 0;                         // second: the CAS targets slot 1 of the bucket
 #pragma unroll
-    for (int u = 0; u < EM_IPT; ++u) {
-        if (u >= skip && u < skip + n_valid) {
-            uint4 v = probe[u];
-            uint64_t s = slot[u];
-            while (true) {
-                unsigned long long k = (static_cast<unsigned long long>(v.y) << 32) | v.x;
-                if (k == key[u]) { id[u] = v.z; break; }
-                if (k == EMPTY_KEY) {
-                    unsigned long long old =
-                        atomicCAS(reinterpret_cast<unsigned long long *>(g.table + s), EMPTY_KEY, key[u]);
-                    if (old == EMPTY_KEY) { won[u] = true; ++n_won; break; }
-                    if (old == key[u]) { id[u] = PENDING_ID; break; }
-                }
-                s = (s + 1 == g.cap) ? 0 : s + 1;
-                v = __ldcg(g.table + s);
+        for (int u = 0; u < EM_IPT; ++u)
+            if (todo >> u & 1u) v[u] = ld_bucket(g.table, slot[u]);
+#pragma unroll
+        for (int u = 0; u < EM_IPT; ++u) {
+            if (todo >> u & 1u) {
+                const unsigned long long k0 = slot_key(v[u].s0), k1 = slot_key(v[u].s1);
+                if (k0 == key[u]) { id[u] = v[u].s0.z; slot[u] = 2 * slot[u]; todo &= ~(1u << u); }
+                else if (k0 == EMPTY_KEY) cas |= 1u << u;
+                else if (k1 == key[u]) { id[u] = v[u].s1.z; slot[u] = 2 * slot[u] + 1; todo &= ~(1u << u); }
+                else if (k1 == EMPTY_KEY) { cas |= 1u << u; second |= 1u << u; }
+                else slot[u] = (slot[u] + 1 == n_buckets) ? 0 : slot[u] + 1;   // both slots taken by other keys
             }
-            slot[u] = s;
+        }
+#pragma unroll
+        for (int u = 0; u < EM_IPT; ++u)
+            if (cas >> u & 1u)
+                old[u] = atomicCAS(reinterpret_cast<unsigned long long *>(g.table + 2 * slot[u] + (second >> u & 1u)),
+                                   EMPTY_KEY, key[u]);
+#pragma unroll
+        for (int u = 0; u < EM_IPT; ++u) {
+            if (cas >> u & 1u) {
+                if (old[u] == EMPTY_KEY) { won |= 1u << u; slot[u] = 2 * slot[u] + (second >> u & 1u); todo &= ~(1u << u); }
+                else if (old[u] == key[u]) { id[u] = PENDING_ID; slot[u] = 2 * slot[u] + (second >> u & 1u); todo &= ~(1u << u); }
+                // else: another key took the slot first -> look at the same bucket again
+            }
         }
     }
+    const uint32_t n_won = __popc(won);
 
     // ---- new state ids: one atomicAdd per block; the new ids of a level are the next frontier
     uint32_t incl = n_won;
@@ -377,7 +458,7 @@ __global__ void __launch_bounds__(EM_THREADS) k_emit(EmitArgs g) {
     uint32_t next_id = static_cast<uint32_t>(s_base) + s_warp[warp] + (incl - n_won);
 #pragma unroll
     for (int u = 0; u < EM_IPT; ++u) {
-        if (won[u]) {
+        if (won >> u & 1u) {
             id[u] = next_id++;
             __stcg(reinterpret_cast<uint32_t *>(g.table + slot[u]) + 2, id[u]);   // publish
             g.pair[id[u]] = tgt_pair[u];
@@ -386,7 +467,7 @@ __global__ void __launch_bounds__(EM_THREADS) k_emit(EmitArgs g) {
     // ---- targets inserted concurrently by another thread: wait for their id to be published
 #pragma unroll
     for (int u = 0; u < EM_IPT; ++u) {
-        if (u >= skip && u < skip + n_valid && !won[u] && id[u] == PENDING_ID) {
+        if (u >= skip && u < skip + n_valid && !(won >> u & 1u) && id[u] == PENDING_ID) {
             const uint32_t *pid = reinterpret_cast<const uint32_t *>(g.table + slot[u]) + 2;
             uint32_t v;
             while ((v = __ldcg(pid)) == PENDING_ID) __nanosleep(20);
@@ -398,12 +479,12 @@ __global__ void __launch_bounds__(EM_THREADS) k_emit(EmitArgs g) {
     if (MODE == EMIT_DIRECT) {
         if (n_valid == EM_IPT) {                               // whole aligned group: 16-byte stores
             const int64_t q = my_pos;
-            *reinterpret_cast<int4 *>(g.o_src + q) = make_int4(static_cast<int>(g.f_lo + pl[0]), static_cast<int>(g.f_lo + pl[1]),
-                                                               static_cast<int>(g.f_lo + pl[2]), static_cast<int>(g.f_lo + pl[3]));
-            *reinterpret_cast<uint4 *>(g.o_il + q) = make_uint4(a_sym[0], a_sym[1], a_sym[2], a_sym[3]);
-            *reinterpret_cast<uint4 *>(g.o_ol + q) = make_uint4(b_sym[0], b_sym[1], b_sym[2], b_sym[3]);
-            *reinterpret_cast<uint4 *>(g.o_tgt + q) = make_uint4(id[0], id[1], id[2], id[3]);
-            *reinterpret_cast<float4 *>(g.o_w + q) = make_float4(w[0], w[1], w[2], w[3]);
+            __stcs(reinterpret_cast<int4 *>(g.o_src + q), make_int4(static_cast<int>(g.f_lo + pl[0]), static_cast<int>(g.f_lo + pl[1]),
+                                                                   static_cast<int>(g.f_lo + pl[2]), static_cast<int>(g.f_lo + pl[3])));
+            __stcs(reinterpret_cast<uint4 *>(g.o_il + q), make_uint4(a_sym[0], a_sym[1], a_sym[2], a_sym[3]));
+            __stcs(reinterpret_cast<uint4 *>(g.o_ol + q), make_uint4(b_sym[0], b_sym[1], b_sym[2], b_sym[3]));
+            __stcs(reinterpret_cast<uint4 *>(g.o_tgt + q), make_uint4(id[0], id[1], id[2], id[3]));
+            __stcs(reinterpret_cast<float4 *>(g.o_w + q), make_float4(w[0], w[1], w[2], w[3]));
         } else {
 #pragma unroll
             for (int u = 0; u < EM_IPT; ++u) {
@@ -514,38 +595,77 @@ __global__ void k_place_merged(const unsigned long long *__restrict__ mkey, cons
 }
 
 // ------------------------------------------------------------------------------------------ assembly
-__global__ void k_accept_flags(const int2 *__restrict__ pair, int64_t n, const uint32_t *__restrict__ acc1,
-                               const uint32_t *__restrict__ acc2, uint8_t *__restrict__ flag) {
-    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    int2 p = pair[i];
-    flag[i] = ((acc1[p.x >> 5] >> (p.x & 31)) & 1u) & ((acc2[p.y >> 5] >> (p.y & 31)) & 1u);
+// Accept list (ascending ids with q1 in F1 and q2 in F2) and expanded flags in two passes over the
+// pair table: pass 1 counts accepting states per 2048-state tile and writes `expanded`; after a scan of the tile
+// counts, pass 2 recomputes the flags and compacts each tile in order.
+constexpr int AS_THREADS = 256;
+constexpr int AS_ITEMS = 8;
+constexpr int AS_TILE = AS_THREADS * AS_ITEMS;
+
+__device__ __forceinline__ uint32_t is_accept(int2 p, const uint32_t *acc1, const uint32_t *acc2) {
+    return ((acc1[p.x >> 5] >> (p.x & 31)) & 1u) & ((acc2[p.y >> 5] >> (p.y & 31)) & 1u);
 }
 
-__global__ void k_accept_scatter(const uint8_t *__restrict__ flag, const int64_t *__restrict__ idx, int64_t n,
-                                 int32_t *__restrict__ out) {
-    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i < n && flag[i]) out[idx[i]] = static_cast<int32_t>(i);
-}
-
-// expanded[i] = 1 for every state before the last frontier [last_lo, last_hi); inside it, 1 iff it was
-// selected; states created while expanding a frontier that stopped the search are never expanded
-__global__ void k_expanded(const int2 *__restrict__ pair, int64_t n, int64_t last_lo, int64_t last_hi,
-                           int last_mode /*0 none,1 all,2 cut*/, uint64_t nq2, uint64_t cut,
-                           uint8_t *__restrict__ expanded) {
-    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    uint8_t e = 1;
-    if (i >= last_hi) e = 0;
-    else if (i >= last_lo) {
-        if (last_mode == 0) e = 0;
-        else if (last_mode == 2) {
-            int2 p = pair[i];
-            uint64_t key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
-            e = key < cut;
+// expanded[i] = 1 for every state before the last frontier [last_lo, last_hi); inside it, 1 iff it was selected;
+// states created while expanding the frontier that stopped the search are never expanded.
+__global__ void __launch_bounds__(AS_THREADS)
+k_assemble_count(const int2 *__restrict__ pair, int64_t n, const uint32_t *__restrict__ acc1,
+                 const uint32_t *__restrict__ acc2, int64_t last_lo, int64_t last_hi,
+                 int last_mode /*0 none, 1 all, 2 cut*/, uint64_t nq2, uint64_t cut, uint8_t *__restrict__ expanded,
+                 uint32_t *__restrict__ tile_count) {
+    __shared__ uint32_t s_cnt;
+    if (threadIdx.x == 0) s_cnt = 0;
+    __syncthreads();
+    const int64_t base = static_cast<int64_t>(blockIdx.x) * AS_TILE;
+    uint32_t cnt = 0;
+#pragma unroll
+    for (int r = 0; r < AS_ITEMS; ++r) {
+        const int64_t i = base + r * AS_THREADS + threadIdx.x;
+        if (i < n) {
+            const int2 p = pair[i];
+            cnt += is_accept(p, acc1, acc2);
+            uint8_t e = 1;
+            if (i >= last_hi) e = 0;
+            else if (i >= last_lo) {
+                if (last_mode == 0) e = 0;
+                else if (last_mode == 2)
+                    e = (static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y)) < cut;
+            }
+            expanded[i] = e;
         }
     }
-    expanded[i] = e;
+    cnt = __reduce_add_sync(0xffffffffu, cnt);
+    if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(&s_cnt, cnt);
+    __syncthreads();
+    if (threadIdx.x == 0) tile_count[blockIdx.x] = s_cnt;
+}
+
+__global__ void __launch_bounds__(AS_THREADS)
+k_assemble_scatter(const int2 *__restrict__ pair, int64_t n, const uint32_t *__restrict__ acc1,
+                   const uint32_t *__restrict__ acc2, const uint32_t *__restrict__ tile_count,
+                   const int64_t *__restrict__ tile_off, int32_t *__restrict__ out) {
+    if (tile_count[blockIdx.x] == 0) return;
+    __shared__ uint32_t s_warp[AS_THREADS / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t base = static_cast<int64_t>(blockIdx.x) * AS_TILE;
+    int64_t off = tile_off[blockIdx.x];
+    for (int r = 0; r < AS_ITEMS; ++r) {                      // rows of 256 consecutive states, in order
+        const int64_t i = base + r * AS_THREADS + threadIdx.x;
+        const uint32_t f = (i < n) ? is_accept(pair[i], acc1, acc2) : 0u;
+        const uint32_t b = __ballot_sync(0xffffffffu, f);
+        if (lane == 0) s_warp[warp] = __popc(b);
+        __syncthreads();
+        uint32_t before = 0, total = 0;
+#pragma unroll
+        for (int wv = 0; wv < AS_THREADS / 32; ++wv) {
+            const uint32_t c = s_warp[wv];
+            if (wv < warp) before += c;
+            total += c;
+        }
+        if (f) out[off + before + __popc(b & ((1u << lane) - 1u))] = static_cast<int32_t>(i);
+        off += total;
+        __syncthreads();
+    }
 }
 
 inline unsigned nblk(int64_t n, int threads = CT_THREADS) { return static_cast<unsigned>(ceil_div(n > 0 ? n : 1, threads)); }
@@ -599,51 +719,80 @@ struct Composer {
         std::memset(&st, 0, sizeof st);
     }
 
-    void ensure_pairs(int64_t need) {
+    // Growable outputs and table.  `need` is what the coming launch requires; `want` >= need is a look-ahead
+    // (next level's predicted size) so that big arrays are not reallocated + copied / rehashed level after level.
+    template <typename F>
+    void grow_to(int64_t need, int64_t want, F &&grow) {
+        if (want > need) {
+            try { grow(want); return; }
+            catch (const Error &e) { if (e.code != FSTC_ERR_OOM) throw; }
+        }
+        grow(need);
+    }
+
+    void ensure_pairs(int64_t need, int64_t want = 0) {
         if (need <= pair_cap) return;
-        int64_t nc = std::max<int64_t>(need, pair_cap * 2);
-        DBuf<int2> np(c, nc);
-        if (n_states > 0)
-            FSTC_CUDA(cudaMemcpyAsync(np.p, pair.p, sizeof(int2) * n_states, cudaMemcpyDeviceToDevice, c.stream));
-        pair = std::move(np);
-        pair_cap = nc;
+        grow_to(need, std::max(want, pair_cap * 2), [&](int64_t nc) {
+            DBuf<int2> np(c, nc);
+            if (n_states > 0)
+                FSTC_CUDA(cudaMemcpyAsync(np.p, pair.p, sizeof(int2) * n_states, cudaMemcpyDeviceToDevice, c.stream));
+            pair = std::move(np);
+            pair_cap = nc;
+        });
         if (n_states > 0) st.n_grow += 1;
     }
 
-    template <typename T>
-    void regrow(DBuf<T> &b, int64_t nc) {
-        DBuf<T> nb(c, nc);
-        if (n_arcs > 0) FSTC_CUDA(cudaMemcpyAsync(nb.p, b.p, sizeof(T) * n_arcs, cudaMemcpyDeviceToDevice, c.stream));
-        b = std::move(nb);
-    }
-    void ensure_arcs(int64_t need) {
+    void ensure_arcs(int64_t need, int64_t want = 0) {
         if (need <= arc_cap) return;
         int h = tm.begin(FSTC_T_ASSEMBLE);
-        int64_t nc = std::max<int64_t>(need, arc_cap + arc_cap / 2);
-        nc = (nc + 3) & ~int64_t(3);
-        regrow(a_src, nc); regrow(a_il, nc); regrow(a_ol, nc); regrow(a_tgt, nc); regrow(a_w, nc);
-        arc_cap = nc;
+        grow_to(need, std::max(want, arc_cap + arc_cap / 2), [&](int64_t nc) {
+            nc = (nc + 3) & ~int64_t(3);
+            DBuf<int32_t> n_src(c, nc), n_il(c, nc), n_ol(c, nc), n_tgt(c, nc);
+            DBuf<float> n_w(c, nc);
+            if (n_arcs > 0) {
+                const size_t b = sizeof(int32_t) * n_arcs;
+                FSTC_CUDA(cudaMemcpyAsync(n_src.p, a_src.p, b, cudaMemcpyDeviceToDevice, c.stream));
+                FSTC_CUDA(cudaMemcpyAsync(n_il.p, a_il.p, b, cudaMemcpyDeviceToDevice, c.stream));
+                FSTC_CUDA(cudaMemcpyAsync(n_ol.p, a_ol.p, b, cudaMemcpyDeviceToDevice, c.stream));
+                FSTC_CUDA(cudaMemcpyAsync(n_tgt.p, a_tgt.p, b, cudaMemcpyDeviceToDevice, c.stream));
+                FSTC_CUDA(cudaMemcpyAsync(n_w.p, a_w.p, b, cudaMemcpyDeviceToDevice, c.stream));
+            }
+            a_src = std::move(n_src); a_il = std::move(n_il); a_ol = std::move(n_ol); a_tgt = std::move(n_tgt);
+            a_w = std::move(n_w);
+            arc_cap = nc;
+        });
         if (n_arcs > 0) st.n_grow += 1;
         tm.end(h);
     }
 
-    // table able to hold `bound` states at load <= 0.6
-    void ensure_table(int64_t bound) {
-        uint64_t need = static_cast<uint64_t>(bound + bound / 2 + bound / 6) + 64;   // bound / 0.6
+    static uint64_t slots_for(int64_t states) { return static_cast<uint64_t>(states) * 100 / FSTC_TABLE_LOAD_PCT + 64; }
+
+    // table able to hold `bound` states at load <= FSTC_TABLE_LOAD_PCT %
+    void ensure_table(int64_t bound, int64_t want_states = 0) {
+        const uint64_t need = slots_for(bound);
         if (need <= cap) return;
         int h = tm.begin(FSTC_T_TABLE);
-        uint64_t nc = std::max<uint64_t>(need, 4096);
-        DBuf<uint4> nt(c, static_cast<int64_t>(nc));
-        FSTC_CUDA(cudaMemsetAsync(nt.p, 0xFF, sizeof(uint4) * nc, c.stream));
-        if (n_states > 0) {
-            tb_insert_ids<<<nblk(n_states), CT_THREADS, 0, c.stream>>>(pair.p, n_states, nq2, nt.p, nc);
-            FSTC_LAUNCH_CHECK();
-            c.n_launch += 1;
+        grow_to(static_cast<int64_t>(need), static_cast<int64_t>(slots_for(std::max(bound, want_states))), [&](int64_t slots) {
+            uint64_t nc = (std::max<uint64_t>(static_cast<uint64_t>(slots), 4096) + 1) & ~uint64_t(1);   // whole buckets
+            DBuf<uint4> nt(c, static_cast<int64_t>(nc));
+            FSTC_CUDA(cudaMemsetAsync(nt.p, 0xFF, sizeof(uint4) * nc, c.stream));
+            if (n_states > 0) {
+                tb_insert_ids<<<nblk(n_states), CT_THREADS, 0, c.stream>>>(pair.p, n_states, nq2, nt.p, nc);
+                FSTC_LAUNCH_CHECK();
+                c.n_launch += 1;
+            }
+            table = std::move(nt);
             if (cap) st.n_rehash += 1;
-        }
-        table = std::move(nt);
-        cap = nc;
+            cap = nc;
+        });
         tm.end(h);
+    }
+
+    // several device scalars, one synchronisation
+    void read_scalars(std::initializer_list<std::pair<const int64_t *, int64_t *>> items) {
+        for (auto &it : items)
+            FSTC_CUDA(cudaMemcpyAsync(it.second, it.first, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
+        c.sync();
     }
 
     void launch_emit(int mode, const MatchList &L, int64_t n_matches, int64_t R, int64_t pos_base, int64_t f_lo,
@@ -684,6 +833,9 @@ fstc_result_t *Composer::run() {
     const uint64_t n_pairs_total = static_cast<uint64_t>(m1.n_states) * nq2;
     const int key_bits = bits_for(n_pairs_total - 1);
 
+    if (const char *e = getenv("FSTC_L2_FETCH")) {            // experiment knob: 32 / 64 / 128
+        (void)cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, static_cast<size_t>(atoi(e)));
+    }
     cudaEvent_t ev0, ev1;
     FSTC_CUDA(cudaEventCreate(&ev0));
     FSTC_CUDA(cudaEventCreate(&ev1));
@@ -708,6 +860,7 @@ fstc_result_t *Composer::run() {
     int last_mode = 1;           // how the last frontier [f_lo, f_hi) was treated: 0 not expanded, 1 all, 2 cut
     uint64_t cut_key = 0;
     int64_t last_lo = 0, last_hi = 1;
+    double last_fan = 0.0;      // raw arcs per expanded pair of the previous level
     int lvl = 0;
     MachineView A = view_of(m1), B = view_of(m2);
 
@@ -721,18 +874,37 @@ fstc_result_t *Composer::run() {
         // ---- count
         DBuf<int64_t> rawU(c, nf), rawF(c, nf);
         DBuf<uint32_t> nmU(c, nf), nmF(c, nf);
-        int h = tm.begin(FSTC_T_COUNT);
-        k_count<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, o.merge_mode, rawU.p, rawF.p, nmU.p, nmF.p);
-        FSTC_LAUNCH_CHECK();
-        c.n_launch += 1;
-        tm.end(h);
-
-        // ---- scan + budget
-        h = tm.begin(FSTC_T_SCAN);
         DBuf<int64_t> roffU(c, nf + 1), roffF(c, nf + 1), moffU(c, nf + 1), moffF(c, nf + 1);
-        exclusive_scan<int64_t>(c, rawU.p, nf, roffU.p);
-        exclusive_scan<int64_t>(c, rawF.p, nf, roffF.p);
-        int64_t RU = read_scalar(c, roffU.p + nf), RF = read_scalar(c, roffF.p + nf);
+        int64_t RU = 0, RF = 0, MU = 0, MF = 0;
+        // A level that will clearly be cut by the budget (predicted from the previous level's fan-out) is counted
+        // only below a key limit: rule T expands a key-ordered prefix, so pairs far above the cut never matter.
+        // Exact: if the counted part does not exceed the budget the limit is raised and the level counted again.
+        uint64_t key_limit = ~0ull;
+        if (o.max_raw_arcs > 0 && nf > 100000 && last_fan > 0) {
+            const double remaining = static_cast<double>(o.max_raw_arcs - cum_raw);
+            const double predicted = static_cast<double>(nf) * last_fan;
+            if (predicted > 4.0 * remaining)
+                key_limit = static_cast<uint64_t>(static_cast<double>(n_pairs_total) * (2.0 * remaining / predicted)) + 1;
+        }
+        int h;
+        while (true) {
+            h = tm.begin(FSTC_T_COUNT);
+            k_count<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, o.merge_mode, nq2, key_limit, rawU.p, rawF.p,
+                                                           nmU.p, nmF.p);
+            FSTC_LAUNCH_CHECK();
+            c.n_launch += 1;
+            tm.end(h);
+            // ---- scan + budget
+            h = tm.begin(FSTC_T_SCAN);
+            exclusive_scan<int64_t>(c, rawU.p, nf, roffU.p);
+            exclusive_scan<int64_t>(c, rawF.p, nf, roffF.p);
+            exclusive_scan<uint32_t>(c, nmU.p, nf, moffU.p);
+            exclusive_scan<uint32_t>(c, nmF.p, nf, moffF.p);
+            read_scalars({{roffU.p + nf, &RU}, {roffF.p + nf, &RF}, {moffU.p + nf, &MU}, {moffF.p + nf, &MF}});
+            if (key_limit >= n_pairs_total || cum_raw + RU + RF > o.max_raw_arcs) break;
+            tm.end(h);
+            key_limit = key_limit > n_pairs_total / 4 ? ~0ull : key_limit * 4;     // the cut lies higher: widen
+        }
         bool stop_after = false;
         int64_t n_sel = nf;
         if (o.max_raw_arcs > 0 && cum_raw + RU + RF > o.max_raw_arcs) {
@@ -742,7 +914,7 @@ fstc_result_t *Composer::run() {
             const int top = ((key_bits + 7) / 8) * 8;
             for (int shift = top - 8; shift >= 0; shift -= 8) {
                 FSTC_CUDA(cudaMemsetAsync(d_counters.p + 4, 0, sizeof(unsigned long long) * 256, c.stream));
-                k_cut_hist<<<nblk(nf), CT_THREADS, 0, c.stream>>>(pair.p, f_lo, nf, nq2, rawU.p, rawF.p, prefix, shift,
+                k_cut_hist<<<std::min<unsigned>(nblk(nf), 8u * c.n_sm), CT_THREADS, 0, c.stream>>>(pair.p, f_lo, nf, nq2, rawU.p, rawF.p, prefix, shift,
                                                                   d_counters.p + 4);
                 FSTC_LAUNCH_CHECK();
                 c.n_launch += 1;
@@ -765,16 +937,14 @@ fstc_result_t *Composer::run() {
             c.n_launch += 1;
             exclusive_scan<int64_t>(c, rawU.p, nf, roffU.p);
             exclusive_scan<int64_t>(c, rawF.p, nf, roffF.p);
-            RU = read_scalar(c, roffU.p + nf);
-            RF = read_scalar(c, roffF.p + nf);
-            n_sel = static_cast<int64_t>(read_scalar(c, d_counters.p + 3));
+            exclusive_scan<uint32_t>(c, nmU.p, nf, moffU.p);
+            exclusive_scan<uint32_t>(c, nmF.p, nf, moffF.p);
+            read_scalars({{roffU.p + nf, &RU}, {roffF.p + nf, &RF}, {moffU.p + nf, &MU}, {moffF.p + nf, &MF},
+                          {reinterpret_cast<const int64_t *>(d_counters.p + 3), &n_sel}});
             st.truncated = 1;
             stop_after = true;
             last_mode = 2;
         }
-        exclusive_scan<uint32_t>(c, nmU.p, nf, moffU.p);
-        exclusive_scan<uint32_t>(c, nmF.p, nf, moffF.p);
-        const int64_t MU = read_scalar(c, moffU.p + nf), MF = read_scalar(c, moffF.p + nf);
         tm.end(h);
 
         const int64_t R = RU + RF;
@@ -782,9 +952,31 @@ fstc_result_t *Composer::run() {
         const uint64_t remaining_pairs = n_pairs_total - static_cast<uint64_t>(n_states);
         const int64_t new_bound = static_cast<int64_t>(std::min<uint64_t>(static_cast<uint64_t>(R), remaining_pairs));
         if (n_states + new_bound >= 0x7FFFFFFFll) fail(FSTC_ERR_CAPACITY, "more than 2^31-1 states");
-        ensure_pairs(n_states + new_bound);
-        ensure_table(n_states + new_bound);
-        ensure_arcs(n_arcs + R);
+        // look-ahead: if the search goes on, the next level is about (new states) x (arcs per expanded pair)
+        int64_t next_R = 0, next_S = 0;
+        const bool must_grow = n_states + new_bound > pair_cap || slots_for(n_states + new_bound) > cap || n_arcs + R > arc_cap;
+        if (must_grow && !stop_after && n_sel > 0 && R > 0) {
+            const double fan = static_cast<double>(R) / static_cast<double>(n_sel);
+            double pr = static_cast<double>(new_bound) * fan;
+            if (o.max_raw_arcs > 0) pr = std::min(pr, static_cast<double>(o.max_raw_arcs - cum_raw - R));
+            size_t free_b = 0, total_b = 0;
+            (void)cudaMemGetInfo(&free_b, &total_b);
+            uint64_t pool_reserved = 0, pool_used = 0;           // cached blocks of our pool are available to us
+            (void)cudaMemPoolGetAttribute(device_pool(), cudaMemPoolAttrReservedMemCurrent, &pool_reserved);
+            (void)cudaMemPoolGetAttribute(device_pool(), cudaMemPoolAttrUsedMemCurrent, &pool_used);
+            if (pool_reserved > pool_used) free_b += pool_reserved - pool_used;
+            pr = std::min(pr, 16.0 * static_cast<double>(n_arcs + R));           // never more than 16x what is needed now
+            const double ps = std::min(pr, static_cast<double>(remaining_pairs - static_cast<uint64_t>(new_bound)));
+            // 20 B per arc; per state 8 B + a table slot at the target load; at most 40 % of what is free
+            const double bytes = 20.0 * pr + (8.0 + 1600.0 / FSTC_TABLE_LOAD_PCT) * ps;
+            const double scale = std::min(1.0, 0.4 * static_cast<double>(free_b) / std::max(bytes, 1.0));
+            next_R = pr > 0 ? static_cast<int64_t>(pr * scale) : 0;
+            next_S = ps > 0 ? static_cast<int64_t>(ps * scale) : 0;
+            if (n_states + new_bound + next_S >= 0x7FFFFFFFll) next_S = 0;
+        }
+        ensure_pairs(n_states + new_bound, n_states + new_bound + next_S);
+        ensure_table(n_states + new_bound, n_states + new_bound + next_S);
+        ensure_arcs(n_arcs + R, n_arcs + R + next_R);
 
         // ---- match work-lists
         MatchList LU{nullptr, nullptr, nullptr}, LF{nullptr, nullptr, nullptr};
@@ -861,6 +1053,7 @@ fstc_result_t *Composer::run() {
         }
         st.n_matches += MU + MF;
         st.n_expanded += n_sel;
+        last_fan = n_sel > 0 ? static_cast<double>(R) / static_cast<double>(n_sel) : 0.0;
         cum_raw += R;
         n_states = ns_after;
         f_lo = f_hi;
@@ -871,19 +1064,22 @@ fstc_result_t *Composer::run() {
 
     // ---- assemble
     int h = tm.begin(FSTC_T_ASSEMBLE);
-    DBuf<uint8_t> accf(c, n_states), expanded(c, n_states);
-    DBuf<int64_t> accidx(c, n_states + 1);
-    k_accept_flags<<<nblk(n_states), CT_THREADS, 0, c.stream>>>(pair.p, n_states, m1.accept_bits, m2.accept_bits, accf.p);
+    DBuf<uint8_t> expanded(c, n_states);
+    const int64_t as_tiles = ceil_div(n_states, AS_TILE);
+    DBuf<uint32_t> tile_count(c, as_tiles);
+    DBuf<int64_t> tile_off(c, as_tiles + 1);
+    k_assemble_count<<<static_cast<unsigned>(as_tiles), AS_THREADS, 0, c.stream>>>(
+        pair.p, n_states, m1.accept_bits, m2.accept_bits, last_lo, last_hi, last_mode, nq2, cut_key, expanded.p, tile_count.p);
     FSTC_LAUNCH_CHECK();
-    exclusive_scan<uint8_t>(c, accf.p, n_states, accidx.p);
-    const int64_t n_accept = read_scalar(c, accidx.p + n_states);
+    exclusive_scan<uint32_t>(c, tile_count.p, as_tiles, tile_off.p);
+    const int64_t n_accept = read_scalar(c, tile_off.p + as_tiles);
     DBuf<int32_t> accept(c, n_accept);
-    k_accept_scatter<<<nblk(n_states), CT_THREADS, 0, c.stream>>>(accf.p, accidx.p, n_states, accept.p);
-    FSTC_LAUNCH_CHECK();
-    k_expanded<<<nblk(n_states), CT_THREADS, 0, c.stream>>>(pair.p, n_states, last_lo, last_hi, last_mode, nq2, cut_key,
-                                                          expanded.p);
-    FSTC_LAUNCH_CHECK();
-    c.n_launch += 3;
+    if (n_accept > 0) {
+        k_assemble_scatter<<<static_cast<unsigned>(as_tiles), AS_THREADS, 0, c.stream>>>(
+            pair.p, n_states, m1.accept_bits, m2.accept_bits, tile_count.p, tile_off.p, accept.p);
+        FSTC_LAUNCH_CHECK();
+    }
+    c.n_launch += 2;
     tm.end(h);
 
     unsigned long long cnt[3];

@@ -15,7 +15,7 @@ from typing import Optional
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libfstc.so")
+LIB_PATH = os.environ.get("FSTC_LIB") or os.path.join(_HERE, "libfstc.so")   # FSTC_LIB: an experiment build
 
 FSTC_MEM_DEVICE, FSTC_MEM_HOST = 0, 1
 MERGE_AUTO, MERGE_OFF, MERGE_SORT_ALL = 0, 1, 2
