@@ -131,8 +131,8 @@ k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_l
             uint8_t fa = A.flags[p.x], fb = B.flags[p.y];
             f = ((fa & FLAG_D) && (fb & FLAG_D)) || (fa & FLAG_X) || (fb & FLAG_X);
         }
-        rawU[i] = f ? 0 : raw; rawF[i] = f ? raw : 0;
-        nmU[i] = f ? 0 : nm;   nmF[i] = f ? nm : 0;
+        rawU[i] = f ? 0 : raw; nmU[i] = f ? 0 : nm;
+        if (rawF) { rawF[i] = f ? raw : 0; nmF[i] = f ? nm : 0; }    // null when no pair of this run can be class F
     }
 }
 
@@ -156,7 +156,7 @@ k_cut_hist(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, uint64_t nq2
             int2 p = pair[f_lo + i];
             uint64_t key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
             uint64_t hi = (shift + 8 >= 64) ? 0 : (key >> (shift + 8));
-            r = static_cast<uint64_t>(rawU[i] + rawF[i]);
+            r = static_cast<uint64_t>(rawU[i] + (rawF ? rawF[i] : 0));
             if (hi == prefix && r > 0) digit = static_cast<uint32_t>(key >> shift) & 255u;
         }
         const uint32_t peers = __match_any_sync(0xffffffffu, digit);
@@ -181,7 +181,10 @@ __global__ void k_apply_cut(const int2 *__restrict__ pair, int64_t f_lo, int64_t
         int2 p = pair[f_lo + i];
         uint64_t key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
         sel = key < cut;
-        if (!sel) { rawU[i] = 0; rawF[i] = 0; nmU[i] = 0; nmF[i] = 0; }
+        if (!sel) {
+            rawU[i] = 0; nmU[i] = 0;
+            if (rawF) { rawF[i] = 0; nmF[i] = 0; }
+        }
     }
     unsigned b = __ballot_sync(0xffffffffu, sel);
     if ((threadIdx.x & 31) == 0 && b) atomicAdd(n_selected, static_cast<unsigned long long>(__popc(b)));
@@ -201,7 +204,7 @@ k_match(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_l
         unsigned long long *__restrict__ counters /* [0] Σ segments visited, [1] Σ (n1+n2) over matches */) {
     int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     unsigned long long segs = 0, marcs = 0;
-    const bool isF = i < nf && nmF[i] != 0;
+    const bool isF = i < nf && nmF && nmF[i] != 0;
     if (i < nf && (isF || nmU[i] != 0)) {
         int2 p = pair[f_lo + i];
         MatchList L = isF ? F : U;
@@ -831,6 +834,10 @@ fstc_result_t *Composer::run() {
     const int bits_a = bits_for(m1.n_outer > 0 ? m1.n_outer - 1 : 0), bits_b = bits_for(m2.n_outer > 0 ? m2.n_outer - 1 : 0);
     const int shift_t = bits_a + bits_b;
     const uint64_t n_pairs_total = static_cast<uint64_t>(m1.n_states) * nq2;
+    // can any pair of this run hold duplicate arcs (N10)?  if not, the whole class-F machinery is skipped
+    const bool has_F = o.merge_mode == FSTC_MERGE_SORT_ALL ||
+                       (o.merge_mode == FSTC_MERGE_AUTO &&
+                        (((m1.any_flags & FLAG_D) && (m2.any_flags & FLAG_D)) || (m1.any_flags & FLAG_X) || (m2.any_flags & FLAG_X)));
     const int key_bits = bits_for(n_pairs_total - 1);
 
     if (const char *e = getenv("FSTC_L2_FETCH")) {            // experiment knob: 32 / 64 / 128
@@ -872,10 +879,24 @@ fstc_result_t *Composer::run() {
         last_mode = 1;
 
         // ---- count
-        DBuf<int64_t> rawU(c, nf), rawF(c, nf);
-        DBuf<uint32_t> nmU(c, nf), nmF(c, nf);
-        DBuf<int64_t> roffU(c, nf + 1), roffF(c, nf + 1), moffU(c, nf + 1), moffF(c, nf + 1);
         int64_t RU = 0, RF = 0, MU = 0, MF = 0;
+        DBuf<int64_t> rawU(c, nf), rawF;
+        DBuf<uint32_t> nmU(c, nf), nmF;
+        DBuf<int64_t> roffU(c, nf + 1), roffF, moffU(c, nf + 1), moffF;
+        if (has_F) { rawF.alloc(c, nf); nmF.alloc(c, nf); roffF.alloc(c, nf + 1); moffF.alloc(c, nf + 1); }
+        auto scan_level = [&](int64_t *n_sel_out) {             // offsets + totals of the level, one synchronisation
+            exclusive_scan2(c, rawU.p, nmU.p, nf, roffU.p, moffU.p);
+            if (has_F) exclusive_scan2(c, rawF.p, nmF.p, nf, roffF.p, moffF.p);
+            RF = 0; MF = 0;
+            if (has_F && n_sel_out)
+                read_scalars({{roffU.p + nf, &RU}, {moffU.p + nf, &MU}, {roffF.p + nf, &RF}, {moffF.p + nf, &MF},
+                              {reinterpret_cast<const int64_t *>(d_counters.p + 3), n_sel_out}});
+            else if (has_F) read_scalars({{roffU.p + nf, &RU}, {moffU.p + nf, &MU}, {roffF.p + nf, &RF}, {moffF.p + nf, &MF}});
+            else if (n_sel_out)
+                read_scalars({{roffU.p + nf, &RU}, {moffU.p + nf, &MU},
+                              {reinterpret_cast<const int64_t *>(d_counters.p + 3), n_sel_out}});
+            else read_scalars({{roffU.p + nf, &RU}, {moffU.p + nf, &MU}});
+        };
         // A level that will clearly be cut by the budget (predicted from the previous level's fan-out) is counted
         // only below a key limit: rule T expands a key-ordered prefix, so pairs far above the cut never matter.
         // Exact: if the counted part does not exceed the budget the limit is raised and the level counted again.
@@ -896,11 +917,7 @@ fstc_result_t *Composer::run() {
             tm.end(h);
             // ---- scan + budget
             h = tm.begin(FSTC_T_SCAN);
-            exclusive_scan<int64_t>(c, rawU.p, nf, roffU.p);
-            exclusive_scan<int64_t>(c, rawF.p, nf, roffF.p);
-            exclusive_scan<uint32_t>(c, nmU.p, nf, moffU.p);
-            exclusive_scan<uint32_t>(c, nmF.p, nf, moffF.p);
-            read_scalars({{roffU.p + nf, &RU}, {roffF.p + nf, &RF}, {moffU.p + nf, &MU}, {moffF.p + nf, &MF}});
+            scan_level(nullptr);
             if (key_limit >= n_pairs_total || cum_raw + RU + RF > o.max_raw_arcs) break;
             tm.end(h);
             key_limit = key_limit > n_pairs_total / 4 ? ~0ull : key_limit * 4;     // the cut lies higher: widen
@@ -935,12 +952,7 @@ fstc_result_t *Composer::run() {
                                                                d_counters.p + 3);
             FSTC_LAUNCH_CHECK();
             c.n_launch += 1;
-            exclusive_scan<int64_t>(c, rawU.p, nf, roffU.p);
-            exclusive_scan<int64_t>(c, rawF.p, nf, roffF.p);
-            exclusive_scan<uint32_t>(c, nmU.p, nf, moffU.p);
-            exclusive_scan<uint32_t>(c, nmF.p, nf, moffF.p);
-            read_scalars({{roffU.p + nf, &RU}, {roffF.p + nf, &RF}, {moffU.p + nf, &MU}, {moffF.p + nf, &MF},
-                          {reinterpret_cast<const int64_t *>(d_counters.p + 3), &n_sel}});
+            scan_level(&n_sel);
             st.truncated = 1;
             stop_after = true;
             last_mode = 2;

@@ -39,6 +39,7 @@ struct fstc_packed_t {
     uint32_t *accept_bits = nullptr;  // [(n_states+31)/32]
     int device = 0;
     int64_t n_launch = 0;         // kernel launches fstc_pack took
+    uint8_t any_flags = 0;        // OR of flags[] over all states
 };
 
 namespace fstc {

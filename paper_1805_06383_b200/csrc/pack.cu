@@ -126,9 +126,12 @@ __global__ void pk_accept_bits(const int32_t *__restrict__ accept, int32_t n_acc
     if (i < n_accept) atomicOr(&bits[accept[i] >> 5], 1u << (accept[i] & 31));
 }
 
-__global__ void pk_narrow_flags(const uint32_t *__restrict__ f32, int32_t n, uint8_t *__restrict__ f8) {
+__global__ void pk_narrow_flags(const uint32_t *__restrict__ f32, int32_t n, uint8_t *__restrict__ f8, int *__restrict__ any) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) f8[i] = static_cast<uint8_t>(f32[i]);
+    uint32_t f = (i < n) ? f32[i] : 0u;
+    if (i < n) f8[i] = static_cast<uint8_t>(f);
+    f = __reduce_or_sync(0xffffffffu, f);
+    if ((threadIdx.x & 31) == 0 && f) atomicOr(any, static_cast<int>(f));
 }
 
 inline unsigned blocks_for(int64_t n) { return static_cast<unsigned>(ceil_div(n > 0 ? n : 1, PK_THREADS)); }
@@ -239,16 +242,17 @@ fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side) {
         FSTC_CUDA(cudaMemsetAsync(seg_ptr.p, 0, sizeof(uint32_t) * (static_cast<size_t>(m.n_states) + 1), c.stream));
         c.sync();
     }
-    pk_narrow_flags<<<blocks_for(m.n_states), PK_THREADS, 0, c.stream>>>(flags32.p, m.n_states, flags.p);
+    pk_narrow_flags<<<blocks_for(m.n_states), PK_THREADS, 0, c.stream>>>(flags32.p, m.n_states, flags.p, bad.p);
     FSTC_LAUNCH_CHECK();
     if (m.n_accept > 0) {
         pk_accept_bits<<<blocks_for(m.n_accept), PK_THREADS, 0, c.stream>>>(f.accept, m.n_accept, accept_bits.p);
         FSTC_LAUNCH_CHECK();
     }
     c.n_launch += 2;
-    c.sync();
+    const int any_flags = read_scalar(c, bad.p);      // `bad` was zero after validation; reused as the OR of all flags
 
     fstc_packed_t *p = new fstc_packed_t();
+    p->any_flags = static_cast<uint8_t>(any_flags);
     p->side = side;
     p->n_states = m.n_states; p->n_inner = n_inner; p->n_outer = n_outer; p->start = m.start;
     p->n_arcs = n; p->n_segs = n_segs;

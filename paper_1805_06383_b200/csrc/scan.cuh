@@ -105,4 +105,86 @@ void exclusive_scan(Ctx &c, const InT *in, int64_t n, int64_t *out) {
     c.n_launch += 2;
 }
 
+// Fused scan of two arrays of equal length (a: int64, b: uint32) in one pass over each: used once per BFS level for
+// (raw arc counts, match counts).  outA / outB have n+1 entries each.
+static __global__ void __launch_bounds__(SCAN_THREADS) scan2_tile_sums(const int64_t *__restrict__ a, const uint32_t *__restrict__ b,
+                                                                 int64_t n, int64_t *__restrict__ sumsA,
+                                                                 int64_t *__restrict__ sumsB) {
+    __shared__ int64_t wa[SCAN_THREADS / 32], wb[SCAN_THREADS / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t base = static_cast<int64_t>(blockIdx.x) * SCAN_TILE + warp * (32 * SCAN_ITEMS);
+    int64_t sa = 0, sb = 0;
+#pragma unroll
+    for (int r = 0; r < SCAN_ITEMS; ++r) {
+        int64_t i = base + r * 32 + lane;
+        if (i < n) { sa += a[i]; sb += b[i]; }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        sa += __shfl_xor_sync(0xffffffffu, sa, d);
+        sb += __shfl_xor_sync(0xffffffffu, sb, d);
+    }
+    if (lane == 0) { wa[warp] = sa; wb[warp] = sb; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int64_t ta = 0, tb = 0;
+#pragma unroll
+        for (int w = 0; w < SCAN_THREADS / 32; ++w) { ta += wa[w]; tb += wb[w]; }
+        sumsA[blockIdx.x] = ta; sumsB[blockIdx.x] = tb;
+    }
+}
+
+static __global__ void __launch_bounds__(SCAN_THREADS) scan2_tile_down(const int64_t *__restrict__ a, const uint32_t *__restrict__ b,
+                                                                 int64_t n, const int64_t *__restrict__ offA,
+                                                                 const int64_t *__restrict__ offB, int64_t *__restrict__ outA,
+                                                                 int64_t *__restrict__ outB) {
+    __shared__ int64_t wa[SCAN_THREADS / 32], wb[SCAN_THREADS / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t base = static_cast<int64_t>(blockIdx.x) * SCAN_TILE + warp * (32 * SCAN_ITEMS);
+    int64_t ea[SCAN_ITEMS], eb[SCAN_ITEMS];
+    int64_t ca = 0, cb = 0;
+#pragma unroll
+    for (int r = 0; r < SCAN_ITEMS; ++r) {
+        int64_t i = base + r * 32 + lane;
+        int64_t xa = (i < n) ? a[i] : 0, xb = (i < n) ? static_cast<int64_t>(b[i]) : 0;
+        int64_t ia = warp_incl_scan(xa, lane), ib = warp_incl_scan(xb, lane);
+        ea[r] = ca + ia - xa; eb[r] = cb + ib - xb;
+        ca += __shfl_sync(0xffffffffu, ia, 31);
+        cb += __shfl_sync(0xffffffffu, ib, 31);
+    }
+    if (lane == 0) { wa[warp] = ca; wb[warp] = cb; }
+    __syncthreads();
+    int64_t oa = offA ? offA[blockIdx.x] : 0, ob = offB ? offB[blockIdx.x] : 0;
+    for (int w = 0; w < warp; ++w) { oa += wa[w]; ob += wb[w]; }
+#pragma unroll
+    for (int r = 0; r < SCAN_ITEMS; ++r) {
+        int64_t i = base + r * 32 + lane;
+        if (i < n) { outA[i] = oa + ea[r]; outB[i] = ob + eb[r]; }
+    }
+    if (blockIdx.x == gridDim.x - 1 && threadIdx.x == SCAN_THREADS - 1) { outA[n] = oa + ca; outB[n] = ob + cb; }
+}
+
+inline void exclusive_scan2(Ctx &c, const int64_t *a, const uint32_t *b, int64_t n, int64_t *outA, int64_t *outB) {
+    if (n <= 0) {
+        FSTC_CUDA(cudaMemsetAsync(outA, 0, sizeof(int64_t), c.stream));
+        FSTC_CUDA(cudaMemsetAsync(outB, 0, sizeof(int64_t), c.stream));
+        return;
+    }
+    const int64_t tiles = ceil_div(n, SCAN_TILE);
+    if (tiles == 1) {
+        scan2_tile_down<<<1, SCAN_THREADS, 0, c.stream>>>(a, b, n, nullptr, nullptr, outA, outB);
+        FSTC_LAUNCH_CHECK();
+        c.n_launch += 1;
+        return;
+    }
+    DBuf<int64_t> sa(c, tiles + 1), sb(c, tiles + 1);
+    scan2_tile_sums<<<static_cast<unsigned>(tiles), SCAN_THREADS, 0, c.stream>>>(a, b, n, sa.p, sb.p);
+    FSTC_LAUNCH_CHECK();
+    exclusive_scan<int64_t>(c, sa.p, tiles, sa.p);
+    exclusive_scan<int64_t>(c, sb.p, tiles, sb.p);
+    scan2_tile_down<<<static_cast<unsigned>(tiles), SCAN_THREADS, 0, c.stream>>>(a, b, n, sa.p, sb.p, outA, outB);
+    FSTC_LAUNCH_CHECK();
+    c.n_launch += 2;
+}
+
 }  // namespace fstc
