@@ -174,6 +174,7 @@ def main():
     ap.add_argument("--workload", default="large", choices=sorted(WORKLOAD_DESC))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--merge-mode", type=int, default=0)
+    ap.add_argument("--resolve-mode", type=int, default=0, help="0 auto, 1 visited table only, 2 partitioned resolve only")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -219,6 +220,7 @@ def main():
         p2 = fstc.fstc_pack(d2, 2)
         e1.record()
         r = fstc.fstc_compose_packed(p1, p2, merge_mode=args.merge_mode, max_raw_arcs=budget, profile=profile,
+                                     resolve_mode=args.resolve_mode,
                                      arc_capacity_hint=hints["arc"], state_capacity_hint=hints["state"])
         e2.record()
         torch.cuda.synchronize()
@@ -271,7 +273,7 @@ def main():
         "warmup": max(args.warmup, 3), "ms_per_step": t_ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": WORKLOAD_DESC[args.workload], "name": args.workload, "seeds": [s1, s2],
-                   "max_raw_arcs": budget, "merge_mode": args.merge_mode, "parallelism": f"replicas x{world}",
+                   "max_raw_arcs": budget, "merge_mode": args.merge_mode, "resolve_mode": args.resolve_mode, "parallelism": f"replicas x{world}",
                    "cache": "L2 flushed (256 MiB write) before every step; working set >> L2"},
         "result": {"n_states": st["n_states"], "n_arcs": st["n_arcs"], "n_raw_arcs": st["n_raw_arcs"],
                    "n_levels": st["n_levels"], "truncated": st["truncated"], "n_expanded": st["n_expanded"],
@@ -318,6 +320,7 @@ def main():
             barrier()
             a.record()
             r = fstc.fstc_compose(hs[0], hs[1], merge_mode=args.merge_mode, max_raw_arcs=budget,
+                                  resolve_mode=args.resolve_mode,
                                   arc_capacity_hint=hints["arc"], state_capacity_hint=hints["state"])
             r.to_host(out)
             b.record()

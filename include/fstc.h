@@ -89,6 +89,12 @@ enum {
   FSTC_MERGE_SORT_ALL = 2   /* every source goes through sort + reduce: arcs sorted by (src,tgt,a,b) */
 };
 
+enum {
+  FSTC_RESOLVE_AUTO = 0,        /* per level: the table while it fits the L2 cache, else the partitioned resolve */
+  FSTC_RESOLVE_TABLE = 1,       /* always the open-addressing visited table (atomicCAS per arc, :237 adapted)  */
+  FSTC_RESOLVE_PARTITIONED = 2  /* always the streaming hash-partitioned resolve         */
+};
+
 /* Options; NULL or all-zero = defaults. */
 typedef struct fstc_opts_t {
   int32_t merge_mode;       /* FSTC_MERGE_*                                                           */
@@ -97,7 +103,7 @@ typedef struct fstc_opts_t {
   int64_t arc_capacity_hint;   /* expected number of output arcs (0 = none): avoids regrowing        */
   int64_t state_capacity_hint; /* expected number of output states (0 = none)                        */
   int32_t profile;          /* 1: time every stage with CUDA events on the stream (fills stats ms)    */
-  int32_t reserved;
+  int32_t resolve_mode;     /* FSTC_RESOLVE_*: how composed arcs find the ids of their target states          */
 } fstc_opts_t;
 
 /* Rule T (the paper only notes that the result may not fit the device, :153).  BFS levels are
@@ -131,6 +137,8 @@ typedef struct fstc_stats_t {
   int64_t table_capacity;   /* final number of visited-table slots                                    */
   int32_t n_rehash, n_grow; /* table rebuilds, output regrow copies                                   */
   int32_t n_emit_launches, n_kernel_launches;
+  int32_t n_resolve, pad_;  /* emit launches whose target ids came from the partitioned resolve                */
+  int64_t n_resolved_arcs;  /* raw arcs of those launches                                                     */
   double ms[FSTC_T_NSTAGES];/* device time per stage (CUDA events), only when opts.profile = 1       */
   double ms_total;          /* device time of the whole call (CUDA events), always                    */
   int64_t level_frontier[FSTC_MAX_LEVEL_STATS];  /* |F_l|                                             */

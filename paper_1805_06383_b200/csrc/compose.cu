@@ -264,6 +264,11 @@ __device__ __forceinline__ uint4 ld_keep(const uint4 *ptr, uint64_t policy) {
 #ifndef FSTC_TABLE_LOAD_PCT
 #define FSTC_TABLE_LOAD_PCT 40
 #endif
+#ifndef FSTC_RESOLVE_MIN_ARCS
+#define FSTC_RESOLVE_MIN_ARCS (int64_t(1) << 24)
+#endif
+constexpr int64_t RESOLVE_MIN_ARCS = FSTC_RESOLVE_MIN_ARCS;          // smaller levels always use the table
+constexpr uint64_t RESOLVE_TABLE_BYTES = 96ull << 20;               // a table beyond this no longer lives in L2
 constexpr int EM_THREADS = FSTC_EM_THREADS;
 constexpr int EM_IPT = 4;                          // consecutive output ranks per thread
 constexpr int EM_TILE = EM_THREADS * EM_IPT;       // 512 arcs per block
@@ -290,6 +295,8 @@ struct EmitArgs {
     uint4 *sortrec;          // SORTREC: {key lo, key hi, pair index, weight}, key = tgt id << shift_t | a << bits_b | b
     int shift_t, bits_b;
     const int64_t *tile_m;   // [n_tiles+1] match index holding the first rank of every tile
+    unsigned long long *keypos;   // KEYS: [R] target key << pos_bits | output position, for the partitioned resolve
+    int pos_bits;
 };
 
 // tile_m[t] = last match whose first rank <= first rank of tile t
@@ -309,7 +316,9 @@ __global__ void k_partition(const int64_t *__restrict__ cum, int64_t n_matches, 
     tile_m[t] = lo - 1;
 }
 
-template <int MODE>
+// KEYS = false: the target ids come from the visited table, inside this kernel.  KEYS = true: the kernel leaves the
+// target column open and writes one (target key, output position) record per arc for resolve_partitioned.
+template <int MODE, bool KEYS>
 __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
     __shared__ uint32_t relcum[EM_TILE + 1];
     __shared__ int64_t s_first_cum;
@@ -397,17 +406,28 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
         }
     }
 
+    uint32_t id[EM_IPT];
+#pragma unroll
+    for (int u = 0; u < EM_IPT; ++u) id[u] = 0;
+    if (KEYS) {
+        // ---- partitioned resolve: leave (key, position) records, in rank order
+#pragma unroll
+        for (int u = 0; u < EM_IPT; ++u) {
+            if (u >= skip && u < skip + n_valid) {
+                const int64_t rank = rank0 + u;
+                int64_t pos = rank;                            // DIRECT: relative to pos_base; SORTREC: record index
+                if (MODE == EMIT_INDIRECT) pos = g.foff[pl[u]] + (rank - g.roff[pl[u]]);
+                __stcs(g.keypos + rank, (key[u] << g.pos_bits) | static_cast<unsigned long long>(pos));
+            }
+        }
+    } else {
     // ---- visited set: find or insert.  Rounds of: all pending bucket reads in flight
     // together, then all pending CAS in flight together; a rank leaves when it finds its key or wins a slot.
     uint64_t slot[EM_IPT];                                    // bucket while searching, then the key's slot
-    uint32_t id[EM_IPT];
     uint32_t won = 0;                                         // bit u: this thread inserted the key (new state)
     const uint64_t n_buckets = g.cap >> 1;
 #pragma unroll
-    for (int u = 0; u < EM_IPT; ++u) {
-        id[u] = 0;
-        slot[u] = (todo >> u & 1u) ? home_bucket(key[u], g.cap) : 0;
-    }
+    for (int u = 0; u < EM_IPT; ++u) slot[u] = (todo >> u & 1u) ? home_bucket(key[u], g.cap) : 0;
     while (todo) {
         Bucket v[EM_IPT];
         unsigned long long old[EM_IPT];
@@ -477,6 +497,7 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
             id[u] = v;
         }
     }
+    }   // !KEYS
 
     // ---- write the composed arcs
     if (MODE == EMIT_DIRECT) {
@@ -486,7 +507,7 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
                                                                    static_cast<int>(g.f_lo + pl[2]), static_cast<int>(g.f_lo + pl[3])));
             __stcs(reinterpret_cast<uint4 *>(g.o_il + q), make_uint4(a_sym[0], a_sym[1], a_sym[2], a_sym[3]));
             __stcs(reinterpret_cast<uint4 *>(g.o_ol + q), make_uint4(b_sym[0], b_sym[1], b_sym[2], b_sym[3]));
-            __stcs(reinterpret_cast<uint4 *>(g.o_tgt + q), make_uint4(id[0], id[1], id[2], id[3]));
+            if (!KEYS) __stcs(reinterpret_cast<uint4 *>(g.o_tgt + q), make_uint4(id[0], id[1], id[2], id[3]));
             __stcs(reinterpret_cast<float4 *>(g.o_w + q), make_float4(w[0], w[1], w[2], w[3]));
         } else {
 #pragma unroll
@@ -494,7 +515,8 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
                 if (u >= skip && u < skip + n_valid) {
                     const int64_t q = my_pos + u;
                     g.o_src[q] = static_cast<int>(g.f_lo + pl[u]);
-                    g.o_il[q] = a_sym[u]; g.o_ol[q] = b_sym[u]; g.o_tgt[q] = id[u]; g.o_w[q] = w[u];
+                    g.o_il[q] = a_sym[u]; g.o_ol[q] = b_sym[u]; g.o_w[q] = w[u];
+                    if (!KEYS) g.o_tgt[q] = id[u];
                 }
             }
         }
@@ -505,7 +527,8 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
                 const int64_t rank = rank0 + u;
                 const int64_t q = g.arc_base + g.foff[pl[u]] + (rank - g.roff[pl[u]]);
                 g.o_src[q] = static_cast<int>(g.f_lo + pl[u]);
-                g.o_il[q] = a_sym[u]; g.o_ol[q] = b_sym[u]; g.o_tgt[q] = id[u]; g.o_w[q] = w[u];
+                g.o_il[q] = a_sym[u]; g.o_ol[q] = b_sym[u]; g.o_w[q] = w[u];
+                if (!KEYS) g.o_tgt[q] = id[u];
             }
         }
     } else {
@@ -798,8 +821,14 @@ struct Composer {
         c.sync();
     }
 
+    // partitioned = true: the level's target ids come from resolve_partitioned (no visited table)
+    bool partitioned = false;
+    int key_bits = 0;
+    int64_t n_states_live = 1;         // states created so far, including those of the launches of this level
+
     void launch_emit(int mode, const MatchList &L, int64_t n_matches, int64_t R, int64_t pos_base, int64_t f_lo,
-                     const int64_t *foff, const int64_t *roff, int64_t arc_base, uint4 *sortrec, int shift_t, int bits_b) {
+                     const int64_t *foff, const int64_t *roff, int64_t arc_base, uint4 *sortrec, int shift_t, int bits_b,
+                     int64_t n_positions = 0) {
         if (R <= 0) return;
         const int64_t tile0 = (pos_base / EM_TILE) * EM_TILE;
         const int64_t n_tiles = ceil_div(pos_base + R - tile0, EM_TILE);
@@ -813,13 +842,40 @@ struct Composer {
         g.table = table.p; g.cap = cap; g.n_states = d_counters.p; g.pair = pair.p;
         g.o_src = a_src.p; g.o_il = a_il.p; g.o_ol = a_ol.p; g.o_tgt = a_tgt.p; g.o_w = a_w.p;
         g.sortrec = sortrec; g.shift_t = shift_t; g.bits_b = bits_b; g.tile_m = tile_m.p;
+        g.keypos = nullptr; g.pos_bits = 0;
         const unsigned grid = static_cast<unsigned>(n_tiles);
-        if (mode == EMIT_DIRECT) k_emit<EMIT_DIRECT><<<grid, EM_THREADS, 0, c.stream>>>(g);
-        else if (mode == EMIT_INDIRECT) k_emit<EMIT_INDIRECT><<<grid, EM_THREADS, 0, c.stream>>>(g);
-        else k_emit<EMIT_SORTREC><<<grid, EM_THREADS, 0, c.stream>>>(g);
+        DBuf<unsigned long long> keypos;
+        if (partitioned) {
+            if (mode == EMIT_DIRECT) n_positions = R;
+            else if (mode == EMIT_SORTREC) n_positions = R;
+            g.pos_bits = bits_for(static_cast<uint64_t>(n_positions > 1 ? n_positions - 1 : 1));
+            keypos.alloc(c, R);
+            g.keypos = keypos.p;
+            if (mode == EMIT_DIRECT) k_emit<EMIT_DIRECT, true><<<grid, EM_THREADS, 0, c.stream>>>(g);
+            else if (mode == EMIT_INDIRECT) k_emit<EMIT_INDIRECT, true><<<grid, EM_THREADS, 0, c.stream>>>(g);
+            else k_emit<EMIT_SORTREC, true><<<grid, EM_THREADS, 0, c.stream>>>(g);
+        } else {
+            if (mode == EMIT_DIRECT) k_emit<EMIT_DIRECT, false><<<grid, EM_THREADS, 0, c.stream>>>(g);
+            else if (mode == EMIT_INDIRECT) k_emit<EMIT_INDIRECT, false><<<grid, EM_THREADS, 0, c.stream>>>(g);
+            else k_emit<EMIT_SORTREC, false><<<grid, EM_THREADS, 0, c.stream>>>(g);
+        }
         FSTC_LAUNCH_CHECK();
         c.n_launch += 2;
         st.n_emit_launches += 1;
+        if (partitioned) {
+            ResolveJob j;
+            j.keypos = keypos.p; j.n_records = R; j.key_bits = key_bits; j.pos_bits = g.pos_bits;
+            j.n_positions = n_positions; j.pair = pair.p; j.n_states_before = n_states_live; j.nq2 = nq2;
+            j.n_states = d_counters.p;
+            j.o_tgt = mode == EMIT_SORTREC ? nullptr : a_tgt.p + (mode == EMIT_DIRECT ? pos_base : arc_base);
+            j.sortrec = mode == EMIT_SORTREC ? sortrec : nullptr;
+            j.shift_t = shift_t;
+            j.force_bits = -1;
+            if (const char *e = getenv("FSTC_RESOLVE_BITS")) j.force_bits = atoi(e);   // test knob: force multi-pass
+            resolve_partitioned(c, j);
+            st.n_resolve += 1;
+            st.n_resolved_arcs += R;
+        }
     }
 
     fstc_result_t *run();
@@ -829,7 +885,7 @@ fstc_result_t *Composer::run() {
     if (m1.side != 1 || m2.side != 2) fail(FSTC_ERR_ARG, "operands must be packed with side 1 (left) and side 2 (right)");
     if (m1.n_inner != m2.n_inner)
         fail(FSTC_ERR_ARG, "inner alphabets differ: |Γ| = %d vs %d (PAPER.md:45)", m1.n_inner, m2.n_inner);
-    if (o.merge_mode < 0 || o.merge_mode > 2 || o.max_levels < 0 || o.max_raw_arcs < 0)
+    if (o.merge_mode < 0 || o.merge_mode > 2 || o.max_levels < 0 || o.max_raw_arcs < 0 || o.resolve_mode < 0 || o.resolve_mode > 2)
         fail(FSTC_ERR_ARG, "bad options");
     const int bits_a = bits_for(m1.n_outer > 0 ? m1.n_outer - 1 : 0), bits_b = bits_for(m2.n_outer > 0 ? m2.n_outer - 1 : 0);
     const int shift_t = bits_a + bits_b;
@@ -838,7 +894,7 @@ fstc_result_t *Composer::run() {
     const bool has_F = o.merge_mode == FSTC_MERGE_SORT_ALL ||
                        (o.merge_mode == FSTC_MERGE_AUTO &&
                         (((m1.any_flags & FLAG_D) && (m2.any_flags & FLAG_D)) || (m1.any_flags & FLAG_X) || (m2.any_flags & FLAG_X)));
-    const int key_bits = bits_for(n_pairs_total - 1);
+    key_bits = bits_for(n_pairs_total - 1);
 
     if (const char *e = getenv("FSTC_L2_FETCH")) {            // experiment knob: 32 / 64 / 128
         (void)cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, static_cast<size_t>(atoi(e)));
@@ -966,7 +1022,8 @@ fstc_result_t *Composer::run() {
         if (n_states + new_bound >= 0x7FFFFFFFll) fail(FSTC_ERR_CAPACITY, "more than 2^31-1 states");
         // look-ahead: if the search goes on, the next level is about (new states) x (arcs per expanded pair)
         int64_t next_R = 0, next_S = 0;
-        const bool must_grow = n_states + new_bound > pair_cap || slots_for(n_states + new_bound) > cap || n_arcs + R > arc_cap;
+        const bool must_grow = n_states + new_bound > pair_cap || (!partitioned && slots_for(n_states + new_bound) > cap) ||
+                               n_arcs + R > arc_cap;
         if (must_grow && !stop_after && n_sel > 0 && R > 0) {
             const double fan = static_cast<double>(R) / static_cast<double>(n_sel);
             double pr = static_cast<double>(new_bound) * fan;
@@ -986,9 +1043,31 @@ fstc_result_t *Composer::run() {
             next_S = ps > 0 ? static_cast<int64_t>(ps * scale) : 0;
             if (n_states + new_bound + next_S >= 0x7FFFFFFFll) next_S = 0;
         }
+        // ---- how this level resolves its target ids: the visited table while it stays small
+        // enough to live in L2, else the streaming partitioned resolve.  The switch is one-way: the table is dropped.
+        {
+            const int pos_bits = bits_for(static_cast<uint64_t>(R > 1 ? R - 1 : 1));
+            const int id_bits = bits_for(static_cast<uint64_t>(n_states + new_bound));
+            const bool fits = key_bits + pos_bits <= 64 && key_bits + id_bits <= 64;
+            if (!partitioned) {
+                bool want = o.resolve_mode == FSTC_RESOLVE_PARTITIONED;
+                if (o.resolve_mode == FSTC_RESOLVE_AUTO)
+                    want = R >= RESOLVE_MIN_ARCS && slots_for(n_states + new_bound) * sizeof(uint4) > RESOLVE_TABLE_BYTES;
+                // later levels must fit too: their positions need at most 31 bits, unless this is the last level
+                if (want && fits && (key_bits + 31 <= 64 || stop_after)) {
+                    partitioned = true;
+                    table = DBuf<uint4>();
+                    cap = 0;
+                }
+            } else if (!fits) {
+                fail(FSTC_ERR_CAPACITY, "level of %lld raw arcs over a %d-bit pair key does not fit the partitioned resolve",
+                     static_cast<long long>(R), key_bits);
+            }
+        }
         ensure_pairs(n_states + new_bound, n_states + new_bound + next_S);
-        ensure_table(n_states + new_bound, n_states + new_bound + next_S);
+        if (!partitioned) ensure_table(n_states + new_bound, n_states + new_bound + next_S);
         ensure_arcs(n_arcs + R, n_arcs + R + next_R);
+        n_states_live = n_states;
 
         // ---- match work-lists
         MatchList LU{nullptr, nullptr, nullptr}, LF{nullptr, nullptr, nullptr};
@@ -1021,6 +1100,7 @@ fstc_result_t *Composer::run() {
             tm.end(h);
             // target ids are now known: n_states bounds them
             const int64_t ns_now = static_cast<int64_t>(read_scalar(c, d_counters.p));
+            n_states_live = ns_now;
             const int tgt_bits = bits_for(static_cast<uint64_t>(ns_now - 1));
             h = tm.begin(FSTC_T_SORT);
             uint4 *sorted = radix_sort_records(c, sa.p, sb.p, RF, make_sort_passes(shift_t + tgt_bits, bits_for(static_cast<uint64_t>(nf - 1))));
@@ -1050,7 +1130,7 @@ fstc_result_t *Composer::run() {
             c.n_launch += 5;
             tm.end(h);
             h = tm.begin(FSTC_T_EMIT);
-            launch_emit(EMIT_INDIRECT, LU, MU, RU, 0, f_lo, foff.p, roffU.p, arc_base, nullptr, 0, 0);
+            launch_emit(EMIT_INDIRECT, LU, MU, RU, 0, f_lo, foff.p, roffU.p, arc_base, nullptr, 0, 0, RU + M);
             tm.end(h);
             n_arcs += RU + M;
             st.n_raw_sorted += RF;

@@ -19,6 +19,7 @@ LIB_PATH = os.environ.get("FSTC_LIB") or os.path.join(_HERE, "libfstc.so")   # F
 
 FSTC_MEM_DEVICE, FSTC_MEM_HOST = 0, 1
 MERGE_AUTO, MERGE_OFF, MERGE_SORT_ALL = 0, 1, 2
+RESOLVE_AUTO, RESOLVE_TABLE, RESOLVE_PARTITIONED = 0, 1, 2
 MAX_LEVEL_STATS = 64
 STAGES = ("count", "scan", "match", "emit", "sort", "reduce", "table", "assemble")
 
@@ -49,7 +50,7 @@ class _Opts(ctypes.Structure):
     _fields_ = [
         ("merge_mode", ctypes.c_int32), ("max_levels", ctypes.c_int32), ("max_raw_arcs", ctypes.c_int64),
         ("arc_capacity_hint", ctypes.c_int64), ("state_capacity_hint", ctypes.c_int64),
-        ("profile", ctypes.c_int32), ("reserved", ctypes.c_int32),
+        ("profile", ctypes.c_int32), ("resolve_mode", ctypes.c_int32),
     ]
 
 
@@ -61,6 +62,7 @@ class _Stats(ctypes.Structure):
         ("n_raw_sorted", ctypes.c_int64), ("table_capacity", ctypes.c_int64),
         ("n_rehash", ctypes.c_int32), ("n_grow", ctypes.c_int32),
         ("n_emit_launches", ctypes.c_int32), ("n_kernel_launches", ctypes.c_int32),
+        ("n_resolve", ctypes.c_int32), ("n_resolve_arcs_pad", ctypes.c_int32), ("n_resolved_arcs", ctypes.c_int64),
         ("ms", ctypes.c_double * len(STAGES)), ("ms_total", ctypes.c_double),
         ("level_frontier", ctypes.c_int64 * MAX_LEVEL_STATS), ("level_raw", ctypes.c_int64 * MAX_LEVEL_STATS),
         ("level_new_states", ctypes.c_int64 * MAX_LEVEL_STATS),
@@ -266,6 +268,7 @@ def stats_dict(s: _Stats) -> dict:
         "n_raw_sorted": int(s.n_raw_sorted), "table_capacity": int(s.table_capacity),
         "n_rehash": int(s.n_rehash), "n_grow": int(s.n_grow), "n_emit_launches": int(s.n_emit_launches),
         "n_kernel_launches": int(s.n_kernel_launches),
+        "n_resolve": int(s.n_resolve), "n_resolved_arcs": int(s.n_resolved_arcs),
         "ms": {k: float(s.ms[i]) for i, k in enumerate(STAGES)}, "ms_total": float(s.ms_total),
         "level_frontier": [int(s.level_frontier[i]) for i in range(nl)],
         "level_raw": [int(s.level_raw[i]) for i in range(nl)],
@@ -274,8 +277,9 @@ def stats_dict(s: _Stats) -> dict:
 
 
 def _opts(merge_mode=MERGE_AUTO, max_raw_arcs=0, max_levels=0, arc_capacity_hint=0, state_capacity_hint=0,
-          profile=False) -> _Opts:
+          profile=False, resolve_mode=0) -> _Opts:
     o = _Opts()
+    o.resolve_mode = int(resolve_mode)
     o.merge_mode, o.max_levels, o.max_raw_arcs = int(merge_mode), int(max_levels), int(max_raw_arcs)
     o.arc_capacity_hint, o.state_capacity_hint, o.profile = int(arc_capacity_hint), int(state_capacity_hint), int(bool(profile))
     return o

@@ -33,11 +33,12 @@ def gpu_tables(res, n_q2):
     return keys, tab, w
 
 
-def check_parity(fstc, m1, m2, *, merge_mode=0, max_raw_arcs=0, max_levels=0, device_inputs=True):
+def check_parity(fstc, m1, m2, *, merge_mode=0, max_raw_arcs=0, max_levels=0, device_inputs=True, resolve_mode=0):
     ref = oracle.compose(m1, m2, merge=True, max_raw_arcs=max_raw_arcs, max_levels=max_levels)
     a = fstc.DeviceFst.from_host(m1) if device_inputs else m1
     b = fstc.DeviceFst.from_host(m2) if device_inputs else m2
-    res = fstc.fstc_compose(a, b, merge_mode=merge_mode, max_raw_arcs=max_raw_arcs, max_levels=max_levels)
+    res = fstc.fstc_compose(a, b, merge_mode=merge_mode, max_raw_arcs=max_raw_arcs, max_levels=max_levels,
+                            resolve_mode=resolve_mode)
     nq2 = m2.n_states
     keys, tab, w = gpu_tables(res, nq2)
     # --- states

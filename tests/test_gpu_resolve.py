@@ -1,0 +1,92 @@
+"""Parity of the PARTITIONED target resolve (csrc/resolve.cu: hash-partitioned records, per-bin dedupe in shared
+memory, id scatter by position window) with the CPU oracle.  The same element-by-element comparison as
+test_gpu_parity.py, with `resolve_mode=RESOLVE_PARTITIONED` forced from level 0 and the number of hash bits forced
+(FSTC_RESOLVE_BITS) so that small inputs run zero, one and two scatter passes.  `-m gpu`."""
+from __future__ import annotations
+
+import os
+
+import pytest
+
+from paper_1805_06383_b200 import workloads
+from helpers import fst_from_arcs, messy_random_fst
+from test_gpu_parity import SMALL, check_parity, fstc  # noqa: F401  (fixture)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(params=["auto", "0", "3", "12"])
+def resolve_bits(request):
+    old = os.environ.pop("FSTC_RESOLVE_BITS", None)
+    if request.param != "auto":
+        os.environ["FSTC_RESOLVE_BITS"] = request.param
+    yield request.param
+    os.environ.pop("FSTC_RESOLVE_BITS", None)
+    if old is not None:
+        os.environ["FSTC_RESOLVE_BITS"] = old
+
+
+@pytest.mark.parametrize("case", SMALL[:3] + SMALL[6:])
+@pytest.mark.parametrize("merge_mode", [0, 1, 2])
+def test_small_random_machines_partitioned(fstc, case, merge_mode, resolve_bits):
+    seed, n1, sig, gam, a1, n2, dlt, a2 = case
+    m1 = messy_random_fst(seed, n1, sig, gam, a1)
+    m2 = messy_random_fst(seed + 100, n2, gam, dlt, a2)
+    res, _ = check_parity(fstc, m1, m2, merge_mode=merge_mode, resolve_mode=fstc.RESOLVE_PARTITIONED)
+    assert res.stats["n_resolve"] > 0 and res.stats["table_capacity"] == 0
+
+
+@pytest.mark.parametrize("merge_mode", [0, 1, 2])
+def test_config_tiny_partitioned(fstc, merge_mode, resolve_bits):
+    m1, m2 = workloads.make_config("tiny")
+    check_parity(fstc, m1, m2, merge_mode=merge_mode, resolve_mode=fstc.RESOLVE_PARTITIONED)
+
+
+@pytest.mark.parametrize("budget", [1, 17, 777, 3739])
+def test_budget_rule_T_partitioned(fstc, budget):
+    m1, m2 = workloads.make_config("tiny")
+    check_parity(fstc, m1, m2, max_raw_arcs=budget, resolve_mode=fstc.RESOLVE_PARTITIONED)
+
+
+@pytest.mark.parametrize("merge_mode", [0, 1])
+def test_config_medium_scaled_partitioned(fstc, merge_mode, resolve_bits):
+    """~250k states, 3e6 arcs: several scatter tiles per segment, bins with a ragged tail, old states re-entered."""
+    m1, m2 = workloads.make_config("medium", scale=0.05)
+    res, ref = check_parity(fstc, m1, m2, merge_mode=merge_mode, resolve_mode=fstc.RESOLVE_PARTITIONED)
+    assert ref.n_states > 10_000 and res.stats["n_resolved_arcs"] == ref.n_raw_arcs
+
+
+def test_config_skewed_scaled_partitioned(fstc, resolve_bits):
+    """Nearly every arc goes through sort + reduce: the ids are scattered into the sort records; the same target key
+    appears up to 10^5 times, so bins are far from uniform (exact-capacity retry of the scatter pass)."""
+    m1, m2 = workloads.make_config("skewed", scale=0.05)
+    res, ref = check_parity(fstc, m1, m2, max_raw_arcs=2_000_000, resolve_mode=fstc.RESOLVE_PARTITIONED)
+    assert res.stats["n_raw_sorted"] > 0 and ref.n_arcs < ref.n_raw_arcs
+
+
+def test_config_nlp_scaled_partitioned(fstc):
+    m1, m2 = workloads.make_config("nlp", scale=0.1)
+    check_parity(fstc, m1, m2, resolve_mode=fstc.RESOLVE_PARTITIONED)
+
+
+def test_config_large_scaled_partitioned(fstc, resolve_bits):
+    m1, m2 = workloads.make_config("large", scale=0.02)
+    check_parity(fstc, m1, m2, max_raw_arcs=3_000_000, resolve_mode=fstc.RESOLVE_PARTITIONED)
+
+
+def test_auto_switches_to_the_partitioned_resolve_on_a_big_level(fstc):
+    """AUTO keeps the table for small levels and switches (one way) once a level is big and its table would not fit L2."""
+    m1, m2 = workloads.make_config("large", scale=0.2)
+    res = fstc.fstc_compose(fstc.DeviceFst.from_host(m1), fstc.DeviceFst.from_host(m2), max_raw_arcs=60_000_000)
+    assert res.stats["n_resolve"] >= 1 and res.n_raw_arcs <= 60_000_000
+
+
+def test_degenerate_partitioned(fstc):
+    m1 = fst_from_arcs(2, 2, 3, [(0, 0, 0, 1, 1.0)], accept=[0])
+    m2 = fst_from_arcs(2, 3, 2, [(0, 1, 0, 1, 1.0)], accept=[0])
+    res, _ = check_parity(fstc, m1, m2, resolve_mode=fstc.RESOLVE_PARTITIONED)
+    assert (res.n_states, res.n_arcs) == (1, 0)
+    m1 = fst_from_arcs(2, 1, 1, [(0, 0, 0, 1, 0.0), (1, 0, 0, 1, 2.0), (1, 0, 0, 0, 3.0), (1, 0, 0, 0, 3.0)])
+    m2 = fst_from_arcs(1, 1, 1, [(0, 0, 0, 0, 0.5)] * 3)
+    for mm in (0, 1, 2):
+        check_parity(fstc, m1, m2, merge_mode=mm, resolve_mode=fstc.RESOLVE_PARTITIONED)
