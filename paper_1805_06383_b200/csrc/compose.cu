@@ -295,8 +295,8 @@ struct EmitArgs {
     uint4 *sortrec;          // SORTREC: {key lo, key hi, pair index, weight}, key = tgt id << shift_t | a << bits_b | b
     int shift_t, bits_b;
     const int64_t *tile_m;   // [n_tiles+1] match index holding the first rank of every tile
-    unsigned long long *keypos;   // KEYS: [R] target key << pos_bits | output position, for the partitioned resolve
-    int pos_bits;
+    unsigned long long *keys;     // KEYS: [R] target key of every rank, for the partitioned resolve
+    uint32_t *posout;             // KEYS + INDIRECT: [R] output position of every rank (relative to arc_base)
 };
 
 // tile_m[t] = last match whose first rank <= first rank of tile t
@@ -410,15 +410,20 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
 #pragma unroll
     for (int u = 0; u < EM_IPT; ++u) id[u] = 0;
     if (KEYS) {
-        // ---- partitioned resolve: leave (key, position) records, in rank order
+        // ---- partitioned resolve: leave the target keys, in rank order
+        if (n_valid == EM_IPT && ((rank0 & 1) == 0)) {
+            __stcs(reinterpret_cast<ulonglong2 *>(g.keys + rank0), make_ulonglong2(key[0], key[1]));
+            __stcs(reinterpret_cast<ulonglong2 *>(g.keys + rank0 + 2), make_ulonglong2(key[2], key[3]));
+        } else {
 #pragma unroll
-        for (int u = 0; u < EM_IPT; ++u) {
-            if (u >= skip && u < skip + n_valid) {
-                const int64_t rank = rank0 + u;
-                int64_t pos = rank;                            // DIRECT: relative to pos_base; SORTREC: record index
-                if (MODE == EMIT_INDIRECT) pos = g.foff[pl[u]] + (rank - g.roff[pl[u]]);
-                __stcs(g.keypos + rank, (key[u] << g.pos_bits) | static_cast<unsigned long long>(pos));
-            }
+            for (int u = 0; u < EM_IPT; ++u)
+                if (u >= skip && u < skip + n_valid) g.keys[rank0 + u] = key[u];
+        }
+        if (MODE == EMIT_INDIRECT) {
+#pragma unroll
+            for (int u = 0; u < EM_IPT; ++u)
+                if (u >= skip && u < skip + n_valid)
+                    g.posout[rank0 + u] = static_cast<uint32_t>(g.foff[pl[u]] + (rank0 + u - g.roff[pl[u]]));
         }
     } else {
     // ---- visited set: find or insert.  Rounds of: all pending bucket reads in flight
@@ -842,15 +847,14 @@ struct Composer {
         g.table = table.p; g.cap = cap; g.n_states = d_counters.p; g.pair = pair.p;
         g.o_src = a_src.p; g.o_il = a_il.p; g.o_ol = a_ol.p; g.o_tgt = a_tgt.p; g.o_w = a_w.p;
         g.sortrec = sortrec; g.shift_t = shift_t; g.bits_b = bits_b; g.tile_m = tile_m.p;
-        g.keypos = nullptr; g.pos_bits = 0;
+        g.keys = nullptr; g.posout = nullptr;
         const unsigned grid = static_cast<unsigned>(n_tiles);
-        DBuf<unsigned long long> keypos;
+        DBuf<unsigned long long> keys;
+        DBuf<uint32_t> posout;
         if (partitioned) {
-            if (mode == EMIT_DIRECT) n_positions = R;
-            else if (mode == EMIT_SORTREC) n_positions = R;
-            g.pos_bits = bits_for(static_cast<uint64_t>(n_positions > 1 ? n_positions - 1 : 1));
-            keypos.alloc(c, R);
-            g.keypos = keypos.p;
+            keys.alloc(c, R + 2);
+            g.keys = keys.p;
+            if (mode == EMIT_INDIRECT) { posout.alloc(c, R); g.posout = posout.p; }
             if (mode == EMIT_DIRECT) k_emit<EMIT_DIRECT, true><<<grid, EM_THREADS, 0, c.stream>>>(g);
             else if (mode == EMIT_INDIRECT) k_emit<EMIT_INDIRECT, true><<<grid, EM_THREADS, 0, c.stream>>>(g);
             else k_emit<EMIT_SORTREC, true><<<grid, EM_THREADS, 0, c.stream>>>(g);
@@ -864,9 +868,11 @@ struct Composer {
         st.n_emit_launches += 1;
         if (partitioned) {
             ResolveJob j;
-            j.keypos = keypos.p; j.n_records = R; j.key_bits = key_bits; j.pos_bits = g.pos_bits;
-            j.n_positions = n_positions; j.pair = pair.p; j.n_states_before = n_states_live; j.nq2 = nq2;
+            j.keys = keys.p; j.n_records = R; j.key_bits = key_bits;
+            j.pair = pair.p; j.n_states_before = n_states_live; j.nq2 = nq2;
             j.n_states = d_counters.p;
+            j.mode = mode == EMIT_DIRECT ? 0 : (mode == EMIT_INDIRECT ? 1 : 2);
+            j.pos = posout.p;
             j.o_tgt = mode == EMIT_SORTREC ? nullptr : a_tgt.p + (mode == EMIT_DIRECT ? pos_base : arc_base);
             j.sortrec = mode == EMIT_SORTREC ? sortrec : nullptr;
             j.shift_t = shift_t;
@@ -1046,22 +1052,20 @@ fstc_result_t *Composer::run() {
         // ---- how this level resolves its target ids: the visited table while it stays small
         // enough to live in L2, else the streaming partitioned resolve.  The switch is one-way: the table is dropped.
         {
-            const int pos_bits = bits_for(static_cast<uint64_t>(R > 1 ? R - 1 : 1));
             const int id_bits = bits_for(static_cast<uint64_t>(n_states + new_bound));
-            const bool fits = key_bits + pos_bits <= 64 && key_bits + id_bits <= 64;
+            const bool fits = key_bits + id_bits <= 64;                // state records are key << id_bits | id
             if (!partitioned) {
                 bool want = o.resolve_mode == FSTC_RESOLVE_PARTITIONED;
                 if (o.resolve_mode == FSTC_RESOLVE_AUTO)
                     want = R >= RESOLVE_MIN_ARCS && slots_for(n_states + new_bound) * sizeof(uint4) > RESOLVE_TABLE_BYTES;
-                // later levels must fit too: their positions need at most 31 bits, unless this is the last level
+                // later levels must fit too (ids have at most 31 bits), unless this is the last level
                 if (want && fits && (key_bits + 31 <= 64 || stop_after)) {
                     partitioned = true;
                     table = DBuf<uint4>();
                     cap = 0;
                 }
             } else if (!fits) {
-                fail(FSTC_ERR_CAPACITY, "level of %lld raw arcs over a %d-bit pair key does not fit the partitioned resolve",
-                     static_cast<long long>(R), key_bits);
+                fail(FSTC_ERR_CAPACITY, "%d-bit pair keys with %d-bit state ids do not fit the partitioned resolve", key_bits, id_bits);
             }
         }
         ensure_pairs(n_states + new_bound, n_states + new_bound + next_S);

@@ -54,19 +54,20 @@ void free_result(fstc_result_t *r);
 
 // ---------------------------------------------------------------- partitioned target resolution (resolve.cu)
 // Finds or creates the state id of every composed arc of a big level without touching a table in DRAM at random:
-// records (target key << pos_bits | position) are hash-partitioned with streaming passes, deduplicated per bin in
-// shared memory against the existing states, and the ids scattered back by position window.
+// the target keys are hash-partitioned with streaming passes, deduplicated per bin in shared memory against the
+// existing states, and the ids gathered back through the recorded permutations.
 struct ResolveJob {
-    const unsigned long long *keypos;   // [n_records] key << pos_bits | position, any order
+    const unsigned long long *keys;     // [n_records] target key q1*|Q2|+q2 of every composed arc, in rank order
     int64_t n_records;
-    int key_bits, pos_bits;
-    int64_t n_positions;                // positions are < n_positions
+    int key_bits;
     int2 *pair;                         // [>= n_states_before + new states] id -> (q1, q2); new entries are written
     int64_t n_states_before;
     uint64_t nq2;
     unsigned long long *n_states;       // device counter: set to n_states_before, advanced by the new states
-    int32_t *o_tgt;                     // o_tgt[position] = id            (when sortrec is null)
-    uint4 *sortrec;                     // or: id OR-ed into key bits [shift_t, ...) of sortrec[position]
+    int mode;                           // 0: o_tgt[r] = id   1: o_tgt[pos[r]] = id   2: id into sortrec[r]
+    const uint32_t *pos;                // mode 1
+    int32_t *o_tgt;                     // modes 0, 1
+    uint4 *sortrec;                     // mode 2: id OR-ed into key bits [shift_t, ...)
     int shift_t;
     int force_bits;                     // >= 0: number of hash bits to partition on (tests); -1: from the sizes
 };

@@ -1,19 +1,20 @@
 // Partitioned target resolution: the visited-set step of a BIG level (PAPER.md:237-239 adapted).
 //
 // The paper tests and sets one entry of a dense |Q1||Q2| table per composed arc (atomicOr, :237).  On a B200 a
-// random 32-byte DRAM sector costs ~21 ps to read and ~45 ps to dirty (measured, profiles/), so at 10^9 arcs per
-// level the per-arc probe of any table that does not fit the 126 MB L2 bounds the whole path.  Big levels are
-// therefore resolved like a radix hash join, with streaming passes only:
+// random 32-byte DRAM sector costs ~21 ps to read and ~45 ps to dirty (measured, profiles/r01_random_access.md), so at
+// 10^9 arcs per level the per-arc probe of any table that does not fit the 126 MB L2 bounds the whole path.  Big
+// levels are therefore resolved like a radix hash join, with streaming passes only:
 //
-//   1. every composed arc leaves a record (target key, output position) — written by the emit kernel in rank order;
-//      every existing state leaves a record (key, id);
-//   2. both record streams are partitioned by the top bits of a hash of the key (one or two staged scatter
-//      passes: a block sorts a tile of 4096 records by bin in shared memory and appends whole runs), until a bin
-//      holds ~10^3 distinct keys;
+//   1. the emit kernel leaves the target key of every composed arc, in rank order; every existing state leaves a
+//      record (key, id);
+//   2. both streams are partitioned by the top bits of a hash of the key (one or two staged scatter passes: a block
+//      sorts a tile of 4096 records by bin in shared memory and appends whole runs), until a bin holds ~10^3 distinct
+//      keys.  A pass also records where every input record went (dest[i]);
 //   3. one block per bin builds the bin's key->id map in SHARED memory (old states first), finds or creates the id
-//      of every arc record, allocates new ids (one global atomicAdd per 1024 records) and writes pair[id];
-//   4. the (position, id) records are partitioned by position window and scattered into the target column; a window
-//      is a few MB, so the scattered 4-byte stores combine in L2 and reach DRAM as full sectors.
+//      of every arc key, allocates new ids (one global atomicAdd per round) and writes pair[id];
+//   4. the ids travel back through the recorded permutations: id1[i] = id2[dest2[i]] (a gather inside one parent
+//      bin, a few MB, L2-resident), then tgt[pos(r)] = id1[dest1[r]] in rank order — records of a bin keep roughly
+//      their rank order, so the gather reads 2^b1 slowly advancing streams and the target column is written coalesced.
 //
 // Nothing persists between levels except pair[] (id -> (q1,q2)): the key->id map is rebuilt per level from it.
 #include <cstdlib>
@@ -28,10 +29,12 @@ namespace {
 
 constexpr unsigned long long RS_EMPTY = ~0ull;
 
+// 64-bit mixer (two multiply / xor-shift rounds).  The bins use its top bits, the shared-memory map its low ones.
 __device__ __forceinline__ uint64_t rmix64(uint64_t k) {
-    k ^= k >> 33; k *= 0xff51afd7ed558ccdULL;
-    k ^= k >> 33; k *= 0xc4ceb9fe1a85ec53ULL;
-    k ^= k >> 33;
+    k *= 0x9E3779B97F4A7C15ULL;
+    k ^= k >> 32;
+    k *= 0xD6E8FEB86659FD93ULL;
+    k ^= k >> 32;
     return k;
 }
 
@@ -49,7 +52,7 @@ constexpr int SC_THREADS = 512;
 constexpr int SC_IPT = SC_TILE / SC_THREADS;
 constexpr int SC_MAX_BINS = 1024;
 
-// tile_first[s] = number of SC_TILE tiles of the segments before s; tile_first[n_seg] = total.  n_seg <= 1024.
+// tile_first[s] = number of tiles of the segments before s; tile_first[n_seg] = total.  n_seg <= 1024.
 __global__ void __launch_bounds__(1024) rs_seg_tiles(SegView in, int tile, int64_t *__restrict__ tile_first) {
     __shared__ int64_t s_w[32];
     const int s = threadIdx.x, lane = s & 31, warp = s >> 5;
@@ -70,13 +73,12 @@ __global__ void __launch_bounds__(1024) rs_seg_tiles(SegView in, int tile, int64
 
 // capacity of every output bin of segment s: exact = 0: cnt[s] / nbins * (1 + 1/slack_div) + slack_add (uniform
 // hashing); exact = 1: the count a previous overflowing attempt left in the cursor.
-__global__ void rs_bin_caps(SegView in, int nbins, int slack_div, uint32_t slack_add, uint32_t fixed_cap,
-                            const uint32_t *__restrict__ cursor, int cur_stride, int exact, uint32_t *__restrict__ cap) {
+__global__ void rs_bin_caps(SegView in, int nbins, int slack_div, uint32_t slack_add, const uint32_t *__restrict__ cursor,
+                            int cur_stride, int exact, uint32_t *__restrict__ cap) {
     const int64_t g = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (g >= static_cast<int64_t>(in.n_seg) * nbins) return;
     if (exact) { cap[g] = cursor[static_cast<size_t>(g) * cur_stride]; return; }
     const uint32_t n = in.cnt[g / nbins];
-    if (fixed_cap) { cap[g] = fixed_cap < n ? fixed_cap : n; return; }
     const uint64_t mean = (static_cast<uint64_t>(n) + nbins - 1) / nbins;
     uint64_t c = mean + mean / slack_div + slack_add;
     if (c > n) c = n;                                           // a bin never holds more than its whole segment
@@ -90,47 +92,54 @@ __global__ void rs_check_overflow(const uint32_t *__restrict__ cursor, int cur_s
     if (__any_sync(0xffffffffu, over) && (threadIdx.x & 31) == 0) atomicOr(flag, 1u);
 }
 
-// ------------------------------------------------------------------------------------------ staged scatter
-// FN 0: bin = bits [hshift, hshift + log2 nbins) of mix64(record >> shift)   (hash partition on the key)
-// FN 1: bin = (record >> 32) >> hshift                                        (position window of a (pos,id) record)
-template <int FN>
-__device__ __forceinline__ uint32_t rs_bin(unsigned long long r, int shift, int hshift, uint32_t mask) {
-    if (FN == 0) return static_cast<uint32_t>(rmix64(r >> shift) >> hshift) & mask;
-    return static_cast<uint32_t>(r >> 32) >> hshift;
+__global__ void rs_compact_counts(const uint32_t *__restrict__ cursor, int cur_stride, int64_t nb, uint32_t *__restrict__ cnt) {
+    const int64_t g = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (g < nb) cnt[g] = cursor[static_cast<size_t>(g) * cur_stride];
 }
 
+// first tile of segment `seg` <= blockIdx.x < first tile of seg + 1
+__device__ __forceinline__ int rs_find_segment(const int64_t *tile_first, int n_seg) {
+    int lo = 0, hi = n_seg;
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (tile_first[mid] <= static_cast<int64_t>(blockIdx.x)) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// ------------------------------------------------------------------------------------------ staged scatter
+// bin of a record = bits [hshift, hshift + log2 nbins) of mix64(record >> shift).  A tile of SC_TILE records is sorted
+// by bin in shared memory; every non-empty bin reserves room for its run with one global atomicAdd and the runs go out
+// with consecutive threads writing consecutive addresses.  DEST: the pass also records, per tile and in sorted order,
+// where every record went (dest) and where it came from (perm), so that ids can travel back with the same locality.
 struct ScatterArgs {
     SegView in;
     const int64_t *tile_first;      // [n_seg + 1]
     unsigned long long *out;
     const int64_t *out_start;       // [n_seg * nbins + 1]
     uint32_t *cursor;               // [n_seg * nbins * cur_stride]
+    uint32_t *dest;                 // DEST: [input buffer length] output index of the record in SORTED slot i of its tile
+    uint16_t *perm;                 // DEST: [input buffer length] tile-local input index of that record
     int cur_stride;
     int shift, hshift, nbins;
 };
 
 #ifndef FSTC_SC_MINB
-#define FSTC_SC_MINB 2
+#define FSTC_SC_MINB 3
 #endif
-template <int FN>
+template <bool DEST>
 __global__ void __launch_bounds__(SC_THREADS, FSTC_SC_MINB) rs_scatter(ScatterArgs a) {
-    extern __shared__ unsigned long long sorted[];             // [SC_TILE], dynamic: the kernel needs > 48 KB in total
+    extern __shared__ unsigned long long sorted[];             // [SC_TILE] records, then uint32 smeta[SC_TILE]
+    uint32_t *smeta = reinterpret_cast<uint32_t *>(sorted + SC_TILE);   // tile-local input index << 16 | bin
     __shared__ uint32_t cnt[SC_MAX_BINS];                       // count, then first slot of the bin in sorted[]
     __shared__ long long gdelta[SC_MAX_BINS];                   // global index of the bin's run minus its first slot
-    __shared__ long long glimit[SC_MAX_BINS];                   // end of the bin's global range
+    __shared__ uint32_t room[SC_MAX_BINS];                      // records of the run that still fit the bin
     __shared__ uint32_t s_warp[SC_THREADS / 32];
     __shared__ int s_seg;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t mask = static_cast<uint32_t>(a.nbins - 1);
 
-    if (tid == 0) {                                             // segment of this tile
-        int lo = 0, hi = a.in.n_seg;                            // last s with tile_first[s] <= blockIdx.x
-        while (hi - lo > 1) {
-            int mid = (lo + hi) >> 1;
-            if (a.tile_first[mid] <= static_cast<int64_t>(blockIdx.x)) lo = mid; else hi = mid;
-        }
-        s_seg = lo;
-    }
+    if (tid == 0) s_seg = rs_find_segment(a.tile_first, a.in.n_seg);
     for (int p = tid; p < a.nbins; p += SC_THREADS) cnt[p] = 0;
     __syncthreads();
     const int seg = s_seg;
@@ -138,16 +147,22 @@ __global__ void __launch_bounds__(SC_THREADS, FSTC_SC_MINB) rs_scatter(ScatterAr
     const int64_t seg_n = a.in.cnt[seg];
     const int64_t lo = tile * SC_TILE;
     const int n = static_cast<int>(seg_n - lo < SC_TILE ? seg_n - lo : SC_TILE);
-    const unsigned long long *src = a.in.data + a.in.start[seg] + lo;
+    const int64_t in_base = a.in.start[seg] + lo;
+    const unsigned long long *src = a.in.data + in_base;
 
     unsigned long long rec[SC_IPT];
-    uint32_t rk[SC_IPT];
+    uint32_t br[SC_IPT];                                        // bin << 16 | rank inside the bin (tile-local)
+#pragma unroll
+    for (int u = 0; u < SC_IPT; ++u) {
+        const int i = u * SC_THREADS + tid;
+        if (i < n) rec[u] = __ldcs(src + i);
+    }
 #pragma unroll
     for (int u = 0; u < SC_IPT; ++u) {
         const int i = u * SC_THREADS + tid;
         if (i < n) {
-            rec[u] = __ldcs(src + i);
-            rk[u] = atomicAdd(&cnt[rs_bin<FN>(rec[u], a.shift, a.hshift, mask)], 1u);
+            const uint32_t b = static_cast<uint32_t>(rmix64(rec[u] >> a.shift) >> a.hshift) & mask;
+            br[u] = (b << 16) | atomicAdd(&cnt[b], 1u);
         }
     }
     __syncthreads();
@@ -172,9 +187,11 @@ __global__ void __launch_bounds__(SC_THREADS, FSTC_SC_MINB) rs_scatter(ScatterAr
         if (p < a.nbins) {
             cnt[p] = ex;
             if (c) {
+                const int64_t b0 = a.out_start[gbin0 + p], b1 = a.out_start[gbin0 + p + 1];
                 const uint32_t g = atomicAdd(&a.cursor[static_cast<size_t>(gbin0 + p) * a.cur_stride], c);
-                gdelta[p] = a.out_start[gbin0 + p] + static_cast<long long>(g) - static_cast<long long>(ex);
-                glimit[p] = a.out_start[gbin0 + p + 1];
+                gdelta[p] = b0 + static_cast<long long>(g) - static_cast<long long>(ex);
+                const int64_t left = (b1 - b0) - static_cast<int64_t>(g);
+                room[p] = left <= 0 ? 0u : (left < c ? static_cast<uint32_t>(left) : c);
             }
             ex += c;
         }
@@ -183,41 +200,49 @@ __global__ void __launch_bounds__(SC_THREADS, FSTC_SC_MINB) rs_scatter(ScatterAr
 #pragma unroll
     for (int u = 0; u < SC_IPT; ++u) {
         const int i = u * SC_THREADS + tid;
-        if (i < n) sorted[cnt[rs_bin<FN>(rec[u], a.shift, a.hshift, mask)] + rk[u]] = rec[u];
+        if (i < n) {
+            const uint32_t b = br[u] >> 16, rk = br[u] & 0xFFFFu;
+            const uint32_t slot = cnt[b] + rk;
+            sorted[slot] = rec[u];
+            smeta[slot] = (static_cast<uint32_t>(i) << 16) | b;
+        }
     }
     __syncthreads();
     for (int i = tid; i < n; i += SC_THREADS) {
-        const unsigned long long r = sorted[i];
-        const uint32_t p = rs_bin<FN>(r, a.shift, a.hshift, mask);
+        const uint32_t m = smeta[i], p = m & 0xFFFFu;
+        const bool fits = static_cast<uint32_t>(i) - cnt[p] < room[p];
         const long long dst = gdelta[p] + i;
-        if (dst < glimit[p]) a.out[dst] = r;                    // a full bin drops the record; the host retries
+        if (fits) a.out[dst] = sorted[i];                       // a full bin drops the record; the host retries
+        if (DEST) {                                             // the way back: sorted slot -> output index, input index
+            a.dest[in_base + i] = fits ? static_cast<uint32_t>(dst) : 0xFFFFFFFFu;
+            a.perm[in_base + i] = static_cast<uint16_t>(m >> 16);
+        }
     }
 }
 
 // ------------------------------------------------------------------------------------------ per-bin dedupe
 // One block per bin.  keys[]/ids[] in shared memory map the bin's keys to state ids: the existing states of the bin
-// are entered first, then every arc record finds its key or creates it.  New ids are handed out per round of
-// DD_TILE records with one global atomicAdd; the winner of a key writes pair[id].  Output: (pos << 32 | id), dense,
-// at out[out_off[bin] + i].
+// are entered first, then every arc key finds its entry or creates it.  New ids are handed out per round of DD_TILE
+// records with one global atomicAdd; the winner of a key writes pair[id].  The id of arc record i of the bin goes to
+// ids_out[start[bin] + i], the index the last scatter pass recorded in dest[].
 constexpr int DD_THREADS = 256;
 constexpr int DD_IPT = 4;
 constexpr int DD_TILE = DD_THREADS * DD_IPT;
 #ifndef FSTC_DD_SLOTS
-#define FSTC_DD_SLOTS 4096
+#define FSTC_DD_SLOTS 2048
 #endif
 #ifndef FSTC_DD_TARGET
-#define FSTC_DD_TARGET 1400
+#define FSTC_DD_TARGET 1000
 #endif
 constexpr int DD_SLOTS = FSTC_DD_SLOTS;        // keys 8 B + ids 4 B per slot, in shared memory
 constexpr int DD_TARGET = FSTC_DD_TARGET;      // aimed maximum of the mean number of distinct keys per bin
 
 struct DedupeArgs {
     SegView st;                // state records  key << ib | id
-    SegView arcs;              // arc records    key << pb | pos
-    int ib, pb;
-    const int64_t *out_off;    // [n_bins + 1]
-    unsigned long long *out;
-    uint64_t nq2;
+    SegView arcs;              // arc records    key
+    int ib;
+    uint32_t *ids_out;         // [length of the arc buffer]
+    uint64_t nq2, nq2_inv;     // |Q2| and floor(2^64 / |Q2|)
     unsigned long long *n_states;
     int2 *pair;
     unsigned *err;             // set when a bin holds more distinct keys than the shared-memory map
@@ -234,43 +259,51 @@ __device__ __forceinline__ int dd_find_or_claim(unsigned long long *keys, unsign
     return -1;
 }
 
+// key = q1 * nq2 + q2 -> (q1, q2) with one multiply-high and a correction step instead of a 64-bit division
+__device__ __forceinline__ int2 dd_split_key(unsigned long long key, uint64_t nq2, uint64_t nq2_inv) {
+    unsigned long long q1 = __umul64hi(key, nq2_inv);
+    long long r = static_cast<long long>(key - q1 * nq2);
+    if (r >= static_cast<long long>(nq2)) { q1 += 1; r -= static_cast<long long>(nq2); }
+    if (r >= static_cast<long long>(nq2)) { q1 += 1; r -= static_cast<long long>(nq2); }
+    return make_int2(static_cast<int>(q1), static_cast<int>(r));
+}
+
 __global__ void __launch_bounds__(DD_THREADS) rs_dedupe(DedupeArgs a) {
-    extern __shared__ unsigned long long keys[];               // [DD_SLOTS]
-    uint32_t *ids = reinterpret_cast<uint32_t *>(keys + DD_SLOTS);
+    __shared__ unsigned long long keys[DD_SLOTS];
+    __shared__ uint32_t ids[DD_SLOTS];
     __shared__ uint32_t s_warp[DD_THREADS / 32];
     __shared__ unsigned long long s_base;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int64_t bin = blockIdx.x;
-    const int64_t sc = a.st.cnt[bin];
     const int64_t ac = a.arcs.cnt[bin];
     if (ac == 0) return;                                       // nothing to resolve in this bin
+    const int64_t sc = a.st.cnt[bin];
+    const int64_t a0 = a.arcs.start[bin], s0 = a.st.start[bin];
     for (int i = tid; i < DD_SLOTS; i += DD_THREADS) keys[i] = RS_EMPTY;
     __syncthreads();
-    const unsigned long long *sp = a.st.data + a.st.start[bin];
     const unsigned long long idmask = (1ull << a.ib) - 1;
     for (int64_t i = tid; i < sc; i += DD_THREADS) {
-        const unsigned long long r = sp[i];
+        const unsigned long long r = a.st.data[s0 + i];
         bool won;
         const int s = dd_find_or_claim(keys, r >> a.ib, &won);
         if (s < 0) atomicOr(a.err, 1u); else ids[s] = static_cast<uint32_t>(r & idmask);
     }
     __syncthreads();
-    const unsigned long long *ap = a.arcs.data + a.arcs.start[bin];
-    unsigned long long *op = a.out + a.out_off[bin];
-    const unsigned long long posmask = (1ull << a.pb) - 1;
+    const unsigned long long *ap = a.arcs.data + a0;
+    uint32_t *op = a.ids_out + a0;
     for (int64_t base = 0; base < ac; base += DD_TILE) {
         unsigned long long key[DD_IPT];
-        uint32_t pos[DD_IPT];
         int slot[DD_IPT];
         uint32_t wonmask = 0;
 #pragma unroll
         for (int u = 0; u < DD_IPT; ++u) {
             const int64_t i = base + u * DD_THREADS + tid;
+            key[u] = i < ac ? __ldcs(ap + i) : RS_EMPTY;
+        }
+#pragma unroll
+        for (int u = 0; u < DD_IPT; ++u) {
             slot[u] = -2;
-            if (i < ac) {
-                const unsigned long long r = __ldcs(ap + i);
-                key[u] = r >> a.pb;
-                pos[u] = static_cast<uint32_t>(r & posmask);
+            if (key[u] != RS_EMPTY) {
                 bool won;
                 slot[u] = dd_find_or_claim(keys, key[u], &won);
                 if (slot[u] < 0) atomicOr(a.err, 1u);
@@ -299,64 +332,80 @@ __global__ void __launch_bounds__(DD_THREADS) rs_dedupe(DedupeArgs a) {
             if (wonmask >> u & 1u) {
                 const uint32_t id = next_id++;
                 ids[slot[u]] = id;
-                const unsigned long long q1 = key[u] / a.nq2;
-                a.pair[id] = make_int2(static_cast<int>(q1), static_cast<int>(key[u] - q1 * a.nq2));
+                a.pair[id] = dd_split_key(key[u], a.nq2, a.nq2_inv);
             }
         }
         __syncthreads();
 #pragma unroll
         for (int u = 0; u < DD_IPT; ++u) {
             const int64_t i = base + u * DD_THREADS + tid;
-            if (i < ac) {
-                const uint32_t id = slot[u] >= 0 ? ids[slot[u]] : 0u;
-                __stcs(op + i, (static_cast<unsigned long long>(pos[u]) << 32) | id);
-            }
+            if (i < ac) __stcs(op + i, slot[u] >= 0 ? ids[slot[u]] : 0u);
         }
     }
 }
 
-// ------------------------------------------------------------------------------------------ id scatter
-// (pos << 32 | id) records of one position window -> the target column.  MODE 0: o_tgt[pos] = id;
-// MODE 1: the id goes into the target field of a sort record (key bits shift_t and up).
-constexpr int SI_THREADS = 256;
-constexpr int SI_IPT = 8;
-constexpr int SI_TILE = SI_THREADS * SI_IPT;
+// ------------------------------------------------------------------------------------------ ids back through the passes
+// A scatter pass undone, tile by tile (the tiles of the pass): thread i reads the id of the record in sorted slot i —
+// slots of a bin are neighbours in the output, so a warp reads a few short runs instead of 32 far-apart words — and
+// drops it at the record's input index in shared memory; the tile is then written out in input order.
+// MODE 0: out[input index] = id (ids of the previous pass's buffer, or the target column when in rank order)
+// MODE 1: o_tgt[pos[rank]] = id;  MODE 2: id into the target field (key bits shift_t and up) of sort record `rank`.
+constexpr int GA_THREADS = 512;
+constexpr int GA_IPT = SC_TILE / GA_THREADS;
+
+struct GatherArgs {
+    SegView seg;                    // the INPUT segments of the pass that is undone
+    const int64_t *tile_first;
+    const uint32_t *dest;           // null: identity (no pass), ids are read at the input index
+    const uint16_t *perm;
+    const uint32_t *in;
+    uint32_t *out;                  // MODE 0
+    const uint32_t *pos;            // MODE 1
+    int32_t *o_tgt;                 // MODE 1
+    uint4 *sortrec;                 // MODE 2
+    int shift_t;
+};
 
 template <int MODE>
-__global__ void __launch_bounds__(SI_THREADS) rs_scatter_ids(SegView in, const int64_t *__restrict__ tile_first,
-                                                             int32_t *__restrict__ o_tgt, uint4 *__restrict__ sortrec,
-                                                             int shift_t) {
+__global__ void __launch_bounds__(GA_THREADS) rs_gather_ids(GatherArgs a) {
+    __shared__ uint32_t s_id[SC_TILE];
     __shared__ int s_seg;
-    if (threadIdx.x == 0) {
-        int lo = 0, hi = in.n_seg;
-        while (hi - lo > 1) {
-            int mid = (lo + hi) >> 1;
-            if (tile_first[mid] <= static_cast<int64_t>(blockIdx.x)) lo = mid; else hi = mid;
-        }
-        s_seg = lo;
-    }
+    const int tid = threadIdx.x;
+    if (tid == 0) s_seg = rs_find_segment(a.tile_first, a.seg.n_seg);
     __syncthreads();
-    const int seg = s_seg;
-    const int64_t lo = (static_cast<int64_t>(blockIdx.x) - tile_first[seg]) * SI_TILE;
-    const int64_t seg_n = in.cnt[seg];
-    const unsigned long long *src = in.data + in.start[seg] + lo;
-    unsigned long long r[SI_IPT];
+    const int s = s_seg;
+    const int64_t lo = (static_cast<int64_t>(blockIdx.x) - a.tile_first[s]) * SC_TILE;
+    const int64_t seg_n = a.seg.cnt[s];
+    const int n = static_cast<int>(seg_n - lo < SC_TILE ? seg_n - lo : SC_TILE);
+    const int64_t base = a.seg.start[s] + lo;
+    if (a.dest) {
+        uint32_t d[GA_IPT], li[GA_IPT];
 #pragma unroll
-    for (int u = 0; u < SI_IPT; ++u) {
-        const int64_t i = lo + u * SI_THREADS + threadIdx.x;
-        r[u] = i < seg_n ? __ldcs(src + u * SI_THREADS + threadIdx.x) : RS_EMPTY;
+        for (int u = 0; u < GA_IPT; ++u) {
+            const int i = u * GA_THREADS + tid;
+            d[u] = i < n ? __ldcs(a.dest + base + i) : 0xFFFFFFFFu;
+            li[u] = i < n ? __ldcs(a.perm + base + i) : 0u;
+        }
+        uint32_t v[GA_IPT];
+#pragma unroll
+        for (int u = 0; u < GA_IPT; ++u) v[u] = d[u] != 0xFFFFFFFFu ? __ldg(a.in + d[u]) : 0u;
+#pragma unroll
+        for (int u = 0; u < GA_IPT; ++u)
+            if (u * GA_THREADS + tid < n) s_id[li[u]] = v[u];
+        __syncthreads();
     }
 #pragma unroll
-    for (int u = 0; u < SI_IPT; ++u) {
-        if (r[u] != RS_EMPTY) {
-            const uint32_t pos = static_cast<uint32_t>(r[u] >> 32), id = static_cast<uint32_t>(r[u]);
-            if (MODE == 0) o_tgt[pos] = static_cast<int32_t>(id);
-            else {
-                const unsigned long long k = static_cast<unsigned long long>(id) << shift_t;
-                uint32_t *w = reinterpret_cast<uint32_t *>(sortrec + pos);
-                w[0] |= static_cast<uint32_t>(k);              // the emit kernel left the target bits zero
-                w[1] |= static_cast<uint32_t>(k >> 32);
-            }
+    for (int u = 0; u < GA_IPT; ++u) {
+        const int i = u * GA_THREADS + tid;
+        if (i >= n) continue;
+        const uint32_t id = a.dest ? s_id[i] : __ldcs(a.in + base + i);
+        if (MODE == 0) __stcs(a.out + base + i, id);
+        else if (MODE == 1) a.o_tgt[a.pos[base + i]] = static_cast<int32_t>(id);
+        else {
+            const unsigned long long k = static_cast<unsigned long long>(id) << a.shift_t;
+            uint32_t *w = reinterpret_cast<uint32_t *>(a.sortrec + base + i);
+            w[0] |= static_cast<uint32_t>(k);                  // the emit kernel left the target bits zero
+            w[1] |= static_cast<uint32_t>(k >> 32);
         }
     }
 }
@@ -369,17 +418,6 @@ __global__ void rs_state_records(const int2 *__restrict__ pair, int64_t n, uint6
     const int2 p = pair[i];
     const unsigned long long key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
     out[i] = (key << ib) | static_cast<unsigned long long>(i);
-}
-
-__global__ void rs_set_u32(uint32_t *p, uint32_t v) { *p = v; }
-__global__ void rs_window_starts(int64_t *start, int n_win, int cshift) {
-    const int w = blockIdx.x * blockDim.x + threadIdx.x;
-    if (w <= n_win) start[w] = static_cast<int64_t>(w) << cshift;
-}
-
-__global__ void rs_compact_counts(const uint32_t *__restrict__ cursor, int cur_stride, int64_t nb, uint32_t *__restrict__ cnt) {
-    const int64_t g = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (g < nb) cnt[g] = cursor[static_cast<size_t>(g) * cur_stride];
 }
 
 // ------------------------------------------------------------------------------------------ host side
@@ -404,7 +442,7 @@ struct RsTrace {
             float ms = 0.f;
             cudaEventSynchronize(s.b);
             cudaEventElapsedTime(&ms, s.a, s.b);
-            fprintf(stderr, "[fstc resolve] %-22s n=%-11lld %8.3f ms\n", s.name, static_cast<long long>(s.n), ms);
+            fprintf(stderr, "[fstc resolve] %-14s n=%-11lld %8.3f ms\n", s.name, static_cast<long long>(s.n), ms);
             cudaEventDestroy(s.a); cudaEventDestroy(s.b);
         }
         spans.clear();
@@ -415,6 +453,7 @@ thread_local RsTrace g_trace;
 struct SegSet {                       // device arrays of a segmented record stream
     DBuf<unsigned long long> own;     // storage, unless the stream borrows the caller's buffer
     const unsigned long long *data = nullptr;
+    int64_t length = 0;               // records the buffer spans (segments + gaps)
     DBuf<int64_t> start;              // [n_seg + 1]
     DBuf<uint32_t> cnt;               // [n_seg]
     int64_t n_seg = 0;
@@ -424,6 +463,7 @@ struct SegSet {                       // device arrays of a segmented record str
 SegSet single_segment(Ctx &c, const unsigned long long *data, int64_t n) {
     SegSet s;
     s.data = data;
+    s.length = n;
     s.n_seg = 1;
     s.start.alloc(c, 2);
     s.cnt.alloc(c, 1);
@@ -435,14 +475,14 @@ SegSet single_segment(Ctx &c, const unsigned long long *data, int64_t n) {
 }
 
 // One staged scatter pass: every segment of `in` is split into `nbins` bins.  Bin capacities are a guess from
-// uniform hashing (or `fixed_cap`); if a bin overflows, the cursors of the failed attempt hold the exact counts
-// and the pass runs once more with those.
-template <int FN>
-SegSet scatter_pass(Ctx &c, const SegSet &in, int shift, int hshift, int nbins, uint32_t fixed_cap) {
+// uniform hashing; if a bin overflows, the cursors of the failed attempt hold the exact counts and the pass runs
+// once more with those.  dest (optional): [in.length], where every input record went.
+SegSet scatter_pass(Ctx &c, const SegSet &in, int shift, int hshift, int nbins, DBuf<uint32_t> *dest, DBuf<uint16_t> *perm) {
     if (in.n_seg > 1024 || nbins > SC_MAX_BINS) fail(FSTC_ERR_CAPACITY, "resolve: too many segments (%lld x %d)",
                                                     static_cast<long long>(in.n_seg), nbins);
     const int64_t nb = in.n_seg * nbins;
     const int cur_stride = nb <= 4096 ? 32 : 8;                  // hot counters sit in sectors of their own
+    const size_t smem = SC_TILE * (sizeof(unsigned long long) + sizeof(uint32_t));
     DBuf<int64_t> tile_first(c, in.n_seg + 1);
     rs_seg_tiles<<<1, 1024, 0, c.stream>>>(in.view(), SC_TILE, tile_first.p);
     FSTC_LAUNCH_CHECK();
@@ -451,29 +491,33 @@ SegSet scatter_pass(Ctx &c, const SegSet &in, int shift, int hshift, int nbins, 
     SegSet out;
     out.n_seg = nb;
     out.start.alloc(c, nb + 1);
+    if (dest) { dest->alloc(c, in.length); perm->alloc(c, in.length); }
     static bool attr_set = false;
     if (!attr_set) {
-        FSTC_CUDA(cudaFuncSetAttribute(rs_scatter<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, SC_TILE * 8));
-        FSTC_CUDA(cudaFuncSetAttribute(rs_scatter<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SC_TILE * 8));
+        FSTC_CUDA(cudaFuncSetAttribute(rs_scatter<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
+        FSTC_CUDA(cudaFuncSetAttribute(rs_scatter<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
         attr_set = true;
     }
     for (int attempt = 0;; ++attempt) {
-        rs_bin_caps<<<rs_blocks(nb), 256, 0, c.stream>>>(in.view(), nbins, 16, 192u, fixed_cap, cursor.p, cur_stride,
-                                                         attempt, cap.p);
+        rs_bin_caps<<<rs_blocks(nb), 256, 0, c.stream>>>(in.view(), nbins, 16, 192u, cursor.p, cur_stride, attempt, cap.p);
         FSTC_LAUNCH_CHECK();
         exclusive_scan<uint32_t>(c, cap.p, nb, out.start.p);
         int64_t totals[2];
         FSTC_CUDA(cudaMemcpyAsync(&totals[0], tile_first.p + in.n_seg, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
         FSTC_CUDA(cudaMemcpyAsync(&totals[1], out.start.p + nb, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
         c.sync();
+        if (totals[1] >= 0xFFFFFFFFll) fail(FSTC_ERR_CAPACITY, "resolve: more than 2^32 records in a pass");
         out.own.alloc(c, totals[1]);
         out.data = out.own.p;
+        out.length = totals[1];
         FSTC_CUDA(cudaMemsetAsync(cursor.p, 0, sizeof(uint32_t) * nb * cur_stride, c.stream));
         FSTC_CUDA(cudaMemsetAsync(flag.p, 0, sizeof(unsigned), c.stream));
         if (totals[0] > 0) {
-            ScatterArgs a{in.view(), tile_first.p, out.own.p, out.start.p, cursor.p, cur_stride, shift, hshift, nbins};
-            const int h = g_trace.begin(c, FN == 0 ? "scatter(key)" : "scatter(pos)", totals[0] * SC_TILE);
-            rs_scatter<FN><<<static_cast<unsigned>(totals[0]), SC_THREADS, SC_TILE * 8, c.stream>>>(a);
+            ScatterArgs a{in.view(), tile_first.p, out.own.p, out.start.p, cursor.p, dest ? dest->p : nullptr, dest ? perm->p : nullptr,
+                          cur_stride, shift, hshift, nbins};
+            const int h = g_trace.begin(c, dest ? "scatter+dest" : "scatter", totals[0] * SC_TILE);
+            if (dest) rs_scatter<true><<<static_cast<unsigned>(totals[0]), SC_THREADS, smem, c.stream>>>(a);
+            else rs_scatter<false><<<static_cast<unsigned>(totals[0]), SC_THREADS, smem, c.stream>>>(a);
             FSTC_LAUNCH_CHECK();
             g_trace.end(c, h);
         }
@@ -490,12 +534,24 @@ SegSet scatter_pass(Ctx &c, const SegSet &in, int shift, int hshift, int nbins, 
     return out;
 }
 
-// hash partition of a record stream into 2^(b1+b2) bins (b1 = the top hash bits, then b2)
-SegSet partition_by_key(Ctx &c, const unsigned long long *recs, int64_t n, int shift, int b1, int b2) {
-    SegSet cur = single_segment(c, recs, n);
-    if (b1 > 0) cur = scatter_pass<0>(c, cur, shift, 64 - b1, 1 << b1, 0);
-    if (b2 > 0) cur = scatter_pass<0>(c, cur, shift, 64 - b1 - b2, 1 << b2, 0);
-    return cur;
+// undoes one scatter pass (or, with dest = null, just delivers the ids): see rs_gather_ids
+void gather_pass(Ctx &c, const SegSet &seg, int mode, GatherArgs a) {
+    DBuf<int64_t> tile_first(c, seg.n_seg + 1);
+    rs_seg_tiles<<<1, 1024, 0, c.stream>>>(seg.view(), SC_TILE, tile_first.p);
+    FSTC_LAUNCH_CHECK();
+    const int64_t tiles = read_scalar(c, tile_first.p + seg.n_seg);
+    a.seg = seg.view();
+    a.tile_first = tile_first.p;
+    if (tiles > 0) {
+        const int h = g_trace.begin(c, mode == 0 && a.dest ? "gather" : "apply", tiles * SC_TILE);
+        const unsigned grid = static_cast<unsigned>(tiles);
+        if (mode == 0) rs_gather_ids<0><<<grid, GA_THREADS, 0, c.stream>>>(a);
+        else if (mode == 1) rs_gather_ids<1><<<grid, GA_THREADS, 0, c.stream>>>(a);
+        else rs_gather_ids<2><<<grid, GA_THREADS, 0, c.stream>>>(a);
+        FSTC_LAUNCH_CHECK();
+        g_trace.end(c, h);
+    }
+    c.n_launch += 2;
 }
 
 }  // namespace
@@ -507,69 +563,59 @@ int resolve_bits_needed(int64_t n_records_and_states) {
 }
 
 void resolve_partitioned(Ctx &c, const ResolveJob &j) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        FSTC_CUDA(cudaFuncSetAttribute(rs_dedupe, cudaFuncAttributeMaxDynamicSharedMemorySize, DD_SLOTS * 12));
-        attr_set = true;
-    }
     const int ib = bits_for(static_cast<uint64_t>(j.n_states_before > 1 ? j.n_states_before - 1 : 1));
-    if (j.key_bits + ib > 64 || j.key_bits + j.pos_bits > 64 || j.pos_bits > 32)
-        fail(FSTC_ERR_CAPACITY, "resolve: key (%d bits) + id/position (%d/%d bits) exceed 64 bits", j.key_bits, ib, j.pos_bits);
+    if (j.key_bits + ib > 64) fail(FSTC_ERR_CAPACITY, "resolve: key (%d bits) + state id (%d bits) exceed 64 bits", j.key_bits, ib);
+    if (j.n_records >= 0xFFFFFFFFll) fail(FSTC_ERR_CAPACITY, "resolve: more than 2^32 records");
     int bits = j.force_bits >= 0 ? j.force_bits : resolve_bits_needed(j.n_states_before + j.n_records);
+    const uint64_t nq2_inv = j.nq2 > 1 ? ~0ull / j.nq2 : ~0ull;      // floor((2^64-1)/d): at most 1 below floor(2^64/d)
     for (;; ++bits) {
         if (bits > 20) fail(FSTC_ERR_CAPACITY, "resolve: more than 2^20 bins needed");
         const int b1 = bits < 10 ? bits : 10, b2 = bits - b1;
-        // 1-2. records of the existing states and of the arcs, partitioned the same way
+        // 1-2. records of the existing states and keys of the arcs, partitioned the same way
         DBuf<unsigned long long> st_recs(c, j.n_states_before);
         rs_state_records<<<rs_blocks(j.n_states_before), 256, 0, c.stream>>>(j.pair, j.n_states_before, j.nq2, ib, st_recs.p);
         FSTC_LAUNCH_CHECK();
         c.n_launch += 1;
-        SegSet st = partition_by_key(c, st_recs.p, j.n_states_before, ib, b1, b2);
+        SegSet st = single_segment(c, st_recs.p, j.n_states_before);
+        if (b1 > 0) st = scatter_pass(c, st, ib, 64 - b1, 1 << b1, nullptr, nullptr);
+        if (b2 > 0) st = scatter_pass(c, st, ib, 64 - b1 - b2, 1 << b2, nullptr, nullptr);
         if (bits > 0) st_recs.release();
-        SegSet arcs = partition_by_key(c, j.keypos, j.n_records, j.pos_bits, b1, b2);
+        SegSet lvl0 = single_segment(c, j.keys, j.n_records), lvl1, lvl2;
+        DBuf<uint32_t> dest1, dest2;
+        DBuf<uint16_t> perm1, perm2;
+        if (b1 > 0) lvl1 = scatter_pass(c, lvl0, 0, 64 - b1, 1 << b1, &dest1, &perm1);
+        if (b2 > 0) lvl2 = scatter_pass(c, lvl1, 0, 64 - b1 - b2, 1 << b2, &dest2, &perm2);
+        const SegSet &arcs = b2 > 0 ? lvl2 : (b1 > 0 ? lvl1 : lvl0);
         // 3. per-bin dedupe
         const int64_t nb = int64_t(1) << bits;
-        DBuf<int64_t> out_off(c, nb + 1);
-        exclusive_scan<uint32_t>(c, arcs.cnt.p, nb, out_off.p);
-        DBuf<unsigned long long> posid(c, j.n_records);
+        DBuf<uint32_t> ids_last(c, arcs.length);
         DBuf<unsigned> err(c, 1);
         FSTC_CUDA(cudaMemsetAsync(err.p, 0, sizeof(unsigned), c.stream));
         const unsigned long long n_before = static_cast<unsigned long long>(j.n_states_before);
         FSTC_CUDA(cudaMemcpyAsync(j.n_states, &n_before, sizeof n_before, cudaMemcpyHostToDevice, c.stream));
-        DedupeArgs d{st.view(), arcs.view(), ib, j.pos_bits, out_off.p, posid.p, j.nq2, j.n_states, j.pair, err.p};
+        DedupeArgs d{st.view(), arcs.view(), ib, ids_last.p, j.nq2, nq2_inv, j.n_states, j.pair, err.p};
         const int hd = g_trace.begin(c, "dedupe", nb);
-        rs_dedupe<<<static_cast<unsigned>(nb), DD_THREADS, DD_SLOTS * 12, c.stream>>>(d);
+        rs_dedupe<<<static_cast<unsigned>(nb), DD_THREADS, 0, c.stream>>>(d);
         FSTC_LAUNCH_CHECK();
         g_trace.end(c, hd);
         c.n_launch += 1;
-        if (read_scalar(c, err.p)) continue;                     // a bin outgrew shared memory: halve the bins, again
+        if (read_scalar(c, err.p)) continue;                     // a bin outgrew shared memory: twice the bins, again
         st = SegSet();
-        arcs = SegSet();
-        // 4. ids back to the target column, one position window at a time
-        const int pbits = bits_for(static_cast<uint64_t>(j.n_positions > 1 ? j.n_positions - 1 : 1));
-        const int cshift = pbits - 10 > 22 ? pbits - 10 : 22;
-        const int n_win = static_cast<int>(((j.n_positions > 0 ? j.n_positions : 1) + (int64_t(1) << cshift) - 1) >> cshift);
-        SegSet win = single_segment(c, posid.p, j.n_records);
-        if (n_win > 1) {
-            win = scatter_pass<1>(c, win, 0, cshift, n_win, static_cast<uint32_t>(1u << cshift));
-            posid.release();
+        // 4. ids back through the passes
+        const uint32_t *ids = ids_last.p;
+        DBuf<uint32_t> ids_mid;
+        if (b2 > 0) {
+            lvl2 = SegSet();
+            ids_mid.alloc(c, lvl1.length);
+            GatherArgs g{};
+            g.dest = dest2.p; g.perm = perm2.p; g.in = ids_last.p; g.out = ids_mid.p;
+            gather_pass(c, lvl1, 0, g);
+            ids = ids_mid.p;
         }
-        DBuf<int64_t> tile_first(c, win.n_seg + 1);
-        rs_seg_tiles<<<1, 1024, 0, c.stream>>>(win.view(), SI_TILE, tile_first.p);
-        FSTC_LAUNCH_CHECK();
-        const int64_t tiles = read_scalar(c, tile_first.p + win.n_seg);
-        const int hs = g_trace.begin(c, "scatter_ids", tiles * SI_TILE);
-        if (tiles > 0) {
-            if (j.sortrec)
-                rs_scatter_ids<1><<<static_cast<unsigned>(tiles), SI_THREADS, 0, c.stream>>>(win.view(), tile_first.p, nullptr,
-                                                                                          j.sortrec, j.shift_t);
-            else
-                rs_scatter_ids<0><<<static_cast<unsigned>(tiles), SI_THREADS, 0, c.stream>>>(win.view(), tile_first.p, j.o_tgt,
-                                                                                          nullptr, 0);
-            FSTC_LAUNCH_CHECK();
-        }
-        g_trace.end(c, hs);
-        c.n_launch += 2;
+        GatherArgs g{};
+        g.dest = b1 > 0 ? dest1.p : nullptr; g.perm = perm1.p; g.in = ids;
+        g.out = reinterpret_cast<uint32_t *>(j.o_tgt); g.pos = j.pos; g.o_tgt = j.o_tgt; g.sortrec = j.sortrec; g.shift_t = j.shift_t;
+        gather_pass(c, lvl0, j.mode, g);
         c.sync();                                                // temporaries are released below
         if (g_trace.on) g_trace.report();
         return;
