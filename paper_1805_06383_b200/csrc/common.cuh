@@ -7,6 +7,8 @@
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
+#include <ctime>
 #include <string>
 #include <utility>
 
@@ -43,6 +45,11 @@ struct Error {
 // One library-owned memory pool per device: freed blocks stay cached (release threshold = max),
 // so repeated compositions do not go back to the driver for memory.
 cudaMemPool_t device_pool();
+// cache of big (>= 64 MB) blocks in front of the pool (api.cu): big_alloc returns null if `bytes` is small or memory is out
+void *big_alloc(size_t bytes, cudaStream_t stream);
+bool big_free(void *p, cudaStream_t stream);   // true if p was a big block (now parked for reuse on that stream)
+void big_forget(void *p);        // p is handed to the caller (result arrays are released with cudaFreeAsync)
+void big_release_all();
 
 struct Ctx {
     cudaStream_t stream = nullptr;
@@ -52,7 +59,16 @@ struct Ctx {
     void *alloc_bytes(size_t bytes) {
         if (bytes == 0) bytes = 16;
         void *p = nullptr;
-        cudaError_t e = cudaMallocFromPoolAsync(&p, bytes, device_pool(), stream);
+        static const bool trace = getenv("FSTC_ALLOC_TRACE") != nullptr;       // debug knob: host time of big allocations
+        timespec t0, t1;
+        if (trace) clock_gettime(CLOCK_MONOTONIC, &t0);
+        p = big_alloc(bytes, stream);
+        cudaError_t e = p ? cudaSuccess : cudaMallocFromPoolAsync(&p, bytes, device_pool(), stream);
+        if (trace && bytes >= (64u << 20)) {
+            clock_gettime(CLOCK_MONOTONIC, &t1);
+            fprintf(stderr, "[fstc alloc] %8.1f MB  %8.3f ms\n", bytes / 1048576.0,
+                    (t1.tv_sec - t0.tv_sec) * 1e3 + (t1.tv_nsec - t0.tv_nsec) * 1e-6);
+        }
         if (e != cudaSuccess) {
             (void)cudaGetLastError();
             fail(e == cudaErrorMemoryAllocation ? FSTC_ERR_OOM : FSTC_ERR_CUDA,
@@ -61,7 +77,16 @@ struct Ctx {
         return p;
     }
     void free_bytes(void *p) {
-        if (p) (void)cudaFreeAsync(p, stream);
+        if (!p) return;
+        static const bool trace = getenv("FSTC_ALLOC_TRACE") != nullptr;
+        timespec t0, t1;
+        if (trace) clock_gettime(CLOCK_MONOTONIC, &t0);
+        if (!big_free(p, stream)) (void)cudaFreeAsync(p, stream);
+        if (trace) {
+            clock_gettime(CLOCK_MONOTONIC, &t1);
+            const double ms = (t1.tv_sec - t0.tv_sec) * 1e3 + (t1.tv_nsec - t0.tv_nsec) * 1e-6;
+            if (ms > 0.2) fprintf(stderr, "[fstc free]  %8.3f ms\n", ms);
+        }
     }
     void sync() { FSTC_CUDA(cudaStreamSynchronize(stream)); }
 };
@@ -97,7 +122,7 @@ struct DBuf {
         p = nullptr;
         n = 0;
     }
-    T *take() { T *q = p; p = nullptr; n = 0; return q; }
+    T *take() { T *q = p; p = nullptr; n = 0; big_forget(q); return q; }
     operator T *() const { return p; }
 };
 

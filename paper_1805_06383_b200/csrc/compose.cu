@@ -1069,7 +1069,12 @@ fstc_result_t *Composer::run() {
             }
         }
         ensure_pairs(n_states + new_bound, n_states + new_bound + next_S);
-        if (!partitioned) ensure_table(n_states + new_bound, n_states + new_bound + next_S);
+        if (!partitioned) {
+            // no look-ahead for the table if the next level will leave it for the partitioned resolve anyway
+            const bool next_partitioned = o.resolve_mode == FSTC_RESOLVE_AUTO && next_R >= RESOLVE_MIN_ARCS &&
+                                          slots_for(n_states + new_bound + next_S) * sizeof(uint4) > RESOLVE_TABLE_BYTES;
+            ensure_table(n_states + new_bound, next_partitioned ? 0 : n_states + new_bound + next_S);
+        }
         ensure_arcs(n_arcs + R, n_arcs + R + next_R);
         n_states_live = n_states;
 

@@ -18,6 +18,7 @@
 //
 // Nothing persists between levels except pair[] (id -> (q1,q2)): the key->id map is rebuilt per level from it.
 #include <cstdlib>
+#include <ctime>
 #include <vector>
 
 #include "internal.h"
@@ -425,12 +426,15 @@ inline unsigned rs_blocks(int64_t n, int threads = 256) { return static_cast<uns
 
 // FSTC_RS_TRACE=1 prints the device time of every resolve kernel to stderr (debug knob, off by default)
 struct RsTrace {
-    struct Span { const char *name; int64_t n; cudaEvent_t a, b; };
+    struct Span { const char *name; int64_t n; cudaEvent_t a, b; double host_us; unsigned long long reserved; };
     std::vector<Span> spans;
     bool on = getenv("FSTC_RS_TRACE") != nullptr;
     int begin(Ctx &c, const char *name, int64_t n) {
         if (!on) return -1;
-        Span s{name, n, nullptr, nullptr};
+        Span s{name, n, nullptr, nullptr, 0.0, 0ull};
+        timespec ts; clock_gettime(CLOCK_MONOTONIC, &ts);
+        s.host_us = ts.tv_sec * 1e6 + ts.tv_nsec * 1e-3;
+        (void)cudaMemPoolGetAttribute(device_pool(), cudaMemPoolAttrReservedMemCurrent, &s.reserved);
         cudaEventCreate(&s.a); cudaEventCreate(&s.b);
         cudaEventRecord(s.a, c.stream);
         spans.push_back(s);
@@ -439,12 +443,14 @@ struct RsTrace {
     void end(Ctx &c, int h) { if (h >= 0) cudaEventRecord(spans[h].b, c.stream); }
     void report() {
         for (auto &s : spans) {
-            float ms = 0.f;
+            float ms = 0.f, at = 0.f;
             cudaEventSynchronize(s.b);
             cudaEventElapsedTime(&ms, s.a, s.b);
-            fprintf(stderr, "[fstc resolve] %-14s n=%-11lld %8.3f ms\n", s.name, static_cast<long long>(s.n), ms);
-            cudaEventDestroy(s.a); cudaEventDestroy(s.b);
+            cudaEventElapsedTime(&at, spans[0].a, s.a);
+            fprintf(stderr, "[fstc resolve] %-18s n=%-11lld at %8.3f  %8.3f ms   host at %9.3f ms  pool %.2f GB\n", s.name,
+                    static_cast<long long>(s.n), at, ms, (s.host_us - spans[0].host_us) * 1e-3, s.reserved / 1e9);
         }
+        for (auto &s : spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
         spans.clear();
     }
 };
@@ -568,6 +574,7 @@ void resolve_partitioned(Ctx &c, const ResolveJob &j) {
     if (j.n_records >= 0xFFFFFFFFll) fail(FSTC_ERR_CAPACITY, "resolve: more than 2^32 records");
     int bits = j.force_bits >= 0 ? j.force_bits : resolve_bits_needed(j.n_states_before + j.n_records);
     const uint64_t nq2_inv = j.nq2 > 1 ? ~0ull / j.nq2 : ~0ull;      // floor((2^64-1)/d): at most 1 below floor(2^64/d)
+    const int h_all = g_trace.begin(c, "RESOLVE TOTAL", j.n_records);
     for (;; ++bits) {
         if (bits > 20) fail(FSTC_ERR_CAPACITY, "resolve: more than 2^20 bins needed");
         const int b1 = bits < 10 ? bits : 10, b2 = bits - b1;
@@ -580,13 +587,18 @@ void resolve_partitioned(Ctx &c, const ResolveJob &j) {
         if (b1 > 0) st = scatter_pass(c, st, ib, 64 - b1, 1 << b1, nullptr, nullptr);
         if (b2 > 0) st = scatter_pass(c, st, ib, 64 - b1 - b2, 1 << b2, nullptr, nullptr);
         if (bits > 0) st_recs.release();
+        const int h_st = g_trace.begin(c, "(states done)", 0); g_trace.end(c, h_st);
         SegSet lvl0 = single_segment(c, j.keys, j.n_records), lvl1, lvl2;
         DBuf<uint32_t> dest1, dest2;
         DBuf<uint16_t> perm1, perm2;
         if (b1 > 0) lvl1 = scatter_pass(c, lvl0, 0, 64 - b1, 1 << b1, &dest1, &perm1);
-        if (b2 > 0) lvl2 = scatter_pass(c, lvl1, 0, 64 - b1 - b2, 1 << b2, &dest2, &perm2);
+        if (b2 > 0) {
+            lvl2 = scatter_pass(c, lvl1, 0, 64 - b1 - b2, 1 << b2, &dest2, &perm2);
+            lvl1.own.release();                                  // only the segment table of level 1 is needed from here on
+        }
         const SegSet &arcs = b2 > 0 ? lvl2 : (b1 > 0 ? lvl1 : lvl0);
         // 3. per-bin dedupe
+        const int h_ar = g_trace.begin(c, "(arcs partitioned)", 0); g_trace.end(c, h_ar);
         const int64_t nb = int64_t(1) << bits;
         DBuf<uint32_t> ids_last(c, arcs.length);
         DBuf<unsigned> err(c, 1);
@@ -616,6 +628,7 @@ void resolve_partitioned(Ctx &c, const ResolveJob &j) {
         g.dest = b1 > 0 ? dest1.p : nullptr; g.perm = perm1.p; g.in = ids;
         g.out = reinterpret_cast<uint32_t *>(j.o_tgt); g.pos = j.pos; g.o_tgt = j.o_tgt; g.sortrec = j.sortrec; g.shift_t = j.shift_t;
         gather_pass(c, lvl0, j.mode, g);
+        g_trace.end(c, h_all);
         c.sync();                                                // temporaries are released below
         if (g_trace.on) g_trace.report();
         return;
