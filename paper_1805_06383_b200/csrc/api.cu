@@ -1,4 +1,5 @@
 // C ABI of libfstc (include/fstc.h): argument checks, error translation, the device memory pool.
+#include <map>
 #include <mutex>
 #include <unordered_map>
 #include <vector>
@@ -33,71 +34,191 @@ cudaMemPool_t device_pool() {
     return g_pools[dev];
 }
 
-// ---- cache of big device blocks.  cudaMallocFromPoolAsync of several GB takes 1-2 ms per GB on the host whenever
-// the pool cannot hand back a block it already has in one piece (measured: 9.7 ms for 8.5 GB), and a composition
-// allocates the same big temporaries level after level, call after call.  Blocks >= 64 MB are therefore parked here
-// when released and handed out again to a request they fit closely ON THE SAME STREAM, so reuse is stream-ordered
-// like the pool's own.
+// ---- workspace arena.  cudaMallocFromPoolAsync of a multi-GB block takes 1-5 ms per GB on the host whenever the
+// pool cannot hand back a block it already holds in one piece (measured: 9.7 ms for 8.5 GB, far more under memory
+// pressure), and a composition allocates dozens of big temporaries per level.  Temporaries are therefore carved out
+// of a few large chunks that the library keeps (first fit, free neighbours coalesce); only the arrays that leave the
+// library (results, packed operands) are separate pool allocations.  One arena per host thread: a thread's calls run
+// one after the other and each ends with a synchronisation of its stream, so a freed range is idle before any later
+// call reuses it; inside a call everything is ordered on one stream.  fstc_trim_pool releases the chunks.
 namespace {
-struct BigBlock { void *p; size_t bytes; int dev; cudaStream_t stream; };
-std::mutex g_cache_mu;
-std::vector<BigBlock> g_parked;
-std::unordered_map<void *, size_t> g_big_live;           // size of every live block that came through big_alloc
-constexpr size_t BIG_BYTES = size_t(64) << 20;
-}  // namespace
-
-void *big_alloc(size_t bytes, cudaStream_t stream) {
-    if (bytes < BIG_BYTES) return nullptr;
+struct ArenaChunk {
+    char *base = nullptr;
+    size_t size = 0;
     int dev = 0;
-    (void)cudaGetDevice(&dev);
-    std::lock_guard<std::mutex> lk(g_cache_mu);
-    int best = -1;
-    for (size_t i = 0; i < g_parked.size(); ++i) {
-        const BigBlock &b = g_parked[i];
-        if (b.dev == dev && b.stream == stream && b.bytes >= bytes && b.bytes <= bytes + bytes / 8 + (size_t(1) << 20) &&
-            (best < 0 || b.bytes < g_parked[best].bytes))
-            best = static_cast<int>(i);
-    }
-    void *p = nullptr;
-    size_t got = bytes;
-    if (best >= 0) {
-        p = g_parked[best].p;
-        got = g_parked[best].bytes;
-        g_parked.erase(g_parked.begin() + best);
-    } else {
-        cudaError_t e = cudaMallocFromPoolAsync(&p, bytes, device_pool(), stream);
-        if (e != cudaSuccess) {                            // out of memory: give the parked blocks back and try again
-            (void)cudaGetLastError();
-            for (auto &b : g_parked) (void)cudaFreeAsync(b.p, stream);
-            g_parked.clear();
-            e = cudaMallocFromPoolAsync(&p, bytes, device_pool(), stream);
-            if (e != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
-        }
-    }
-    g_big_live[p] = got;
+    std::map<size_t, size_t> free_ranges;                  // offset -> length
+};
+struct Arena {
+    std::vector<ArenaChunk> chunks;
+    std::unordered_map<void *, std::pair<int, size_t>> live;   // pointer -> (chunk, length)
+    ~Arena() {}                                             // chunks die with the context
+};
+thread_local Arena g_arena;
+constexpr size_t ARENA_ALIGN = 512;
+constexpr size_t ARENA_MIN_CHUNK = size_t(1) << 30;
+
+// carves `bytes` out of the free range at `off` of chunk ci
+void *arena_carve(int ci, size_t off, size_t bytes) {
+    ArenaChunk &ch = g_arena.chunks[ci];
+    auto it = ch.free_ranges.find(off);
+    const size_t len = it->second;
+    ch.free_ranges.erase(it);
+    if (len > bytes) ch.free_ranges[off + bytes] = len - bytes;
+    void *p = ch.base + off;
+    g_arena.live[p] = {ci, bytes};
     return p;
 }
+}  // namespace
 
-bool big_free(void *p, cudaStream_t stream) {
+void arena_release_all() {
+    for (auto &ch : g_arena.chunks)
+        if (ch.base) (void)cudaFreeAsync(ch.base, nullptr);
+    g_arena.chunks.clear();
+    g_arena.live.clear();
+}
+
+void *arena_alloc(size_t bytes, cudaStream_t stream) {
+    bytes = (bytes + ARENA_ALIGN - 1) / ARENA_ALIGN * ARENA_ALIGN;
     int dev = 0;
     (void)cudaGetDevice(&dev);
-    std::lock_guard<std::mutex> lk(g_cache_mu);
-    auto it = g_big_live.find(p);
-    if (it == g_big_live.end()) return false;
-    g_parked.push_back(BigBlock{p, it->second, dev, stream});
-    g_big_live.erase(it);
+    // best fit over all chunks: small requests fill small holes and leave the large ranges whole, so a caller that
+    // repeats the same sequence of requests finds the same layout again
+    int best_ci = -1;
+    size_t best_off = 0, best_len = ~size_t(0);
+    for (size_t ci = 0; ci < g_arena.chunks.size(); ++ci) {
+        if (g_arena.chunks[ci].dev != dev) continue;
+        for (auto &r : g_arena.chunks[ci].free_ranges)
+            if (r.second >= bytes && r.second < best_len) { best_ci = static_cast<int>(ci); best_off = r.first; best_len = r.second; }
+    }
+    if (best_ci >= 0) return arena_carve(best_ci, best_off, bytes);
+    ArenaChunk ch;
+    ch.size = bytes > ARENA_MIN_CHUNK ? bytes : ARENA_MIN_CHUNK;
+    ch.dev = dev;
+    void *base = nullptr;
+    cudaError_t e = cudaMallocFromPoolAsync(&base, ch.size, device_pool(), stream);
+    if (e != cudaSuccess && ch.size > bytes) {             // no room for a whole chunk: just what is asked for
+        (void)cudaGetLastError();
+        ch.size = bytes;
+        e = cudaMallocFromPoolAsync(&base, ch.size, device_pool(), stream);
+    }
+    if (e != cudaSuccess) {                                // still none: drop the chunks nobody uses, once
+        (void)cudaGetLastError();
+        bool dropped = false;
+        for (auto &c2 : g_arena.chunks)
+            if (c2.base && c2.free_ranges.size() == 1 && c2.free_ranges.begin()->second == c2.size) {
+                (void)cudaFreeAsync(c2.base, stream);
+                c2.base = nullptr; c2.size = 0; c2.free_ranges.clear();
+                dropped = true;
+            }
+        if (dropped) e = cudaMallocFromPoolAsync(&base, ch.size, device_pool(), stream);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+    }
+    ch.base = static_cast<char *>(base);
+    ch.free_ranges[0] = ch.size;
+    g_arena.chunks.push_back(std::move(ch));
+    return arena_carve(static_cast<int>(g_arena.chunks.size()) - 1, 0, bytes);
+}
+
+bool arena_free(void *p) {
+    auto it = g_arena.live.find(p);
+    if (it == g_arena.live.end()) return false;
+    ArenaChunk &ch = g_arena.chunks[it->second.first];
+    size_t off = static_cast<char *>(p) - ch.base, len = it->second.second;
+    g_arena.live.erase(it);
+    auto nxt = ch.free_ranges.lower_bound(off);
+    if (nxt != ch.free_ranges.end() && off + len == nxt->first) {   // merge with the free range behind
+        len += nxt->second;
+        nxt = ch.free_ranges.erase(nxt);
+    }
+    if (nxt != ch.free_ranges.begin()) {                            // and with the one in front
+        auto prv = std::prev(nxt);
+        if (prv->first + prv->second == off) { prv->second += len; return true; }
+    }
+    ch.free_ranges[off] = len;
     return true;
 }
 
-void big_forget(void *p) {                                 // the block leaves the library's hands (a result array)
-    std::lock_guard<std::mutex> lk(g_cache_mu);
-    g_big_live.erase(p);
+// ---- arrays that leave the library (results, packed operands, and the growing output arrays on the way there).
+// They are pool allocations of their own; when one is released it is parked, with an event that marks the point of
+// release, and the next request of (nearly) the same size takes it over after waiting on that event.  A caller that
+// composes in a loop thus gets the same blocks back instead of paying the pool's multi-millisecond path every time.
+namespace {
+struct ParkedBlock { void *p; size_t bytes; int dev; cudaEvent_t ev; };
+std::mutex g_park_mu;
+std::vector<ParkedBlock> g_parked;
+std::unordered_map<void *, size_t> g_persist_size;
+size_t g_parked_bytes = 0;
+constexpr size_t PARK_MIN_BYTES = size_t(32) << 20;
+constexpr size_t PARK_MAX_TOTAL = size_t(64) << 30;
+}  // namespace
+
+void *persist_alloc(size_t bytes, cudaStream_t stream) {
+    int dev = 0;
+    (void)cudaGetDevice(&dev);
+    void *p = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(g_park_mu);
+        int best = -1;
+        for (size_t i = 0; i < g_parked.size(); ++i) {
+            const ParkedBlock &b = g_parked[i];
+            if (b.dev == dev && b.bytes >= bytes && b.bytes <= bytes + bytes / 8 && (best < 0 || b.bytes < g_parked[best].bytes))
+                best = static_cast<int>(i);
+        }
+        if (best >= 0) {
+            ParkedBlock b = g_parked[best];
+            g_parked.erase(g_parked.begin() + best);
+            g_parked_bytes -= b.bytes;
+            (void)cudaStreamWaitEvent(stream, b.ev, 0);
+            (void)cudaEventDestroy(b.ev);
+            g_persist_size[b.p] = b.bytes;
+            return b.p;
+        }
+    }
+    cudaError_t e = cudaMallocFromPoolAsync(&p, bytes, device_pool(), stream);
+    if (e != cudaSuccess) {                                // out of memory: hand the parked blocks back, once
+        (void)cudaGetLastError();
+        persist_release_all();
+        e = cudaMallocFromPoolAsync(&p, bytes, device_pool(), stream);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+    }
+    if (bytes >= PARK_MIN_BYTES) {
+        std::lock_guard<std::mutex> lk(g_park_mu);
+        g_persist_size[p] = bytes;
+    }
+    return p;
 }
 
-void big_release_all() {
-    std::lock_guard<std::mutex> lk(g_cache_mu);
-    for (auto &b : g_parked) (void)cudaFreeAsync(b.p, nullptr);
+void persist_free(void *p, cudaStream_t stream) {
+    if (!p) return;
+    int dev = 0;
+    (void)cudaGetDevice(&dev);
+    {
+        std::lock_guard<std::mutex> lk(g_park_mu);
+        auto it = g_persist_size.find(p);
+        if (it != g_persist_size.end()) {
+            const size_t bytes = it->second;
+            g_persist_size.erase(it);
+            cudaEvent_t ev;
+            if (g_parked_bytes + bytes <= PARK_MAX_TOTAL &&
+                cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) == cudaSuccess) {
+                (void)cudaEventRecord(ev, stream);         // the legacy stream (null) orders after all blocking streams
+                g_parked.push_back(ParkedBlock{p, bytes, dev, ev});
+                g_parked_bytes += bytes;
+                return;
+            }
+        }
+    }
+    (void)cudaFreeAsync(p, stream);
+}
+
+void persist_release_all() {
+    std::lock_guard<std::mutex> lk(g_park_mu);
+    for (auto &b : g_parked) {
+        (void)cudaFreeAsync(b.p, nullptr);
+        (void)cudaEventDestroy(b.ev);
+    }
     g_parked.clear();
+    g_parked_bytes = 0;
 }
 
 namespace {
@@ -245,7 +366,8 @@ void fstc_result_free(fstc_result_t *r) { free_result(r); }
 int fstc_trim_pool(void) {
     return guarded([&] {
         FSTC_CUDA(cudaDeviceSynchronize());
-        big_release_all();
+        arena_release_all();
+        persist_release_all();
         FSTC_CUDA(cudaDeviceSynchronize());
         FSTC_CUDA(cudaMemPoolTrimTo(device_pool(), 0));
     });

@@ -45,25 +45,30 @@ struct Error {
 // One library-owned memory pool per device: freed blocks stay cached (release threshold = max),
 // so repeated compositions do not go back to the driver for memory.
 cudaMemPool_t device_pool();
-// cache of big (>= 64 MB) blocks in front of the pool (api.cu): big_alloc returns null if `bytes` is small or memory is out
-void *big_alloc(size_t bytes, cudaStream_t stream);
-bool big_free(void *p, cudaStream_t stream);   // true if p was a big block (now parked for reuse on that stream)
-void big_forget(void *p);        // p is handed to the caller (result arrays are released with cudaFreeAsync)
-void big_release_all();
+// workspace arena of the calling thread (api.cu): temporaries are carved out of a few large chunks the library keeps
+void *arena_alloc(size_t bytes, cudaStream_t stream);   // null when device memory is out
+bool arena_free(void *p);                               // false if p is not an arena block
+void arena_release_all();
+// blocks that outlive a call (api.cu): pool allocations, parked on release and handed out again to a like-sized request
+void *persist_alloc(size_t bytes, cudaStream_t stream);   // null when device memory is out
+void persist_free(void *p, cudaStream_t stream);
+void persist_release_all();
 
 struct Ctx {
     cudaStream_t stream = nullptr;
     int n_sm = 148;
     int64_t n_launch = 0;
 
-    void *alloc_bytes(size_t bytes) {
+    // persistent: the block outlives the call (a result or packed array): a pool allocation of its own
+    void *alloc_bytes(size_t bytes, bool persistent = false) {
         if (bytes == 0) bytes = 16;
         void *p = nullptr;
         static const bool trace = getenv("FSTC_ALLOC_TRACE") != nullptr;       // debug knob: host time of big allocations
         timespec t0, t1;
         if (trace) clock_gettime(CLOCK_MONOTONIC, &t0);
-        p = big_alloc(bytes, stream);
-        cudaError_t e = p ? cudaSuccess : cudaMallocFromPoolAsync(&p, bytes, device_pool(), stream);
+        cudaError_t e = cudaSuccess;
+        p = persistent ? persist_alloc(bytes, stream) : arena_alloc(bytes, stream);
+        if (!p) e = cudaErrorMemoryAllocation;
         if (trace && bytes >= (64u << 20)) {
             clock_gettime(CLOCK_MONOTONIC, &t1);
             fprintf(stderr, "[fstc alloc] %8.1f MB  %8.3f ms\n", bytes / 1048576.0,
@@ -81,7 +86,7 @@ struct Ctx {
         static const bool trace = getenv("FSTC_ALLOC_TRACE") != nullptr;
         timespec t0, t1;
         if (trace) clock_gettime(CLOCK_MONOTONIC, &t0);
-        if (!big_free(p, stream)) (void)cudaFreeAsync(p, stream);
+        if (!arena_free(p)) persist_free(p, stream);
         if (trace) {
             clock_gettime(CLOCK_MONOTONIC, &t1);
             const double ms = (t1.tv_sec - t0.tv_sec) * 1e3 + (t1.tv_nsec - t0.tv_nsec) * 1e-6;
@@ -98,7 +103,7 @@ struct DBuf {
     int64_t n = 0;
     Ctx *ctx = nullptr;
     DBuf() = default;
-    DBuf(Ctx &c, int64_t count) { alloc(c, count); }
+    DBuf(Ctx &c, int64_t count, bool persistent = false) { alloc(c, count, persistent); }
     DBuf(const DBuf &) = delete;
     DBuf &operator=(const DBuf &) = delete;
     DBuf(DBuf &&o) noexcept : p(o.p), n(o.n), ctx(o.ctx) { o.p = nullptr; o.n = 0; }
@@ -111,18 +116,18 @@ struct DBuf {
         return *this;
     }
     ~DBuf() { release(); }
-    void alloc(Ctx &c, int64_t count) {
+    void alloc(Ctx &c, int64_t count, bool persistent = false) {
         release();
         ctx = &c;
         n = count;
-        p = static_cast<T *>(c.alloc_bytes(static_cast<size_t>(count > 0 ? count : 0) * sizeof(T)));
+        p = static_cast<T *>(c.alloc_bytes(static_cast<size_t>(count > 0 ? count : 0) * sizeof(T), persistent));
     }
     void release() {
         if (p && ctx) ctx->free_bytes(p);
         p = nullptr;
         n = 0;
     }
-    T *take() { T *q = p; p = nullptr; n = 0; big_forget(q); return q; }
+    T *take() { T *q = p; p = nullptr; n = 0; return q; }   // only for blocks allocated `persistent`
     operator T *() const { return p; }
 };
 

@@ -111,12 +111,13 @@ __device__ __forceinline__ void intersect(const MachineView &A, const MachineVie
 
 // class U = arcs go straight to the output; class F = arcs go through sort + reduce first
 __global__ void __launch_bounds__(CT_THREADS)
-k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, int merge_mode,
+k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_lo, int64_t nf,
+        const uint32_t *__restrict__ sel /* null: all pairs of the level */, int merge_mode,
         uint64_t nq2, uint64_t key_limit /* pairs with key >= key_limit are left uncounted (raw = 0) */,
         int64_t *__restrict__ rawU, int64_t *__restrict__ rawF, uint32_t *__restrict__ nmU, uint32_t *__restrict__ nmF) {
     int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (i < nf) {
-        int2 p = pair[f_lo + i];
+        int2 p = pair[f_lo + (sel ? sel[i] : i)];
         int64_t raw = 0;
         uint32_t nm = 0;
         const uint64_t key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
@@ -141,7 +142,8 @@ k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_l
 // so 32 lanes cannot overflow 32 bits) and issue ONE shared-memory atomic: the top digits, which are nearly
 // constant over the frontier, no longer serialise.
 __global__ void __launch_bounds__(CT_THREADS)
-k_cut_hist(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, uint64_t nq2, const int64_t *__restrict__ rawU,
+k_cut_hist(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, const uint32_t *__restrict__ sel, uint64_t nq2,
+           const int64_t *__restrict__ rawU,
            const int64_t *__restrict__ rawF, uint64_t prefix, int shift, unsigned long long *__restrict__ hist) {
     __shared__ unsigned long long h[256];
     h[threadIdx.x] = 0;
@@ -153,7 +155,7 @@ k_cut_hist(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, uint64_t nq2
         uint32_t digit = 0xFFFFu;                            // lanes without a contribution
         uint64_t r = 0;
         if (i < nf) {
-            int2 p = pair[f_lo + i];
+            int2 p = pair[f_lo + (sel ? sel[i] : i)];
             uint64_t key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
             uint64_t hi = (shift + 8 >= 64) ? 0 : (key >> (shift + 8));
             r = static_cast<uint64_t>(rawU[i] + (rawF ? rawF[i] : 0));
@@ -172,21 +174,22 @@ k_cut_hist(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, uint64_t nq2
 }
 
 // pairs with key >= cut are not expanded in this (last) level
-__global__ void k_apply_cut(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, uint64_t nq2, uint64_t cut,
+__global__ void k_apply_cut(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, const uint32_t *__restrict__ sel,
+                            uint64_t nq2, uint64_t cut,
                             int64_t *__restrict__ rawU, int64_t *__restrict__ rawF, uint32_t *__restrict__ nmU,
                             uint32_t *__restrict__ nmF, unsigned long long *__restrict__ n_selected) {
     int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    bool sel = false;
+    bool keep = false;
     if (i < nf) {
-        int2 p = pair[f_lo + i];
+        int2 p = pair[f_lo + (sel ? sel[i] : i)];
         uint64_t key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
-        sel = key < cut;
-        if (!sel) {
+        keep = key < cut;
+        if (!keep) {
             rawU[i] = 0; nmU[i] = 0;
             if (rawF) { rawF[i] = 0; nmF[i] = 0; }
         }
     }
-    unsigned b = __ballot_sync(0xffffffffu, sel);
+    unsigned b = __ballot_sync(0xffffffffu, keep);
     if ((threadIdx.x & 31) == 0 && b) atomicAdd(n_selected, static_cast<unsigned long long>(__popc(b)));
 }
 
@@ -197,7 +200,7 @@ struct MatchList {           // SoA work-list of one class
 };
 
 __global__ void __launch_bounds__(CT_THREADS)
-k_match(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_lo, int64_t nf,
+k_match(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, const uint32_t *__restrict__ sel,
         const uint32_t *__restrict__ nmU, const uint32_t *__restrict__ nmF, const int64_t *__restrict__ moffU,
         const int64_t *__restrict__ moffF, const int64_t *__restrict__ roffU, const int64_t *__restrict__ roffF,
         MatchList U, MatchList F,
@@ -206,7 +209,7 @@ k_match(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_l
     unsigned long long segs = 0, marcs = 0;
     const bool isF = i < nf && nmF && nmF[i] != 0;
     if (i < nf && (isF || nmU[i] != 0)) {
-        int2 p = pair[f_lo + i];
+        int2 p = pair[f_lo + (sel ? sel[i] : i)];
         MatchList L = isF ? F : U;
         int64_t m = isF ? moffF[i] : moffU[i];
         int64_t run = isF ? roffF[i] : roffU[i];
@@ -281,7 +284,8 @@ struct EmitArgs {
     int64_t n_matches;
     int64_t R;               // ranks [0, R)
     int64_t pos_base;        // DIRECT: output position of rank 0 (tiles are aligned on absolute positions)
-    int64_t f_lo;            // source id = f_lo + pair index
+    int64_t f_lo;            // source id = f_lo + pair index (through sel, if the level was compacted)
+    const uint32_t *sel;
     const int64_t *foff;     // INDIRECT: final position of the pair's first arc (relative to arc_base)
     const int64_t *roff;     // INDIRECT: rank of the pair's first arc
     int64_t arc_base;        // INDIRECT
@@ -505,11 +509,12 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
     }   // !KEYS
 
     // ---- write the composed arcs
+#define SRC(u) (g.sel ? g.sel[pl[u]] : pl[u])
     if (MODE == EMIT_DIRECT) {
         if (n_valid == EM_IPT) {                               // whole aligned group: 16-byte stores
             const int64_t q = my_pos;
-            __stcs(reinterpret_cast<int4 *>(g.o_src + q), make_int4(static_cast<int>(g.f_lo + pl[0]), static_cast<int>(g.f_lo + pl[1]),
-                                                                   static_cast<int>(g.f_lo + pl[2]), static_cast<int>(g.f_lo + pl[3])));
+            __stcs(reinterpret_cast<int4 *>(g.o_src + q), make_int4(static_cast<int>(g.f_lo + SRC(0)), static_cast<int>(g.f_lo + SRC(1)),
+                                                                   static_cast<int>(g.f_lo + SRC(2)), static_cast<int>(g.f_lo + SRC(3))));
             __stcs(reinterpret_cast<uint4 *>(g.o_il + q), make_uint4(a_sym[0], a_sym[1], a_sym[2], a_sym[3]));
             __stcs(reinterpret_cast<uint4 *>(g.o_ol + q), make_uint4(b_sym[0], b_sym[1], b_sym[2], b_sym[3]));
             if (!KEYS) __stcs(reinterpret_cast<uint4 *>(g.o_tgt + q), make_uint4(id[0], id[1], id[2], id[3]));
@@ -519,7 +524,7 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
             for (int u = 0; u < EM_IPT; ++u) {
                 if (u >= skip && u < skip + n_valid) {
                     const int64_t q = my_pos + u;
-                    g.o_src[q] = static_cast<int>(g.f_lo + pl[u]);
+                    g.o_src[q] = static_cast<int>(g.f_lo + SRC(u));
                     g.o_il[q] = a_sym[u]; g.o_ol[q] = b_sym[u]; g.o_w[q] = w[u];
                     if (!KEYS) g.o_tgt[q] = id[u];
                 }
@@ -531,7 +536,7 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
             if (u >= skip && u < skip + n_valid) {
                 const int64_t rank = rank0 + u;
                 const int64_t q = g.arc_base + g.foff[pl[u]] + (rank - g.roff[pl[u]]);
-                g.o_src[q] = static_cast<int>(g.f_lo + pl[u]);
+                g.o_src[q] = static_cast<int>(g.f_lo + SRC(u));
                 g.o_il[q] = a_sym[u]; g.o_ol[q] = b_sym[u]; g.o_w[q] = w[u];
                 if (!KEYS) g.o_tgt[q] = id[u];
             }
@@ -547,6 +552,7 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
             }
         }
     }
+#undef SRC
 }
 
 // ------------------------------------------------------------------------------------------ merge (reduce by key)
@@ -610,15 +616,15 @@ __global__ void k_final_counts(const int64_t *__restrict__ rawU, const int64_t *
 
 __global__ void k_place_merged(const unsigned long long *__restrict__ mkey, const uint32_t *__restrict__ msrc,
                                const float *__restrict__ mw, int64_t n_merged, const int64_t *__restrict__ mstart,
-                               const int64_t *__restrict__ foff, int64_t arc_base, int64_t f_lo, int shift_t, int bits_b,
-                               int32_t *__restrict__ o_src, int32_t *__restrict__ o_il, int32_t *__restrict__ o_ol,
+                               const int64_t *__restrict__ foff, int64_t arc_base, int64_t f_lo,
+                               const uint32_t *__restrict__ sel, int shift_t, int bits_b, int32_t *__restrict__ o_src, int32_t *__restrict__ o_il, int32_t *__restrict__ o_ol,
                                int32_t *__restrict__ o_tgt, float *__restrict__ o_w) {
     int64_t j = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (j >= n_merged) return;
     uint32_t p = msrc[j];
     unsigned long long k = mkey[j];
     int64_t q = arc_base + foff[p] + (j - mstart[p]);
-    o_src[q] = static_cast<int>(f_lo + p);
+    o_src[q] = static_cast<int>(f_lo + (sel ? sel[p] : p));
     o_tgt[q] = static_cast<int>(k >> shift_t);
     o_il[q] = static_cast<int>((k & ((1ull << shift_t) - 1)) >> bits_b);
     o_ol[q] = static_cast<int>(k & ((1ull << bits_b) - 1));
@@ -699,6 +705,20 @@ k_assemble_scatter(const int2 *__restrict__ pair, int64_t n, const uint32_t *__r
     }
 }
 
+// Level compaction: when rule T will clearly cut the level, only the pairs below a key limit are worked on.
+__global__ void k_flag_below(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, uint64_t nq2, uint64_t key_limit,
+                             uint8_t *__restrict__ flag) {
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= nf) return;
+    int2 p = pair[f_lo + i];
+    flag[i] = (static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y)) < key_limit;
+}
+__global__ void k_compact_sel(const uint8_t *__restrict__ flag, const int64_t *__restrict__ off, int64_t nf,
+                              uint32_t *__restrict__ sel) {
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i < nf && flag[i]) sel[off[i]] = static_cast<uint32_t>(i);
+}
+
 inline unsigned nblk(int64_t n, int threads = CT_THREADS) { return static_cast<unsigned>(ceil_div(n > 0 ? n : 1, threads)); }
 
 // ------------------------------------------------------------------------------------------ host side
@@ -764,7 +784,7 @@ struct Composer {
     void ensure_pairs(int64_t need, int64_t want = 0) {
         if (need <= pair_cap) return;
         grow_to(need, std::max(want, pair_cap * 2), [&](int64_t nc) {
-            DBuf<int2> np(c, nc);
+            DBuf<int2> np(c, nc, true);
             if (n_states > 0)
                 FSTC_CUDA(cudaMemcpyAsync(np.p, pair.p, sizeof(int2) * n_states, cudaMemcpyDeviceToDevice, c.stream));
             pair = std::move(np);
@@ -778,8 +798,8 @@ struct Composer {
         int h = tm.begin(FSTC_T_ASSEMBLE);
         grow_to(need, std::max(want, arc_cap + arc_cap / 2), [&](int64_t nc) {
             nc = (nc + 3) & ~int64_t(3);
-            DBuf<int32_t> n_src(c, nc), n_il(c, nc), n_ol(c, nc), n_tgt(c, nc);
-            DBuf<float> n_w(c, nc);
+            DBuf<int32_t> n_src(c, nc, true), n_il(c, nc, true), n_ol(c, nc, true), n_tgt(c, nc, true);
+            DBuf<float> n_w(c, nc, true);
             if (n_arcs > 0) {
                 const size_t b = sizeof(int32_t) * n_arcs;
                 FSTC_CUDA(cudaMemcpyAsync(n_src.p, a_src.p, b, cudaMemcpyDeviceToDevice, c.stream));
@@ -829,6 +849,7 @@ struct Composer {
     // partitioned = true: the level's target ids come from resolve_partitioned (no visited table)
     bool partitioned = false;
     int key_bits = 0;
+    const uint32_t *cur_sel = nullptr;  // compaction of the level being expanded (null: none)
     int64_t n_states_live = 1;         // states created so far, including those of the launches of this level
 
     void launch_emit(int mode, const MatchList &L, int64_t n_matches, int64_t R, int64_t pos_base, int64_t f_lo,
@@ -842,7 +863,7 @@ struct Composer {
         FSTC_LAUNCH_CHECK();
         EmitArgs g;
         g.A = view_of(m1); g.B = view_of(m2);
-        g.L = L; g.n_matches = n_matches; g.R = R; g.pos_base = pos_base; g.f_lo = f_lo;
+        g.L = L; g.n_matches = n_matches; g.R = R; g.pos_base = pos_base; g.f_lo = f_lo; g.sel = cur_sel;
         g.foff = foff; g.roff = roff; g.arc_base = arc_base; g.nq2 = nq2;
         g.table = table.p; g.cap = cap; g.n_states = d_counters.p; g.pair = pair.p;
         g.o_src = a_src.p; g.o_il = a_il.p; g.o_ol = a_ol.p; g.o_tgt = a_tgt.p; g.o_w = a_w.p;
@@ -934,18 +955,19 @@ fstc_result_t *Composer::run() {
     MachineView A = view_of(m1), B = view_of(m2);
 
     for (;; ++lvl) {
-        const int64_t nf = f_hi - f_lo;
-        if (nf == 0) break;
+        const int64_t nf_all = f_hi - f_lo;                      // the frontier
+        if (nf_all == 0) break;
+        int64_t nf = nf_all;                                     // the pairs of it this level works on (see `sel`)
         last_lo = f_lo; last_hi = f_hi;
         if (o.max_levels > 0 && lvl == o.max_levels) { st.truncated = 1; last_mode = 0; break; }
         last_mode = 1;
 
         // ---- count
         int64_t RU = 0, RF = 0, MU = 0, MF = 0;
-        DBuf<int64_t> rawU(c, nf), rawF;
-        DBuf<uint32_t> nmU(c, nf), nmF;
-        DBuf<int64_t> roffU(c, nf + 1), roffF, moffU(c, nf + 1), moffF;
-        if (has_F) { rawF.alloc(c, nf); nmF.alloc(c, nf); roffF.alloc(c, nf + 1); moffF.alloc(c, nf + 1); }
+        DBuf<int64_t> rawU, rawF;
+        DBuf<uint32_t> nmU, nmF;
+        DBuf<int64_t> roffU, roffF, moffU, moffF;
+        DBuf<uint32_t> sel;                                      // compacted level: frontier index of working pair i
         auto scan_level = [&](int64_t *n_sel_out) {             // offsets + totals of the level, one synchronisation
             exclusive_scan2(c, rawU.p, nmU.p, nf, roffU.p, moffU.p);
             if (has_F) exclusive_scan2(c, rawF.p, nmF.p, nf, roffF.p, moffF.p);
@@ -972,7 +994,29 @@ fstc_result_t *Composer::run() {
         int h;
         while (true) {
             h = tm.begin(FSTC_T_COUNT);
-            k_count<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, o.merge_mode, nq2, key_limit, rawU.p, rawF.p,
+            nf = nf_all;
+            sel.release();
+            if (key_limit < n_pairs_total) {                     // work on the pairs below the limit only
+                DBuf<uint8_t> flag(c, nf_all);
+                DBuf<int64_t> off(c, nf_all + 1);
+                k_flag_below<<<nblk(nf_all), CT_THREADS, 0, c.stream>>>(pair.p, f_lo, nf_all, nq2, key_limit, flag.p);
+                FSTC_LAUNCH_CHECK();
+                exclusive_scan<uint8_t>(c, flag.p, nf_all, off.p);
+                nf = read_scalar(c, off.p + nf_all);
+                sel.alloc(c, nf);
+                k_compact_sel<<<nblk(nf_all), CT_THREADS, 0, c.stream>>>(flag.p, off.p, nf_all, sel.p);
+                FSTC_LAUNCH_CHECK();
+                c.n_launch += 2;
+                c.sync();                                        // flag / off go out of scope
+                if (nf == 0) {                                   // nothing below the limit: widen
+                    tm.end(h);
+                    key_limit = key_limit > n_pairs_total / 4 ? ~0ull : key_limit * 4;
+                    continue;
+                }
+            }
+            rawU.alloc(c, nf); nmU.alloc(c, nf); roffU.alloc(c, nf + 1); moffU.alloc(c, nf + 1);
+            if (has_F) { rawF.alloc(c, nf); nmF.alloc(c, nf); roffF.alloc(c, nf + 1); moffF.alloc(c, nf + 1); }
+            k_count<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, sel.p, o.merge_mode, nq2, key_limit, rawU.p, rawF.p,
                                                            nmU.p, nmF.p);
             FSTC_LAUNCH_CHECK();
             c.n_launch += 1;
@@ -993,7 +1037,7 @@ fstc_result_t *Composer::run() {
             const int top = ((key_bits + 7) / 8) * 8;
             for (int shift = top - 8; shift >= 0; shift -= 8) {
                 FSTC_CUDA(cudaMemsetAsync(d_counters.p + 4, 0, sizeof(unsigned long long) * 256, c.stream));
-                k_cut_hist<<<std::min<unsigned>(nblk(nf), 8u * c.n_sm), CT_THREADS, 0, c.stream>>>(pair.p, f_lo, nf, nq2, rawU.p, rawF.p, prefix, shift,
+                k_cut_hist<<<std::min<unsigned>(nblk(nf), 8u * c.n_sm), CT_THREADS, 0, c.stream>>>(pair.p, f_lo, nf, sel.p, nq2, rawU.p, rawF.p, prefix, shift,
                                                                   d_counters.p + 4);
                 FSTC_LAUNCH_CHECK();
                 c.n_launch += 1;
@@ -1010,7 +1054,7 @@ fstc_result_t *Composer::run() {
             }
             cut_key = prefix;
             FSTC_CUDA(cudaMemsetAsync(d_counters.p + 3, 0, sizeof(unsigned long long), c.stream));
-            k_apply_cut<<<nblk(nf), CT_THREADS, 0, c.stream>>>(pair.p, f_lo, nf, nq2, cut_key, rawU.p, rawF.p, nmU.p, nmF.p,
+            k_apply_cut<<<nblk(nf), CT_THREADS, 0, c.stream>>>(pair.p, f_lo, nf, sel.p, nq2, cut_key, rawU.p, rawF.p, nmU.p, nmF.p,
                                                                d_counters.p + 3);
             FSTC_LAUNCH_CHECK();
             c.n_launch += 1;
@@ -1022,10 +1066,32 @@ fstc_result_t *Composer::run() {
         tm.end(h);
 
         const int64_t R = RU + RF;
+        cur_sel = sel.p;
         // ---- capacities for this level
         const uint64_t remaining_pairs = n_pairs_total - static_cast<uint64_t>(n_states);
         const int64_t new_bound = static_cast<int64_t>(std::min<uint64_t>(static_cast<uint64_t>(R), remaining_pairs));
         if (n_states + new_bound >= 0x7FFFFFFFll) fail(FSTC_ERR_CAPACITY, "more than 2^31-1 states");
+        // ---- how this level resolves its target ids (DESIGN.md "resolve"): the visited table while it stays small
+        // enough to live in L2, else the streaming partitioned resolve.  The switch is one-way: the table is dropped.
+        {
+            const int id_bits = bits_for(static_cast<uint64_t>(n_states + new_bound));
+            const bool fits = key_bits + id_bits <= 64;                // state records are key << id_bits | id
+            if (!partitioned) {
+                bool want = o.resolve_mode == FSTC_RESOLVE_PARTITIONED;
+                if (o.resolve_mode == FSTC_RESOLVE_AUTO)
+                    want = R >= RESOLVE_MIN_ARCS && slots_for(n_states + new_bound) * sizeof(uint4) > RESOLVE_TABLE_BYTES;
+                // later levels must fit too, unless this is the last level: bound the number of states the run can reach
+                uint64_t max_states = std::min<uint64_t>(n_pairs_total, 0x7FFFFFFFull);
+                if (o.max_raw_arcs > 0) max_states = std::min<uint64_t>(max_states, static_cast<uint64_t>(o.max_raw_arcs) + 1);
+                if (want && fits && (key_bits + bits_for(max_states) <= 64 || stop_after)) {
+                    partitioned = true;
+                    table = DBuf<uint4>();
+                    cap = 0;
+                }
+            } else if (!fits) {
+                fail(FSTC_ERR_CAPACITY, "%d-bit pair keys with %d-bit state ids do not fit the partitioned resolve", key_bits, id_bits);
+            }
+        }
         // look-ahead: if the search goes on, the next level is about (new states) x (arcs per expanded pair)
         int64_t next_R = 0, next_S = 0;
         const bool must_grow = n_states + new_bound > pair_cap || (!partitioned && slots_for(n_states + new_bound) > cap) ||
@@ -1043,30 +1109,11 @@ fstc_result_t *Composer::run() {
             pr = std::min(pr, 16.0 * static_cast<double>(n_arcs + R));           // never more than 16x what is needed now
             const double ps = std::min(pr, static_cast<double>(remaining_pairs - static_cast<uint64_t>(new_bound)));
             // 20 B per arc; per state 8 B + a table slot at the target load; at most 40 % of what is free
-            const double bytes = 20.0 * pr + (8.0 + 1600.0 / FSTC_TABLE_LOAD_PCT) * ps;
+            const double bytes = 20.0 * pr + (partitioned ? 8.0 : 8.0 + 1600.0 / FSTC_TABLE_LOAD_PCT) * ps;
             const double scale = std::min(1.0, 0.4 * static_cast<double>(free_b) / std::max(bytes, 1.0));
             next_R = pr > 0 ? static_cast<int64_t>(pr * scale) : 0;
             next_S = ps > 0 ? static_cast<int64_t>(ps * scale) : 0;
             if (n_states + new_bound + next_S >= 0x7FFFFFFFll) next_S = 0;
-        }
-        // ---- how this level resolves its target ids (DESIGN.md "resolve"): the visited table while it stays small
-        // enough to live in L2, else the streaming partitioned resolve.  The switch is one-way: the table is dropped.
-        {
-            const int id_bits = bits_for(static_cast<uint64_t>(n_states + new_bound));
-            const bool fits = key_bits + id_bits <= 64;                // state records are key << id_bits | id
-            if (!partitioned) {
-                bool want = o.resolve_mode == FSTC_RESOLVE_PARTITIONED;
-                if (o.resolve_mode == FSTC_RESOLVE_AUTO)
-                    want = R >= RESOLVE_MIN_ARCS && slots_for(n_states + new_bound) * sizeof(uint4) > RESOLVE_TABLE_BYTES;
-                // later levels must fit too (ids have at most 31 bits), unless this is the last level
-                if (want && fits && (key_bits + 31 <= 64 || stop_after)) {
-                    partitioned = true;
-                    table = DBuf<uint4>();
-                    cap = 0;
-                }
-            } else if (!fits) {
-                fail(FSTC_ERR_CAPACITY, "%d-bit pair keys with %d-bit state ids do not fit the partitioned resolve", key_bits, id_bits);
-            }
         }
         ensure_pairs(n_states + new_bound, n_states + new_bound + next_S);
         if (!partitioned) {
@@ -1087,7 +1134,7 @@ fstc_result_t *Composer::run() {
         LF = MatchList{cumF.p, recF.p, plF.p};
         if (MU + MF > 0) {
             h = tm.begin(FSTC_T_MATCH);
-            k_match<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, nmU.p, nmF.p, moffU.p, moffF.p, roffU.p,
+            k_match<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, sel.p, nmU.p, nmF.p, moffU.p, moffF.p, roffU.p,
                                                            roffF.p, LU, LF, d_counters.p + 1);
             FSTC_LAUNCH_CHECK();
             c.n_launch += 1;
@@ -1133,7 +1180,7 @@ fstc_result_t *Composer::run() {
             k_final_counts<<<nblk(nf), CT_THREADS, 0, c.stream>>>(rawU.p, mstart.p, nf, fc.p);
             FSTC_LAUNCH_CHECK();
             exclusive_scan<int64_t>(c, fc.p, nf, foff.p);
-            k_place_merged<<<nblk(M), CT_THREADS, 0, c.stream>>>(mkey.p, msrc.p, mw.p, M, mstart.p, foff.p, arc_base, f_lo,
+            k_place_merged<<<nblk(M), CT_THREADS, 0, c.stream>>>(mkey.p, msrc.p, mw.p, M, mstart.p, foff.p, arc_base, f_lo, sel.p,
                                                                  shift_t, bits_b, a_src.p, a_il.p, a_ol.p, a_tgt.p, a_w.p);
             FSTC_LAUNCH_CHECK();
             c.n_launch += 5;
@@ -1148,7 +1195,7 @@ fstc_result_t *Composer::run() {
 
         const int64_t ns_after = static_cast<int64_t>(read_scalar(c, d_counters.p));
         if (lvl < FSTC_MAX_LEVEL_STATS) {
-            st.level_frontier[lvl] = nf;
+            st.level_frontier[lvl] = nf_all;
             st.level_raw[lvl] = R;
             st.level_new_states[lvl] = ns_after - n_states;
         }
@@ -1165,7 +1212,7 @@ fstc_result_t *Composer::run() {
 
     // ---- assemble
     int h = tm.begin(FSTC_T_ASSEMBLE);
-    DBuf<uint8_t> expanded(c, n_states);
+    DBuf<uint8_t> expanded(c, n_states, true);
     const int64_t as_tiles = ceil_div(n_states, AS_TILE);
     DBuf<uint32_t> tile_count(c, as_tiles);
     DBuf<int64_t> tile_off(c, as_tiles + 1);
@@ -1174,7 +1221,7 @@ fstc_result_t *Composer::run() {
     FSTC_LAUNCH_CHECK();
     exclusive_scan<uint32_t>(c, tile_count.p, as_tiles, tile_off.p);
     const int64_t n_accept = read_scalar(c, tile_off.p + as_tiles);
-    DBuf<int32_t> accept(c, n_accept);
+    DBuf<int32_t> accept(c, n_accept, true);
     if (n_accept > 0) {
         k_assemble_scatter<<<static_cast<unsigned>(as_tiles), AS_THREADS, 0, c.stream>>>(
             pair.p, n_states, m1.accept_bits, m2.accept_bits, tile_count.p, tile_off.p, accept.p);
@@ -1228,7 +1275,7 @@ void free_result(fstc_result_t *r) {
     ResultImpl *impl = static_cast<ResultImpl *>(r->impl);
     if (impl) {
         for (void *p : impl->bufs)
-            if (p) (void)cudaFreeAsync(p, nullptr);
+            if (p) persist_free(p, nullptr);
         delete impl;
     }
     delete r;

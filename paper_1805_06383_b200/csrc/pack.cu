@@ -149,11 +149,11 @@ const T *stage(Ctx &c, const T *p, int64_t n, int mem, DBuf<T> &hold) {
 void free_packed(fstc_packed_t *p) {
     if (!p) return;
     // freed stream-ordered on the legacy stream: safe after any stream of ours has been synchronised
-    if (p->arcs) (void)cudaFreeAsync(p->arcs, nullptr);
-    if (p->segs) (void)cudaFreeAsync(p->segs, nullptr);
-    if (p->seg_ptr) (void)cudaFreeAsync(p->seg_ptr, nullptr);
-    if (p->flags) (void)cudaFreeAsync(p->flags, nullptr);
-    if (p->accept_bits) (void)cudaFreeAsync(p->accept_bits, nullptr);
+    if (p->arcs) persist_free(p->arcs, nullptr);
+    if (p->segs) persist_free(p->segs, nullptr);
+    if (p->seg_ptr) persist_free(p->seg_ptr, nullptr);
+    if (p->flags) persist_free(p->flags, nullptr);
+    if (p->accept_bits) persist_free(p->accept_bits, nullptr);
     delete p;
 }
 
@@ -197,11 +197,11 @@ fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side) {
     }
     if (read_scalar(c, bad.p)) fail(FSTC_ERR_INPUT, "a state or symbol id is out of range");
 
-    DBuf<uint4> arcs(c, n);
+    DBuf<uint4> arcs(c, n, true);                             // the five arrays of the packed form outlive the call
     DBuf<uint2> segs;
-    DBuf<uint32_t> seg_ptr(c, static_cast<int64_t>(m.n_states) + 1);
-    DBuf<uint8_t> flags(c, m.n_states);
-    DBuf<uint32_t> accept_bits(c, (m.n_states + 31) / 32);
+    DBuf<uint32_t> seg_ptr(c, static_cast<int64_t>(m.n_states) + 1, true);
+    DBuf<uint8_t> flags(c, m.n_states, true);
+    DBuf<uint32_t> accept_bits(c, (m.n_states + 31) / 32, true);
     DBuf<uint32_t> flags32(c, m.n_states);
     FSTC_CUDA(cudaMemsetAsync(flags32.p, 0, sizeof(uint32_t) * m.n_states, c.stream));
     FSTC_CUDA(cudaMemsetAsync(accept_bits.p, 0, sizeof(uint32_t) * ((m.n_states + 31) / 32), c.stream));
@@ -226,7 +226,7 @@ fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side) {
         FSTC_LAUNCH_CHECK();
         exclusive_scan<uint32_t>(c, head.p, n, seg_idx.p);
         n_segs = read_scalar(c, seg_idx.p + n);
-        segs.alloc(c, n_segs + 1);
+        segs.alloc(c, n_segs + 1, true);
         DBuf<uint32_t> seg_src(c, n_segs);
         pk_fill_segs<<<blocks_for(n), PK_THREADS, 0, c.stream>>>(s2, arcs.p, head.p, seg_idx.p, n, segs.p, seg_src.p);
         FSTC_LAUNCH_CHECK();
@@ -236,7 +236,7 @@ fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side) {
         c.n_launch += 5;
         c.sync();   // temporaries (ra, rb, head, ...) are released below; keep the stream ordered and simple
     } else {
-        segs.alloc(c, 1);
+        segs.alloc(c, 1, true);
         uint2 sentinel = make_uint2(0xFFFFFFFFu, 0u);
         FSTC_CUDA(cudaMemcpyAsync(segs.p, &sentinel, sizeof sentinel, cudaMemcpyHostToDevice, c.stream));
         FSTC_CUDA(cudaMemsetAsync(seg_ptr.p, 0, sizeof(uint32_t) * (static_cast<size_t>(m.n_states) + 1), c.stream));
