@@ -107,12 +107,27 @@ class ClockSampler:
 
 
 def alg_bytes(st: dict, n_new_states: int) -> dict:
-    """Algorithmic bytes of one composition, from exact device-side counts."""
+    """Algorithmic bytes from exact device-side counts: of one composition (SURVEY §8(d) model) and
+    of every hot kernel, summed over its launches in the step."""
     E, R, S, M = st["n_expanded"], st["n_raw_arcs"], st["n_states"], st["n_arcs"]
     Rm = st["n_raw_sorted"]
     path = (16 * E + 8 * st["n_seg_visited"] + 12 * st["n_match_arcs"] + 12 * R + 12 * S + 20 * M + 9 * S + 40 * Rm)
-    emit = 12 * st["n_match_arcs"] + 12 * R + 12 * n_new_states + 8 * n_new_states + 20 * (R - Rm) + 16 * Rm
-    return {"path": path, "emit": emit}
+    Rp = st["n_resolved_arcs"]                      # arcs whose targets went through the partitioned resolve
+    Rt = R - Rp                                     # arcs resolved in the visited table, inside the emit kernel
+    new_p = st["rs_dedupe_new"]
+    new_t = max(0, n_new_states - new_p)
+    kern = {
+        # arc payload of the matching segments + the four final columns (or the 16-byte sort record) per arc
+        # + table levels: target column, one probe per arc, insert + pair per new state; resolve levels: the key
+        "k_emit": 12 * st["n_match_arcs"] + 16 * R + (4 + 12) * Rt + 20 * new_t + 8 * Rp,
+        # record in + out (8 + 8), and the recorded permutation (4 + 2) on the arc stream
+        "rs_scatter": 16 * (st["rs_scatter_recs"] + st["rs_scatter_dest_recs"]) + 6 * st["rs_scatter_dest_recs"],
+        # state record, arc key in + id out, pair of every new state
+        "rs_dedupe": 8 * st["rs_dedupe_states"] + 12 * st["rs_dedupe_arcs"] + 8 * new_p,
+        # permutation (4 + 2), id in, id out
+        "rs_gather": 14 * st["rs_gather_recs"],
+    }
+    return {"path": path, "kernels": kern}
 
 
 def rank_seeds(workload: str, rank: int):
@@ -253,17 +268,28 @@ def main():
     peak, peak_src = _peaks()
     new_states = st["n_states"] - 1
     ab = alg_bytes(st, new_states)
-    emit_ms = sum(s["ms"]["emit"] for s in stats) / max(1, sum(s["n_emit_launches"] for s in stats))
-    emit_bytes_per_launch = ab["emit"] / max(1, st["n_emit_launches"])
-    emit_gbs = emit_bytes_per_launch / (emit_ms * 1e-3) / 1e9 if emit_ms > 0 else 0.0
+    # the dominant kernel of the step, by device time measured live (CUDA events on the compose stream, library
+    # `profile` mode): each of these stages is ONE kernel, launched several times per step
+    kstage = {"k_emit": ("emit", "n_emit_launches"), "rs_scatter": ("rs_scatter", "rs_scatter_launches"),
+              "rs_dedupe": ("rs_dedupe", "rs_dedupe_launches"), "rs_gather": ("rs_gather", "rs_gather_launches")}
+    kms = {k: sum(s["ms"][v[0]] for s in stats) / len(stats) for k, v in kstage.items()}
+    dom = max(kms, key=kms.get)
+    dom_launches = max(1, st[kstage[dom][1]])
+    dom_ms = kms[dom] / dom_launches
+    dom_bytes_per_launch = ab["kernels"][dom] / dom_launches
+    dom_gbs = dom_bytes_per_launch / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", f"emit_traffic_{args.workload}.json")
+    tpath = os.path.join(ROOT, "profiles", f"kernel_traffic_{args.workload}.json")
     if os.path.exists(tpath):
         try:
-            # measured DRAM bytes per raw arc of the captured launch x arcs per launch (average, like `achieved`)
-            traffic = json.load(open(tpath))["dram_bytes_per_raw_arc"] * st["n_raw_arcs"] / max(1, st["n_emit_launches"])
+            # measured DRAM bytes per launch of that kernel (ncu --set full, averaged over its launches in one step)
+            traffic = json.load(open(tpath))["dram_bytes_per_launch"].get(dom)
         except Exception:
             traffic = None
+    per_kernel = {k: {"ms_per_step": kms[k], "launches_per_step": st[kstage[k][1]],
+                      "alg_bytes_per_step": ab["kernels"][k],
+                      "achieved_GBs": (ab["kernels"][k] / (kms[k] * 1e-3) / 1e9) if kms[k] > 0 else 0.0}
+                  for k in kstage}
     compose_ms = sum(s["compose_ms"] for s in stats) / len(stats)
     pack_ms = sum(s["pack_ms"] for s in stats) / len(stats)
     path_gbs = ab["path"] / (compose_ms * 1e-3) / 1e9
@@ -281,10 +307,11 @@ def main():
         "timing_ms": {"pack": pack_ms, "compose_packed": compose_ms,
                       "stages": {k: sum(s["ms"][k] for s in stats) / len(stats) for k in fstc.STAGES},
                       "compose_raw_arcs_per_sec": st["n_raw_arcs"] / (compose_ms * 1e-3)},
-        "roofline": {"bound": "hbm", "kernel": "k_emit (emit + visited-set find-or-insert)", "achieved": emit_gbs,
-                     "peak": peak, "unit": "GB/s", "frac": emit_gbs / peak, "peak_source": peak_src,
-                     "traffic": traffic, "alg_bytes_per_launch": emit_bytes_per_launch, "ms_per_launch": emit_ms,
-                     "launches_per_step": st["n_emit_launches"], "frac_of_8TBs_nominal": emit_gbs / 8000.0},
+        "roofline": {"bound": "hbm", "kernel": dom, "achieved": dom_gbs, "peak": peak, "unit": "GB/s",
+                     "frac": dom_gbs / peak, "peak_source": peak_src, "traffic": traffic,
+                     "alg_bytes_per_launch": dom_bytes_per_launch, "ms_per_launch": dom_ms,
+                     "launches_per_step": dom_launches, "share_of_step": kms[dom] / (t_ms / args.steps / max(1, world)) if world == 1 else None,
+                     "frac_of_8TBs_nominal": dom_gbs / 8000.0, "kernels": per_kernel},
         "roofline_path": {"alg_bytes": ab["path"], "achieved": path_gbs, "frac": path_gbs / peak,
                           "frac_of_8TBs_nominal": path_gbs / 8000.0,
                           "alg_bytes_per_raw_arc": ab["path"] / max(1, st["n_raw_arcs"])},

@@ -118,12 +118,15 @@ enum {                      /* indices into fstc_stats_t.ms[] (filled when opts.
   FSTC_T_COUNT = 0,         /* per-pair inner-symbol intersection + raw counts                       */
   FSTC_T_SCAN = 1,          /* exclusive scans and the budget cut                                    */
   FSTC_T_MATCH = 2,         /* match work-list construction                                          */
-  FSTC_T_EMIT = 3,          /* load-balanced product-arc emission fused with visited-set find-or-insert */
+  FSTC_T_EMIT = 3,          /* the emit kernel: load-balanced product arcs (+ visited-table find-or-insert when the level uses the table) */
   FSTC_T_SORT = 4,          /* radix sort of the arcs that may merge                                 */
   FSTC_T_REDUCE = 5,        /* segmented reduction + placement of merged arcs                        */
   FSTC_T_TABLE = 6,         /* visited table clear / grow + rehash                                   */
   FSTC_T_ASSEMBLE = 7,      /* accept list, expanded flags, output growth copies                     */
-  FSTC_T_NSTAGES = 8
+  FSTC_T_RS_SCATTER = 8,    /* partitioned resolve: staged scatter passes (states and arc keys)                */
+  FSTC_T_RS_DEDUPE = 9,     /* partitioned resolve: per-bin dedupe in shared memory, new ids, pair table        */
+  FSTC_T_RS_GATHER = 10,    /* partitioned resolve: ids back through the recorded permutations                  */
+  FSTC_T_NSTAGES = 11
 };
 
 typedef struct fstc_stats_t {
@@ -139,6 +142,10 @@ typedef struct fstc_stats_t {
   int32_t n_emit_launches, n_kernel_launches;
   int32_t n_resolve, pad_;  /* emit launches whose target ids came from the partitioned resolve                */
   int64_t n_resolved_arcs;  /* raw arcs of those launches                                                     */
+  /* work of the partitioned resolve, for its roofline: records through the scatter passes without / with
+   * the recorded permutation, arc keys and state records through the dedupe, ids through the gathers; launches    */
+  int64_t rs_scatter_recs, rs_scatter_dest_recs, rs_dedupe_arcs, rs_dedupe_states, rs_dedupe_new, rs_gather_recs;
+  int32_t rs_scatter_launches, rs_dedupe_launches, rs_gather_launches, pad2_;
   double ms[FSTC_T_NSTAGES];/* device time per stage (CUDA events), only when opts.profile = 1       */
   double ms_total;          /* device time of the whole call (CUDA events), always                    */
   int64_t level_frontier[FSTC_MAX_LEVEL_STATS];  /* |F_l|                                             */

@@ -859,6 +859,7 @@ struct Composer {
         const int64_t tile0 = (pos_base / EM_TILE) * EM_TILE;
         const int64_t n_tiles = ceil_div(pos_base + R - tile0, EM_TILE);
         DBuf<int64_t> tile_m(c, n_tiles + 1);
+        const int h_emit = tm.begin(FSTC_T_EMIT);
         k_partition<<<nblk(n_tiles + 1), CT_THREADS, 0, c.stream>>>(L.cum, n_matches, R, pos_base, n_tiles, tile_m.p);
         FSTC_LAUNCH_CHECK();
         EmitArgs g;
@@ -885,6 +886,7 @@ struct Composer {
             else k_emit<EMIT_SORTREC, false><<<grid, EM_THREADS, 0, c.stream>>>(g);
         }
         FSTC_LAUNCH_CHECK();
+        tm.end(h_emit);
         c.n_launch += 2;
         st.n_emit_launches += 1;
         if (partitioned) {
@@ -898,6 +900,8 @@ struct Composer {
             j.sortrec = mode == EMIT_SORTREC ? sortrec : nullptr;
             j.shift_t = shift_t;
             j.force_bits = -1;
+            j.stats = &st;
+            j.profile = o.profile != 0;
             if (const char *e = getenv("FSTC_RESOLVE_BITS")) j.force_bits = atoi(e);   // test knob: force multi-pass
             resolve_partitioned(c, j);
             st.n_resolve += 1;
@@ -1144,16 +1148,12 @@ fstc_result_t *Composer::run() {
         const int64_t arc_base = n_arcs;
         if (RF == 0) {
             // no source of this level can hold duplicates: arcs go straight to their final place
-            h = tm.begin(FSTC_T_EMIT);
             launch_emit(EMIT_DIRECT, LU, MU, RU, arc_base, f_lo, nullptr, nullptr, 0, nullptr, 0, 0);
-            tm.end(h);
             n_arcs += RU;
         } else {
             if (shift_t > 32) fail(FSTC_ERR_CAPACITY, "bits(|Σ|)+bits(|Δ|) = %d > 32: merge key does not fit 64 bits", shift_t);
             DBuf<uint4> sa(c, RF), sb(c, RF);
-            h = tm.begin(FSTC_T_EMIT);
             launch_emit(EMIT_SORTREC, LF, MF, RF, 0, f_lo, nullptr, nullptr, 0, sa.p, shift_t, bits_b);
-            tm.end(h);
             // target ids are now known: n_states bounds them
             const int64_t ns_now = static_cast<int64_t>(read_scalar(c, d_counters.p));
             n_states_live = ns_now;
@@ -1185,9 +1185,7 @@ fstc_result_t *Composer::run() {
             FSTC_LAUNCH_CHECK();
             c.n_launch += 5;
             tm.end(h);
-            h = tm.begin(FSTC_T_EMIT);
             launch_emit(EMIT_INDIRECT, LU, MU, RU, 0, f_lo, foff.p, roffU.p, arc_base, nullptr, 0, 0, RU + M);
-            tm.end(h);
             n_arcs += RU + M;
             st.n_raw_sorted += RF;
             c.sync();   // the level's temporaries go out of scope below
@@ -1199,6 +1197,7 @@ fstc_result_t *Composer::run() {
             st.level_raw[lvl] = R;
             st.level_new_states[lvl] = ns_after - n_states;
         }
+        if (partitioned) st.rs_dedupe_new += ns_after - n_states;
         st.n_matches += MU + MF;
         st.n_expanded += n_sel;
         last_fan = n_sel > 0 ? static_cast<double>(R) / static_cast<double>(n_sel) : 0.0;

@@ -70,6 +70,8 @@ struct ResolveJob {
     uint4 *sortrec;                     // mode 2: id OR-ed into key bits [shift_t, ...)
     int shift_t;
     int force_bits;                     // >= 0: number of hash bits to partition on (tests); -1: from the sizes
+    fstc_stats_t *stats;                // nullable: work counters and (profile) stage times are added here
+    bool profile;
 };
 int resolve_bits_needed(int64_t n_records_and_states);
 void resolve_partitioned(Ctx &c, const ResolveJob &j);

@@ -426,12 +426,13 @@ inline unsigned rs_blocks(int64_t n, int threads = 256) { return static_cast<uns
 
 // FSTC_RS_TRACE=1 prints the device time of every resolve kernel to stderr (debug knob, off by default)
 struct RsTrace {
-    struct Span { const char *name; int64_t n; cudaEvent_t a, b; double host_us; unsigned long long reserved; };
+    struct Span { const char *name; int64_t n; cudaEvent_t a, b; double host_us; unsigned long long reserved; int kind; };
     std::vector<Span> spans;
-    bool on = getenv("FSTC_RS_TRACE") != nullptr;
-    int begin(Ctx &c, const char *name, int64_t n) {
+    bool print = getenv("FSTC_RS_TRACE") != nullptr;
+    bool on = print;                                            // also switched on by opts.profile (stage times)
+    int begin(Ctx &c, const char *name, int64_t n, int kind = -1) {
         if (!on) return -1;
-        Span s{name, n, nullptr, nullptr, 0.0, 0ull};
+        Span s{name, n, nullptr, nullptr, 0.0, 0ull, kind};
         timespec ts; clock_gettime(CLOCK_MONOTONIC, &ts);
         s.host_us = ts.tv_sec * 1e6 + ts.tv_nsec * 1e-3;
         (void)cudaMemPoolGetAttribute(device_pool(), cudaMemPoolAttrReservedMemCurrent, &s.reserved);
@@ -441,13 +442,14 @@ struct RsTrace {
         return static_cast<int>(spans.size()) - 1;
     }
     void end(Ctx &c, int h) { if (h >= 0) cudaEventRecord(spans[h].b, c.stream); }
-    void report() {
+    void report(double *stage_ms) {
         for (auto &s : spans) {
             float ms = 0.f, at = 0.f;
             cudaEventSynchronize(s.b);
             cudaEventElapsedTime(&ms, s.a, s.b);
             cudaEventElapsedTime(&at, spans[0].a, s.a);
-            fprintf(stderr, "[fstc resolve] %-18s n=%-11lld at %8.3f  %8.3f ms   host at %9.3f ms  pool %.2f GB\n", s.name,
+            if (stage_ms && s.kind >= 0) stage_ms[s.kind] += ms;
+            if (print) fprintf(stderr, "[fstc resolve] %-18s n=%-11lld at %8.3f  %8.3f ms   host at %9.3f ms  pool %.2f GB\n", s.name,
                     static_cast<long long>(s.n), at, ms, (s.host_us - spans[0].host_us) * 1e-3, s.reserved / 1e9);
         }
         for (auto &s : spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
@@ -521,7 +523,7 @@ SegSet scatter_pass(Ctx &c, const SegSet &in, int shift, int hshift, int nbins, 
         if (totals[0] > 0) {
             ScatterArgs a{in.view(), tile_first.p, out.own.p, out.start.p, cursor.p, dest ? dest->p : nullptr, dest ? perm->p : nullptr,
                           cur_stride, shift, hshift, nbins};
-            const int h = g_trace.begin(c, dest ? "scatter+dest" : "scatter", totals[0] * SC_TILE);
+            const int h = g_trace.begin(c, dest ? "scatter+dest" : "scatter", totals[0] * SC_TILE, FSTC_T_RS_SCATTER);
             if (dest) rs_scatter<true><<<static_cast<unsigned>(totals[0]), SC_THREADS, smem, c.stream>>>(a);
             else rs_scatter<false><<<static_cast<unsigned>(totals[0]), SC_THREADS, smem, c.stream>>>(a);
             FSTC_LAUNCH_CHECK();
@@ -549,7 +551,7 @@ void gather_pass(Ctx &c, const SegSet &seg, int mode, GatherArgs a) {
     a.seg = seg.view();
     a.tile_first = tile_first.p;
     if (tiles > 0) {
-        const int h = g_trace.begin(c, mode == 0 && a.dest ? "gather" : "apply", tiles * SC_TILE);
+        const int h = g_trace.begin(c, mode == 0 && a.dest ? "gather" : "apply", tiles * SC_TILE, FSTC_T_RS_GATHER);
         const unsigned grid = static_cast<unsigned>(tiles);
         if (mode == 0) rs_gather_ids<0><<<grid, GA_THREADS, 0, c.stream>>>(a);
         else if (mode == 1) rs_gather_ids<1><<<grid, GA_THREADS, 0, c.stream>>>(a);
@@ -574,6 +576,7 @@ void resolve_partitioned(Ctx &c, const ResolveJob &j) {
     if (j.n_records >= 0xFFFFFFFFll) fail(FSTC_ERR_CAPACITY, "resolve: more than 2^32 records");
     int bits = j.force_bits >= 0 ? j.force_bits : resolve_bits_needed(j.n_states_before + j.n_records);
     const uint64_t nq2_inv = j.nq2 > 1 ? ~0ull / j.nq2 : ~0ull;      // floor((2^64-1)/d): at most 1 below floor(2^64/d)
+    g_trace.on = g_trace.print || j.profile;
     const int h_all = g_trace.begin(c, "RESOLVE TOTAL", j.n_records);
     for (;; ++bits) {
         if (bits > 20) fail(FSTC_ERR_CAPACITY, "resolve: more than 2^20 bins needed");
@@ -606,12 +609,23 @@ void resolve_partitioned(Ctx &c, const ResolveJob &j) {
         const unsigned long long n_before = static_cast<unsigned long long>(j.n_states_before);
         FSTC_CUDA(cudaMemcpyAsync(j.n_states, &n_before, sizeof n_before, cudaMemcpyHostToDevice, c.stream));
         DedupeArgs d{st.view(), arcs.view(), ib, ids_last.p, j.nq2, nq2_inv, j.n_states, j.pair, err.p};
-        const int hd = g_trace.begin(c, "dedupe", nb);
+        const int hd = g_trace.begin(c, "dedupe", nb, FSTC_T_RS_DEDUPE);
         rs_dedupe<<<static_cast<unsigned>(nb), DD_THREADS, 0, c.stream>>>(d);
         FSTC_LAUNCH_CHECK();
         g_trace.end(c, hd);
         c.n_launch += 1;
         if (read_scalar(c, err.p)) continue;                     // a bin outgrew shared memory: twice the bins, again
+        if (j.stats) {
+            const int passes = (b1 > 0) + (b2 > 0);
+            j.stats->rs_scatter_recs += passes * j.n_states_before;
+            j.stats->rs_scatter_dest_recs += passes * j.n_records;
+            j.stats->rs_scatter_launches += 2 * passes;
+            j.stats->rs_dedupe_arcs += j.n_records;
+            j.stats->rs_dedupe_states += j.n_states_before;
+            j.stats->rs_dedupe_launches += 1;
+            j.stats->rs_gather_recs += (passes > 0 ? passes : 1) * j.n_records;
+            j.stats->rs_gather_launches += passes > 0 ? passes : 1;
+        }
         st = SegSet();
         // 4. ids back through the passes
         const uint32_t *ids = ids_last.p;
@@ -630,7 +644,8 @@ void resolve_partitioned(Ctx &c, const ResolveJob &j) {
         gather_pass(c, lvl0, j.mode, g);
         g_trace.end(c, h_all);
         c.sync();                                                // temporaries are released below
-        if (g_trace.on) g_trace.report();
+        if (g_trace.on) g_trace.report(j.stats ? j.stats->ms : nullptr);
+        g_trace.on = g_trace.print;
         return;
     }
 }

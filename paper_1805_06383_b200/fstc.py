@@ -21,7 +21,7 @@ FSTC_MEM_DEVICE, FSTC_MEM_HOST = 0, 1
 MERGE_AUTO, MERGE_OFF, MERGE_SORT_ALL = 0, 1, 2
 RESOLVE_AUTO, RESOLVE_TABLE, RESOLVE_PARTITIONED = 0, 1, 2
 MAX_LEVEL_STATS = 64
-STAGES = ("count", "scan", "match", "emit", "sort", "reduce", "table", "assemble")
+STAGES = ("count", "scan", "match", "emit", "sort", "reduce", "table", "assemble", "rs_scatter", "rs_dedupe", "rs_gather")
 
 EXPORTS = (
     "fstc_pack", "fstc_packed_free", "fstc_packed_info", "fstc_packed_to_host", "fstc_compose_packed",
@@ -63,6 +63,10 @@ class _Stats(ctypes.Structure):
         ("n_rehash", ctypes.c_int32), ("n_grow", ctypes.c_int32),
         ("n_emit_launches", ctypes.c_int32), ("n_kernel_launches", ctypes.c_int32),
         ("n_resolve", ctypes.c_int32), ("n_resolve_arcs_pad", ctypes.c_int32), ("n_resolved_arcs", ctypes.c_int64),
+        ("rs_scatter_recs", ctypes.c_int64), ("rs_scatter_dest_recs", ctypes.c_int64), ("rs_dedupe_arcs", ctypes.c_int64),
+        ("rs_dedupe_states", ctypes.c_int64), ("rs_dedupe_new", ctypes.c_int64), ("rs_gather_recs", ctypes.c_int64),
+        ("rs_scatter_launches", ctypes.c_int32), ("rs_dedupe_launches", ctypes.c_int32),
+        ("rs_gather_launches", ctypes.c_int32), ("pad2_", ctypes.c_int32),
         ("ms", ctypes.c_double * len(STAGES)), ("ms_total", ctypes.c_double),
         ("level_frontier", ctypes.c_int64 * MAX_LEVEL_STATS), ("level_raw", ctypes.c_int64 * MAX_LEVEL_STATS),
         ("level_new_states", ctypes.c_int64 * MAX_LEVEL_STATS),
@@ -269,6 +273,9 @@ def stats_dict(s: _Stats) -> dict:
         "n_rehash": int(s.n_rehash), "n_grow": int(s.n_grow), "n_emit_launches": int(s.n_emit_launches),
         "n_kernel_launches": int(s.n_kernel_launches),
         "n_resolve": int(s.n_resolve), "n_resolved_arcs": int(s.n_resolved_arcs),
+        **{k: int(getattr(s, k)) for k in ("rs_scatter_recs", "rs_scatter_dest_recs", "rs_dedupe_arcs", "rs_dedupe_states",
+                                           "rs_dedupe_new", "rs_gather_recs", "rs_scatter_launches", "rs_dedupe_launches",
+                                           "rs_gather_launches")},
         "ms": {k: float(s.ms[i]) for i, k in enumerate(STAGES)}, "ms_total": float(s.ms_total),
         "level_frontier": [int(s.level_frontier[i]) for i in range(nl)],
         "level_raw": [int(s.level_raw[i]) for i in range(nl)],
