@@ -272,6 +272,12 @@ __device__ __forceinline__ uint4 ld_keep(const uint4 *ptr, uint64_t policy) {
 #endif
 constexpr int64_t RESOLVE_MIN_ARCS = FSTC_RESOLVE_MIN_ARCS;          // smaller levels always use the table
 constexpr uint64_t RESOLVE_TABLE_BYTES = 96ull << 20;               // a table beyond this no longer lives in L2
+// unit costs measured on a B200, in picoseconds
+constexpr double COST_PROBE_PS = 21.0;            // random 32-byte sector read: one probe
+constexpr double COST_INSERT_PS = 75.0;           // CAS write-back + id publish of a new state
+constexpr double COST_STREAM_PS_PER_BYTE = 0.2;   // memset / streaming at ~5 TB/s
+constexpr double COST_PART_ARC_PS = 45.0;         // keys + 2 scatter passes + dedupe + 2 gathers, per arc
+constexpr double COST_PART_STATE_PS = 30.0;       // re-entering an existing state, per level
 constexpr int EM_THREADS = FSTC_EM_THREADS;
 constexpr int EM_IPT = 4;                          // consecutive output ranks per thread
 constexpr int EM_TILE = EM_THREADS * EM_IPT;       // 512 arcs per block
@@ -1075,26 +1081,26 @@ fstc_result_t *Composer::run() {
         const uint64_t remaining_pairs = n_pairs_total - static_cast<uint64_t>(n_states);
         const int64_t new_bound = static_cast<int64_t>(std::min<uint64_t>(static_cast<uint64_t>(R), remaining_pairs));
         if (n_states + new_bound >= 0x7FFFFFFFll) fail(FSTC_ERR_CAPACITY, "more than 2^31-1 states");
-        // ---- how this level resolves its target ids: the visited table while it stays small
-        // enough to live in L2, else the streaming partitioned resolve.  The switch is one-way: the table is dropped.
+        // ---- how this level resolves its target ids, decided per level from measured unit costs: the
+        // visited table pays a random DRAM read per arc and a random write-back + publish per NEW state (and a rebuild
+        // if it was dropped or must grow); the partitioned resolve pays streaming passes per arc and per existing state.
+        auto prefer_partitioned = [&](int64_t r, int64_t bound, int64_t states_now, uint64_t slots_ready) {
+            if (o.resolve_mode == FSTC_RESOLVE_TABLE) return false;
+            if (key_bits + bits_for(static_cast<uint64_t>(states_now + bound)) > 64) return false;   // state records: key << id_bits | id
+            if (o.resolve_mode == FSTC_RESOLVE_PARTITIONED) return true;
+            const uint64_t slots = slots_for(states_now + bound);
+            if (r < RESOLVE_MIN_ARCS || slots * sizeof(uint4) <= RESOLVE_TABLE_BYTES) return false;  // small, or the table lives in L2
+            double t_table = COST_PROBE_PS * r + COST_INSERT_PS * bound;
+            if (slots > slots_ready) t_table += COST_INSERT_PS * 0.6 * states_now + COST_STREAM_PS_PER_BYTE * 16.0 * slots;
+            const double t_part = COST_PART_ARC_PS * r + COST_PART_STATE_PS * states_now + 1e9;      // + 1 ms of launches
+            // a clear win only: leaving the table also costs the next table level a rebuild, and ids in bin order cost
+            // the next level's count / match their cache locality
+            return t_part < 0.6 * t_table;
+        };
         {
-            const int id_bits = bits_for(static_cast<uint64_t>(n_states + new_bound));
-            const bool fits = key_bits + id_bits <= 64;                // state records are key << id_bits | id
-            if (!partitioned) {
-                bool want = o.resolve_mode == FSTC_RESOLVE_PARTITIONED;
-                if (o.resolve_mode == FSTC_RESOLVE_AUTO)
-                    want = R >= RESOLVE_MIN_ARCS && slots_for(n_states + new_bound) * sizeof(uint4) > RESOLVE_TABLE_BYTES;
-                // later levels must fit too, unless this is the last level: bound the number of states the run can reach
-                uint64_t max_states = std::min<uint64_t>(n_pairs_total, 0x7FFFFFFFull);
-                if (o.max_raw_arcs > 0) max_states = std::min<uint64_t>(max_states, static_cast<uint64_t>(o.max_raw_arcs) + 1);
-                if (want && fits && (key_bits + bits_for(max_states) <= 64 || stop_after)) {
-                    partitioned = true;
-                    table = DBuf<uint4>();
-                    cap = 0;
-                }
-            } else if (!fits) {
-                fail(FSTC_ERR_CAPACITY, "%d-bit pair keys with %d-bit state ids do not fit the partitioned resolve", key_bits, id_bits);
-            }
+            const bool want = prefer_partitioned(R, new_bound, n_states, cap);
+            if (want && !partitioned) { table = DBuf<uint4>(); cap = 0; }    // the table is dropped; ensure_table rebuilds it from pair[]
+            partitioned = want;
         }
         // look-ahead: if the search goes on, the next level is about (new states) x (arcs per expanded pair)
         int64_t next_R = 0, next_S = 0;
@@ -1121,9 +1127,9 @@ fstc_result_t *Composer::run() {
         }
         ensure_pairs(n_states + new_bound, n_states + new_bound + next_S);
         if (!partitioned) {
-            // no look-ahead for the table if the next level will leave it for the partitioned resolve anyway
-            const bool next_partitioned = o.resolve_mode == FSTC_RESOLVE_AUTO && next_R >= RESOLVE_MIN_ARCS &&
-                                          slots_for(n_states + new_bound + next_S) * sizeof(uint4) > RESOLVE_TABLE_BYTES;
+            // no look-ahead for the table if the next level is expected to leave it for the partitioned resolve anyway
+            const bool next_partitioned = next_R > 0 && prefer_partitioned(next_R, next_S, n_states + new_bound,
+                                                                           slots_for(n_states + new_bound + next_S));
             ensure_table(n_states + new_bound, next_partitioned ? 0 : n_states + new_bound + next_S);
         }
         ensure_arcs(n_arcs + R, n_arcs + R + next_R);
