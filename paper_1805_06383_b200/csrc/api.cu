@@ -51,7 +51,11 @@ struct ArenaChunk {
 struct Arena {
     std::vector<ArenaChunk> chunks;
     std::unordered_map<void *, std::pair<int, size_t>> live;   // pointer -> (chunk, length)
-    ~Arena() {}                                             // chunks die with the context
+    ~Arena() {                                              // the thread ends: its calls are complete, give the chunks back
+        for (auto &ch : chunks)
+            if (ch.base) (void)cudaFreeAsync(ch.base, nullptr);
+        (void)cudaGetLastError();                           // (at process exit the context may already be gone)
+    }
 };
 thread_local Arena g_arena;
 constexpr size_t ARENA_ALIGN = 512;
