@@ -48,9 +48,10 @@ struct SegView {
     int n_seg;
 };
 
-constexpr int SC_TILE = 4096;
+// Tile of a scatter pass (template parameter): 8192 for the first pass — its runs are twice as long, which makes the
+// last gather, the one that writes the target column, read whole sectors — and 4096 for the second.
+constexpr int SC_TILE_BIG = 8192, SC_TILE_SMALL = 4096;
 constexpr int SC_THREADS = 512;
-constexpr int SC_IPT = SC_TILE / SC_THREADS;
 constexpr int SC_MAX_BINS = 1024;
 
 // tile_first[s] = number of tiles of the segments before s; tile_first[n_seg] = total.  n_seg <= 1024.
@@ -128,8 +129,9 @@ struct ScatterArgs {
 #ifndef FSTC_SC_MINB
 #define FSTC_SC_MINB 3
 #endif
-template <bool DEST>
-__global__ void __launch_bounds__(SC_THREADS, FSTC_SC_MINB) rs_scatter(ScatterArgs a) {
+template <bool DEST, int SC_TILE>
+__global__ void __launch_bounds__(SC_THREADS, SC_TILE == SC_TILE_BIG ? 2 : FSTC_SC_MINB) rs_scatter(ScatterArgs a) {
+    constexpr int SC_IPT = SC_TILE / SC_THREADS;
     extern __shared__ unsigned long long sorted[];             // [SC_TILE] records, then uint32 smeta[SC_TILE]
     uint32_t *smeta = reinterpret_cast<uint32_t *>(sorted + SC_TILE);   // tile-local input index << 16 | bin
     __shared__ uint32_t cnt[SC_MAX_BINS];                       // count, then first slot of the bin in sorted[]
@@ -351,8 +353,10 @@ __global__ void __launch_bounds__(DD_THREADS) rs_dedupe(DedupeArgs a) {
 // drops it at the record's input index in shared memory; the tile is then written out in input order.
 // MODE 0: out[input index] = id (ids of the previous pass's buffer, or the target column when in rank order)
 // MODE 1: o_tgt[pos[rank]] = id;  MODE 2: id into the target field (key bits shift_t and up) of sort record `rank`.
-constexpr int GA_THREADS = 512;
-constexpr int GA_IPT = SC_TILE / GA_THREADS;
+#ifndef FSTC_GA_THREADS
+#define FSTC_GA_THREADS 512
+#endif
+constexpr int GA_THREADS = FSTC_GA_THREADS;
 
 struct GatherArgs {
     SegView seg;                    // the INPUT segments of the pass that is undone
@@ -367,8 +371,9 @@ struct GatherArgs {
     int shift_t;
 };
 
-template <int MODE>
+template <int MODE, int SC_TILE>
 __global__ void __launch_bounds__(GA_THREADS) rs_gather_ids(GatherArgs a) {
+    constexpr int GA_IPT = SC_TILE / GA_THREADS;
     __shared__ uint32_t s_id[SC_TILE];
     __shared__ int s_seg;
     const int tid = threadIdx.x;
@@ -485,7 +490,9 @@ SegSet single_segment(Ctx &c, const unsigned long long *data, int64_t n) {
 // One staged scatter pass: every segment of `in` is split into `nbins` bins.  Bin capacities are a guess from
 // uniform hashing; if a bin overflows, the cursors of the failed attempt hold the exact counts and the pass runs
 // once more with those.  dest (optional): [in.length], where every input record went.
-SegSet scatter_pass(Ctx &c, const SegSet &in, int shift, int hshift, int nbins, DBuf<uint32_t> *dest, DBuf<uint16_t> *perm) {
+SegSet scatter_pass(Ctx &c, const SegSet &in, int shift, int hshift, int nbins, bool big_tile, DBuf<uint32_t> *dest,
+                    DBuf<uint16_t> *perm) {
+    const int SC_TILE = big_tile ? SC_TILE_BIG : SC_TILE_SMALL;
     if (in.n_seg > 1024 || nbins > SC_MAX_BINS) fail(FSTC_ERR_CAPACITY, "resolve: too many segments (%lld x %d)",
                                                     static_cast<long long>(in.n_seg), nbins);
     const int64_t nb = in.n_seg * nbins;
@@ -502,8 +509,11 @@ SegSet scatter_pass(Ctx &c, const SegSet &in, int shift, int hshift, int nbins, 
     if (dest) { dest->alloc(c, in.length); perm->alloc(c, in.length); }
     static bool attr_set = false;
     if (!attr_set) {
-        FSTC_CUDA(cudaFuncSetAttribute(rs_scatter<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
-        FSTC_CUDA(cudaFuncSetAttribute(rs_scatter<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
+        const int s_big = SC_TILE_BIG * 12, s_small = SC_TILE_SMALL * 12;
+        FSTC_CUDA(cudaFuncSetAttribute(rs_scatter<false, SC_TILE_BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, s_big));
+        FSTC_CUDA(cudaFuncSetAttribute(rs_scatter<true, SC_TILE_BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, s_big));
+        FSTC_CUDA(cudaFuncSetAttribute(rs_scatter<false, SC_TILE_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, s_small));
+        FSTC_CUDA(cudaFuncSetAttribute(rs_scatter<true, SC_TILE_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, s_small));
         attr_set = true;
     }
     for (int attempt = 0;; ++attempt) {
@@ -524,8 +534,11 @@ SegSet scatter_pass(Ctx &c, const SegSet &in, int shift, int hshift, int nbins, 
             ScatterArgs a{in.view(), tile_first.p, out.own.p, out.start.p, cursor.p, dest ? dest->p : nullptr, dest ? perm->p : nullptr,
                           cur_stride, shift, hshift, nbins};
             const int h = g_trace.begin(c, dest ? "scatter+dest" : "scatter", totals[0] * SC_TILE, FSTC_T_RS_SCATTER);
-            if (dest) rs_scatter<true><<<static_cast<unsigned>(totals[0]), SC_THREADS, smem, c.stream>>>(a);
-            else rs_scatter<false><<<static_cast<unsigned>(totals[0]), SC_THREADS, smem, c.stream>>>(a);
+            const unsigned grid = static_cast<unsigned>(totals[0]);
+            if (dest && big_tile) rs_scatter<true, SC_TILE_BIG><<<grid, SC_THREADS, smem, c.stream>>>(a);
+            else if (dest) rs_scatter<true, SC_TILE_SMALL><<<grid, SC_THREADS, smem, c.stream>>>(a);
+            else if (big_tile) rs_scatter<false, SC_TILE_BIG><<<grid, SC_THREADS, smem, c.stream>>>(a);
+            else rs_scatter<false, SC_TILE_SMALL><<<grid, SC_THREADS, smem, c.stream>>>(a);
             FSTC_LAUNCH_CHECK();
             g_trace.end(c, h);
         }
@@ -543,7 +556,8 @@ SegSet scatter_pass(Ctx &c, const SegSet &in, int shift, int hshift, int nbins, 
 }
 
 // undoes one scatter pass (or, with dest = null, just delivers the ids): see rs_gather_ids
-void gather_pass(Ctx &c, const SegSet &seg, int mode, GatherArgs a) {
+void gather_pass(Ctx &c, const SegSet &seg, int mode, bool big_tile, GatherArgs a) {
+    const int SC_TILE = big_tile ? SC_TILE_BIG : SC_TILE_SMALL;
     DBuf<int64_t> tile_first(c, seg.n_seg + 1);
     rs_seg_tiles<<<1, 1024, 0, c.stream>>>(seg.view(), SC_TILE, tile_first.p);
     FSTC_LAUNCH_CHECK();
@@ -553,9 +567,15 @@ void gather_pass(Ctx &c, const SegSet &seg, int mode, GatherArgs a) {
     if (tiles > 0) {
         const int h = g_trace.begin(c, mode == 0 && a.dest ? "gather" : "apply", tiles * SC_TILE, FSTC_T_RS_GATHER);
         const unsigned grid = static_cast<unsigned>(tiles);
-        if (mode == 0) rs_gather_ids<0><<<grid, GA_THREADS, 0, c.stream>>>(a);
-        else if (mode == 1) rs_gather_ids<1><<<grid, GA_THREADS, 0, c.stream>>>(a);
-        else rs_gather_ids<2><<<grid, GA_THREADS, 0, c.stream>>>(a);
+        if (big_tile) {
+            if (mode == 0) rs_gather_ids<0, SC_TILE_BIG><<<grid, GA_THREADS, 0, c.stream>>>(a);
+            else if (mode == 1) rs_gather_ids<1, SC_TILE_BIG><<<grid, GA_THREADS, 0, c.stream>>>(a);
+            else rs_gather_ids<2, SC_TILE_BIG><<<grid, GA_THREADS, 0, c.stream>>>(a);
+        } else {
+            if (mode == 0) rs_gather_ids<0, SC_TILE_SMALL><<<grid, GA_THREADS, 0, c.stream>>>(a);
+            else if (mode == 1) rs_gather_ids<1, SC_TILE_SMALL><<<grid, GA_THREADS, 0, c.stream>>>(a);
+            else rs_gather_ids<2, SC_TILE_SMALL><<<grid, GA_THREADS, 0, c.stream>>>(a);
+        }
         FSTC_LAUNCH_CHECK();
         g_trace.end(c, h);
     }
@@ -587,16 +607,16 @@ void resolve_partitioned(Ctx &c, const ResolveJob &j) {
         FSTC_LAUNCH_CHECK();
         c.n_launch += 1;
         SegSet st = single_segment(c, st_recs.p, j.n_states_before);
-        if (b1 > 0) st = scatter_pass(c, st, ib, 64 - b1, 1 << b1, nullptr, nullptr);
-        if (b2 > 0) st = scatter_pass(c, st, ib, 64 - b1 - b2, 1 << b2, nullptr, nullptr);
+        if (b1 > 0) st = scatter_pass(c, st, ib, 64 - b1, 1 << b1, true, nullptr, nullptr);
+        if (b2 > 0) st = scatter_pass(c, st, ib, 64 - b1 - b2, 1 << b2, false, nullptr, nullptr);
         if (bits > 0) st_recs.release();
         const int h_st = g_trace.begin(c, "(states done)", 0); g_trace.end(c, h_st);
         SegSet lvl0 = single_segment(c, j.keys, j.n_records), lvl1, lvl2;
         DBuf<uint32_t> dest1, dest2;
         DBuf<uint16_t> perm1, perm2;
-        if (b1 > 0) lvl1 = scatter_pass(c, lvl0, 0, 64 - b1, 1 << b1, &dest1, &perm1);
+        if (b1 > 0) lvl1 = scatter_pass(c, lvl0, 0, 64 - b1, 1 << b1, true, &dest1, &perm1);
         if (b2 > 0) {
-            lvl2 = scatter_pass(c, lvl1, 0, 64 - b1 - b2, 1 << b2, &dest2, &perm2);
+            lvl2 = scatter_pass(c, lvl1, 0, 64 - b1 - b2, 1 << b2, false, &dest2, &perm2);
             lvl1.own.release();                                  // only the segment table of level 1 is needed from here on
         }
         const SegSet &arcs = b2 > 0 ? lvl2 : (b1 > 0 ? lvl1 : lvl0);
@@ -635,13 +655,13 @@ void resolve_partitioned(Ctx &c, const ResolveJob &j) {
             ids_mid.alloc(c, lvl1.length);
             GatherArgs g{};
             g.dest = dest2.p; g.perm = perm2.p; g.in = ids_last.p; g.out = ids_mid.p;
-            gather_pass(c, lvl1, 0, g);
+            gather_pass(c, lvl1, 0, false, g);
             ids = ids_mid.p;
         }
         GatherArgs g{};
         g.dest = b1 > 0 ? dest1.p : nullptr; g.perm = perm1.p; g.in = ids;
         g.out = reinterpret_cast<uint32_t *>(j.o_tgt); g.pos = j.pos; g.o_tgt = j.o_tgt; g.sortrec = j.sortrec; g.shift_t = j.shift_t;
-        gather_pass(c, lvl0, j.mode, g);
+        gather_pass(c, lvl0, j.mode, true, g);
         g_trace.end(c, h_all);
         c.sync();                                                // temporaries are released below
         if (g_trace.on) g_trace.report(j.stats ? j.stats->ms : nullptr);
