@@ -306,6 +306,7 @@ struct EmitArgs {
     int shift_t, bits_b;
     const int64_t *tile_m;   // [n_tiles+1] match index holding the first rank of every tile
     unsigned long long *keys;     // KEYS: [R] target key of every rank, for the partitioned resolve
+    int q2_bits;                  // KEYS: the resolve key is (r1 << q2_bits) | r2
     uint32_t *posout;             // KEYS + INDIRECT: [R] output position of every rank (relative to arc_base)
 };
 
@@ -411,7 +412,7 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
             a_sym[u] = e1.y; b_sym[u] = e2.y;
             w[u] = __uint_as_float(e1.z) * __uint_as_float(e2.z);
             tgt_pair[u] = make_int2(static_cast<int>(e1.x), static_cast<int>(e2.x));
-            key[u] = static_cast<uint64_t>(e1.x) * g.nq2 + e2.x;
+            key[u] = KEYS ? ((static_cast<unsigned long long>(e1.x) << g.q2_bits) | e2.x) : static_cast<uint64_t>(e1.x) * g.nq2 + e2.x;
             todo |= 1u << u;
         }
     }
@@ -876,6 +877,7 @@ struct Composer {
         g.o_src = a_src.p; g.o_il = a_il.p; g.o_ol = a_ol.p; g.o_tgt = a_tgt.p; g.o_w = a_w.p;
         g.sortrec = sortrec; g.shift_t = shift_t; g.bits_b = bits_b; g.tile_m = tile_m.p;
         g.keys = nullptr; g.posout = nullptr;
+        g.q2_bits = bits_for(nq2 > 1 ? nq2 - 1 : 1);
         const unsigned grid = static_cast<unsigned>(n_tiles);
         DBuf<unsigned long long> keys;
         DBuf<uint32_t> posout;
@@ -897,8 +899,9 @@ struct Composer {
         st.n_emit_launches += 1;
         if (partitioned) {
             ResolveJob j;
-            j.keys = keys.p; j.n_records = R; j.key_bits = key_bits;
-            j.pair = pair.p; j.n_states_before = n_states_live; j.nq2 = nq2;
+            j.keys = keys.p; j.n_records = R; j.q2_bits = g.q2_bits;
+            j.key_bits = g.q2_bits + bits_for(static_cast<uint64_t>(m1.n_states > 1 ? m1.n_states - 1 : 1));
+            j.pair = pair.p; j.n_states_before = n_states_live;
             j.n_states = d_counters.p;
             j.mode = mode == EMIT_DIRECT ? 0 : (mode == EMIT_INDIRECT ? 1 : 2);
             j.pos = posout.p;
@@ -1084,9 +1087,10 @@ fstc_result_t *Composer::run() {
         // ---- how this level resolves its target ids, decided per level from measured unit costs: the
         // visited table pays a random DRAM read per arc and a random write-back + publish per NEW state (and a rebuild
         // if it was dropped or must grow); the partitioned resolve pays streaming passes per arc and per existing state.
+        const int rkey_bits = bits_for(nq2 > 1 ? nq2 - 1 : 1) + bits_for(static_cast<uint64_t>(m1.n_states > 1 ? m1.n_states - 1 : 1));
         auto prefer_partitioned = [&](int64_t r, int64_t bound, int64_t states_now, uint64_t slots_ready) {
             if (o.resolve_mode == FSTC_RESOLVE_TABLE) return false;
-            if (key_bits + bits_for(static_cast<uint64_t>(states_now + bound)) > 64) return false;   // state records: key << id_bits | id
+            if (rkey_bits + bits_for(static_cast<uint64_t>(states_now + bound)) > 64) return false;  // state records: key << id_bits | id
             if (o.resolve_mode == FSTC_RESOLVE_PARTITIONED) return true;
             const uint64_t slots = slots_for(states_now + bound);
             if (r < RESOLVE_MIN_ARCS || slots * sizeof(uint4) <= RESOLVE_TABLE_BYTES) return false;  // small, or the table lives in L2

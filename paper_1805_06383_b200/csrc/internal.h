@@ -57,12 +57,12 @@ void free_result(fstc_result_t *r);
 // the target keys are hash-partitioned with streaming passes, deduplicated per bin in shared memory against the
 // existing states, and the ids gathered back through the recorded permutations.
 struct ResolveJob {
-    const unsigned long long *keys;     // [n_records] target key q1*|Q2|+q2 of every composed arc, in rank order
+    const unsigned long long *keys;     // [n_records] target (q1 << q2_bits) | q2 of every composed arc, in rank order
     int64_t n_records;
-    int key_bits;
+    int key_bits;                       // bits of such a key
+    int q2_bits;
     int2 *pair;                         // [>= n_states_before + new states] id -> (q1, q2); new entries are written
     int64_t n_states_before;
-    uint64_t nq2;
     unsigned long long *n_states;       // device counter: set to n_states_before, advanced by the new states
     int mode;                           // 0: o_tgt[r] = id   1: o_tgt[pos[r]] = id   2: id into sortrec[r]
     const uint32_t *pos;                // mode 1

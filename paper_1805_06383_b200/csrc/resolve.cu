@@ -232,12 +232,14 @@ constexpr int DD_THREADS = 256;
 constexpr int DD_IPT = 4;
 constexpr int DD_TILE = DD_THREADS * DD_IPT;
 #ifndef FSTC_DD_SLOTS
-#define FSTC_DD_SLOTS 2048
+#define FSTC_DD_SLOTS 4096
 #endif
 #ifndef FSTC_DD_TARGET
-#define FSTC_DD_TARGET 1000
+#define FSTC_DD_TARGET 2000
 #endif
-constexpr int DD_SLOTS = FSTC_DD_SLOTS;        // keys 8 B + ids 4 B per slot, in shared memory
+constexpr int DD_SLOTS = FSTC_DD_SLOTS;        // keys 8 B + ids 4 B per slot, in shared memory (a power of two)
+constexpr int DD_SLOT_BITS = DD_SLOTS == 2048 ? 11 : (DD_SLOTS == 4096 ? 12 : (DD_SLOTS == 8192 ? 13 : -1));
+static_assert(DD_SLOT_BITS > 0, "DD_SLOTS must be 2048, 4096 or 8192");
 constexpr int DD_TARGET = FSTC_DD_TARGET;      // aimed maximum of the mean number of distinct keys per bin
 
 struct DedupeArgs {
@@ -245,35 +247,27 @@ struct DedupeArgs {
     SegView arcs;              // arc records    key
     int ib;
     uint32_t *ids_out;         // [length of the arc buffer]
-    uint64_t nq2, nq2_inv;     // |Q2| and floor(2^64 / |Q2|)
+    int q2_bits;               // a key is (q1 << q2_bits) | q2
     unsigned long long *n_states;
     int2 *pair;
     unsigned *err;             // set when a bin holds more distinct keys than the shared-memory map
 };
 
 __device__ __forceinline__ int dd_find_or_claim(unsigned long long *keys, unsigned long long key, bool *won) {
-    uint32_t s = static_cast<uint32_t>(rmix64(key)) & (DD_SLOTS - 1);   // low hash bits: the bins use the top ones
+    // the bins took the top bits of mix64(key); inside a bin a multiplicative hash of the folded key is independent enough
+    uint32_t s = ((static_cast<uint32_t>(key) ^ (static_cast<uint32_t>(key >> 32) * 0x85EBCA6Bu)) * 0x9E3779B1u) >> (32 - DD_SLOT_BITS);
     for (int probes = 0; probes < DD_SLOTS; ++probes) {
         const unsigned long long old = atomicCAS(&keys[s], RS_EMPTY, key);
         if (old == RS_EMPTY) { *won = true; return static_cast<int>(s); }
         if (old == key) { *won = false; return static_cast<int>(s); }
-        s = (s + 1) & (DD_SLOTS - 1);
+        s = (s + static_cast<uint32_t>(probes) + 1) & (DD_SLOTS - 1);   // triangular steps: no primary clustering, every slot is visited
     }
     return -1;
 }
 
-// key = q1 * nq2 + q2 -> (q1, q2) with one multiply-high and a correction step instead of a 64-bit division
-__device__ __forceinline__ int2 dd_split_key(unsigned long long key, uint64_t nq2, uint64_t nq2_inv) {
-    unsigned long long q1 = __umul64hi(key, nq2_inv);
-    long long r = static_cast<long long>(key - q1 * nq2);
-    if (r >= static_cast<long long>(nq2)) { q1 += 1; r -= static_cast<long long>(nq2); }
-    if (r >= static_cast<long long>(nq2)) { q1 += 1; r -= static_cast<long long>(nq2); }
-    return make_int2(static_cast<int>(q1), static_cast<int>(r));
-}
-
 __global__ void __launch_bounds__(DD_THREADS) rs_dedupe(DedupeArgs a) {
-    __shared__ unsigned long long keys[DD_SLOTS];
-    __shared__ uint32_t ids[DD_SLOTS];
+    extern __shared__ unsigned long long keys[];               // [DD_SLOTS], then uint32 ids[DD_SLOTS]
+    uint32_t *ids = reinterpret_cast<uint32_t *>(keys + DD_SLOTS);
     __shared__ uint32_t s_warp[DD_THREADS / 32];
     __shared__ unsigned long long s_base;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -335,7 +329,7 @@ __global__ void __launch_bounds__(DD_THREADS) rs_dedupe(DedupeArgs a) {
             if (wonmask >> u & 1u) {
                 const uint32_t id = next_id++;
                 ids[slot[u]] = id;
-                a.pair[id] = dd_split_key(key[u], a.nq2, a.nq2_inv);
+                a.pair[id] = make_int2(static_cast<int>(key[u] >> a.q2_bits), static_cast<int>(key[u] & ((1ull << a.q2_bits) - 1)));
             }
         }
         __syncthreads();
@@ -417,12 +411,12 @@ __global__ void __launch_bounds__(GA_THREADS) rs_gather_ids(GatherArgs a) {
 }
 
 // state records key << ib | id, in id order
-__global__ void rs_state_records(const int2 *__restrict__ pair, int64_t n, uint64_t nq2, int ib,
+__global__ void rs_state_records(const int2 *__restrict__ pair, int64_t n, int q2_bits, int ib,
                                  unsigned long long *__restrict__ out) {
     const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const int2 p = pair[i];
-    const unsigned long long key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
+    const unsigned long long key = (static_cast<unsigned long long>(static_cast<uint32_t>(p.x)) << q2_bits) | static_cast<uint32_t>(p.y);
     out[i] = (key << ib) | static_cast<unsigned long long>(i);
 }
 
@@ -591,11 +585,15 @@ int resolve_bits_needed(int64_t n_records_and_states) {
 }
 
 void resolve_partitioned(Ctx &c, const ResolveJob &j) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        FSTC_CUDA(cudaFuncSetAttribute(rs_dedupe, cudaFuncAttributeMaxDynamicSharedMemorySize, DD_SLOTS * 12));
+        attr_set = true;
+    }
     const int ib = bits_for(static_cast<uint64_t>(j.n_states_before > 1 ? j.n_states_before - 1 : 1));
     if (j.key_bits + ib > 64) fail(FSTC_ERR_CAPACITY, "resolve: key (%d bits) + state id (%d bits) exceed 64 bits", j.key_bits, ib);
     if (j.n_records >= 0xFFFFFFFFll) fail(FSTC_ERR_CAPACITY, "resolve: more than 2^32 records");
     int bits = j.force_bits >= 0 ? j.force_bits : resolve_bits_needed(j.n_states_before + j.n_records);
-    const uint64_t nq2_inv = j.nq2 > 1 ? ~0ull / j.nq2 : ~0ull;      // floor((2^64-1)/d): at most 1 below floor(2^64/d)
     g_trace.on = g_trace.print || j.profile;
     const int h_all = g_trace.begin(c, "RESOLVE TOTAL", j.n_records);
     for (;; ++bits) {
@@ -603,7 +601,7 @@ void resolve_partitioned(Ctx &c, const ResolveJob &j) {
         const int b1 = bits < 10 ? bits : 10, b2 = bits - b1;
         // 1-2. records of the existing states and keys of the arcs, partitioned the same way
         DBuf<unsigned long long> st_recs(c, j.n_states_before);
-        rs_state_records<<<rs_blocks(j.n_states_before), 256, 0, c.stream>>>(j.pair, j.n_states_before, j.nq2, ib, st_recs.p);
+        rs_state_records<<<rs_blocks(j.n_states_before), 256, 0, c.stream>>>(j.pair, j.n_states_before, j.q2_bits, ib, st_recs.p);
         FSTC_LAUNCH_CHECK();
         c.n_launch += 1;
         SegSet st = single_segment(c, st_recs.p, j.n_states_before);
@@ -628,9 +626,9 @@ void resolve_partitioned(Ctx &c, const ResolveJob &j) {
         FSTC_CUDA(cudaMemsetAsync(err.p, 0, sizeof(unsigned), c.stream));
         const unsigned long long n_before = static_cast<unsigned long long>(j.n_states_before);
         FSTC_CUDA(cudaMemcpyAsync(j.n_states, &n_before, sizeof n_before, cudaMemcpyHostToDevice, c.stream));
-        DedupeArgs d{st.view(), arcs.view(), ib, ids_last.p, j.nq2, nq2_inv, j.n_states, j.pair, err.p};
+        DedupeArgs d{st.view(), arcs.view(), ib, ids_last.p, j.q2_bits, j.n_states, j.pair, err.p};
         const int hd = g_trace.begin(c, "dedupe", nb, FSTC_T_RS_DEDUPE);
-        rs_dedupe<<<static_cast<unsigned>(nb), DD_THREADS, 0, c.stream>>>(d);
+        rs_dedupe<<<static_cast<unsigned>(nb), DD_THREADS, DD_SLOTS * 12, c.stream>>>(d);
         FSTC_LAUNCH_CHECK();
         g_trace.end(c, hd);
         c.n_launch += 1;
