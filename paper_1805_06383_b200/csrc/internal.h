@@ -10,14 +10,14 @@ namespace fstc {
 // ---------------------------------------------------------------- radix sort (radix_sort.cu)
 // Records are 16 bytes: {x,y} = 64-bit key (x low word), z = 32-bit high key ("src"), w = payload.
 // The sort order is (z, key64) ascending, restricted to the bits the passes name; it is a stable
-// least-significant-digit radix sort with digits of up to 8 bits.
+// least-significant-digit radix sort with digits of up to 8 bits that may straddle key and z.
 struct SortPass {
-    int word;   // 0: digit taken from the 64-bit key; 1: from z
-    int shift;  // bit offset inside that word
+    int word;   // number of key bits: a record sorts as the number (z << key_bits) | key64
+    int shift;  // bit offset of the digit inside that number (a digit may straddle key and z)
     int bits;   // 1..8
 };
-// LSD pass list covering key bits [0, key_bits) then z bits [0, z_bits).
-std::vector<SortPass> make_sort_passes(int key_bits, int z_bits);
+// LSD pass list over bits [from_bit, key_bits + z_bits) of (z << key_bits) | key, 8 bits at a time.
+std::vector<SortPass> make_sort_passes(int key_bits, int z_bits, int from_bit = 0);
 // Sorts n records.  `a` holds the input; `b` is scratch of the same size.  Returns the buffer
 // (a or b) that holds the sorted records.
 uint4 *radix_sort_records(Ctx &c, uint4 *a, uint4 *b, int64_t n, const std::vector<SortPass> &passes);

@@ -216,9 +216,8 @@ fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side) {
         pk_flags_rekey<<<blocks_for(n), PK_THREADS, 0, c.stream>>>(s1, n, bi, bt, bo, flags32.p, o1);
         FSTC_LAUNCH_CHECK();
         // stable sort on (src, inner) only: (outer, tgt) order inside a segment is inherited from sort #1
-        std::vector<SortPass> p2;
-        for (int s = 0; s < bi; s += 8) p2.push_back(SortPass{0, bo + bt + s, bi - s < 8 ? bi - s : 8});
-        for (int s = 0; s < bs; s += 8) p2.push_back(SortPass{1, s, bs - s < 8 ? bs - s : 8});
+        // only the (inner, src) bits: the key is (inner, outer, tgt) with inner on top, directly below z = src
+        std::vector<SortPass> p2 = make_sort_passes(bi + bo + bt, bs, bo + bt);
         uint4 *s2 = radix_sort_records(c, o1, s1, n, p2);
         DBuf<uint32_t> head(c, n);
         DBuf<int64_t> seg_idx(c, n + 1);

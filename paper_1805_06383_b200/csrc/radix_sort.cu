@@ -16,12 +16,14 @@ constexpr int RS_ITEMS = 8;
 constexpr int RS_TILE = RS_THREADS * RS_ITEMS;   // 2048 records = 32 KB per tile
 constexpr int RS_RADIX = 256;
 
-__device__ __forceinline__ uint32_t digit_of(const uint4 &r, int word, int shift, uint32_t mask) {
-    if (word == 0) {
-        uint64_t k = (static_cast<uint64_t>(r.y) << 32) | r.x;
-        return static_cast<uint32_t>(k >> shift) & mask;
-    }
-    return (r.z >> shift) & mask;
+// A record sorts as the number (z << key_bits) | key; a digit is `mask` at bit `shift` of it and may straddle the two.
+// `word` carries key_bits.
+__device__ __forceinline__ uint32_t digit_of(const uint4 &r, int key_bits, int shift, uint32_t mask) {
+    const uint64_t k = (static_cast<uint64_t>(r.y) << 32) | r.x;
+    const uint64_t lo = shift < key_bits ? k >> shift : 0ull;
+    const uint64_t hi = shift <= key_bits ? (key_bits - shift < 64 ? static_cast<uint64_t>(r.z) << (key_bits - shift) : 0ull)
+                                          : static_cast<uint64_t>(r.z) >> (shift - key_bits);
+    return static_cast<uint32_t>(lo | hi) & mask;
 }
 
 __global__ void __launch_bounds__(RS_THREADS) rs_upsweep(const uint4 *__restrict__ in, int64_t n,
@@ -109,10 +111,10 @@ __global__ void __launch_bounds__(RS_THREADS) rs_downsweep(const uint4 *__restri
 
 }  // namespace
 
-std::vector<SortPass> make_sort_passes(int key_bits, int z_bits) {
+std::vector<SortPass> make_sort_passes(int key_bits, int z_bits, int from_bit) {
     std::vector<SortPass> p;
-    for (int s = 0; s < key_bits; s += 8) p.push_back(SortPass{0, s, key_bits - s < 8 ? key_bits - s : 8});
-    for (int s = 0; s < z_bits; s += 8) p.push_back(SortPass{1, s, z_bits - s < 8 ? z_bits - s : 8});
+    const int total = key_bits + z_bits;
+    for (int s = from_bit; s < total; s += 8) p.push_back(SortPass{key_bits, s, total - s < 8 ? total - s : 8});
     return p;
 }
 
