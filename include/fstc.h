@@ -91,8 +91,10 @@ enum {
 
 enum {
   FSTC_RESOLVE_AUTO = 0,        /* per level: the table while it fits the L2 cache, else the partitioned resolve */
-  FSTC_RESOLVE_TABLE = 1,       /* always the open-addressing visited table (atomicCAS per arc, :237 adapted)  */
-  FSTC_RESOLVE_PARTITIONED = 2  /* always the streaming hash-partitioned resolve         */
+  FSTC_RESOLVE_TABLE = 1,       /* always a visited table (atomicCAS per arc, :237): the paper's dense table of one
+                                   entry per pair when |Q1||Q2| <= 2^29, else the open-addressing hash table   */
+  FSTC_RESOLVE_PARTITIONED = 2, /* always the streaming hash-partitioned resolve         */
+  FSTC_RESOLVE_HASH = 3         /* always the open-addressing hash table, whatever |Q1||Q2|                    */
 };
 
 /* Options; NULL or all-zero = defaults. */

@@ -83,6 +83,13 @@ __global__ void tb_insert_ids(const int2 *__restrict__ pair, int64_t n, uint64_t
     reinterpret_cast<uint32_t *>(table + s)[2] = static_cast<uint32_t>(i);
 }
 
+__global__ void tb_dense_insert_ids(const int2 *__restrict__ pair, int64_t n, uint64_t nq2, uint32_t *__restrict__ dense) {
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int2 p = pair[i];
+    dense[static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y)] = static_cast<uint32_t>(i) + 1u;
+}
+
 // ------------------------------------------------------------------------------------------ count / match
 // Intersection of the two states' sorted inner-symbol lists.  F is called for every shared symbol with
 // (first arc of q1's segment, n1, first arc of q2's segment, n2).
@@ -271,6 +278,7 @@ __device__ __forceinline__ uint4 ld_keep(const uint4 *ptr, uint64_t policy) {
 #define FSTC_RESOLVE_MIN_ARCS (int64_t(1) << 24)
 #endif
 constexpr int64_t RESOLVE_MIN_ARCS = FSTC_RESOLVE_MIN_ARCS;          // smaller levels always use the table
+constexpr uint64_t DENSE_MAX_PAIRS = 1ull << 29;                     // dense visited table (4 B per pair) up to 2 GB
 constexpr uint64_t RESOLVE_TABLE_BYTES = 96ull << 20;               // a table beyond this no longer lives in L2
 // unit costs measured on a B200, in picoseconds
 constexpr double COST_PROBE_PS = 21.0;            // random 32-byte sector read: one probe
@@ -298,6 +306,7 @@ struct EmitArgs {
     uint64_t nq2;
     uint4 *table;
     uint64_t cap;
+    uint32_t *dense;         // RES_DENSE: [|Q1||Q2|] id + 1 of every pair, 0 = not visited
     unsigned long long *n_states;
     int2 *pair;
     int32_t *o_src, *o_il, *o_ol, *o_tgt;
@@ -327,10 +336,14 @@ __global__ void k_partition(const int64_t *__restrict__ cum, int64_t n_matches, 
     tile_m[t] = lo - 1;
 }
 
-// KEYS = false: the target ids come from the visited table, inside this kernel.  KEYS = true: the kernel leaves the
-// target column open and writes one (target key, output position) record per arc for resolve_partitioned.
-template <int MODE, bool KEYS>
+// RES_HASH / RES_DENSE: the target ids come from the visited table, inside this kernel — the open-addressing hash
+// table, or, when |Q1||Q2| is small enough, the paper's dense table of one entry per pair (entry =
+// id + 1, 0 = not visited).  RES_KEYS: the kernel leaves the target column open and writes the target key of every
+// arc for resolve_partitioned.
+enum { RES_HASH = 0, RES_KEYS = 1, RES_DENSE = 2 };
+template <int MODE, int RES>
 __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
+    constexpr bool KEYS = RES == RES_KEYS, DENSE = RES == RES_DENSE;
     __shared__ uint32_t relcum[EM_TILE + 1];
     __shared__ int64_t s_first_cum;
     __shared__ uint32_t s_warp[EM_THREADS / 32];
@@ -441,9 +454,28 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
     // together, then all pending CAS in flight together; a rank leaves when it finds its key or wins a slot.
     uint64_t slot[EM_IPT];                                    // bucket while searching, then the key's slot
     uint32_t won = 0;                                         // bit u: this thread inserted the key (new state)
+    if (DENSE) {
+        uint32_t v[EM_IPT];
+#pragma unroll
+        for (int u = 0; u < EM_IPT; ++u) {
+            slot[u] = key[u];
+            if (todo >> u & 1u) v[u] = __ldcg(g.dense + key[u]);
+        }
+#pragma unroll
+        for (int u = 0; u < EM_IPT; ++u)
+            if ((todo >> u & 1u) && v[u] == 0u) v[u] = atomicCAS(g.dense + key[u], 0u, PENDING_ID);   // 0: this thread won
+#pragma unroll
+        for (int u = 0; u < EM_IPT; ++u) {
+            if (todo >> u & 1u) {
+                if (v[u] == 0u) won |= 1u << u;
+                else id[u] = v[u] == PENDING_ID ? PENDING_ID : v[u] - 1u;
+            }
+        }
+        todo = 0;
+    }
     const uint64_t n_buckets = g.cap >> 1;
 #pragma unroll
-    for (int u = 0; u < EM_IPT; ++u) slot[u] = (todo >> u & 1u) ? home_bucket(key[u], g.cap) : 0;
+    for (int u = 0; u < EM_IPT; ++u) if (!DENSE) slot[u] = (todo >> u & 1u) ? home_bucket(key[u], g.cap) : 0;
     while (todo) {
         Bucket v[EM_IPT];
         unsigned long long old[EM_IPT];
@@ -499,7 +531,8 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
     for (int u = 0; u < EM_IPT; ++u) {
         if (won >> u & 1u) {
             id[u] = next_id++;
-            __stcg(reinterpret_cast<uint32_t *>(g.table + slot[u]) + 2, id[u]);   // publish
+            if (DENSE) __stcg(g.dense + slot[u], id[u] + 1u);
+            else __stcg(reinterpret_cast<uint32_t *>(g.table + slot[u]) + 2, id[u]);   // publish
             g.pair[id[u]] = tgt_pair[u];
         }
     }
@@ -507,10 +540,10 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
 #pragma unroll
     for (int u = 0; u < EM_IPT; ++u) {
         if (u >= skip && u < skip + n_valid && !(won >> u & 1u) && id[u] == PENDING_ID) {
-            const uint32_t *pid = reinterpret_cast<const uint32_t *>(g.table + slot[u]) + 2;
+            const uint32_t *pid = DENSE ? g.dense + slot[u] : reinterpret_cast<const uint32_t *>(g.table + slot[u]) + 2;
             uint32_t v;
             while ((v = __ldcg(pid)) == PENDING_ID) __nanosleep(20);
-            id[u] = v;
+            id[u] = DENSE ? v - 1u : v;
         }
     }
     }   // !KEYS
@@ -770,6 +803,8 @@ struct Composer {
     int64_t n_arcs = 0, n_states = 0;
     // visited table
     DBuf<uint4> table; uint64_t cap = 0;
+    DBuf<uint32_t> dense; bool use_dense = false;   // the dense |Q1||Q2| table instead of the hash table (small products)
+    uint64_t n_pairs_all = 0;
     DBuf<unsigned long long> d_counters;   // [0] n_states, [1] seg visited, [2] match arcs, [3] n_selected, [4..259] hist
 
     Composer(Ctx &ctx, const fstc_packed_t &a, const fstc_packed_t &b, const fstc_opts_t &opts)
@@ -827,6 +862,19 @@ struct Composer {
 
     // table able to hold `bound` states at load <= FSTC_TABLE_LOAD_PCT %
     void ensure_table(int64_t bound, int64_t want_states = 0) {
+        if (use_dense) {                                     // one entry per pair: never grows; rebuilt only after it was dropped
+            if (dense.p) return;
+            int h = tm.begin(FSTC_T_TABLE);
+            dense.alloc(c, static_cast<int64_t>(n_pairs_all));
+            FSTC_CUDA(cudaMemsetAsync(dense.p, 0, sizeof(uint32_t) * n_pairs_all, c.stream));
+            if (n_states > 0) {
+                tb_dense_insert_ids<<<nblk(n_states), CT_THREADS, 0, c.stream>>>(pair.p, n_states, nq2, dense.p);
+                FSTC_LAUNCH_CHECK();
+                c.n_launch += 1;
+            }
+            tm.end(h);
+            return;
+        }
         const uint64_t need = slots_for(bound);
         if (need <= cap) return;
         int h = tm.begin(FSTC_T_TABLE);
@@ -873,7 +921,7 @@ struct Composer {
         g.A = view_of(m1); g.B = view_of(m2);
         g.L = L; g.n_matches = n_matches; g.R = R; g.pos_base = pos_base; g.f_lo = f_lo; g.sel = cur_sel;
         g.foff = foff; g.roff = roff; g.arc_base = arc_base; g.nq2 = nq2;
-        g.table = table.p; g.cap = cap; g.n_states = d_counters.p; g.pair = pair.p;
+        g.table = table.p; g.cap = cap; g.dense = dense.p; g.n_states = d_counters.p; g.pair = pair.p;
         g.o_src = a_src.p; g.o_il = a_il.p; g.o_ol = a_ol.p; g.o_tgt = a_tgt.p; g.o_w = a_w.p;
         g.sortrec = sortrec; g.shift_t = shift_t; g.bits_b = bits_b; g.tile_m = tile_m.p;
         g.keys = nullptr; g.posout = nullptr;
@@ -885,13 +933,17 @@ struct Composer {
             keys.alloc(c, R + 2);
             g.keys = keys.p;
             if (mode == EMIT_INDIRECT) { posout.alloc(c, R); g.posout = posout.p; }
-            if (mode == EMIT_DIRECT) k_emit<EMIT_DIRECT, true><<<grid, EM_THREADS, 0, c.stream>>>(g);
-            else if (mode == EMIT_INDIRECT) k_emit<EMIT_INDIRECT, true><<<grid, EM_THREADS, 0, c.stream>>>(g);
-            else k_emit<EMIT_SORTREC, true><<<grid, EM_THREADS, 0, c.stream>>>(g);
+            if (mode == EMIT_DIRECT) k_emit<EMIT_DIRECT, RES_KEYS><<<grid, EM_THREADS, 0, c.stream>>>(g);
+            else if (mode == EMIT_INDIRECT) k_emit<EMIT_INDIRECT, RES_KEYS><<<grid, EM_THREADS, 0, c.stream>>>(g);
+            else k_emit<EMIT_SORTREC, RES_KEYS><<<grid, EM_THREADS, 0, c.stream>>>(g);
+        } else if (use_dense) {
+            if (mode == EMIT_DIRECT) k_emit<EMIT_DIRECT, RES_DENSE><<<grid, EM_THREADS, 0, c.stream>>>(g);
+            else if (mode == EMIT_INDIRECT) k_emit<EMIT_INDIRECT, RES_DENSE><<<grid, EM_THREADS, 0, c.stream>>>(g);
+            else k_emit<EMIT_SORTREC, RES_DENSE><<<grid, EM_THREADS, 0, c.stream>>>(g);
         } else {
-            if (mode == EMIT_DIRECT) k_emit<EMIT_DIRECT, false><<<grid, EM_THREADS, 0, c.stream>>>(g);
-            else if (mode == EMIT_INDIRECT) k_emit<EMIT_INDIRECT, false><<<grid, EM_THREADS, 0, c.stream>>>(g);
-            else k_emit<EMIT_SORTREC, false><<<grid, EM_THREADS, 0, c.stream>>>(g);
+            if (mode == EMIT_DIRECT) k_emit<EMIT_DIRECT, RES_HASH><<<grid, EM_THREADS, 0, c.stream>>>(g);
+            else if (mode == EMIT_INDIRECT) k_emit<EMIT_INDIRECT, RES_HASH><<<grid, EM_THREADS, 0, c.stream>>>(g);
+            else k_emit<EMIT_SORTREC, RES_HASH><<<grid, EM_THREADS, 0, c.stream>>>(g);
         }
         FSTC_LAUNCH_CHECK();
         tm.end(h_emit);
@@ -925,7 +977,7 @@ fstc_result_t *Composer::run() {
     if (m1.side != 1 || m2.side != 2) fail(FSTC_ERR_ARG, "operands must be packed with side 1 (left) and side 2 (right)");
     if (m1.n_inner != m2.n_inner)
         fail(FSTC_ERR_ARG, "inner alphabets differ: |Γ| = %d vs %d (PAPER.md:45)", m1.n_inner, m2.n_inner);
-    if (o.merge_mode < 0 || o.merge_mode > 2 || o.max_levels < 0 || o.max_raw_arcs < 0 || o.resolve_mode < 0 || o.resolve_mode > 2)
+    if (o.merge_mode < 0 || o.merge_mode > 2 || o.max_levels < 0 || o.max_raw_arcs < 0 || o.resolve_mode < 0 || o.resolve_mode > 3)
         fail(FSTC_ERR_ARG, "bad options");
     const int bits_a = bits_for(m1.n_outer > 0 ? m1.n_outer - 1 : 0), bits_b = bits_for(m2.n_outer > 0 ? m2.n_outer - 1 : 0);
     const int shift_t = bits_a + bits_b;
@@ -935,6 +987,8 @@ fstc_result_t *Composer::run() {
                        (o.merge_mode == FSTC_MERGE_AUTO &&
                         (((m1.any_flags & FLAG_D) && (m2.any_flags & FLAG_D)) || (m1.any_flags & FLAG_X) || (m2.any_flags & FLAG_X)));
     key_bits = bits_for(n_pairs_total - 1);
+    n_pairs_all = n_pairs_total;
+    use_dense = o.resolve_mode != FSTC_RESOLVE_HASH && n_pairs_total <= DENSE_MAX_PAIRS;
 
     if (const char *e = getenv("FSTC_L2_FETCH")) {            // experiment knob: 32 / 64 / 128
         (void)cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, static_cast<size_t>(atoi(e)));
@@ -1089,26 +1143,27 @@ fstc_result_t *Composer::run() {
         // if it was dropped or must grow); the partitioned resolve pays streaming passes per arc and per existing state.
         const int rkey_bits = bits_for(nq2 > 1 ? nq2 - 1 : 1) + bits_for(static_cast<uint64_t>(m1.n_states > 1 ? m1.n_states - 1 : 1));
         auto prefer_partitioned = [&](int64_t r, int64_t bound, int64_t states_now, uint64_t slots_ready) {
-            if (o.resolve_mode == FSTC_RESOLVE_TABLE) return false;
+            if (o.resolve_mode == FSTC_RESOLVE_TABLE || o.resolve_mode == FSTC_RESOLVE_HASH) return false;
             if (rkey_bits + bits_for(static_cast<uint64_t>(states_now + bound)) > 64) return false;  // state records: key << id_bits | id
             if (o.resolve_mode == FSTC_RESOLVE_PARTITIONED) return true;
-            const uint64_t slots = slots_for(states_now + bound);
-            if (r < RESOLVE_MIN_ARCS || slots * sizeof(uint4) <= RESOLVE_TABLE_BYTES) return false;  // small, or the table lives in L2
+            const uint64_t slots = use_dense ? n_pairs_all : slots_for(states_now + bound);
+            const uint64_t table_bytes = slots * (use_dense ? sizeof(uint32_t) : sizeof(uint4));
+            if (r < RESOLVE_MIN_ARCS || table_bytes <= RESOLVE_TABLE_BYTES) return false;            // small, or the table lives in L2
             double t_table = COST_PROBE_PS * r + COST_INSERT_PS * bound;
-            if (slots > slots_ready) t_table += COST_INSERT_PS * 0.6 * states_now + COST_STREAM_PS_PER_BYTE * 16.0 * slots;
+            if (slots > slots_ready) t_table += COST_INSERT_PS * 0.6 * states_now + COST_STREAM_PS_PER_BYTE * table_bytes;
             const double t_part = COST_PART_ARC_PS * r + COST_PART_STATE_PS * states_now + 1e9;      // + 1 ms of launches
             // a clear win only: leaving the table also costs the next table level a rebuild, and ids in bin order cost
             // the next level's count / match their cache locality
             return t_part < 0.6 * t_table;
         };
         {
-            const bool want = prefer_partitioned(R, new_bound, n_states, cap);
-            if (want && !partitioned) { table = DBuf<uint4>(); cap = 0; }    // the table is dropped; ensure_table rebuilds it from pair[]
+            const bool want = prefer_partitioned(R, new_bound, n_states, use_dense ? (dense.p ? n_pairs_all : 0) : cap);
+            if (want && !partitioned) { table = DBuf<uint4>(); cap = 0; dense = DBuf<uint32_t>(); }    // the table is dropped; ensure_table rebuilds it from pair[]
             partitioned = want;
         }
         // look-ahead: if the search goes on, the next level is about (new states) x (arcs per expanded pair)
         int64_t next_R = 0, next_S = 0;
-        const bool must_grow = n_states + new_bound > pair_cap || (!partitioned && slots_for(n_states + new_bound) > cap) ||
+        const bool must_grow = n_states + new_bound > pair_cap || (!partitioned && (use_dense ? dense.p == nullptr : slots_for(n_states + new_bound) > cap)) ||
                                n_arcs + R > arc_cap;
         if (must_grow && !stop_after && n_sel > 0 && R > 0) {
             const double fan = static_cast<double>(R) / static_cast<double>(n_sel);
@@ -1253,7 +1308,7 @@ fstc_result_t *Composer::run() {
     st.n_states = n_states; st.n_arcs = n_arcs; st.n_raw_arcs = cum_raw;
     st.n_seg_visited = static_cast<int64_t>(cnt[1]);
     st.n_match_arcs = static_cast<int64_t>(cnt[2]);
-    st.table_capacity = static_cast<int64_t>(cap);
+    st.table_capacity = static_cast<int64_t>(use_dense && dense.p ? n_pairs_all : cap);
     st.n_kernel_launches = static_cast<int32_t>(c.n_launch);
 
     fstc_result_t *r = new fstc_result_t();

@@ -19,7 +19,7 @@ LIB_PATH = os.environ.get("FSTC_LIB") or os.path.join(_HERE, "libfstc.so")   # F
 
 FSTC_MEM_DEVICE, FSTC_MEM_HOST = 0, 1
 MERGE_AUTO, MERGE_OFF, MERGE_SORT_ALL = 0, 1, 2
-RESOLVE_AUTO, RESOLVE_TABLE, RESOLVE_PARTITIONED = 0, 1, 2
+RESOLVE_AUTO, RESOLVE_TABLE, RESOLVE_PARTITIONED, RESOLVE_HASH = 0, 1, 2, 3
 MAX_LEVEL_STATS = 64
 STAGES = ("count", "scan", "match", "emit", "sort", "reduce", "table", "assemble", "rs_scatter", "rs_dedupe", "rs_gather")
 

@@ -75,8 +75,9 @@ def test_config_large_scaled_partitioned(fstc, resolve_bits):
 
 
 def test_auto_switches_to_the_partitioned_resolve_on_a_big_level(fstc):
-    """AUTO keeps the table for small levels and switches (one way) once a level is big and its table would not fit L2."""
-    m1, m2 = workloads.make_config("large", scale=0.2)
+    """AUTO keeps the table for small levels and leaves it for a level that is big, creates a state per arc and whose
+    table would not fit L2 (|Q1||Q2| = 9e8 here: too big for the dense table, so the hash table would have to grow)."""
+    m1, m2 = workloads.make_config("large", scale=0.3)
     res = fstc.fstc_compose(fstc.DeviceFst.from_host(m1), fstc.DeviceFst.from_host(m2), max_raw_arcs=60_000_000)
     assert res.stats["n_resolve"] >= 1 and res.n_raw_arcs <= 60_000_000
 
@@ -150,3 +151,37 @@ def test_two_host_threads_compose_concurrently(fstc):
     [t.join() for t in ts]
     assert not errs, errs
     assert len(got) == 6 and all(g == want for g in got)
+
+
+# ---- the two visited tables: the paper's dense table (one entry per pair, |Q1||Q2| <= 2^29: every config of this file)
+# ---- is what RESOLVE_TABLE / AUTO use here, so the open-addressing hash table is forced explicitly
+@pytest.mark.parametrize("case", SMALL)
+@pytest.mark.parametrize("merge_mode", [0, 1, 2])
+def test_small_random_machines_hash_table(fstc, case, merge_mode):
+    seed, n1, sig, gam, a1, n2, dlt, a2 = case
+    m1 = messy_random_fst(seed, n1, sig, gam, a1)
+    m2 = messy_random_fst(seed + 100, n2, gam, dlt, a2)
+    check_parity(fstc, m1, m2, merge_mode=merge_mode, resolve_mode=fstc.RESOLVE_HASH)
+
+
+@pytest.mark.parametrize("budget", [0, 17, 777, 3739])
+def test_config_tiny_hash_table(fstc, budget):
+    m1, m2 = workloads.make_config("tiny")
+    check_parity(fstc, m1, m2, max_raw_arcs=budget, resolve_mode=fstc.RESOLVE_HASH)
+
+
+def test_scaled_configs_hash_table(fstc):
+    for name, scale, budget in (("medium", 0.05, 0), ("skewed", 0.05, 2_000_000), ("large", 0.02, 3_000_000), ("nlp", 0.1, 0)):
+        m1, m2 = workloads.make_config(name, scale=scale)
+        res, _ = check_parity(fstc, m1, m2, max_raw_arcs=budget, resolve_mode=fstc.RESOLVE_HASH)
+        assert res.stats["n_resolve"] == 0
+
+
+def test_dense_table_is_rebuilt_after_partitioned_levels(fstc):
+    """AUTO on a product small enough for the dense table: forced here by comparing TABLE (dense) with HASH and with the
+    partitioned resolve on the same input."""
+    m1, m2 = workloads.make_config("medium", scale=0.05)
+    a, b = fstc.DeviceFst.from_host(m1), fstc.DeviceFst.from_host(m2)
+    rs = [fstc.fstc_compose(a, b, resolve_mode=m) for m in (fstc.RESOLVE_TABLE, fstc.RESOLVE_HASH, fstc.RESOLVE_PARTITIONED)]
+    assert len({(r.n_states, r.n_arcs, tuple(r.stats["level_new_states"])) for r in rs}) == 1
+    assert rs[0].stats["table_capacity"] == m1.n_states * m2.n_states
