@@ -1,20 +1,20 @@
 // Partitioned target resolution: the visited-set step of a BIG level (PAPER.md:237-239 adapted).
 //
 // The paper tests and sets one entry of a dense |Q1||Q2| table per composed arc (atomicOr, :237).  On a B200 a
-// random 32-byte DRAM sector costs ~21 ps to read and ~45 ps to dirty (measured, profiles/r01_random_access.md), so at
+// random 32-byte DRAM sector costs ~21 ps to read and ~45 ps to dirty (measured), so at
 // 10^9 arcs per level the per-arc probe of any table that does not fit the 126 MB L2 bounds the whole path.  Big
 // levels are therefore resolved like a radix hash join, with streaming passes only:
 //
 //   1. the emit kernel leaves the target key of every composed arc, in rank order; every existing state leaves a
 //      record (key, id);
 //   2. both streams are partitioned by the top bits of a hash of the key (one or two staged scatter passes: a block
-//      sorts a tile of 4096 records by bin in shared memory and appends whole runs), until a bin holds ~10^3 distinct
-//      keys.  A pass also records where every input record went (dest[i]);
+//      sorts a tile of 8192 / 4096 records by bin in shared memory and appends whole runs), until a bin holds at most
+//      ~2000 distinct keys.  On the arc stream a pass also records where every record went and came from;
 //   3. one block per bin builds the bin's key->id map in SHARED memory (old states first), finds or creates the id
 //      of every arc key, allocates new ids (one global atomicAdd per round) and writes pair[id];
-//   4. the ids travel back through the recorded permutations: id1[i] = id2[dest2[i]] (a gather inside one parent
-//      bin, a few MB, L2-resident), then tgt[pos(r)] = id1[dest1[r]] in rank order — records of a bin keep roughly
-//      their rank order, so the gather reads 2^b1 slowly advancing streams and the target column is written coalesced.
+//   4. the ids travel back through the recorded permutations, tile by tile: a block reads the ids of its tile's records
+//      in SORTED order (runs of neighbours, not 32 far-apart words per warp), un-permutes them in shared memory and
+//      writes them out in input order; the last pass writes the target column, coalesced, in rank order.
 //
 // Nothing persists between levels except pair[] (id -> (q1,q2)): the key->id map is rebuilt per level from it.
 #include <cstdlib>
@@ -501,14 +501,12 @@ SegSet scatter_pass(Ctx &c, const SegSet &in, int shift, int hshift, int nbins, 
     out.n_seg = nb;
     out.start.alloc(c, nb + 1);
     if (dest) { dest->alloc(c, in.length); perm->alloc(c, in.length); }
-    static bool attr_set = false;
-    if (!attr_set) {
+    {   // per device and cheap: set on every pass rather than remembered per process
         const int s_big = SC_TILE_BIG * 12, s_small = SC_TILE_SMALL * 12;
         FSTC_CUDA(cudaFuncSetAttribute(rs_scatter<false, SC_TILE_BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, s_big));
         FSTC_CUDA(cudaFuncSetAttribute(rs_scatter<true, SC_TILE_BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, s_big));
         FSTC_CUDA(cudaFuncSetAttribute(rs_scatter<false, SC_TILE_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, s_small));
         FSTC_CUDA(cudaFuncSetAttribute(rs_scatter<true, SC_TILE_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, s_small));
-        attr_set = true;
     }
     for (int attempt = 0;; ++attempt) {
         rs_bin_caps<<<rs_blocks(nb), 256, 0, c.stream>>>(in.view(), nbins, 16, 192u, cursor.p, cur_stride, attempt, cap.p);
@@ -585,11 +583,7 @@ int resolve_bits_needed(int64_t n_records_and_states) {
 }
 
 void resolve_partitioned(Ctx &c, const ResolveJob &j) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        FSTC_CUDA(cudaFuncSetAttribute(rs_dedupe, cudaFuncAttributeMaxDynamicSharedMemorySize, DD_SLOTS * 12));
-        attr_set = true;
-    }
+    FSTC_CUDA(cudaFuncSetAttribute(rs_dedupe, cudaFuncAttributeMaxDynamicSharedMemorySize, DD_SLOTS * 12));   // per device
     const int ib = bits_for(static_cast<uint64_t>(j.n_states_before > 1 ? j.n_states_before - 1 : 1));
     if (j.key_bits + ib > 64) fail(FSTC_ERR_CAPACITY, "resolve: key (%d bits) + state id (%d bits) exceed 64 bits", j.key_bits, ib);
     if (j.n_records >= 0xFFFFFFFFll) fail(FSTC_ERR_CAPACITY, "resolve: more than 2^32 records");
