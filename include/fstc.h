@@ -139,6 +139,7 @@ typedef struct fstc_stats_t {
   int64_t n_matches;        /* number of (pair, inner symbol) matches                                 */
   int64_t n_match_arcs;     /* Σ over matches of (n1 + n2) input arcs read                            */
   int64_t n_raw_sorted;     /* raw arcs that went through sort + reduce                               */
+  int64_t n_raw_grouped;    /* raw arcs merged by construction (class G: never materialised)          */
   int64_t table_capacity;   /* final number of visited-table slots                                    */
   int32_t n_rehash, n_grow; /* table rebuilds, output regrow copies                                   */
   int32_t n_emit_launches, n_kernel_launches;

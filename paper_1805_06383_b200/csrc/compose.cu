@@ -29,6 +29,7 @@ namespace {
 constexpr unsigned long long EMPTY_KEY = ~0ull;
 constexpr uint32_t PENDING_ID = 0xFFFFFFFFu;
 constexpr int CT_THREADS = 256;
+constexpr int64_t GROUP_MAX_RATIO = 8;     // class G while (groups of q1) x (groups of q2) <= 8 x raw arcs of the pair
 
 __device__ __forceinline__ int64_t ceil_div_dev(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
@@ -37,9 +38,15 @@ struct MachineView {
     const uint2 *segs;
     const uint32_t *seg_ptr;
     const uint8_t *flags;
+    const uint2 *garcs;          // grouped copy (internal.h): {inner, weight} sorted by (src, outer, tgt, inner)
+    const uint32_t *goff;
+    const uint2 *gkey;
+    const uint32_t *gptr;
 };
 
-inline MachineView view_of(const fstc_packed_t &p) { return MachineView{p.arcs, p.segs, p.seg_ptr, p.flags}; }
+inline MachineView view_of(const fstc_packed_t &p) {
+    return MachineView{p.arcs, p.segs, p.seg_ptr, p.flags, p.garcs, p.goff, p.gkey, p.gptr};
+}
 
 // ------------------------------------------------------------------------------------------ hash table
 // Open addressing over 32-byte BUCKETS of two 16-byte slots {key lo, key hi, id, unused}: a bucket is exactly
@@ -121,7 +128,8 @@ __global__ void __launch_bounds__(CT_THREADS)
 k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_lo, int64_t nf,
         const uint32_t *__restrict__ sel /* null: all pairs of the level */, int merge_mode,
         uint64_t nq2, uint64_t key_limit /* pairs with key >= key_limit are left uncounted (raw = 0) */,
-        int64_t *__restrict__ rawU, int64_t *__restrict__ rawF, uint32_t *__restrict__ nmU, uint32_t *__restrict__ nmF) {
+        int64_t *__restrict__ rawU, int64_t *__restrict__ rawF, uint32_t *__restrict__ nmU, uint32_t *__restrict__ nmF,
+        int64_t *__restrict__ rawG, int64_t *__restrict__ gwork, uint32_t *__restrict__ nmG) {
     int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (i < nf) {
         int2 p = pair[f_lo + (sel ? sel[i] : i)];
@@ -139,8 +147,17 @@ k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_l
             uint8_t fa = A.flags[p.x], fb = B.flags[p.y];
             f = ((fa & FLAG_D) && (fb & FLAG_D)) || (fa & FLAG_X) || (fb & FLAG_X);
         }
+        // class G (merge by construction): a class-F pair whose (a,r1) x (b,r2) group product is not much larger than its
+        // raw arc count composes group by group instead of arc by arc and needs no sort
+        bool gcls = false;
+        int64_t work = 0;
+        if (f && rawG && raw > 0) {
+            work = static_cast<int64_t>(A.gptr[p.x + 1] - A.gptr[p.x]) * static_cast<int64_t>(B.gptr[p.y + 1] - B.gptr[p.y]);
+            gcls = work <= GROUP_MAX_RATIO * raw;
+        }
         rawU[i] = f ? 0 : raw; nmU[i] = f ? 0 : nm;
-        if (rawF) { rawF[i] = f ? raw : 0; nmF[i] = f ? nm : 0; }    // null when no pair of this run can be class F
+        if (rawF) { rawF[i] = (f && !gcls) ? raw : 0; nmF[i] = (f && !gcls) ? nm : 0; }   // null when no pair of this run can be class F
+        if (rawG) { rawG[i] = gcls ? raw : 0; gwork[i] = gcls ? work : 0; nmG[i] = gcls ? 1u : 0u; }
     }
 }
 
@@ -151,7 +168,8 @@ k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_l
 __global__ void __launch_bounds__(CT_THREADS)
 k_cut_hist(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, const uint32_t *__restrict__ sel, uint64_t nq2,
            const int64_t *__restrict__ rawU,
-           const int64_t *__restrict__ rawF, uint64_t prefix, int shift, unsigned long long *__restrict__ hist) {
+           const int64_t *__restrict__ rawF, const int64_t *__restrict__ rawG, uint64_t prefix, int shift,
+           unsigned long long *__restrict__ hist) {
     __shared__ unsigned long long h[256];
     h[threadIdx.x] = 0;
     __syncthreads();
@@ -165,7 +183,7 @@ k_cut_hist(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, const uint32
             int2 p = pair[f_lo + (sel ? sel[i] : i)];
             uint64_t key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
             uint64_t hi = (shift + 8 >= 64) ? 0 : (key >> (shift + 8));
-            r = static_cast<uint64_t>(rawU[i] + (rawF ? rawF[i] : 0));
+            r = static_cast<uint64_t>(rawU[i] + (rawF ? rawF[i] : 0) + (rawG ? rawG[i] : 0));
             if (hi == prefix && r > 0) digit = static_cast<uint32_t>(key >> shift) & 255u;
         }
         const uint32_t peers = __match_any_sync(0xffffffffu, digit);
@@ -184,7 +202,8 @@ k_cut_hist(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, const uint32
 __global__ void k_apply_cut(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, const uint32_t *__restrict__ sel,
                             uint64_t nq2, uint64_t cut,
                             int64_t *__restrict__ rawU, int64_t *__restrict__ rawF, uint32_t *__restrict__ nmU,
-                            uint32_t *__restrict__ nmF, unsigned long long *__restrict__ n_selected) {
+                            uint32_t *__restrict__ nmF, int64_t *__restrict__ rawG, int64_t *__restrict__ gwork,
+                            uint32_t *__restrict__ nmG, unsigned long long *__restrict__ n_selected) {
     int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     bool keep = false;
     if (i < nf) {
@@ -194,6 +213,7 @@ __global__ void k_apply_cut(const int2 *__restrict__ pair, int64_t f_lo, int64_t
         if (!keep) {
             rawU[i] = 0; nmU[i] = 0;
             if (rawF) { rawF[i] = 0; nmF[i] = 0; }
+            if (rawG) { rawG[i] = 0; gwork[i] = 0; nmG[i] = 0; }
         }
     }
     unsigned b = __ballot_sync(0xffffffffu, keep);
@@ -595,6 +615,244 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
 #undef SRC
 }
 
+// ------------------------------------------------------------------------------------------ merge by construction
+// Class G.  Seen from a source pair (q1,q2), M1 only contributes (a, r1) and M2 only (b, r2): group q1's arcs by
+// (a, r1) and q2's by (b, r2) (the packer's grouped copy); every composed-and-merged arc of the pair is one pair of
+// groups that share an inner symbol, and its weight is sum_c (sum of p1 over the group's arcs with c) x (same for p2)
+// (PAPER.md:53,65 regrouped).  So the merged arcs come out directly, in (a, r1, b, r2) order, with no sort and no
+// reduce: work = groups x groups per pair (load-balanced over ranks like the emit kernel), not raw arcs.
+// The match list of this class has one entry per pair: {first group of q1, first group of q2, #groups, #groups}.
+__global__ void __launch_bounds__(CT_THREADS)
+k_gmatch(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, const uint32_t *__restrict__ sel,
+         const uint32_t *__restrict__ nmG, const int64_t *__restrict__ moffG, const int64_t *__restrict__ woff, MatchList G) {
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= nf || nmG[i] == 0) return;
+    int2 p = pair[f_lo + (sel ? sel[i] : i)];
+    const int64_t m = moffG[i];
+    const uint32_t g1 = A.gptr[p.x], g2 = B.gptr[p.y];
+    G.cum[m] = woff[i];
+    G.rec[m] = make_uint4(g1, g2, A.gptr[p.x + 1] - g1, B.gptr[p.y + 1] - g2);
+    G.pl[m] = static_cast<uint32_t>(i);
+}
+
+struct GProdArgs {
+    MachineView A, B;
+    MatchList L;
+    int64_t n_matches, W;        // ranks [0, W) = group pairs
+    const int64_t *tile_m;
+    uint32_t *tile_cnt;          // pass 0: arcs found per tile
+    const int64_t *tile_off;     // pass 1: first output slot of every tile
+    uint32_t *msrc;              // pass 1 outputs, compact, in rank order: pair index,
+    uint32_t *mab;               //   a << bits_b | b,
+    float *mw;                   //   merged weight,
+    unsigned long long *mkey;    //   target key (table: r1 * |Q2| + r2; partitioned resolve: (r1 << q2_bits) | r2)
+    int bits_b, q2_bits;         // q2_bits < 0: table key
+    uint64_t nq2;
+};
+
+// sum over the common inner symbols of two groups; *found = at least one common symbol
+__device__ __forceinline__ float group_dot(const uint2 *__restrict__ ga, uint32_t a0, uint32_t a1, const uint2 *__restrict__ gb,
+                                           uint32_t b0, uint32_t b1, bool first_only, bool *found) {
+    float sum = 0.f;
+    bool any = false;
+    uint2 x = ga[a0], y = gb[b0];
+    while (true) {
+        if (x.x == y.x) {
+            any = true;
+            if (first_only) break;
+            const uint32_t c = x.x;                              // runs of equal symbols (parallel duplicate arcs) first
+            float sa = 0.f, sb = 0.f;
+            while (true) { sa += __uint_as_float(x.y); if (++a0 == a1) break; x = ga[a0]; if (x.x != c) break; }
+            while (true) { sb += __uint_as_float(y.y); if (++b0 == b1) break; y = gb[b0]; if (y.x != c) break; }
+            sum += sa * sb;
+            if (a0 == a1 || b0 == b1) break;
+        } else if (x.x < y.x) {
+            if (++a0 == a1) break;
+            x = ga[a0];
+        } else {
+            if (++b0 == b1) break;
+            y = gb[b0];
+        }
+    }
+    *found = any;
+    return sum;
+}
+
+constexpr int GP_THREADS = 128, GP_IPT = 4, GP_TILE = GP_THREADS * GP_IPT;
+static_assert(GP_TILE == EM_TILE, "k_partition places tiles of EM_TILE ranks");
+
+template <int PASS>
+__global__ void __launch_bounds__(GP_THREADS) k_gprod(GProdArgs g) {
+    __shared__ uint32_t relcum[GP_TILE + 1];
+    __shared__ int64_t s_first_cum;
+    __shared__ uint32_t s_warp[GP_THREADS / 32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t rank_lo = static_cast<int64_t>(blockIdx.x) * GP_TILE;
+    const int64_t rank_hi = rank_lo + GP_TILE < g.W ? rank_lo + GP_TILE : g.W;
+    const int64_t m_lo = g.tile_m[blockIdx.x];
+    int64_t m_hi = g.tile_m[blockIdx.x + 1];
+    if (m_hi >= g.n_matches) m_hi = g.n_matches - 1;
+    const int nm = static_cast<int>(m_hi - m_lo + 1);
+    for (int j = tid; j < nm; j += GP_THREADS) {
+        int64_t c = g.L.cum[m_lo + j] - rank_lo;
+        relcum[j] = c < 0 ? 0u : static_cast<uint32_t>(c > GP_TILE ? GP_TILE : c);
+    }
+    if (tid == 0) s_first_cum = g.L.cum[m_lo];
+    __syncthreads();
+    const int64_t rank0 = rank_lo + tid * GP_IPT;
+    int n_valid = rank0 < rank_hi ? static_cast<int>(rank_hi - rank0 < GP_IPT ? rank_hi - rank0 : GP_IPT) : 0;
+    uint32_t exists = 0;
+    float w[GP_IPT];
+    uint32_t g1v[GP_IPT], g2v[GP_IPT], plv[GP_IPT];
+    if (n_valid > 0) {
+        const uint32_t rr = static_cast<uint32_t>(rank0 - rank_lo);
+        int lo = 0, hi = nm;
+        while (lo < hi) {
+            int mid = (lo + hi) >> 1;
+            if (relcum[mid] <= rr) lo = mid + 1; else hi = mid;
+        }
+        int j = lo - 1;
+        int64_t m = m_lo + j;
+        uint64_t r = (j == 0) ? static_cast<uint64_t>(rank0 - s_first_cum) : static_cast<uint64_t>(rr - relcum[j]);
+        uint4 rec = g.L.rec[m];
+        uint32_t p = g.L.pl[m];
+        uint32_t i1 = static_cast<uint32_t>(r / rec.w), i2 = static_cast<uint32_t>(r - static_cast<uint64_t>(i1) * rec.w);
+#pragma unroll
+        for (int u = 0; u < GP_IPT; ++u) {
+            if (u < n_valid) {
+                g1v[u] = rec.x + i1; g2v[u] = rec.y + i2; plv[u] = p;
+                if (++i2 == rec.w) {
+                    i2 = 0;
+                    if (++i1 == rec.z) {
+                        i1 = 0; ++m;
+                        if (m <= m_hi) { rec = g.L.rec[m]; p = g.L.pl[m]; }
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < GP_IPT; ++u) {
+            if (u < n_valid) {
+                bool found;
+                w[u] = group_dot(g.A.garcs, g.A.goff[g1v[u]], g.A.goff[g1v[u] + 1], g.B.garcs, g.B.goff[g2v[u]],
+                                 g.B.goff[g2v[u] + 1], PASS == 0, &found);
+                if (found) exists |= 1u << u;
+            }
+        }
+    }
+    const uint32_t n_mine = __popc(exists);
+    uint32_t incl = n_mine;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += t;
+    }
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    uint32_t before = incl - n_mine, total = 0;
+#pragma unroll
+    for (int wv = 0; wv < GP_THREADS / 32; ++wv) { if (wv < warp) before += s_warp[wv]; total += s_warp[wv]; }
+    if (PASS == 0) {
+        if (tid == 0) g.tile_cnt[blockIdx.x] = total;
+        return;
+    }
+    int64_t q = g.tile_off[blockIdx.x] + before;
+#pragma unroll
+    for (int u = 0; u < GP_IPT; ++u) {
+        if (exists >> u & 1u) {
+            const uint2 k1 = g.A.gkey[g1v[u]], k2 = g.B.gkey[g2v[u]];      // {outer, tgt}
+            g.msrc[q] = plv[u];
+            g.mab[q] = (k1.x << g.bits_b) | k2.x;
+            g.mw[q] = w[u];
+            g.mkey[q] = g.q2_bits >= 0 ? ((static_cast<unsigned long long>(k1.y) << g.q2_bits) | k2.y)
+                                       : static_cast<unsigned long long>(k1.y) * g.nq2 + k2.y;
+            ++q;
+        }
+    }
+}
+
+// Ids of a list of target keys through the visited table (dense or hash), outside the emit kernel: one key per thread,
+// new ids per block with one atomicAdd.  Same protocol as in k_emit.
+template <bool DENSE>
+__global__ void __launch_bounds__(CT_THREADS)
+k_resolve_keys(const unsigned long long *__restrict__ keys, int64_t n, uint32_t *dense, uint4 *table, uint64_t cap, uint64_t nq2,
+               unsigned long long *n_states, int2 *pair, int32_t *__restrict__ ids) {
+    __shared__ uint32_t s_warp[CT_THREADS / 32];
+    __shared__ unsigned long long s_base;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + tid;
+    const bool valid = i < n;
+    unsigned long long key = valid ? keys[i] : 0ull;
+    uint32_t id = 0;
+    bool won = false;
+    uint32_t *slotp = nullptr;                                   // where the id is (or will be) published
+    if (valid) {
+        if (DENSE) {
+            slotp = dense + key;
+            uint32_t v = __ldcg(slotp);
+            if (v == 0u) v = atomicCAS(slotp, 0u, PENDING_ID);
+            if (v == 0u) won = true; else id = v == PENDING_ID ? PENDING_ID : v - 1u;
+        } else {
+            const uint64_t n_buckets = cap >> 1;
+            uint64_t b = home_bucket(key, cap);
+            while (true) {
+                Bucket v = ld_bucket(table, b);
+                const unsigned long long k0 = slot_key(v.s0), k1 = slot_key(v.s1);
+                int cas = -1;
+                if (k0 == key) { id = v.s0.z; slotp = reinterpret_cast<uint32_t *>(table + 2 * b) + 2; break; }
+                else if (k0 == EMPTY_KEY) cas = 0;
+                else if (k1 == key) { id = v.s1.z; slotp = reinterpret_cast<uint32_t *>(table + 2 * b + 1) + 2; break; }
+                else if (k1 == EMPTY_KEY) cas = 1;
+                if (cas < 0) { b = (b + 1 == n_buckets) ? 0 : b + 1; continue; }
+                const unsigned long long old = atomicCAS(reinterpret_cast<unsigned long long *>(table + 2 * b + cas), EMPTY_KEY, key);
+                if (old == EMPTY_KEY || old == key) {
+                    slotp = reinterpret_cast<uint32_t *>(table + 2 * b + cas) + 2;
+                    if (old == EMPTY_KEY) won = true; else id = PENDING_ID;
+                    break;
+                }                                                // another key took the slot: look at the bucket again
+            }
+        }
+    }
+    const uint32_t bal = __ballot_sync(0xffffffffu, won);
+    if (lane == 0) s_warp[warp] = __popc(bal);
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t tot = 0;
+#pragma unroll
+        for (int wv = 0; wv < CT_THREADS / 32; ++wv) { uint32_t cnt = s_warp[wv]; s_warp[wv] = tot; tot += cnt; }
+        s_base = tot ? atomicAdd(n_states, static_cast<unsigned long long>(tot)) : 0ull;
+    }
+    __syncthreads();
+    if (won) {
+        id = static_cast<uint32_t>(s_base) + s_warp[warp] + __popc(bal & ((1u << lane) - 1u));
+        __stcg(slotp, DENSE ? id + 1u : id);
+        const unsigned long long q1 = key / nq2;
+        pair[id] = make_int2(static_cast<int>(q1), static_cast<int>(key - q1 * nq2));
+    } else if (valid && id == PENDING_ID) {
+        uint32_t v;
+        while ((v = __ldcg(slotp)) == PENDING_ID) __nanosleep(20);
+        id = DENSE ? v - 1u : v;
+    }
+    if (valid) ids[i] = static_cast<int32_t>(id);
+}
+
+__global__ void k_place_grouped(const uint32_t *__restrict__ mab, const int32_t *__restrict__ mtgt, const uint32_t *__restrict__ msrc,
+                                const float *__restrict__ mw, int64_t n_merged, const int64_t *__restrict__ mstart,
+                                const int64_t *__restrict__ foff, int64_t arc_base, int64_t f_lo,
+                                const uint32_t *__restrict__ sel, int bits_b, int32_t *__restrict__ o_src,
+                                int32_t *__restrict__ o_il, int32_t *__restrict__ o_ol, int32_t *__restrict__ o_tgt,
+                                float *__restrict__ o_w) {
+    int64_t j = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (j >= n_merged) return;
+    const uint32_t p = msrc[j], ab = mab[j];
+    const int64_t q = arc_base + foff[p] + (j - mstart[p]);
+    o_src[q] = static_cast<int>(f_lo + (sel ? sel[p] : p));
+    o_tgt[q] = mtgt[j];
+    o_il[q] = static_cast<int>(ab >> bits_b);
+    o_ol[q] = static_cast<int>(ab & ((1u << bits_b) - 1u));
+    o_w[q] = mw[j];
+}
+
 // ------------------------------------------------------------------------------------------ merge (reduce by key)
 __global__ void k_heads(const uint4 *__restrict__ rec, int64_t n, uint8_t *__restrict__ head) {
     int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
@@ -648,10 +906,10 @@ __global__ void k_mstart(const uint32_t *__restrict__ msrc, int64_t n_merged, in
     mstart[p] = lo;
 }
 
-__global__ void k_final_counts(const int64_t *__restrict__ rawU, const int64_t *__restrict__ mstart, int64_t nf,
-                               int64_t *__restrict__ fc) {
+__global__ void k_final_counts(const int64_t *__restrict__ rawU, const int64_t *__restrict__ mstartS,
+                               const int64_t *__restrict__ mstartG, int64_t nf, int64_t *__restrict__ fc) {
     int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i < nf) fc[i] = rawU[i] + (mstart[i + 1] - mstart[i]);
+    if (i < nf) fc[i] = rawU[i] + (mstartS ? mstartS[i + 1] - mstartS[i] : 0) + (mstartG ? mstartG[i + 1] - mstartG[i] : 0);
 }
 
 __global__ void k_place_merged(const unsigned long long *__restrict__ mkey, const uint32_t *__restrict__ msrc,
@@ -987,6 +1245,8 @@ fstc_result_t *Composer::run() {
                        (o.merge_mode == FSTC_MERGE_AUTO &&
                         (((m1.any_flags & FLAG_D) && (m2.any_flags & FLAG_D)) || (m1.any_flags & FLAG_X) || (m2.any_flags & FLAG_X)));
     key_bits = bits_for(n_pairs_total - 1);
+    // class G (merge by construction) replaces sort + reduce for the pairs it suits; FSTC_MERGE_SORT_ALL keeps the sort
+    const bool has_G = has_F && o.merge_mode == FSTC_MERGE_AUTO && getenv("FSTC_NO_GROUP_MERGE") == nullptr;
     n_pairs_all = n_pairs_total;
     use_dense = o.resolve_mode != FSTC_RESOLVE_HASH && n_pairs_total <= DENSE_MAX_PAIRS;
 
@@ -1031,22 +1291,33 @@ fstc_result_t *Composer::run() {
 
         // ---- count
         int64_t RU = 0, RF = 0, MU = 0, MF = 0;
-        DBuf<int64_t> rawU, rawF;
-        DBuf<uint32_t> nmU, nmF;
-        DBuf<int64_t> roffU, roffF, moffU, moffF;
+        DBuf<int64_t> rawU, rawF, rawG, gwork;
+        DBuf<uint32_t> nmU, nmF, nmG;
+        DBuf<int64_t> roffU, roffF, moffU, moffF, roffG, moffG, woff;
+        int64_t RG = 0, MG = 0, WG = 0;                          // class G: raw arcs, pairs, group pairs of the level
         DBuf<uint32_t> sel;                                      // compacted level: frontier index of working pair i
         auto scan_level = [&](int64_t *n_sel_out) {             // offsets + totals of the level, one synchronisation
             exclusive_scan2(c, rawU.p, nmU.p, nf, roffU.p, moffU.p);
             if (has_F) exclusive_scan2(c, rawF.p, nmF.p, nf, roffF.p, moffF.p);
-            RF = 0; MF = 0;
-            if (has_F && n_sel_out)
-                read_scalars({{roffU.p + nf, &RU}, {moffU.p + nf, &MU}, {roffF.p + nf, &RF}, {moffF.p + nf, &MF},
-                              {reinterpret_cast<const int64_t *>(d_counters.p + 3), n_sel_out}});
-            else if (has_F) read_scalars({{roffU.p + nf, &RU}, {moffU.p + nf, &MU}, {roffF.p + nf, &RF}, {moffF.p + nf, &MF}});
-            else if (n_sel_out)
-                read_scalars({{roffU.p + nf, &RU}, {moffU.p + nf, &MU},
-                              {reinterpret_cast<const int64_t *>(d_counters.p + 3), n_sel_out}});
-            else read_scalars({{roffU.p + nf, &RU}, {moffU.p + nf, &MU}});
+            if (has_G) {
+                exclusive_scan2(c, rawG.p, nmG.p, nf, roffG.p, moffG.p);
+                exclusive_scan<int64_t>(c, gwork.p, nf, woff.p);
+            }
+            RF = 0; MF = 0; RG = 0; MG = 0; WG = 0;
+            int64_t dummy = 0;
+            FSTC_CUDA(cudaMemcpyAsync(&RU, roffU.p + nf, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
+            FSTC_CUDA(cudaMemcpyAsync(&MU, moffU.p + nf, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
+            if (has_F) {
+                FSTC_CUDA(cudaMemcpyAsync(&RF, roffF.p + nf, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
+                FSTC_CUDA(cudaMemcpyAsync(&MF, moffF.p + nf, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
+            }
+            if (has_G) {
+                FSTC_CUDA(cudaMemcpyAsync(&RG, roffG.p + nf, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
+                FSTC_CUDA(cudaMemcpyAsync(&MG, moffG.p + nf, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
+                FSTC_CUDA(cudaMemcpyAsync(&WG, woff.p + nf, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
+            }
+            FSTC_CUDA(cudaMemcpyAsync(n_sel_out ? n_sel_out : &dummy, d_counters.p + 3, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
+            c.sync();
         };
         // A level that will clearly be cut by the budget (predicted from the previous level's fan-out) is counted
         // only below a key limit: rule T expands a key-ordered prefix, so pairs far above the cut never matter.
@@ -1083,28 +1354,32 @@ fstc_result_t *Composer::run() {
             }
             rawU.alloc(c, nf); nmU.alloc(c, nf); roffU.alloc(c, nf + 1); moffU.alloc(c, nf + 1);
             if (has_F) { rawF.alloc(c, nf); nmF.alloc(c, nf); roffF.alloc(c, nf + 1); moffF.alloc(c, nf + 1); }
+            if (has_G) {
+                rawG.alloc(c, nf); gwork.alloc(c, nf); nmG.alloc(c, nf);
+                roffG.alloc(c, nf + 1); moffG.alloc(c, nf + 1); woff.alloc(c, nf + 1);
+            }
             k_count<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, sel.p, o.merge_mode, nq2, key_limit, rawU.p, rawF.p,
-                                                           nmU.p, nmF.p);
+                                                           nmU.p, nmF.p, rawG.p, gwork.p, nmG.p);
             FSTC_LAUNCH_CHECK();
             c.n_launch += 1;
             tm.end(h);
             // ---- scan + budget
             h = tm.begin(FSTC_T_SCAN);
             scan_level(nullptr);
-            if (key_limit >= n_pairs_total || cum_raw + RU + RF > o.max_raw_arcs) break;
+            if (key_limit >= n_pairs_total || cum_raw + RU + RF + RG > o.max_raw_arcs) break;
             tm.end(h);
             key_limit = key_limit > n_pairs_total / 4 ? ~0ull : key_limit * 4;     // the cut lies higher: widen
         }
         bool stop_after = false;
         int64_t n_sel = nf;
-        if (o.max_raw_arcs > 0 && cum_raw + RU + RF > o.max_raw_arcs) {
+        if (o.max_raw_arcs > 0 && cum_raw + RU + RF + RG > o.max_raw_arcs) {
             // rule T: find the key of the first pair (ascending key order) whose arcs no longer fit
             const uint64_t remaining = static_cast<uint64_t>(o.max_raw_arcs - cum_raw);
             uint64_t prefix = 0, before = 0;
             const int top = ((key_bits + 7) / 8) * 8;
             for (int shift = top - 8; shift >= 0; shift -= 8) {
                 FSTC_CUDA(cudaMemsetAsync(d_counters.p + 4, 0, sizeof(unsigned long long) * 256, c.stream));
-                k_cut_hist<<<std::min<unsigned>(nblk(nf), 8u * c.n_sm), CT_THREADS, 0, c.stream>>>(pair.p, f_lo, nf, sel.p, nq2, rawU.p, rawF.p, prefix, shift,
+                k_cut_hist<<<std::min<unsigned>(nblk(nf), 8u * c.n_sm), CT_THREADS, 0, c.stream>>>(pair.p, f_lo, nf, sel.p, nq2, rawU.p, rawF.p, rawG.p, prefix, shift,
                                                                   d_counters.p + 4);
                 FSTC_LAUNCH_CHECK();
                 c.n_launch += 1;
@@ -1122,6 +1397,7 @@ fstc_result_t *Composer::run() {
             cut_key = prefix;
             FSTC_CUDA(cudaMemsetAsync(d_counters.p + 3, 0, sizeof(unsigned long long), c.stream));
             k_apply_cut<<<nblk(nf), CT_THREADS, 0, c.stream>>>(pair.p, f_lo, nf, sel.p, nq2, cut_key, rawU.p, rawF.p, nmU.p, nmF.p,
+                                                               rawG.p, gwork.p, nmG.p,
                                                                d_counters.p + 3);
             FSTC_LAUNCH_CHECK();
             c.n_launch += 1;
@@ -1132,7 +1408,7 @@ fstc_result_t *Composer::run() {
         }
         tm.end(h);
 
-        const int64_t R = RU + RF;
+        const int64_t R = RU + RF + RG;
         cur_sel = sel.p;
         // ---- capacities for this level
         const uint64_t remaining_pairs = n_pairs_total - static_cast<uint64_t>(n_states);
@@ -1211,47 +1487,140 @@ fstc_result_t *Composer::run() {
         }
 
         const int64_t arc_base = n_arcs;
-        if (RF == 0) {
+        if (RF == 0 && RG == 0) {
             // no source of this level can hold duplicates: arcs go straight to their final place
             launch_emit(EMIT_DIRECT, LU, MU, RU, arc_base, f_lo, nullptr, nullptr, 0, nullptr, 0, 0);
             n_arcs += RU;
         } else {
             if (shift_t > 32) fail(FSTC_ERR_CAPACITY, "bits(|Σ|)+bits(|Δ|) = %d > 32: merge key does not fit 64 bits", shift_t);
-            DBuf<uint4> sa(c, RF), sb(c, RF);
-            launch_emit(EMIT_SORTREC, LF, MF, RF, 0, f_lo, nullptr, nullptr, 0, sa.p, shift_t, bits_b);
-            // target ids are now known: n_states bounds them
-            const int64_t ns_now = static_cast<int64_t>(read_scalar(c, d_counters.p));
-            n_states_live = ns_now;
-            const int tgt_bits = bits_for(static_cast<uint64_t>(ns_now - 1));
-            h = tm.begin(FSTC_T_SORT);
-            uint4 *sorted = radix_sort_records(c, sa.p, sb.p, RF, make_sort_passes(shift_t + tgt_bits, bits_for(static_cast<uint64_t>(nf - 1))));
-            tm.end(h);
+            // ---- class F: sort + reduce
+            int64_t M = 0;
+            DBuf<uint4> sa, sb;
+            DBuf<unsigned long long> mkey;
+            DBuf<uint32_t> msrc;
+            DBuf<float> mw;
+            DBuf<int64_t> mstartS;
+            if (RF > 0) {
+                sa.alloc(c, RF); sb.alloc(c, RF);
+                launch_emit(EMIT_SORTREC, LF, MF, RF, 0, f_lo, nullptr, nullptr, 0, sa.p, shift_t, bits_b);
+                // target ids are now known: n_states bounds them
+                const int64_t ns_now = static_cast<int64_t>(read_scalar(c, d_counters.p));
+                n_states_live = ns_now;
+                const int tgt_bits = bits_for(static_cast<uint64_t>(ns_now - 1));
+                h = tm.begin(FSTC_T_SORT);
+                uint4 *sorted = radix_sort_records(c, sa.p, sb.p, RF, make_sort_passes(shift_t + tgt_bits, bits_for(static_cast<uint64_t>(nf - 1))));
+                tm.end(h);
+                h = tm.begin(FSTC_T_REDUCE);
+                DBuf<uint8_t> head(c, RF);
+                DBuf<int64_t> hidx(c, RF + 1);
+                k_heads<<<nblk(RF), CT_THREADS, 0, c.stream>>>(sorted, RF, head.p);
+                FSTC_LAUNCH_CHECK();
+                exclusive_scan<uint8_t>(c, head.p, RF, hidx.p);
+                M = read_scalar(c, hidx.p + RF);
+                mkey.alloc(c, M); msrc.alloc(c, M); mw.alloc(c, M);
+                FSTC_CUDA(cudaMemsetAsync(mw.p, 0, sizeof(float) * M, c.stream));
+                k_reduce<<<nblk(RF), CT_THREADS, 0, c.stream>>>(sorted, head.p, hidx.p, RF, mkey.p, msrc.p, mw.p);
+                FSTC_LAUNCH_CHECK();
+                mstartS.alloc(c, nf + 1);
+                k_mstart<<<nblk(nf + 1), CT_THREADS, 0, c.stream>>>(msrc.p, M, nf, mstartS.p);
+                FSTC_LAUNCH_CHECK();
+                c.n_launch += 3;
+                tm.end(h);
+                c.sync();
+                sa.release(); sb.release();
+            }
+            // ---- class G: merge by construction (group products)
+            int64_t MGm = 0;
+            DBuf<uint32_t> gsrc, gab;
+            DBuf<float> gw;
+            DBuf<int32_t> gtgt;
+            DBuf<int64_t> mstartG;
+            if (RG > 0) {
+                h = tm.begin(FSTC_T_REDUCE);
+                DBuf<int64_t> cumG(c, MG + 1);
+                DBuf<uint4> recG(c, MG);
+                DBuf<uint32_t> plG(c, MG);
+                MatchList LG{cumG.p, recG.p, plG.p};
+                k_gmatch<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, sel.p, nmG.p, moffG.p, woff.p, LG);
+                FSTC_LAUNCH_CHECK();
+                FSTC_CUDA(cudaMemcpyAsync(cumG.p + MG, woff.p + nf, sizeof(int64_t), cudaMemcpyDeviceToDevice, c.stream));
+                const int64_t n_tiles = ceil_div(WG, GP_TILE);
+                DBuf<int64_t> tile_m(c, n_tiles + 1), tile_off(c, n_tiles + 1);
+                DBuf<uint32_t> tile_cnt(c, n_tiles);
+                k_partition<<<nblk(n_tiles + 1), CT_THREADS, 0, c.stream>>>(cumG.p, MG, WG, 0, n_tiles, tile_m.p);
+                FSTC_LAUNCH_CHECK();
+                GProdArgs g;
+                g.A = A; g.B = B; g.L = LG; g.n_matches = MG; g.W = WG; g.tile_m = tile_m.p;
+                g.tile_cnt = tile_cnt.p; g.tile_off = nullptr;
+                g.msrc = nullptr; g.mab = nullptr; g.mw = nullptr; g.mkey = nullptr;
+                g.bits_b = bits_b; g.nq2 = nq2;
+                g.q2_bits = partitioned ? bits_for(nq2 > 1 ? nq2 - 1 : 1) : -1;
+                k_gprod<0><<<static_cast<unsigned>(n_tiles), GP_THREADS, 0, c.stream>>>(g);
+                FSTC_LAUNCH_CHECK();
+                exclusive_scan<uint32_t>(c, tile_cnt.p, n_tiles, tile_off.p);
+                MGm = read_scalar(c, tile_off.p + n_tiles);
+                gsrc.alloc(c, MGm); gab.alloc(c, MGm); gw.alloc(c, MGm); gtgt.alloc(c, MGm);
+                DBuf<unsigned long long> gkeys(c, MGm + 2);
+                g.tile_off = tile_off.p; g.msrc = gsrc.p; g.mab = gab.p; g.mw = gw.p; g.mkey = gkeys.p;
+                k_gprod<1><<<static_cast<unsigned>(n_tiles), GP_THREADS, 0, c.stream>>>(g);
+                FSTC_LAUNCH_CHECK();
+                c.n_launch += 4;
+                tm.end(h);
+                // target ids of the merged arcs
+                if (MGm > 0) {
+                    if (partitioned) {
+                        ResolveJob j;
+                        j.keys = gkeys.p; j.n_records = MGm; j.q2_bits = g.q2_bits;
+                        j.key_bits = g.q2_bits + bits_for(static_cast<uint64_t>(m1.n_states > 1 ? m1.n_states - 1 : 1));
+                        j.pair = pair.p; j.n_states_before = n_states_live; j.n_states = d_counters.p;
+                        j.mode = 0; j.pos = nullptr; j.o_tgt = gtgt.p; j.sortrec = nullptr; j.shift_t = 0;
+                        j.force_bits = -1;
+                        if (const char *e = getenv("FSTC_RESOLVE_BITS")) j.force_bits = atoi(e);
+                        j.stats = &st; j.profile = o.profile != 0;
+                        resolve_partitioned(c, j);
+                        st.n_resolve += 1;
+                        st.n_resolved_arcs += MGm;
+                    } else {
+                        h = tm.begin(FSTC_T_EMIT);
+                        if (use_dense)
+                            k_resolve_keys<true><<<nblk(MGm), CT_THREADS, 0, c.stream>>>(gkeys.p, MGm, dense.p, nullptr, 0, nq2, d_counters.p,
+                                                                                        pair.p, gtgt.p);
+                        else
+                            k_resolve_keys<false><<<nblk(MGm), CT_THREADS, 0, c.stream>>>(gkeys.p, MGm, nullptr, table.p, cap, nq2,
+                                                                                         d_counters.p, pair.p, gtgt.p);
+                        FSTC_LAUNCH_CHECK();
+                        c.n_launch += 1;
+                        tm.end(h);
+                    }
+                    n_states_live = static_cast<int64_t>(read_scalar(c, d_counters.p));
+                }
+                mstartG.alloc(c, nf + 1);
+                k_mstart<<<nblk(nf + 1), CT_THREADS, 0, c.stream>>>(gsrc.p, MGm, nf, mstartG.p);
+                FSTC_LAUNCH_CHECK();
+                c.n_launch += 1;
+                st.n_raw_grouped += RG;
+                c.sync();
+            }
+            // ---- final place of every arc of the level
             h = tm.begin(FSTC_T_REDUCE);
-            DBuf<uint8_t> head(c, RF);
-            DBuf<int64_t> hidx(c, RF + 1);
-            k_heads<<<nblk(RF), CT_THREADS, 0, c.stream>>>(sorted, RF, head.p);
-            FSTC_LAUNCH_CHECK();
-            exclusive_scan<uint8_t>(c, head.p, RF, hidx.p);
-            const int64_t M = read_scalar(c, hidx.p + RF);
-            DBuf<unsigned long long> mkey(c, M);
-            DBuf<uint32_t> msrc(c, M);
-            DBuf<float> mw(c, M);
-            FSTC_CUDA(cudaMemsetAsync(mw.p, 0, sizeof(float) * M, c.stream));
-            k_reduce<<<nblk(RF), CT_THREADS, 0, c.stream>>>(sorted, head.p, hidx.p, RF, mkey.p, msrc.p, mw.p);
-            FSTC_LAUNCH_CHECK();
-            DBuf<int64_t> mstart(c, nf + 1), fc(c, nf), foff(c, nf + 1);
-            k_mstart<<<nblk(nf + 1), CT_THREADS, 0, c.stream>>>(msrc.p, M, nf, mstart.p);
-            FSTC_LAUNCH_CHECK();
-            k_final_counts<<<nblk(nf), CT_THREADS, 0, c.stream>>>(rawU.p, mstart.p, nf, fc.p);
+            DBuf<int64_t> fc(c, nf), foff(c, nf + 1);
+            k_final_counts<<<nblk(nf), CT_THREADS, 0, c.stream>>>(rawU.p, mstartS.p, mstartG.p, nf, fc.p);
             FSTC_LAUNCH_CHECK();
             exclusive_scan<int64_t>(c, fc.p, nf, foff.p);
-            k_place_merged<<<nblk(M), CT_THREADS, 0, c.stream>>>(mkey.p, msrc.p, mw.p, M, mstart.p, foff.p, arc_base, f_lo, sel.p,
-                                                                 shift_t, bits_b, a_src.p, a_il.p, a_ol.p, a_tgt.p, a_w.p);
-            FSTC_LAUNCH_CHECK();
-            c.n_launch += 5;
+            if (M > 0) {
+                k_place_merged<<<nblk(M), CT_THREADS, 0, c.stream>>>(mkey.p, msrc.p, mw.p, M, mstartS.p, foff.p, arc_base, f_lo, sel.p,
+                                                                     shift_t, bits_b, a_src.p, a_il.p, a_ol.p, a_tgt.p, a_w.p);
+                FSTC_LAUNCH_CHECK();
+            }
+            if (MGm > 0) {
+                k_place_grouped<<<nblk(MGm), CT_THREADS, 0, c.stream>>>(gab.p, gtgt.p, gsrc.p, gw.p, MGm, mstartG.p, foff.p, arc_base,
+                                                                       f_lo, sel.p, bits_b, a_src.p, a_il.p, a_ol.p, a_tgt.p, a_w.p);
+                FSTC_LAUNCH_CHECK();
+            }
+            c.n_launch += 3;
             tm.end(h);
-            launch_emit(EMIT_INDIRECT, LU, MU, RU, 0, f_lo, foff.p, roffU.p, arc_base, nullptr, 0, 0, RU + M);
-            n_arcs += RU + M;
+            launch_emit(EMIT_INDIRECT, LU, MU, RU, 0, f_lo, foff.p, roffU.p, arc_base, nullptr, 0, 0, RU + M + MGm);
+            n_arcs += RU + M + MGm;
             st.n_raw_sorted += RF;
             c.sync();   // the level's temporaries go out of scope below
         }

@@ -40,6 +40,14 @@ struct fstc_packed_t {
     int device = 0;
     int64_t n_launch = 0;         // kernel launches fstc_pack took
     uint8_t any_flags = 0;        // OR of flags[] over all states
+    // The same arcs grouped by (source, outer symbol, target): a group is what a composed arc sees of this operand
+    // (its a or b, and its r1 or r2); inside a group the arcs are sorted by inner symbol.  Used by the merge by
+    // construction (compose.cu, class G).
+    int64_t n_groups = 0;
+    uint2 *garcs = nullptr;       // [n_arcs]     {inner symbol, weight bits}, sorted by (src, outer, tgt, inner)
+    uint32_t *goff = nullptr;     // [n_groups+1] first arc of each group; goff[n_groups] = n_arcs
+    uint2 *gkey = nullptr;        // [n_groups]   {outer symbol, target}
+    uint32_t *gptr = nullptr;     // [n_states+1] first group of each state
 };
 
 namespace fstc {

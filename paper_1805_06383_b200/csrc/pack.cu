@@ -74,6 +74,36 @@ __global__ void pk_flags_rekey(uint4 *__restrict__ rec, int64_t n_arcs, int bits
     out[i] = make_uint4(static_cast<uint32_t>(k2), static_cast<uint32_t>(k2 >> 32), r.z, r.w);
 }
 
+// On the (src, outer, tgt, inner) order of sort #1: the grouped copy of the arcs.  A group = equal (src, outer, tgt).
+__global__ void pk_group_heads(const uint4 *__restrict__ rec, int64_t n_arcs, int bits_inner, uint2 *__restrict__ garcs,
+                               uint32_t *__restrict__ head) {
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= n_arcs) return;
+    uint4 r = rec[i];
+    uint64_t key = (static_cast<uint64_t>(r.y) << 32) | r.x;
+    garcs[i] = make_uint2(static_cast<uint32_t>(key & ((uint64_t(1) << bits_inner) - 1)), r.w);
+    uint32_t h = 1;
+    if (i > 0) {
+        uint4 p = rec[i - 1];
+        uint64_t pkey = (static_cast<uint64_t>(p.y) << 32) | p.x;
+        h = (p.z != r.z) || ((pkey >> bits_inner) != (key >> bits_inner));
+    }
+    head[i] = h;
+}
+__global__ void pk_fill_groups(const uint4 *__restrict__ rec, const uint32_t *__restrict__ head, const int64_t *__restrict__ gidx,
+                               int64_t n_arcs, int bits_inner, int bits_tgt, uint32_t *__restrict__ goff,
+                               uint2 *__restrict__ gkey, uint32_t *__restrict__ gsrc) {
+    int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i == 0) goff[gidx[n_arcs]] = static_cast<uint32_t>(n_arcs);
+    if (i >= n_arcs || !head[i]) return;
+    const int64_t g = gidx[i];
+    uint4 r = rec[i];
+    uint64_t key = ((static_cast<uint64_t>(r.y) << 32) | r.x) >> bits_inner;        // (outer, tgt)
+    goff[g] = static_cast<uint32_t>(i);
+    gkey[g] = make_uint2(static_cast<uint32_t>(key >> bits_tgt), static_cast<uint32_t>(key & ((uint64_t(1) << bits_tgt) - 1)));
+    gsrc[g] = r.z;
+}
+
 // On the final (src, inner, outer, tgt) order: unpack the arc record and mark segment heads.
 __global__ void pk_unpack(const uint4 *__restrict__ rec, int64_t n_arcs, int bits_tgt, int bits_outer,
                           uint4 *__restrict__ arcs, uint32_t *__restrict__ head) {
@@ -154,6 +184,10 @@ void free_packed(fstc_packed_t *p) {
     if (p->seg_ptr) persist_free(p->seg_ptr, nullptr);
     if (p->flags) persist_free(p->flags, nullptr);
     if (p->accept_bits) persist_free(p->accept_bits, nullptr);
+    if (p->garcs) persist_free(p->garcs, nullptr);
+    if (p->goff) persist_free(p->goff, nullptr);
+    if (p->gkey) persist_free(p->gkey, nullptr);
+    if (p->gptr) persist_free(p->gptr, nullptr);
     delete p;
 }
 
@@ -205,7 +239,9 @@ fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side) {
     DBuf<uint32_t> flags32(c, m.n_states);
     FSTC_CUDA(cudaMemsetAsync(flags32.p, 0, sizeof(uint32_t) * m.n_states, c.stream));
     FSTC_CUDA(cudaMemsetAsync(accept_bits.p, 0, sizeof(uint32_t) * ((m.n_states + 31) / 32), c.stream));
-    int64_t n_segs = 0;
+    int64_t n_segs = 0, n_groups = 0;
+    DBuf<uint2> garcs(c, n, true), gkey;
+    DBuf<uint32_t> goff, gptr(c, static_cast<int64_t>(m.n_states) + 1, true);
 
     if (n > 0) {
         DBuf<uint4> ra(c, n), rb(c, n);
@@ -213,6 +249,24 @@ fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side) {
         FSTC_LAUNCH_CHECK();
         uint4 *s1 = radix_sort_records(c, ra.p, rb.p, n, make_sort_passes(bi + bt + bo, bs));
         uint4 *o1 = (s1 == ra.p) ? rb.p : ra.p;
+        {   // grouped copy, on this (src, outer, tgt, inner) order
+            DBuf<uint32_t> ghead(c, n);
+            DBuf<int64_t> gidx(c, n + 1);
+            pk_group_heads<<<blocks_for(n), PK_THREADS, 0, c.stream>>>(s1, n, bi, garcs.p, ghead.p);
+            FSTC_LAUNCH_CHECK();
+            exclusive_scan<uint32_t>(c, ghead.p, n, gidx.p);
+            n_groups = read_scalar(c, gidx.p + n);
+            goff.alloc(c, n_groups + 1, true);
+            gkey.alloc(c, n_groups, true);
+            DBuf<uint32_t> gsrc(c, n_groups);
+            pk_fill_groups<<<blocks_for(n), PK_THREADS, 0, c.stream>>>(s1, ghead.p, gidx.p, n, bi, bt, goff.p, gkey.p, gsrc.p);
+            FSTC_LAUNCH_CHECK();
+            pk_seg_ptr<<<blocks_for(static_cast<int64_t>(m.n_states) + 1), PK_THREADS, 0, c.stream>>>(gsrc.p, n_groups, m.n_states,
+                                                                                                     gptr.p);
+            FSTC_LAUNCH_CHECK();
+            c.n_launch += 3;
+            c.sync();
+        }
         pk_flags_rekey<<<blocks_for(n), PK_THREADS, 0, c.stream>>>(s1, n, bi, bt, bo, flags32.p, o1);
         FSTC_LAUNCH_CHECK();
         // stable sort on (src, inner) only: (outer, tgt) order inside a segment is inherited from sort #1
@@ -236,6 +290,10 @@ fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side) {
         c.sync();   // temporaries (ra, rb, head, ...) are released below; keep the stream ordered and simple
     } else {
         segs.alloc(c, 1, true);
+        goff.alloc(c, 1, true);
+        gkey.alloc(c, 1, true);
+        FSTC_CUDA(cudaMemsetAsync(goff.p, 0, sizeof(uint32_t), c.stream));
+        FSTC_CUDA(cudaMemsetAsync(gptr.p, 0, sizeof(uint32_t) * (static_cast<size_t>(m.n_states) + 1), c.stream));
         uint2 sentinel = make_uint2(0xFFFFFFFFu, 0u);
         FSTC_CUDA(cudaMemcpyAsync(segs.p, &sentinel, sizeof sentinel, cudaMemcpyHostToDevice, c.stream));
         FSTC_CUDA(cudaMemsetAsync(seg_ptr.p, 0, sizeof(uint32_t) * (static_cast<size_t>(m.n_states) + 1), c.stream));
@@ -257,6 +315,8 @@ fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side) {
     p->n_arcs = n; p->n_segs = n_segs;
     p->arcs = arcs.take(); p->segs = segs.take(); p->seg_ptr = seg_ptr.take();
     p->flags = flags.take(); p->accept_bits = accept_bits.take();
+    p->n_groups = n_groups;
+    p->garcs = garcs.take(); p->goff = goff.take(); p->gkey = gkey.take(); p->gptr = gptr.take();
     FSTC_CUDA(cudaGetDevice(&p->device));
     p->n_launch = c.n_launch - launch0;
     return p;

@@ -61,7 +61,7 @@ def test_config_skewed_scaled_partitioned(fstc, resolve_bits):
     appears up to 10^5 times, so bins are far from uniform (exact-capacity retry of the scatter pass)."""
     m1, m2 = workloads.make_config("skewed", scale=0.05)
     res, ref = check_parity(fstc, m1, m2, max_raw_arcs=2_000_000, resolve_mode=fstc.RESOLVE_PARTITIONED)
-    assert res.stats["n_raw_sorted"] > 0 and ref.n_arcs < ref.n_raw_arcs
+    assert res.stats["n_raw_sorted"] + res.stats["n_raw_grouped"] > 0 and ref.n_arcs < ref.n_raw_arcs
 
 
 def test_config_nlp_scaled_partitioned(fstc):
