@@ -641,6 +641,7 @@ struct GProdArgs {
     int64_t n_matches, W;        // ranks [0, W) = group pairs
     const int64_t *tile_m;
     uint32_t *tile_cnt;          // pass 0: arcs found per tile
+    uint8_t *ebits;              // [tiles * GP_THREADS] which of a thread's ranks give an arc: written by pass 0, read by pass 1
     const int64_t *tile_off;     // pass 1: first output slot of every tile
     uint32_t *msrc;              // pass 1 outputs, compact, in rank order: pair index,
     uint32_t *mab;               //   a << bits_b | b,
@@ -730,9 +731,10 @@ __global__ void __launch_bounds__(GP_THREADS) k_gprod(GProdArgs g) {
                 }
             }
         }
+        const uint32_t known = PASS == 1 ? g.ebits[static_cast<int64_t>(blockIdx.x) * GP_THREADS + tid] : 0xFu;
 #pragma unroll
         for (int u = 0; u < GP_IPT; ++u) {
-            if (u < n_valid) {
+            if (u < n_valid && (known >> u & 1u)) {
                 bool found;
                 w[u] = group_dot(g.A.garcs, g.A.goff[g1v[u]], g.A.goff[g1v[u] + 1], g.B.garcs, g.B.goff[g2v[u]],
                                  g.B.goff[g2v[u] + 1], PASS == 0, &found);
@@ -753,6 +755,7 @@ __global__ void __launch_bounds__(GP_THREADS) k_gprod(GProdArgs g) {
 #pragma unroll
     for (int wv = 0; wv < GP_THREADS / 32; ++wv) { if (wv < warp) before += s_warp[wv]; total += s_warp[wv]; }
     if (PASS == 0) {
+        g.ebits[static_cast<int64_t>(blockIdx.x) * GP_THREADS + tid] = static_cast<uint8_t>(exists);
         if (tid == 0) g.tile_cnt[blockIdx.x] = total;
         return;
     }
@@ -1547,11 +1550,12 @@ fstc_result_t *Composer::run() {
                 const int64_t n_tiles = ceil_div(WG, GP_TILE);
                 DBuf<int64_t> tile_m(c, n_tiles + 1), tile_off(c, n_tiles + 1);
                 DBuf<uint32_t> tile_cnt(c, n_tiles);
+                DBuf<uint8_t> ebits(c, n_tiles * GP_THREADS);
                 k_partition<<<nblk(n_tiles + 1), CT_THREADS, 0, c.stream>>>(cumG.p, MG, WG, 0, n_tiles, tile_m.p);
                 FSTC_LAUNCH_CHECK();
                 GProdArgs g;
                 g.A = A; g.B = B; g.L = LG; g.n_matches = MG; g.W = WG; g.tile_m = tile_m.p;
-                g.tile_cnt = tile_cnt.p; g.tile_off = nullptr;
+                g.tile_cnt = tile_cnt.p; g.tile_off = nullptr; g.ebits = ebits.p;
                 g.msrc = nullptr; g.mab = nullptr; g.mw = nullptr; g.mkey = nullptr;
                 g.bits_b = bits_b; g.nq2 = nq2;
                 g.q2_bits = partitioned ? bits_for(nq2 > 1 ? nq2 - 1 : 1) : -1;
