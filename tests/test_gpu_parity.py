@@ -235,3 +235,26 @@ def test_result_to_host_roundtrip(fstc):
     h = res.to_host()
     for k in ("pair", "src", "ilabel", "olabel", "tgt", "weight", "accept", "expanded"):
         assert (h[k].numpy() == getattr(res, k).cpu().numpy()).all(), k
+
+
+def test_merge_by_construction_and_sort_merge_agree(fstc):
+    """Class G (group products, no sort) and class F (radix sort + segmented sum) are two ways to the same merged arcs:
+    both against the oracle, on an input where nearly every source can hold duplicates; the packed operand's grouped
+    copy is checked against a host grouping on the way."""
+    import os
+    m1, m2 = workloads.make_config("skewed", scale=0.05)
+    res_g, ref = check_parity(fstc, m1, m2, max_raw_arcs=2_000_000)
+    assert res_g.stats["n_raw_grouped"] > 0
+    os.environ["FSTC_NO_GROUP_MERGE"] = "1"
+    try:
+        res_f, _ = check_parity(fstc, m1, m2, max_raw_arcs=2_000_000)
+    finally:
+        del os.environ["FSTC_NO_GROUP_MERGE"]
+    assert res_f.stats["n_raw_grouped"] == 0 and res_f.stats["n_raw_sorted"] > 0
+    assert (res_f.n_arcs, res_f.n_states) == (res_g.n_arcs, res_g.n_states)
+    # small machines with parallel duplicate arcs and zero weights (messy_random_fst): both classes, all merge modes
+    for case in SMALL[4:8]:
+        seed, n1, sig, gam, a1, n2, dlt, a2 = case
+        a = messy_random_fst(seed, n1, sig, gam, a1)
+        b = messy_random_fst(seed + 100, n2, gam, dlt, a2)
+        check_parity(fstc, a, b)
