@@ -6,14 +6,17 @@
 //   scan     exclusive scans of the raw counts / match counts, budget rule T                      (step 4)
 //   match    work-list of (pair, inner symbol) matches with the running arc rank                  (step 3b)
 //   emit     one thread per 4 consecutive output ranks (load-balanced over matches, so a match of
-//            10^9 arcs is spread over many blocks): read e1,e2, w = p1·p2, find-or-insert the
-//            target pair in the visited hash table (64-bit key q1·|Q2|+q2, atomicCAS), new ids are
-//            the next frontier                                                                     (steps 5-6)
-//   merge    sources that can hold duplicate (tgt,a,b) go through radix sort + segmented sum      (step 7)
+//            10^9 arcs is spread over many blocks): read e1,e2, w = p1·p2, write the arc               (step 5)
+//   resolve  the id of every target pair: find-or-insert in the visited table inside the emit kernel (the paper's
+//            dense |Q1||Q2| table when it is small, else a hash table on the 64-bit key q1·|Q2|+q2, atomicCAS), or,
+//            for a big level that creates about a state per arc, the streaming partitioned resolve of
+//            resolve.cu; new ids are the next frontier                                                  (step 6)
+//   merge    sources that can hold duplicate (tgt,a,b): merged arcs computed directly from the (a,r1) x (b,r2)
+//            groups of the pair (class G), or radix sort + segmented sum (class F)                      (step 7)
 //   assemble accept list, expanded flags                                                           (step 8)
 //
 // What differs from the paper's own kernel design (one launch per inner symbol per popped pair, 32-thread
-// blocks, host-side queue, dense |Q1||Q2| visited table, lossy table H — PAPER.md:219-243) is listed in
+// blocks, host-side queue, lossy table H, sort + reduce of every flagged source — PAPER.md:219-243) is listed in
 // DESIGN.md "differences".
 #include <algorithm>
 #include <cstdlib>
@@ -1169,8 +1172,7 @@ struct Composer {
     int64_t n_states_live = 1;         // states created so far, including those of the launches of this level
 
     void launch_emit(int mode, const MatchList &L, int64_t n_matches, int64_t R, int64_t pos_base, int64_t f_lo,
-                     const int64_t *foff, const int64_t *roff, int64_t arc_base, uint4 *sortrec, int shift_t, int bits_b,
-                     int64_t n_positions = 0) {
+                     const int64_t *foff, const int64_t *roff, int64_t arc_base, uint4 *sortrec, int shift_t, int bits_b) {
         if (R <= 0) return;
         const int64_t tile0 = (pos_base / EM_TILE) * EM_TILE;
         const int64_t n_tiles = ceil_div(pos_base + R - tile0, EM_TILE);
@@ -1253,9 +1255,6 @@ fstc_result_t *Composer::run() {
     n_pairs_all = n_pairs_total;
     use_dense = o.resolve_mode != FSTC_RESOLVE_HASH && n_pairs_total <= DENSE_MAX_PAIRS;
 
-    if (const char *e = getenv("FSTC_L2_FETCH")) {            // experiment knob: 32 / 64 / 128
-        (void)cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, static_cast<size_t>(atoi(e)));
-    }
     cudaEvent_t ev0, ev1;
     FSTC_CUDA(cudaEventCreate(&ev0));
     FSTC_CUDA(cudaEventCreate(&ev1));
@@ -1623,7 +1622,7 @@ fstc_result_t *Composer::run() {
             }
             c.n_launch += 3;
             tm.end(h);
-            launch_emit(EMIT_INDIRECT, LU, MU, RU, 0, f_lo, foff.p, roffU.p, arc_base, nullptr, 0, 0, RU + M + MGm);
+            launch_emit(EMIT_INDIRECT, LU, MU, RU, 0, f_lo, foff.p, roffU.p, arc_base, nullptr, 0, 0);
             n_arcs += RU + M + MGm;
             st.n_raw_sorted += RF;
             c.sync();   // the level's temporaries go out of scope below
