@@ -1023,6 +1023,13 @@ __global__ void k_compact_sel(const uint8_t *__restrict__ flag, const int64_t *_
     if (i < nf && flag[i]) sel[off[i]] = static_cast<uint32_t>(i);
 }
 
+// several device scalars -> one contiguous block, so that the host reads them with ONE copy (a level costs a fixed
+// number of host round trips; on small levels those are the whole cost)
+struct ScalarPtrs { const int64_t *p[8]; };
+__global__ void k_gather_scalars(ScalarPtrs s, int n, int64_t *__restrict__ out) {
+    if (static_cast<int>(threadIdx.x) < n) out[threadIdx.x] = s.p[threadIdx.x] ? *s.p[threadIdx.x] : 0;
+}
+
 inline unsigned nblk(int64_t n, int threads = CT_THREADS) { return static_cast<unsigned>(ceil_div(n > 0 ? n : 1, threads)); }
 
 // ------------------------------------------------------------------------------------------ host side
@@ -1298,6 +1305,7 @@ fstc_result_t *Composer::run() {
         DBuf<int64_t> roffU, roffF, moffU, moffF, roffG, moffG, woff;
         int64_t RG = 0, MG = 0, WG = 0;                          // class G: raw arcs, pairs, group pairs of the level
         DBuf<uint32_t> sel;                                      // compacted level: frontier index of working pair i
+        DBuf<int64_t> level_totals(c, 8);
         auto scan_level = [&](int64_t *n_sel_out) {             // offsets + totals of the level, one synchronisation
             exclusive_scan2(c, rawU.p, nmU.p, nf, roffU.p, moffU.p);
             if (has_F) exclusive_scan2(c, rawF.p, nmF.p, nf, roffF.p, moffF.p);
@@ -1305,21 +1313,16 @@ fstc_result_t *Composer::run() {
                 exclusive_scan2(c, rawG.p, nmG.p, nf, roffG.p, moffG.p);
                 exclusive_scan<int64_t>(c, gwork.p, nf, woff.p);
             }
-            RF = 0; MF = 0; RG = 0; MG = 0; WG = 0;
-            int64_t dummy = 0;
-            FSTC_CUDA(cudaMemcpyAsync(&RU, roffU.p + nf, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
-            FSTC_CUDA(cudaMemcpyAsync(&MU, moffU.p + nf, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
-            if (has_F) {
-                FSTC_CUDA(cudaMemcpyAsync(&RF, roffF.p + nf, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
-                FSTC_CUDA(cudaMemcpyAsync(&MF, moffF.p + nf, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
-            }
-            if (has_G) {
-                FSTC_CUDA(cudaMemcpyAsync(&RG, roffG.p + nf, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
-                FSTC_CUDA(cudaMemcpyAsync(&MG, moffG.p + nf, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
-                FSTC_CUDA(cudaMemcpyAsync(&WG, woff.p + nf, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
-            }
-            FSTC_CUDA(cudaMemcpyAsync(n_sel_out ? n_sel_out : &dummy, d_counters.p + 3, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
+            ScalarPtrs sp{{roffU.p + nf, moffU.p + nf, has_F ? roffF.p + nf : nullptr, has_F ? moffF.p + nf : nullptr,
+                           has_G ? roffG.p + nf : nullptr, has_G ? moffG.p + nf : nullptr, has_G ? woff.p + nf : nullptr,
+                           reinterpret_cast<const int64_t *>(d_counters.p + 3)}};
+            k_gather_scalars<<<1, 32, 0, c.stream>>>(sp, 8, level_totals.p);
+            FSTC_LAUNCH_CHECK();
+            int64_t t[8];
+            FSTC_CUDA(cudaMemcpyAsync(t, level_totals.p, sizeof t, cudaMemcpyDeviceToHost, c.stream));
             c.sync();
+            RU = t[0]; MU = t[1]; RF = t[2]; MF = t[3]; RG = t[4]; MG = t[5]; WG = t[6];
+            if (n_sel_out) *n_sel_out = t[7];
         };
         // A level that will clearly be cut by the budget (predicted from the previous level's fan-out) is counted
         // only below a key limit: rule T expands a key-ordered prefix, so pairs far above the cut never matter.
