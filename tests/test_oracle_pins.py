@@ -321,3 +321,30 @@ def test_tiny_config_invariants_and_pair_expander():
         assert len(w) == sum(1 for k in whole if k[0] == (q1, q2))
         n += len(w)
     assert n > 0
+
+
+@pytest.mark.parametrize("seed", [11, 12, 13, 14])
+def test_merged_weights_are_a_contraction_over_the_inner_symbol(seed):
+    """PAPER.md:53 read as tensors: with A[q1,a,c,r1] and B[q2,c,b,r2] the summed input weights (and their structural
+    0/1 versions), the merged arc (q1q2, a, b, r1r2) exists iff the structural contraction over c is non-zero and weighs
+    sum_c A·B.  Checked with numpy.einsum for every reached source: a dropped duplicate, a product summed in the wrong
+    group or a transposed operand fails it.  (Also the identity behind the CUDA path's merge by construction.)"""
+    n1, n2, sig, gam, dlt = 5, 4, 3, 4, 3
+    m1 = messy_random_fst(seed, n1, sig, gam, 60, dup_frac=0.3)
+    m2 = messy_random_fst(seed + 50, n2, gam, dlt, 50, dup_frac=0.3)
+    A = np.zeros((n1, sig, gam, n1)); As = np.zeros_like(A)
+    B = np.zeros((n2, gam, dlt, n2)); Bs = np.zeros_like(B)
+    np.add.at(A, (m1.src, m1.ilabel, m1.olabel, m1.tgt), m1.weight.astype(np.float64))
+    np.add.at(As, (m1.src, m1.ilabel, m1.olabel, m1.tgt), 1.0)
+    np.add.at(B, (m2.src, m2.ilabel, m2.olabel, m2.tgt), m2.weight.astype(np.float64))
+    np.add.at(Bs, (m2.src, m2.ilabel, m2.olabel, m2.tgt), 1.0)
+    W = np.einsum("pacr,qcbs->pqabrs", A, B)            # [q1, q2, a, b, r1, r2]
+    S = np.einsum("pacr,qcbs->pqabrs", As, Bs) > 0
+    res = oracle.compose(m1, m2, merge=True)
+    got = _oracle_canon(res)
+    want = {}
+    for q1, q2 in zip(res.q1, res.q2):                   # every reached (and here expanded) source pair
+        for a, b, r1, r2 in zip(*np.nonzero(S[q1, q2])):
+            want[((int(q1), int(q2)), int(a), int(b), (int(r1), int(r2)))] = float(W[q1, q2, a, b, r1, r2])
+    _assert_arcs_equal(got, want, rtol=1e-12)
+    assert len(got) < res.n_raw_arcs                     # the inputs are made so that merging really happens
