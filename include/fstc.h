@@ -215,7 +215,8 @@ FSTC_API int fstc_compose(const fstc_fst_t *m1, const fstc_fst_t *m2, const fstc
 FSTC_API int fstc_result_to_host(const fstc_result_t *r, void *cuda_stream, const fstc_host_result_t *dst);
 FSTC_API void fstc_result_free(fstc_result_t *r);
 
-/* Releases the cached device memory of the library's pool back to the driver. */
+/* Releases the cached device memory back to the driver: the calling thread's workspace arena, the parked result /
+ * packed blocks and the pool's free blocks.  (Device memory the library caches is otherwise kept for reuse.) */
 FSTC_API int fstc_trim_pool(void);
 
 FSTC_API const char *fstc_strerror(int code);
