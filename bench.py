@@ -263,20 +263,28 @@ def main():
         flush.fill_(1)                                                   # L2 flush, outside the timed region
         e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
         torch.cuda.synchronize()
+        t0 = time.perf_counter()
         e0.record()
         p1 = fstc.fstc_pack(d1, 1)
+        t1 = time.perf_counter()
         p2 = fstc.fstc_pack(d2, 2)
+        t2 = time.perf_counter()
         e1.record()
         r = fstc.fstc_compose_packed(p1, p2, merge_mode=args.merge_mode, max_raw_arcs=budget, profile=profile,
                                      resolve_mode=args.resolve_mode,
                                      arc_capacity_hint=hints["arc"], state_capacity_hint=hints["state"])
+        t3 = time.perf_counter()
         e2.record()
         torch.cuda.synchronize()
         st = r.stats
+        host_ms = [round(1e3 * (b - a), 2) for a, b in ((t0, t1), (t1, t2), (t2, t3))]      # pack, pack, compose on the host clock
         st["pack_ms"], st["compose_ms"] = e0.elapsed_time(e1), e1.elapsed_time(e2)
         launches = st["n_kernel_launches"] + p1.info().get("n_kernel_launches", 0) + p2.info().get("n_kernel_launches", 0)
         del r
         p1.free(); p2.free()
+        if os.environ.get("FSTC_ALLOC_TRACE") or os.environ.get("FSTC_RS_TRACE"):   # debug knobs of the library: mark the steps
+            print(f"[bench] step done: {e0.elapsed_time(e2):.2f} ms, stages {sum(st['ms'].values()):.2f} ms, host {host_ms}, "
+                  f"lib total {st['ms_total']:.2f}", file=sys.stderr, flush=True)
         return e0.elapsed_time(e2), st, launches
 
     # warm-up: at least W (>= 3) untimed steps; then, while the machine is still settling (right after another GPU

@@ -1,4 +1,6 @@
 // C ABI of libfstc (include/fstc.h): argument checks, error translation, the device memory pool.
+#include <cstdio>
+#include <cstdlib>
 #include <map>
 #include <mutex>
 #include <unordered_map>
@@ -95,6 +97,8 @@ void *arena_alloc(size_t bytes, cudaStream_t stream) {
             if (r.second >= bytes && r.second < best_len) { best_ci = static_cast<int>(ci); best_off = r.first; best_len = r.second; }
     }
     if (best_ci >= 0) return arena_carve(best_ci, best_off, bytes);
+    static const bool trace = getenv("FSTC_ALLOC_TRACE") != nullptr;
+    if (trace) fprintf(stderr, "[fstc arena] new chunk for %.1f MB (chunks so far %zu)\n", bytes / 1048576.0, g_arena.chunks.size());
     ArenaChunk ch;
     ch.size = bytes > ARENA_MIN_CHUNK ? bytes : ARENA_MIN_CHUNK;
     ch.dev = dev;
@@ -178,6 +182,9 @@ void *persist_alloc(size_t bytes, cudaStream_t stream) {
             return b.p;
         }
     }
+    static const bool trace = getenv("FSTC_ALLOC_TRACE") != nullptr;
+    if (trace && bytes >= PARK_MIN_BYTES) fprintf(stderr, "[fstc persist] pool allocation of %.1f MB (parked %zu blocks, %.1f GB)\n",
+                                                  bytes / 1048576.0, g_parked.size(), g_parked_bytes / 1e9);
     cudaError_t e = cudaMallocFromPoolAsync(&p, bytes, device_pool(), stream);
     if (e != cudaSuccess) {                                // out of memory: hand the parked blocks back, once
         (void)cudaGetLastError();
@@ -212,6 +219,8 @@ void persist_free(void *p, cudaStream_t stream) {
             }
         }
     }
+    static const bool trace = getenv("FSTC_ALLOC_TRACE") != nullptr;
+    if (trace) fprintf(stderr, "[fstc persist] block goes back to the pool (not parked)\n");
     (void)cudaFreeAsync(p, stream);
 }
 

@@ -21,6 +21,7 @@
 #include <algorithm>
 #include <cstdlib>
 #include <cstring>
+#include <ctime>
 
 #include "internal.h"
 #include "scan.cuh"
@@ -1262,6 +1263,19 @@ fstc_result_t *Composer::run() {
     n_pairs_all = n_pairs_total;
     use_dense = o.resolve_mode != FSTC_RESOLVE_HASH && n_pairs_total <= DENSE_MAX_PAIRS;
 
+    // FSTC_ALLOC_TRACE: host clock at the main points of the run (debug knob; finds host-side stalls)
+    static const bool host_trace = getenv("FSTC_ALLOC_TRACE") != nullptr;
+    timespec ht0;
+    clock_gettime(CLOCK_MONOTONIC, &ht0);
+    double ht_last = 0.0;
+    auto hostmark = [&](const char *what, int level) {
+        if (!host_trace) return;
+        timespec t;
+        clock_gettime(CLOCK_MONOTONIC, &t);
+        const double ms = (t.tv_sec - ht0.tv_sec) * 1e3 + (t.tv_nsec - ht0.tv_nsec) * 1e-6;
+        if (ms - ht_last > 3.0) fprintf(stderr, "[fstc host] level %d %-12s at %8.2f ms (+%.2f)\n", level, what, ms, ms - ht_last);
+        ht_last = ms;
+    };
     cudaEvent_t ev0, ev1;
     FSTC_CUDA(cudaEventCreate(&ev0));
     FSTC_CUDA(cudaEventCreate(&ev1));
@@ -1413,6 +1427,7 @@ fstc_result_t *Composer::run() {
         }
         tm.end(h);
 
+        hostmark("count+scan", lvl);
         const int64_t R = RU + RF + RG;
         cur_sel = sel.p;
         // ---- capacities for this level
@@ -1450,12 +1465,17 @@ fstc_result_t *Composer::run() {
             const double fan = static_cast<double>(R) / static_cast<double>(n_sel);
             double pr = static_cast<double>(new_bound) * fan;
             if (o.max_raw_arcs > 0) pr = std::min(pr, static_cast<double>(o.max_raw_arcs - cum_raw - R));
-            size_t free_b = 0, total_b = 0;
-            (void)cudaMemGetInfo(&free_b, &total_b);
-            uint64_t pool_reserved = 0, pool_used = 0;           // cached blocks of our pool are available to us
-            (void)cudaMemPoolGetAttribute(device_pool(), cudaMemPoolAttrReservedMemCurrent, &pool_reserved);
+            // what is free for us: the device's memory minus what our pool has handed out.  (cudaMemGetInfo would say it
+            // exactly, but it goes to the driver and was seen to take 10-50 ms at times: the device size is read once.)
+            static size_t device_bytes = 0;
+            if (device_bytes == 0) {
+                size_t f = 0, t = 0;
+                (void)cudaMemGetInfo(&f, &t);
+                device_bytes = t > 0 ? t - t / 16 : size_t(64) << 30;            // leave 1/16 to others on the device
+            }
+            uint64_t pool_used = 0;
             (void)cudaMemPoolGetAttribute(device_pool(), cudaMemPoolAttrUsedMemCurrent, &pool_used);
-            if (pool_reserved > pool_used) free_b += pool_reserved - pool_used;
+            const size_t free_b = device_bytes > pool_used ? device_bytes - pool_used : 0;
             pr = std::min(pr, 16.0 * static_cast<double>(n_arcs + R));           // never more than 16x what is needed now
             const double ps = std::min(pr, static_cast<double>(remaining_pairs - static_cast<uint64_t>(new_bound)));
             // 20 B per arc; per state 8 B + a table slot at the target load; at most 40 % of what is free
@@ -1465,6 +1485,7 @@ fstc_result_t *Composer::run() {
             next_S = ps > 0 ? static_cast<int64_t>(ps * scale) : 0;
             if (n_states + new_bound + next_S >= 0x7FFFFFFFll) next_S = 0;
         }
+        hostmark("lookahead", lvl);
         ensure_pairs(n_states + new_bound, n_states + new_bound + next_S);
         if (!partitioned) {
             // no look-ahead for the table if the next level is expected to leave it for the partitioned resolve anyway
@@ -1474,6 +1495,7 @@ fstc_result_t *Composer::run() {
         }
         ensure_arcs(n_arcs + R, n_arcs + R + next_R);
         n_states_live = n_states;
+        hostmark("ensure", lvl);
 
         // ---- match work-lists
         MatchList LU{nullptr, nullptr, nullptr}, LF{nullptr, nullptr, nullptr};
@@ -1491,6 +1513,7 @@ fstc_result_t *Composer::run() {
             tm.end(h);
         }
 
+        hostmark("match", lvl);
         const int64_t arc_base = n_arcs;
         if (RF == 0 && RG == 0) {
             // no source of this level can hold duplicates: arcs go straight to their final place
@@ -1631,7 +1654,9 @@ fstc_result_t *Composer::run() {
             c.sync();   // the level's temporaries go out of scope below
         }
 
+        hostmark("emit+resolve", lvl);
         const int64_t ns_after = static_cast<int64_t>(read_scalar(c, d_counters.p));
+        hostmark("ns read", lvl);
         if (lvl < FSTC_MAX_LEVEL_STATS) {
             st.level_frontier[lvl] = nf_all;
             st.level_raw[lvl] = R;
@@ -1649,6 +1674,7 @@ fstc_result_t *Composer::run() {
         if (stop_after) break;
     }
 
+    hostmark("levels done", lvl);
     // ---- assemble
     int h = tm.begin(FSTC_T_ASSEMBLE);
     DBuf<uint8_t> expanded(c, n_states, true);
@@ -1678,6 +1704,7 @@ fstc_result_t *Composer::run() {
     cudaEventDestroy(ev0);
     cudaEventDestroy(ev1);
     tm.collect(st.ms);
+    hostmark("assembled", lvl);
 
     st.ms_total = ms;
     st.n_states = n_states; st.n_arcs = n_arcs; st.n_raw_arcs = cum_raw;

@@ -228,7 +228,13 @@ __global__ void __launch_bounds__(SC_THREADS, SC_TILE == SC_TILE_BIG ? 2 : FSTC_
 // are entered first, then every arc key finds its entry or creates it.  New ids are handed out per round of DD_TILE
 // records with one global atomicAdd; the winner of a key writes pair[id].  The id of arc record i of the bin goes to
 // ids_out[start[bin] + i], the index the last scatter pass recorded in dest[].
-constexpr int DD_THREADS = 256;
+#ifndef FSTC_DD_THREADS
+#define FSTC_DD_THREADS 512
+#endif
+#ifndef FSTC_DD_MINB
+#define FSTC_DD_MINB 3
+#endif
+constexpr int DD_THREADS = FSTC_DD_THREADS;
 constexpr int DD_IPT = 4;
 constexpr int DD_TILE = DD_THREADS * DD_IPT;
 #ifndef FSTC_DD_SLOTS
@@ -265,7 +271,7 @@ __device__ __forceinline__ int dd_find_or_claim(unsigned long long *keys, unsign
     return -1;
 }
 
-__global__ void __launch_bounds__(DD_THREADS) rs_dedupe(DedupeArgs a) {
+__global__ void __launch_bounds__(DD_THREADS, FSTC_DD_MINB) rs_dedupe(DedupeArgs a) {
     extern __shared__ unsigned long long keys[];               // [DD_SLOTS], then uint32 ids[DD_SLOTS]
     uint32_t *ids = reinterpret_cast<uint32_t *>(keys + DD_SLOTS);
     __shared__ uint32_t s_warp[DD_THREADS / 32];
