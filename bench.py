@@ -56,8 +56,8 @@ def _peaks():
 
 
 class ClockSampler:
-    """Samples SM clocks and throttle reasons during the timed region: NVML in a thread (light; `nvidia-smi -lms`
-    polling was seen to stall CUDA calls of the timed process for milliseconds), nvidia-smi only as a fallback."""
+    """Samples SM clocks and throttle reasons during the timed region: NVML in a thread of this process (no subprocess
+    polling the driver beside the timed work), nvidia-smi only as a fallback."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -287,9 +287,8 @@ def main():
                   f"lib total {st['ms_total']:.2f}", file=sys.stderr, flush=True)
         return e0.elapsed_time(e2), st, launches
 
-    # warm-up: at least W (>= 3) untimed steps; then, while the machine is still settling (right after another GPU
-    # process ended, the first seconds show sporadic host-side stalls of 5-40 ms per step), up to 30 more until three
-    # steps in a row agree within 2 % of the fastest step seen
+    # warm-up: at least W (>= 3) untimed steps; then, while the machine is still settling (memory pools filling, clocks
+    # ramping), up to 30 more until three steps in a row agree within 2 % of the fastest step seen
     n_warm, recent, best = 0, [], float("inf")
     while n_warm < max(args.warmup, 3) + 30:
         ms, st, _ = step()
