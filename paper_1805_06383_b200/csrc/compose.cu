@@ -1346,7 +1346,7 @@ fstc_result_t *Composer::run() {
             const double remaining = static_cast<double>(o.max_raw_arcs - cum_raw);
             const double predicted = static_cast<double>(nf) * last_fan;
             if (predicted > 4.0 * remaining)
-                key_limit = static_cast<uint64_t>(static_cast<double>(n_pairs_total) * (2.0 * remaining / predicted)) + 1;
+                key_limit = static_cast<uint64_t>(static_cast<double>(n_pairs_total) * (1.5 * remaining / predicted)) + 1;
         }
         int h;
         while (true) {
