@@ -5,9 +5,15 @@
                     [--impl ours|reference] [--no-e2e] [--no-cpu-baseline]
 
 One "step" = one pass of the whole hot path over one pair of synthetic transducers: pack(M1),
-pack(M2), compose_packed (count, scan, match, emit + visited set, merge, assembly).  Inputs are resident
-in HBM when the timed region of `value` starts; `e2e` repeats the step through the C ABI with HOST
-buffers (H2D of the inputs and D2H of the whole result inside the timed region).
+pack(M2), compose_packed (count, scan, match, emit, target resolve — visited table or partitioned —, merge,
+assembly).  Inputs are resident in HBM when the timed region of `value` starts; `e2e` repeats the step
+through the C ABI with HOST buffers (H2D of the inputs and D2H of the whole result inside the timed region).
+
+`roofline` describes the kernel with the largest device time in the step among k_emit, rs_scatter, rs_dedupe and
+rs_gather_ids (each one kernel per library stage, timed live with CUDA events on the compose stream): algorithmic
+bytes per launch from exact device-side counts (DESIGN.md §7) / average launch time, against the measured HBM peak;
+`traffic` = DRAM bytes per launch of that kernel from the committed ncu capture; `roofline.kernels` lists all four and
+`roofline_path` the whole composition against SURVEY's byte model.  `ms_steps` carries every timed step.
 
 N > 1 (torchrun): the path shards by independent problems — every rank composes its own seeded pair of
 the same shape, no data-path collective ("scaling": "weak"); time = max over ranks, value = Σ arcs / time.
