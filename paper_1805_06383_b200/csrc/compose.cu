@@ -1345,8 +1345,11 @@ fstc_result_t *Composer::run() {
         if (o.max_raw_arcs > 0 && nf > 100000 && last_fan > 0) {
             const double remaining = static_cast<double>(o.max_raw_arcs - cum_raw);
             const double predicted = static_cast<double>(nf) * last_fan;
-            if (predicted > 4.0 * remaining)
-                key_limit = static_cast<uint64_t>(static_cast<double>(n_pairs_total) * (1.5 * remaining / predicted)) + 1;
+            if (predicted > 4.0 * remaining) {
+                double margin = 1.5;                                 // test knob: a margin < 1 forces the widening path
+                if (const char *e = getenv("FSTC_KEY_LIMIT_MARGIN")) margin = atof(e);
+                key_limit = static_cast<uint64_t>(static_cast<double>(n_pairs_total) * (margin * remaining / predicted)) + 1;
+            }
         }
         int h;
         while (true) {

@@ -149,3 +149,17 @@ def test_nlp_full_size_exact(fstc):
     m1, m2 = workloads.make_config("nlp")
     res, ref = check_parity(fstc, m1, m2)
     assert ref.n_levels == 51
+
+
+@pytest.mark.parametrize("margin", ["0.02", "0.3", "40"])
+def test_cut_level_key_limit_is_exact_whatever_the_guess(fstc, margin):
+    """A level that rule T will cut is counted only below a guessed key limit (1.5 x the predicted cut).  The guess must
+    not matter: far too low (the level is recounted with a 4x wider limit, several times), too low, far too high."""
+    import os
+    m1, m2 = workloads.make_config("large", scale=0.1)
+    os.environ["FSTC_KEY_LIMIT_MARGIN"] = margin
+    try:
+        res, ref = check_parity(fstc, m1, m2, max_raw_arcs=2_000_000)
+    finally:
+        del os.environ["FSTC_KEY_LIMIT_MARGIN"]
+    assert res.truncated == 1 and ref.level_size[-1] > 100_000       # the cut level is big enough to be compacted
