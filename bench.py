@@ -107,7 +107,7 @@ class ClockSampler:
                                                            ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")])
             except Exception:
                 pass
-            time.sleep(float(os.environ.get("FSTC_BENCH_CLOCK_PERIOD", "0.05")))
+            time.sleep(0.05)
 
     def _read(self):
         for line in self.proc.stdout:
