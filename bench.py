@@ -9,11 +9,12 @@ pack(M2), compose_packed (count, scan, match, emit, target resolve — visited t
 assembly).  Inputs are resident in HBM when the timed region of `value` starts; `e2e` repeats the step
 through the C ABI with HOST buffers (H2D of the inputs and D2H of the whole result inside the timed region).
 
-`roofline` describes the kernel with the largest device time in the step among k_emit, rs_scatter, rs_dedupe and
-rs_gather_ids (each one kernel per library stage, timed live with CUDA events on the compose stream): algorithmic
-bytes per launch from exact device-side counts (DESIGN.md §7) / average launch time, against the measured HBM peak;
-`traffic` = DRAM bytes per launch of that kernel from the committed ncu capture; `roofline.kernels` lists all four and
-`roofline_path` the whole composition against SURVEY's byte model.  `ms_steps` carries every timed step.
+`roofline` is SURVEY §8(d)'s number: the algorithmic bytes of the whole composition (exact device-side counts) divided by
+the device time of fstc_compose_packed, against the measured HBM peak; `roofline.stage_groups` splits the same terms over
+the stage groups that serve them (CUDA events on the compose stream, library `profile` mode) and names the dominant one;
+`roofline.achieved_vs_own_traffic` keeps the achieved bandwidth of the resolve kernels on the bytes their design moves
+(not a fraction of the method's bytes); `traffic` = DRAM bytes of one composition from the committed ncu capture.
+`ms_steps` carries every timed step.
 
 N > 1 (torchrun): the path shards by independent problems — every rank composes its own seeded pair of
 the same shape, no data-path collective ("scaling": "weak"); time = max over ranks, value = Σ arcs / time.
@@ -145,28 +146,40 @@ class ClockSampler:
                 "reasons": sorted(reasons), "source": "nvml" if self.nvml else "nvidia-smi"}
 
 
-def alg_bytes(st: dict, n_new_states: int) -> dict:
-    """Algorithmic bytes from exact device-side counts: of one composition (SURVEY §8(d) model) and
-    of every hot kernel, summed over its launches in the step."""
+# Stage groups of the library's `profile` times, and the SURVEY §8(d) terms each one serves.
+STAGE_GROUPS = {
+    "index": ("count", "scan", "match"),                       # 16·E + 8·Σ_E(s1+s2)
+    "expand": ("emit", "sort", "reduce"),                      # 12·Σ_matches(n1+n2) + 20·M + 40·R_m (+ table-level probes, fused)
+    "visited": ("table", "rs_scatter", "rs_dedupe", "rs_gather"),   # 12·R + 12·S of the levels resolved outside the emit kernel
+    "assemble": ("assemble",),                                 # 9·S
+}
+
+
+def alg_bytes(st: dict) -> dict:
+    """SURVEY §8(d) algorithmic bytes from exact device-side counts: of the whole composition, and split over the
+    stage groups that serve each term.  The visited-set term (12 per raw arc + 12 per state) of the levels whose targets
+    are resolved inside the emit kernel (visited table) is charged to `expand`; the rest to `visited`."""
     E, R, S, M = st["n_expanded"], st["n_raw_arcs"], st["n_states"], st["n_arcs"]
     Rm = st["n_raw_sorted"]
-    path = (16 * E + 8 * st["n_seg_visited"] + 12 * st["n_match_arcs"] + 12 * R + 12 * S + 20 * M + 9 * S + 40 * Rm)
-    Rp = st["n_resolved_arcs"]                      # arcs whose targets went through the partitioned resolve
-    Rt = R - Rp                                     # arcs resolved in the visited table, inside the emit kernel
-    new_p = st["rs_dedupe_new"]
-    new_t = max(0, n_new_states - new_p)
-    kern = {
-        # arc payload of the matching segments + the four final columns (or the 16-byte sort record) per arc
-        # + table levels: target column, one probe per arc, insert + pair per new state; resolve levels: the key
-        "k_emit": 12 * st["n_match_arcs"] + 16 * R + (4 + 12) * Rt + 20 * new_t + 8 * Rp,
-        # record in + out (8 + 8), and the recorded permutation (4 + 2) on the arc stream
-        "rs_scatter": 16 * (st["rs_scatter_recs"] + st["rs_scatter_dest_recs"]) + 6 * st["rs_scatter_dest_recs"],
-        # state record, arc key in + id out, pair of every new state
-        "rs_dedupe": 8 * st["rs_dedupe_states"] + 12 * st["rs_dedupe_arcs"] + 8 * new_p,
-        # permutation (4 + 2), id in, id out
+    Rp, Sp = st["n_resolved_arcs"], st["rs_dedupe_new"]        # arcs / new states of the partitioned-resolve levels
+    groups = {
+        "index": 16 * E + 8 * st["n_seg_visited"],
+        "expand": 12 * st["n_match_arcs"] + 20 * M + 40 * Rm + 12 * (R - Rp) + 12 * (S - Sp),
+        "visited": 12 * Rp + 12 * Sp,
+        "assemble": 9 * S,
+    }
+    return {"path": sum(groups.values()), "groups": groups}
+
+
+def own_traffic(st: dict) -> dict:
+    """Bytes each hot kernel of the partitioned resolve moves BY DESIGN (not SURVEY's model): what its
+    achieved bandwidth is measured on (`achieved_vs_own_traffic`)."""
+    rec = st.get("rs_rec_bytes", 8)
+    return {
+        "rs_scatter": (2 * rec) * (st["rs_scatter_recs"] + st["rs_scatter_dest_recs"]) + 6 * st["rs_scatter_dest_recs"],
+        "rs_dedupe": 8 * st["rs_dedupe_states"] + (rec + 4) * st["rs_dedupe_arcs"] + 8 * st["rs_dedupe_new"],
         "rs_gather": 14 * st["rs_gather_recs"],
     }
-    return {"path": path, "kernels": kern}
 
 
 def rank_seeds(workload: str, rank: int):
@@ -262,7 +275,6 @@ def main():
     budget = int(workloads.CONFIGS[args.workload]["max_raw_arcs"])
     d1, d2 = fstc.DeviceFst.from_host(m1), fstc.DeviceFst.from_host(m2)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
-    hints = {"arc": 0, "state": 0}
 
     def step(profile=True):
         """pack + compose on device-resident inputs; returns (ms, stats, pack_launches)."""
@@ -277,8 +289,7 @@ def main():
         t2 = time.perf_counter()
         e1.record()
         r = fstc.fstc_compose_packed(p1, p2, merge_mode=args.merge_mode, max_raw_arcs=budget, profile=profile,
-                                     resolve_mode=args.resolve_mode,
-                                     arc_capacity_hint=hints["arc"], state_capacity_hint=hints["state"])
+                                     resolve_mode=args.resolve_mode)
         t3 = time.perf_counter()
         e2.record()
         torch.cuda.synchronize()
@@ -321,33 +332,38 @@ def main():
 
     st = stats[-1]
     peak, peak_src = _peaks()
-    new_states = st["n_states"] - 1
-    ab = alg_bytes(st, new_states)
-    # the dominant kernel of the step, by device time measured live (CUDA events on the compose stream, library
-    # `profile` mode): each of these stages is ONE kernel, launched several times per step
-    kstage = {"k_emit": ("emit", "n_emit_launches"), "rs_scatter": ("rs_scatter", "rs_scatter_launches"),
-              "rs_dedupe": ("rs_dedupe", "rs_dedupe_launches"), "rs_gather": ("rs_gather", "rs_gather_launches")}
-    kms = {k: sum(s["ms"][v[0]] for s in stats) / len(stats) for k, v in kstage.items()}
-    dom = max(kms, key=kms.get)
-    dom_launches = max(1, st[kstage[dom][1]])
-    dom_ms = kms[dom] / dom_launches
-    dom_bytes_per_launch = ab["kernels"][dom] / dom_launches
-    dom_gbs = dom_bytes_per_launch / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0
+    ab = alg_bytes(st)
+    compose_ms = sum(s["compose_ms"] for s in stats) / len(stats)
+    pack_ms = sum(s["pack_ms"] for s in stats) / len(stats)
+    stage_ms = {k: sum(s["ms"][k] for s in stats) / len(stats) for k in fstc.STAGES}
+    # the headline fraction is B_alg / t_compose_packed / peak; per stage group the same terms over the
+    # group's device time (CUDA events on the compose stream, library `profile` mode)
+    path_gbs = ab["path"] / (compose_ms * 1e-3) / 1e9
+    groups = {}
+    for gname, members in STAGE_GROUPS.items():
+        ms = sum(stage_ms[m] for m in members)
+        gb = ab["groups"][gname]
+        groups[gname] = {"stages": list(members), "ms_per_step": ms, "alg_bytes_per_step": gb,
+                         "achieved_GBs": gb / (ms * 1e-3) / 1e9 if ms > 0 else 0.0,
+                         "frac": gb / (ms * 1e-3) / 1e9 / peak if ms > 0 else 0.0,
+                         "share_of_compose": ms / compose_ms if compose_ms > 0 else 0.0}
+    dom = max(groups, key=lambda g: groups[g]["ms_per_step"])
+    own = own_traffic(st)
+    own_k = {}
+    for k, (stage, nl) in {"rs_scatter": ("rs_scatter", "rs_scatter_launches"), "rs_dedupe": ("rs_dedupe", "rs_dedupe_launches"),
+                           "rs_gather": ("rs_gather", "rs_gather_launches")}.items():
+        if stage_ms[stage] > 0:
+            own_k[k] = {"ms_per_step": stage_ms[stage], "launches_per_step": st[nl], "own_bytes_per_step": own[k],
+                        "achieved_GBs": own[k] / (stage_ms[stage] * 1e-3) / 1e9}
     traffic = None
     tpath = os.path.join(ROOT, "profiles", f"kernel_traffic_{args.workload}.json")
     if os.path.exists(tpath):
         try:
-            # measured DRAM bytes per launch of that kernel (ncu --set full, averaged over its launches in one step)
-            traffic = json.load(open(tpath))["dram_bytes_per_launch"].get(dom)
+            # measured DRAM bytes of one whole composition (ncu --set full, summed over the kernels of one step)
+            traffic = json.load(open(tpath)).get("dram_bytes_per_step")
         except Exception:
             traffic = None
-    per_kernel = {k: {"ms_per_step": kms[k], "launches_per_step": st[kstage[k][1]],
-                      "alg_bytes_per_step": ab["kernels"][k],
-                      "achieved_GBs": (ab["kernels"][k] / (kms[k] * 1e-3) / 1e9) if kms[k] > 0 else 0.0}
-                  for k in kstage}
-    compose_ms = sum(s["compose_ms"] for s in stats) / len(stats)
-    pack_ms = sum(s["pack_ms"] for s in stats) / len(stats)
-    path_gbs = ab["path"] / (compose_ms * 1e-3) / 1e9
+    latency_bound = st["n_raw_arcs"] < 10_000_000
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -359,17 +375,18 @@ def main():
         "result": {"n_states": st["n_states"], "n_arcs": st["n_arcs"], "n_raw_arcs": st["n_raw_arcs"],
                    "n_levels": st["n_levels"], "truncated": st["truncated"], "n_expanded": st["n_expanded"],
                    "merged_arcs_per_sec": st["n_arcs"] * world / (t_ms / args.steps * 1e-3)},
-        "timing_ms": {"pack": pack_ms, "compose_packed": compose_ms,
-                      "stages": {k: sum(s["ms"][k] for s in stats) / len(stats) for k in fstc.STAGES},
+        "timing_ms": {"pack": pack_ms, "compose_packed": compose_ms, "stages": stage_ms,
                       "compose_raw_arcs_per_sec": st["n_raw_arcs"] / (compose_ms * 1e-3)},
-        "roofline": {"bound": "hbm", "kernel": dom, "achieved": dom_gbs, "peak": peak, "unit": "GB/s",
-                     "frac": dom_gbs / peak, "peak_source": peak_src, "traffic": traffic,
-                     "alg_bytes_per_launch": dom_bytes_per_launch, "ms_per_launch": dom_ms,
-                     "launches_per_step": dom_launches, "share_of_step": kms[dom] / (t_ms / args.steps / max(1, world)) if world == 1 else None,
-                     "frac_of_8TBs_nominal": dom_gbs / 8000.0, "kernels": per_kernel},
-        "roofline_path": {"alg_bytes": ab["path"], "achieved": path_gbs, "frac": path_gbs / peak,
-                          "frac_of_8TBs_nominal": path_gbs / 8000.0,
-                          "alg_bytes_per_raw_arc": ab["path"] / max(1, st["n_raw_arcs"])},
+        # algorithmic bytes of the whole composition / compose time, against the measured HBM peak
+        "roofline": {"bound": "hbm", "kernel": "path: every kernel of fstc_compose_packed", "achieved": path_gbs, "peak": peak,
+                     "unit": "GB/s", "frac": path_gbs / peak, "peak_source": peak_src, "traffic": traffic,
+                     "alg_bytes_per_step": ab["path"], "alg_bytes_per_raw_arc": ab["path"] / max(1, st["n_raw_arcs"]),
+                     "ms_per_step": compose_ms, "frac_of_8TBs_nominal": path_gbs / 8000.0,
+                     "meaningful": not latency_bound,
+                     "note": ("latency-bound workload (< 1e7 arcs): report ms, the HBM fraction says nothing" if latency_bound else
+                              "B_alg = 16E + 8Σ(s1+s2) + 12Σ(n1+n2) + 12R + 12S + 20M + 9S + 40R_m (SURVEY §8(d))"),
+                     "dominant_stage_group": dom, "stage_groups": groups,
+                     "achieved_vs_own_traffic": own_k},
         "ms_steps": [round(x, 3) for x in ms_steps], "compose_ms_steps": [round(s_["compose_ms"], 3) for s_ in stats],
         "clocks": clocks, "gpu_launches": int(launches),
         "host": {"nproc": os.cpu_count()},
@@ -403,8 +420,7 @@ def main():
             barrier()
             a.record()
             r = fstc.fstc_compose(hs[0], hs[1], merge_mode=args.merge_mode, max_raw_arcs=budget,
-                                  resolve_mode=args.resolve_mode,
-                                  arc_capacity_hint=hints["arc"], state_capacity_hint=hints["state"])
+                                  resolve_mode=args.resolve_mode)
             r.to_host(out)
             b.record()
             torch.cuda.synchronize()

@@ -62,6 +62,8 @@ def test_matches_brute_force_full_product_then_trim(case, force_map):
     for p, l in level.items():
         by_level[l] += raw[p]
     assert [int(x) for x in res.level_raw] == [by_level[l] for l in range(res.n_levels)]
+    # |F_l|, the frontier sizes (the GPU tests use them as the expected `level_frontier`): counted from the brute force's levels
+    assert [int(x) for x in res.level_size] == [sum(1 for l in level.values() if l == i) for i in range(res.n_levels)]
 
 
 @pytest.mark.parametrize("case", CASES[:4])
