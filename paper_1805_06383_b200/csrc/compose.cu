@@ -1235,7 +1235,6 @@ struct Composer {
             j.stats = &st;
             j.profile = o.profile != 0;
             if (const char *e = getenv("FSTC_RESOLVE_BITS")) j.force_bits = atoi(e);   // test knob: force multi-pass
-            j.generic = getenv("FSTC_RESOLVE_GENERIC") != nullptr;                        // test knob: never the compact path
             resolve_partitioned(c, j);
             st.n_resolve += 1;
             st.n_resolved_arcs += R;
@@ -1609,7 +1608,6 @@ fstc_result_t *Composer::run() {
                         j.mode = 0; j.pos = nullptr; j.o_tgt = gtgt.p; j.sortrec = nullptr; j.shift_t = 0;
                         j.force_bits = -1;
                         if (const char *e = getenv("FSTC_RESOLVE_BITS")) j.force_bits = atoi(e);
-                        j.generic = getenv("FSTC_RESOLVE_GENERIC") != nullptr;
                         j.stats = &st; j.profile = o.profile != 0;
                         resolve_partitioned(c, j);
                         st.n_resolve += 1;

@@ -78,7 +78,6 @@ struct ResolveJob {
     uint4 *sortrec;                     // mode 2: id OR-ed into key bits [shift_t, ...)
     int shift_t;
     int force_bits;                     // >= 0: number of hash bits to partition on (tests); -1: from the sizes
-    bool generic;                       // true: never the compact path (tests)
     fstc_stats_t *stats;                // nullable: work counters and (profile) stage times are added here
     bool profile;
 };

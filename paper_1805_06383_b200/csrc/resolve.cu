@@ -17,7 +17,6 @@
 //      writes them out in input order; the last pass writes the target column, coalesced, in rank order.
 //
 // Nothing persists between levels except pair[] (id -> (q1,q2)): the key->id map is rebuilt per level from it.
-#include <algorithm>
 #include <cstdlib>
 #include <ctime>
 #include <vector>
@@ -43,7 +42,7 @@ __device__ __forceinline__ uint64_t rmix64(uint64_t k) {
 // ------------------------------------------------------------------------------------------ segment bookkeeping
 // A record stream is a set of segments inside one buffer: segment s = data[start[s] .. start[s] + cnt[s]).
 struct SegView {
-    const void *data;          // records: u64 in the generic path; u64 / u32 / u16 in the compact path
+    const unsigned long long *data;
     const int64_t *start;      // [n_seg + 1]
     const uint32_t *cnt;       // [n_seg]
     int n_seg;
@@ -152,7 +151,7 @@ __global__ void __launch_bounds__(SC_THREADS, SC_TILE == SC_TILE_BIG ? 2 : FSTC_
     const int64_t lo = tile * SC_TILE;
     const int n = static_cast<int>(seg_n - lo < SC_TILE ? seg_n - lo : SC_TILE);
     const int64_t in_base = a.in.start[seg] + lo;
-    const unsigned long long *src = static_cast<const unsigned long long *>(a.in.data) + in_base;
+    const unsigned long long *src = a.in.data + in_base;
 
     unsigned long long rec[SC_IPT];
     uint32_t br[SC_IPT];                                        // bin << 16 | rank inside the bin (tile-local)
@@ -287,13 +286,13 @@ __global__ void __launch_bounds__(DD_THREADS, FSTC_DD_MINB) rs_dedupe(DedupeArgs
     __syncthreads();
     const unsigned long long idmask = (1ull << a.ib) - 1;
     for (int64_t i = tid; i < sc; i += DD_THREADS) {
-        const unsigned long long r = static_cast<const unsigned long long *>(a.st.data)[s0 + i];
+        const unsigned long long r = a.st.data[s0 + i];
         bool won;
         const int s = dd_find_or_claim(keys, r >> a.ib, &won);
         if (s < 0) atomicOr(a.err, 1u); else ids[s] = static_cast<uint32_t>(r & idmask);
     }
     __syncthreads();
-    const unsigned long long *ap = static_cast<const unsigned long long *>(a.arcs.data) + a0;
+    const unsigned long long *ap = a.arcs.data + a0;
     uint32_t *op = a.ids_out + a0;
     for (int64_t base = 0; base < ac; base += DD_TILE) {
         unsigned long long key[DD_IPT];
@@ -427,404 +426,6 @@ __global__ void rs_state_records(const int2 *__restrict__ pair, int64_t n, int q
     out[i] = (key << ib) | static_cast<unsigned long long>(i);
 }
 
-// ========================================================================================== compact path
-// Keys of at most ~36 bits (|Q1||Q2| up to 6.9e10: every BASELINE.json config).  Three changes against the generic
-// path above, all from one measurement: a shared-memory atomic costs 2 cycles per LANE on this SM (64 cycles per warp
-// instruction, B300_MICROARCH.md "Atomics"), so one atomic per record caps a pass at 0.5 record per SM clock, which is
-// where rs_scatter and rs_dedupe sat (0.39 and 0.31).
-//   * the bins come from a BIJECTION h on key_bits bits, not from a 64-bit hash: a record only has to carry the bits
-//     of h(key) below its bin, 4 bytes after the first pass and 2 after the second;
-//   * the scatter ranks its records without atomics: each warp counts into its own row of bin counters
-//     (match-any inside the warp, plain loads and stores), a scan over (bin, warp) turns the rows into slots;
-//   * the dedupe needs no hash map: a bin spans <= 2^16 possible keys, so a WARP owns a bin and keeps two bitmaps of
-//     it in shared memory (existing states, new keys; bits set with match-any + reduce-or, no atomics); the id of a new
-//     key is base + its rank in the bitmap, so ids inside a bin ascend with h(key); pair[id] comes from h^-1.
-struct KeyHash {
-    uint64_t c1, c2, c1inv, c2inv, mask;
-    int s, kb;
-};
-__host__ __device__ __forceinline__ uint64_t kh_fwd(const KeyHash &h, uint64_t k) {
-    k = (k * h.c1) & h.mask; k ^= k >> h.s;
-    k = (k * h.c2) & h.mask; k ^= k >> h.s;
-    return k;
-}
-__host__ __device__ __forceinline__ uint64_t kh_unshift(uint64_t y, int s, int) {   // inverse of x ^= x >> s when 2s >= kb
-    return y ^ (y >> s);
-}
-__host__ __device__ __forceinline__ uint64_t kh_inv(const KeyHash &h, uint64_t k) {
-    k = kh_unshift(k, h.s, h.kb); k = (k * h.c2inv) & h.mask;
-    k = kh_unshift(k, h.s, h.kb); k = (k * h.c1inv) & h.mask;
-    return k;
-}
-inline uint64_t odd_inverse(uint64_t c) {          // c * x = 1 mod 2^64 (Newton), hence mod every 2^kb
-    uint64_t x = c;
-    for (int i = 0; i < 6; ++i) x *= 2 - c * x;
-    return x;
-}
-inline KeyHash make_key_hash(int kb) {
-    KeyHash h;
-    h.kb = kb;
-    h.mask = kb >= 64 ? ~0ull : ((1ull << kb) - 1);
-    h.c1 = 0x9E3779B97F4A7C15ULL; h.c2 = 0xD6E8FEB86659FD93ULL;
-    h.c1inv = odd_inverse(h.c1); h.c2inv = odd_inverse(h.c2);
-    h.s = (kb + 1) / 2;                               // 2s >= kb: the xor-shift is its own inverse
-    return h;
-}
-
-// state records h(key) << ib | id, in id order
-__global__ void rs_state_records_h(const int2 *__restrict__ pair, int64_t n, int q2_bits, int ib, KeyHash h,
-                                   unsigned long long *__restrict__ out) {
-    const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const int2 p = pair[i];
-    const unsigned long long key = (static_cast<unsigned long long>(static_cast<uint32_t>(p.x)) << q2_bits) | static_cast<uint32_t>(p.y);
-    out[i] = (kh_fwd(h, key) << ib) | static_cast<unsigned long long>(i);
-}
-
-// lanes of the warp whose `v` agrees with this lane's on the low `nbits` bits: one ballot per bit.  (MATCH.ANY and a
-// REDUX under a per-lane mask both serialise over the distinct values of the warp: measured 4x slower than the atomics
-// they were meant to replace.)
-template <int NBITS_MAX>
-__device__ __forceinline__ uint32_t warp_peers(uint32_t v, int nbits) {
-    uint32_t peers = 0xffffffffu;
-#pragma unroll
-    for (int b = 0; b < NBITS_MAX; ++b) {
-        if (b < nbits) {                                       // nbits is a constant at every call site
-            const uint32_t m = __ballot_sync(0xffffffffu, (v >> b) & 1u);
-            peers &= ((v >> b) & 1u) ? m : ~m;
-        }
-    }
-    return peers;
-}
-
-struct Scatter2Args {
-    SegView in;
-    const int64_t *tile_first;
-    void *out;
-    const int64_t *out_start;
-    uint32_t *cursor;
-    uint32_t *dest;
-    uint16_t *perm;
-    int cur_stride;
-    int bin_shift, nbins, nbits;    // bin = (record >> bin_shift) & (nbins - 1), nbins = 2^nbits; record hashed first when HASH
-    uint64_t out_mask;              // what the output record keeps of the (hashed) input record
-    KeyHash h;
-};
-constexpr int S2_THREADS = 512, S2_WARPS = S2_THREADS / 32;
-constexpr size_t s2_smem_bytes(int tile, int out_bytes) {
-    return static_cast<size_t>(tile) * (out_bytes + 4) + SC_MAX_BINS * (8 + 2 * S2_WARPS);
-}
-
-// One tile of TILE records: warp w of the block ranks the records it loads inside ITS row of bin counters (plain
-// shared-memory loads and stores; lanes of the warp that share a bin are told apart with match-any), a scan over
-// (bin, warp) turns the rows into first slots, the records are staged in bin order and the runs go out like in
-// rs_scatter (one global reservation per non-empty bin, dest / perm for the way back).
-template <typename TIn, typename TOut, bool DEST, bool HASH, int TILE>
-__global__ void __launch_bounds__(S2_THREADS, 2) rs_scatter2(Scatter2Args a) {
-    constexpr int IPT = TILE / S2_THREADS;
-    extern __shared__ __align__(16) unsigned char s2_raw[];
-    TOut *stage = reinterpret_cast<TOut *>(s2_raw);                               // [TILE] records in bin order
-    uint32_t *smeta = reinterpret_cast<uint32_t *>(s2_raw + sizeof(TOut) * TILE);  // [TILE] tile-local input index << 16 | bin
-    uint2 *binfo = reinterpret_cast<uint2 *>(smeta + TILE);                        // [nbins] {global index - slot, first slot that no longer fits}
-    uint16_t *wcnt = reinterpret_cast<uint16_t *>(binfo + SC_MAX_BINS);            // [S2_WARPS][nbins]
-    __shared__ uint32_t s_warp[S2_WARPS];
-    __shared__ int s_seg;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int nb = a.nbins;
-    const uint32_t bmask = static_cast<uint32_t>(nb - 1);
-
-    if (tid == 0) s_seg = rs_find_segment(a.tile_first, a.in.n_seg);
-    for (int p = tid; p < nb * S2_WARPS / 2; p += S2_THREADS) reinterpret_cast<uint32_t *>(wcnt)[p] = 0u;
-    __syncthreads();
-    const int seg = s_seg;
-    const int64_t tile = static_cast<int64_t>(blockIdx.x) - a.tile_first[seg];
-    const int64_t seg_n = a.in.cnt[seg];
-    const int64_t lo = tile * TILE;
-    const int n = static_cast<int>(seg_n - lo < TILE ? seg_n - lo : TILE);
-    const int64_t in_base = a.in.start[seg] + lo;
-    const TIn *src = static_cast<const TIn *>(a.in.data) + in_base;
-
-    TIn raw[IPT];
-#pragma unroll
-    for (int u = 0; u < IPT; ++u) {
-        const int i = u * S2_THREADS + tid;
-        raw[u] = i < n ? __ldcs(src + i) : TIn(0);
-    }
-    TOut val[IPT];
-    uint32_t br[IPT];                                           // bin << 16 | rank among the warp's records of the bin
-    volatile uint16_t *wc = wcnt + warp * nb;
-    const uint32_t lt_mask = (1u << lane) - 1u;
-    static_assert(TILE / S2_WARPS <= 1023, "a warp's count of one bin must fit 10 bits");
-#pragma unroll
-    for (int u = 0; u < IPT; ++u) {
-        const int i = u * S2_THREADS + tid;
-        const bool valid = i < n;
-        uint64_t k = static_cast<uint64_t>(raw[u]);
-        if (HASH) k = kh_fwd(a.h, k);
-        const uint32_t b = static_cast<uint32_t>(k >> a.bin_shift) & bmask;
-        val[u] = static_cast<TOut>(k & a.out_mask);
-        // rank among the warp's records of bin b: counter = count (10 bits) | lane that wrote it last (5 bits).  Every
-        // pending lane writes count + 1 with its lane number; of the lanes of one instruction that hit the same counter one
-        // store lands, and the lane that reads its own number back owns the increment; the others go round again (with
-        // 1024 bins a warp has a collision in about a third of its rounds).  Shared-memory accesses of a warp are in order.
-        uint32_t rank = 0;
-        bool pending = valid;
-        for (int it = 0; __any_sync(0xffffffffu, pending); ++it) {
-            if (it < 2) {
-                if (pending) {
-                    const uint32_t c = wc[b] & 0x3FFu;
-                    wc[b] = static_cast<uint16_t>((c + 1u) | (static_cast<uint32_t>(lane) << 10));
-                    if ((wc[b] >> 10) == static_cast<uint32_t>(lane)) { rank = c; pending = false; }
-                }
-            } else {
-                // many lanes on one bin (input already in bin order, e.g. states created by an earlier partitioned
-                // level): rank the pending lanes exactly, one ballot per bin bit
-                const uint32_t peers = warp_peers<10>(b, 10) & __ballot_sync(0xffffffffu, pending);
-                uint32_t c = 0;
-                if (pending) { c = wc[b] & 0x3FFu; rank = c + __popc(peers & lt_mask); }
-                __syncwarp();
-                if (pending && (peers & lt_mask) == 0u) wc[b] = static_cast<uint16_t>(c + __popc(peers));
-                pending = false;
-            }
-            __syncwarp();
-        }
-        br[u] = (b << 16) | rank;
-        __syncwarp();
-    }
-    __syncthreads();
-    // per bin: exclusive prefix over the warps' counts (in place), then an exclusive scan of the bin totals over the block
-    const int p0 = 2 * tid;
-    uint32_t c0 = 0, c1 = 0;
-    if (p0 < nb) {
-#pragma unroll
-        for (int w = 0; w < S2_WARPS; ++w) {
-            uint32_t *q = reinterpret_cast<uint32_t *>(wcnt + w * nb + p0);
-            const uint32_t v = *q & 0x03FF03FFu;               // counts without the lane tags
-            *q = c0 | (c1 << 16);
-            c0 += v & 0xFFFFu; c1 += v >> 16;
-        }
-    }
-    uint32_t incl = c0 + c1;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        uint32_t v = __shfl_up_sync(0xffffffffu, incl, d);
-        if (lane >= d) incl += v;
-    }
-    if (lane == 31) s_warp[warp] = incl;
-    __syncthreads();
-    uint32_t ex = incl - (c0 + c1);
-    for (int w = 0; w < warp; ++w) ex += s_warp[w];
-    if (p0 < nb) {
-        const uint32_t st0 = ex, st1 = ex + c0;
-        const uint32_t add = st0 | (st1 << 16);
-#pragma unroll
-        for (int w = 0; w < S2_WARPS; ++w) *reinterpret_cast<uint32_t *>(wcnt + w * nb + p0) += add;   // halves stay < 2^16: no carry
-        const int64_t gbin0 = static_cast<int64_t>(seg) * nb;
-#pragma unroll
-        for (int k = 0; k < 2; ++k) {
-            const int p = p0 + k;
-            const uint32_t c = k ? c1 : c0, st = k ? st1 : st0;
-            if (c) {
-                const int64_t b0 = a.out_start[gbin0 + p], b1 = a.out_start[gbin0 + p + 1];
-                const uint32_t g = atomicAdd(&a.cursor[static_cast<size_t>(gbin0 + p) * a.cur_stride], c);
-                const int64_t left = (b1 - b0) - static_cast<int64_t>(g);
-                const uint32_t room = left <= 0 ? 0u : (left < c ? static_cast<uint32_t>(left) : c);
-                binfo[p] = make_uint2(static_cast<uint32_t>(b0 + g) - st, st + room);   // modulo 2^32: a pass holds < 2^32 records
-            }
-        }
-    }
-    __syncthreads();
-#pragma unroll
-    for (int u = 0; u < IPT; ++u) {
-        const int i = u * S2_THREADS + tid;
-        if (i < n) {
-            const uint32_t b = br[u] >> 16;
-            const uint32_t slot = wc[b] + (br[u] & 0xFFFFu);
-            stage[slot] = val[u];
-            smeta[slot] = (static_cast<uint32_t>(i) << 16) | b;
-        }
-    }
-    __syncthreads();
-    TOut *out = static_cast<TOut *>(a.out);
-    for (int i = tid; i < n; i += S2_THREADS) {
-        const uint32_t m = smeta[i];
-        const uint2 bi = binfo[m & 0xFFFFu];
-        const bool fits = static_cast<uint32_t>(i) < bi.y;
-        const uint32_t dst = bi.x + static_cast<uint32_t>(i);
-        if (fits) out[dst] = stage[i];                          // a full bin drops the record; the host retries
-        if (DEST) {
-            a.dest[in_base + i] = fits ? dst : 0xFFFFFFFFu;
-            a.perm[in_base + i] = static_cast<uint16_t>(m >> 16);
-        }
-    }
-}
-
-// ------------------------------------------------------------------------------------------ per-bin dedupe, bitmaps
-// A WARP per bin.  rem = the bits of h(key) below the bin (<= 16): bm_old / bm_new are bitmaps over rem of the bin's
-// existing states and of its new keys.  No atomics: lanes that fall into the same bitmap word are found with match-any,
-// their bits OR-reduced, and the first of them does a plain read-modify-write (nobody else touches the warp's bitmaps).
-// id of an existing key: old_ids[first state of the bin + rank of rem in bm_old] (filled from the state records);
-// id of a new key: base + rank of rem in bm_new, base from one global atomicAdd per bin.
-struct Dedupe2Args {
-    SegView st;                // u64 state records  h(key) << ib | id, partitioned like the arcs
-    SegView arcs;              // rem of every arc (u16), or the raw key (u64) when no scatter pass ran
-    int64_t n_bins;
-    int ib, rem_bits, q2_bits;
-    KeyHash h;
-    uint32_t *ids_out;         // [length of the arc buffer]
-    uint32_t *old_ids;         // [length of the state buffer] scratch
-    unsigned long long *n_states;
-    int2 *pair;
-};
-
-// Sets `bit` of bm[word] for the lanes that are `on`; returns true to the lane (or lanes, if several of one instruction carry
-// the same bit) whose store set it.  Optimistic read-modify-write: of the lanes of one instruction that hit the same word
-// one store lands; a lane that does not find its bit in the word afterwards goes round again.
-__device__ __forceinline__ bool bm_set(volatile uint32_t *bm, uint32_t word, uint32_t bit, bool on) {
-    bool pending = on, won = false;
-    while (__any_sync(0xffffffffu, pending)) {
-        if (pending) {
-            const uint32_t old = bm[word];
-            if (old & bit) pending = false;
-            else {
-                bm[word] = old | bit;
-                if (bm[word] & bit) { pending = false; won = true; }
-            }
-        }
-        __syncwarp();
-    }
-    return won;
-}
-// pre[w] = number of set bits in the words before w; returns the total
-__device__ __forceinline__ uint32_t bm_prefix(const volatile uint32_t *bm, uint16_t *pre, int W, int lane) {
-    uint32_t base = 0;
-    for (int j = 0; j < W; j += 32) {
-        const int wi = j + lane;
-        const uint32_t c = wi < W ? __popc(bm[wi]) : 0u;
-        uint32_t incl = c;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            uint32_t v = __shfl_up_sync(0xffffffffu, incl, d);
-            if (lane >= d) incl += v;
-        }
-        if (wi < W) pre[wi] = static_cast<uint16_t>(base + incl - c);
-        base += __shfl_sync(0xffffffffu, incl, 31);
-    }
-    __syncwarp();
-    return base;
-}
-
-constexpr int DB_MLP = 4;
-template <typename TArc, bool HASH>
-__global__ void __launch_bounds__(512) rs_dedupe_bm(Dedupe2Args a) {
-    extern __shared__ __align__(16) unsigned char db_raw[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, warps = blockDim.x >> 5;
-    const int64_t bin = static_cast<int64_t>(blockIdx.x) * warps + warp;
-    if (bin >= a.n_bins) return;
-    const int64_t ac = a.arcs.cnt[bin];
-    if (ac == 0) return;                                       // nothing to resolve in this bin
-    const int wbits = a.rem_bits > 5 ? a.rem_bits - 5 : 0;
-    const int W = 1 << wbits;
-    volatile uint32_t *bm_old = reinterpret_cast<uint32_t *>(db_raw) + static_cast<size_t>(warp) * 3 * W;
-    volatile uint32_t *bm_new = bm_old + W;
-    uint16_t *pre_old = reinterpret_cast<uint16_t *>(const_cast<uint32_t *>(bm_new) + W), *pre_new = pre_old + W;
-    const uint32_t rmask = (1u << a.rem_bits) - 1u;
-    const int64_t sc = a.st.cnt[bin];
-    const int64_t a0 = a.arcs.start[bin], s0 = a.st.start[bin];
-    for (int j = lane; j < W; j += 32) { bm_old[j] = 0u; bm_new[j] = 0u; }
-    __syncwarp();
-    // ---- existing states of the bin
-    const unsigned long long *sp = static_cast<const unsigned long long *>(a.st.data) + s0;
-    for (int64_t i0 = 0; i0 < sc; i0 += 32 * DB_MLP) {           // DB_MLP loads in flight per lane
-        unsigned long long rec[DB_MLP];
-#pragma unroll
-        for (int k = 0; k < DB_MLP; ++k) { const int64_t i = i0 + k * 32 + lane; rec[k] = i < sc ? sp[i] : 0ull; }
-#pragma unroll
-        for (int k = 0; k < DB_MLP; ++k) {
-            if (i0 + k * 32 >= sc) break;
-            const uint32_t rem = static_cast<uint32_t>(rec[k] >> a.ib) & rmask;
-            bm_set(bm_old, rem >> 5, 1u << (rem & 31u), i0 + k * 32 + lane < sc);
-        }
-    }
-    if (sc > 0) {
-        bm_prefix(bm_old, pre_old, W, lane);
-        const unsigned long long idmask = (1ull << a.ib) - 1;
-        for (int64_t i = lane; i < sc; i += 32) {
-            const unsigned long long r = sp[i];
-            const uint32_t rem = static_cast<uint32_t>(r >> a.ib) & rmask;
-            const uint32_t word = rem >> 5, bit = rem & 31u;
-            a.old_ids[s0 + pre_old[word] + __popc(bm_old[word] & ((1u << bit) - 1u))] = static_cast<uint32_t>(r & idmask);
-        }
-        __syncwarp();
-    }
-    // ---- arcs: the new keys of the bin
-    const TArc *ap = static_cast<const TArc *>(a.arcs.data) + a0;
-    auto rem_of = [&](int64_t i) -> uint32_t {
-        uint64_t k = static_cast<uint64_t>(ap[i]);
-        if (HASH) k = kh_fwd(a.h, k);
-        return static_cast<uint32_t>(k) & rmask;
-    };
-    // the lane whose store set the bit of a new key writes pair[id] once the ids are known: its flags wait in `wonbits`
-    // (bit r = the lane's r-th record); a bin of more than 2048 arcs writes the pairs from the bitmap instead
-    const bool flags_fit = ac <= 64 * 32;
-    unsigned long long wonbits = 0ull;
-    for (int64_t i0 = 0; i0 < ac; i0 += 32 * DB_MLP) {
-        uint32_t rem[DB_MLP];
-#pragma unroll
-        for (int k = 0; k < DB_MLP; ++k) { const int64_t i = i0 + k * 32 + lane; rem[k] = i < ac ? rem_of(i) : 0u; }
-#pragma unroll
-        for (int k = 0; k < DB_MLP; ++k) {
-            if (i0 + k * 32 >= ac) break;
-            const uint32_t word = rem[k] >> 5, bit = rem[k] & 31u;
-            const bool fresh = i0 + k * 32 + lane < ac && !((bm_old[word] >> bit) & 1u);
-            const bool won = bm_set(bm_new, word, 1u << bit, fresh);
-            if (flags_fit && won) wonbits |= 1ull << (i0 / 32 + k);
-        }
-    }
-    const uint32_t total_new = bm_prefix(bm_new, pre_new, W, lane);
-    uint32_t base = 0;
-    if (total_new) {
-        if (lane == 0) base = static_cast<uint32_t>(atomicAdd(a.n_states, static_cast<unsigned long long>(total_new)));
-        base = __shfl_sync(0xffffffffu, base, 0);
-    }
-    uint32_t *op = a.ids_out + a0;
-    const uint32_t q2mask = (1u << a.q2_bits) - 1u;
-    const uint64_t hk_bin = static_cast<uint64_t>(bin) << a.rem_bits;
-    for (int64_t i0 = 0; i0 < ac; i0 += 32 * DB_MLP) {
-        uint32_t remv[DB_MLP];
-#pragma unroll
-        for (int k = 0; k < DB_MLP; ++k) { const int64_t i = i0 + k * 32 + lane; remv[k] = i < ac ? rem_of(i) : 0u; }
-#pragma unroll
-        for (int k = 0; k < DB_MLP; ++k) {
-            const int64_t i = i0 + k * 32 + lane;
-            if (i >= ac) continue;
-            const uint32_t rem = remv[k];
-            const uint32_t word = rem >> 5, bit = rem & 31u, below = (1u << bit) - 1u;
-            const uint32_t bo = bm_old[word];
-            uint32_t id;
-            if ((bo >> bit) & 1u) id = __ldcg(a.old_ids + s0 + pre_old[word] + __popc(bo & below));
-            else id = base + pre_new[word] + __popc(bm_new[word] & below);
-            __stcs(op + i, id);
-            if ((wonbits >> (i0 / 32 + k)) & 1ull) {            // h^-1 gives the pair back (several lanes may write the same value)
-                const uint64_t key = kh_inv(a.h, hk_bin | rem);
-                a.pair[id] = make_int2(static_cast<int>(key >> a.q2_bits), static_cast<int>(static_cast<uint32_t>(key) & q2mask));
-            }
-        }
-    }
-    if (!flags_fit) {
-        for (int j = lane; j < W; j += 32) {
-            uint32_t bits = bm_new[j];
-            uint32_t id = base + pre_new[j];
-            while (bits) {
-                const uint32_t bit = __ffs(bits) - 1;
-                bits &= bits - 1;
-                const uint64_t key = kh_inv(a.h, hk_bin | (static_cast<uint32_t>(j) * 32u + bit));
-                a.pair[id++] = make_int2(static_cast<int>(key >> a.q2_bits), static_cast<int>(static_cast<uint32_t>(key) & q2mask));
-            }
-        }
-    }
-}
-
 // ------------------------------------------------------------------------------------------ host side
 inline unsigned rs_blocks(int64_t n, int threads = 256) { return static_cast<unsigned>(ceil_div(n > 0 ? n : 1, threads)); }
 
@@ -864,7 +465,7 @@ thread_local RsTrace g_trace;
 
 struct SegSet {                       // device arrays of a segmented record stream
     DBuf<unsigned long long> own;     // storage, unless the stream borrows the caller's buffer
-    const void *data = nullptr;
+    const unsigned long long *data = nullptr;
     int64_t length = 0;               // records the buffer spans (segments + gaps)
     DBuf<int64_t> start;              // [n_seg + 1]
     DBuf<uint32_t> cnt;               // [n_seg]
@@ -872,7 +473,7 @@ struct SegSet {                       // device arrays of a segmented record str
     SegView view() const { return SegView{data, start.p, cnt.p, static_cast<int>(n_seg)}; }
 };
 
-SegSet single_segment(Ctx &c, const void *data, int64_t n) {
+SegSet single_segment(Ctx &c, const unsigned long long *data, int64_t n) {
     SegSet s;
     s.data = data;
     s.length = n;
@@ -979,168 +580,6 @@ void gather_pass(Ctx &c, const SegSet &seg, int mode, bool big_tile, GatherArgs 
     c.n_launch += 2;
 }
 
-// ---- compact path, host side
-enum { REC_U64 = 8, REC_U32 = 4, REC_U16 = 2 };
-
-template <typename TIn, typename TOut, bool DEST, bool HASH, int TILE>
-void launch_scatter2(Ctx &c, unsigned grid, const Scatter2Args &a) {
-    constexpr size_t smem = s2_smem_bytes(TILE, sizeof(TOut));
-    FSTC_CUDA(cudaFuncSetAttribute(rs_scatter2<TIn, TOut, DEST, HASH, TILE>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
-    rs_scatter2<TIn, TOut, DEST, HASH, TILE><<<grid, S2_THREADS, smem, c.stream>>>(a);
-}
-
-constexpr int S2_TILE_ARCS = 8192, S2_TILE_STATES = 4096;
-#ifndef FSTC_RS_REM_BITS
-#define FSTC_RS_REM_BITS 14
-#endif
-constexpr int RS_REM_BITS = FSTC_RS_REM_BITS;     // aimed number of key bits left below the bins (bitmaps of 2^14 bits = 2 KB)
-
-// One pass of the compact scatter.  Arc streams (dest != null): u64 raw keys -> u32 / u16, or u32 -> u16; the state
-// stream (dest == null) keeps its u64 records whole.  Capacities and the retry on overflow are those of scatter_pass.
-SegSet scatter2_pass(Ctx &c, const SegSet &in, int in_bytes, int out_bytes, bool hash, const KeyHash &kh, int bin_shift, int nbins,
-                     uint64_t out_mask, DBuf<uint32_t> *dest, DBuf<uint16_t> *perm) {
-    const int TILE = dest ? S2_TILE_ARCS : S2_TILE_STATES;
-    if (in.n_seg > 1024 || nbins > SC_MAX_BINS) fail(FSTC_ERR_CAPACITY, "resolve: too many segments (%lld x %d)",
-                                                    static_cast<long long>(in.n_seg), nbins);
-    const int64_t nb = in.n_seg * nbins;
-    const int cur_stride = nb <= 4096 ? 32 : 8;
-    DBuf<int64_t> tile_first(c, in.n_seg + 1);
-    rs_seg_tiles<<<1, 1024, 0, c.stream>>>(in.view(), TILE, tile_first.p);
-    FSTC_LAUNCH_CHECK();
-    DBuf<uint32_t> cap(c, nb), cursor(c, nb * cur_stride);
-    DBuf<unsigned> flag(c, 1);
-    SegSet out;
-    out.n_seg = nb;
-    out.start.alloc(c, nb + 1);
-    if (dest) { dest->alloc(c, in.length); perm->alloc(c, in.length); }
-    for (int attempt = 0;; ++attempt) {
-        rs_bin_caps<<<rs_blocks(nb), 256, 0, c.stream>>>(in.view(), nbins, 16, 192u, cursor.p, cur_stride, attempt, cap.p);
-        FSTC_LAUNCH_CHECK();
-        exclusive_scan<uint32_t>(c, cap.p, nb, out.start.p);
-        int64_t totals[2];
-        FSTC_CUDA(cudaMemcpyAsync(&totals[0], tile_first.p + in.n_seg, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
-        FSTC_CUDA(cudaMemcpyAsync(&totals[1], out.start.p + nb, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
-        c.sync();
-        if (totals[1] >= 0xFFFFFFFFll) fail(FSTC_ERR_CAPACITY, "resolve: more than 2^32 records in a pass");
-        out.own.alloc(c, (totals[1] * out_bytes + 7) / 8 + 1);
-        out.data = out.own.p;
-        out.length = totals[1];
-        FSTC_CUDA(cudaMemsetAsync(cursor.p, 0, sizeof(uint32_t) * nb * cur_stride, c.stream));
-        FSTC_CUDA(cudaMemsetAsync(flag.p, 0, sizeof(unsigned), c.stream));
-        if (totals[0] > 0) {
-            Scatter2Args a{in.view(), tile_first.p, out.own.p, out.start.p, cursor.p, dest ? dest->p : nullptr, dest ? perm->p : nullptr,
-                           cur_stride, bin_shift, nbins, bits_for(static_cast<uint64_t>(nbins - 1)), out_mask, kh};
-            const int h = g_trace.begin(c, dest ? "scatter2+dest" : "scatter2", totals[0] * TILE, FSTC_T_RS_SCATTER);
-            const unsigned grid = static_cast<unsigned>(totals[0]);
-            if (!dest) launch_scatter2<unsigned long long, unsigned long long, false, false, S2_TILE_STATES>(c, grid, a);
-            else if (in_bytes == REC_U64 && out_bytes == REC_U32 && hash) launch_scatter2<unsigned long long, uint32_t, true, true, S2_TILE_ARCS>(c, grid, a);
-            else if (in_bytes == REC_U64 && out_bytes == REC_U16 && hash) launch_scatter2<unsigned long long, uint16_t, true, true, S2_TILE_ARCS>(c, grid, a);
-            else if (in_bytes == REC_U32 && out_bytes == REC_U16 && !hash) launch_scatter2<uint32_t, uint16_t, true, false, S2_TILE_ARCS>(c, grid, a);
-            else fail(FSTC_ERR_CUDA, "internal: no scatter kernel for %d -> %d bytes", in_bytes, out_bytes);
-            FSTC_LAUNCH_CHECK();
-            g_trace.end(c, h);
-        }
-        rs_check_overflow<<<rs_blocks(nb), 256, 0, c.stream>>>(cursor.p, cur_stride, cap.p, nb, flag.p);
-        FSTC_LAUNCH_CHECK();
-        c.n_launch += 4;
-        if (!read_scalar(c, flag.p)) break;
-        if (attempt == 1) fail(FSTC_ERR_CUDA, "internal: resolve scatter overflowed with exact capacities");
-    }
-    out.cnt.alloc(c, nb);
-    rs_compact_counts<<<rs_blocks(nb), 256, 0, c.stream>>>(cursor.p, cur_stride, nb, out.cnt.p);
-    FSTC_LAUNCH_CHECK();
-    c.n_launch += 1;
-    return out;
-}
-
-void gather_pass(Ctx &c, const SegSet &seg, int mode, bool big_tile, GatherArgs a);
-
-// `bits` hash bits (<= 20, <= key_bits); key_bits - bits <= 16
-void resolve_compact(Ctx &c, const ResolveJob &j, int bits) {
-    const int kb = j.key_bits;
-    const int ib = bits_for(static_cast<uint64_t>(j.n_states_before > 1 ? j.n_states_before - 1 : 1));
-    const KeyHash kh = make_key_hash(kb);
-    const int b1 = bits < 10 ? bits : 10, b2 = bits - b1;
-    const int rem_bits = kb - bits;
-    g_trace.on = g_trace.print || j.profile;
-    const int h_all = g_trace.begin(c, "RESOLVE TOTAL", j.n_records);
-    // 1. records of the existing states, partitioned like the arcs
-    DBuf<unsigned long long> st_recs(c, j.n_states_before);
-    rs_state_records_h<<<rs_blocks(j.n_states_before), 256, 0, c.stream>>>(j.pair, j.n_states_before, j.q2_bits, ib, kh, st_recs.p);
-    FSTC_LAUNCH_CHECK();
-    c.n_launch += 1;
-    SegSet st = single_segment(c, st_recs.p, j.n_states_before);
-    if (b1 > 0) st = scatter2_pass(c, st, REC_U64, REC_U64, false, kh, ib + kb - b1, 1 << b1, ~0ull, nullptr, nullptr);
-    if (b2 > 0) st = scatter2_pass(c, st, REC_U64, REC_U64, false, kh, ib + kb - bits, 1 << b2, ~0ull, nullptr, nullptr);
-    if (bits > 0) st_recs.release();
-    // 2. the arc keys: u64 -> (u32 ->) u16
-    SegSet lvl0 = single_segment(c, j.keys, j.n_records), lvl1, lvl2;
-    DBuf<uint32_t> dest1, dest2;
-    DBuf<uint16_t> perm1, perm2;
-    if (b1 > 0) {
-        const int w1 = b2 > 0 ? REC_U32 : REC_U16;
-        lvl1 = scatter2_pass(c, lvl0, REC_U64, w1, true, kh, kb - b1, 1 << b1, (1ull << (kb - b1)) - 1, &dest1, &perm1);
-    }
-    if (b2 > 0) {
-        lvl2 = scatter2_pass(c, lvl1, REC_U32, REC_U16, false, kh, kb - bits, 1 << b2, (1ull << rem_bits) - 1, &dest2, &perm2);
-        lvl1.own.release();
-    }
-    const SegSet &arcs = b2 > 0 ? lvl2 : (b1 > 0 ? lvl1 : lvl0);
-    // 3. per-bin dedupe
-    const int64_t nb = int64_t(1) << bits;
-    DBuf<uint32_t> ids_last(c, arcs.length), old_ids(c, st.length);
-    const unsigned long long n_before = static_cast<unsigned long long>(j.n_states_before);
-    FSTC_CUDA(cudaMemcpyAsync(j.n_states, &n_before, sizeof n_before, cudaMemcpyHostToDevice, c.stream));
-    Dedupe2Args d{st.view(), arcs.view(), nb, ib, rem_bits, j.q2_bits, kh, ids_last.p, old_ids.p, j.n_states, j.pair};
-    const int W = rem_bits > 5 ? 1 << (rem_bits - 5) : 1;
-    int warps = static_cast<int>((96 * 1024) / (12 * W));
-    warps = warps > 16 ? 16 : (warps < 1 ? 1 : warps);
-    if (nb < warps) warps = static_cast<int>(nb);
-    const size_t smem = static_cast<size_t>(warps) * 12 * W;
-    const unsigned grid = static_cast<unsigned>(ceil_div(nb, warps));
-    const int hd = g_trace.begin(c, "dedupe bitmaps", nb, FSTC_T_RS_DEDUPE);
-    if (bits > 0) {
-        FSTC_CUDA(cudaFuncSetAttribute(rs_dedupe_bm<uint16_t, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
-        rs_dedupe_bm<uint16_t, false><<<grid, warps * 32, smem, c.stream>>>(d);
-    } else {
-        FSTC_CUDA(cudaFuncSetAttribute(rs_dedupe_bm<unsigned long long, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
-        rs_dedupe_bm<unsigned long long, true><<<grid, warps * 32, smem, c.stream>>>(d);
-    }
-    FSTC_LAUNCH_CHECK();
-    g_trace.end(c, hd);
-    c.n_launch += 1;
-    if (j.stats) {
-        const int passes = (b1 > 0) + (b2 > 0);
-        j.stats->rs_scatter_recs += passes * j.n_states_before;
-        j.stats->rs_scatter_dest_recs += passes * j.n_records;
-        j.stats->rs_scatter_launches += 2 * passes;
-        j.stats->rs_dedupe_arcs += j.n_records;
-        j.stats->rs_dedupe_states += j.n_states_before;
-        j.stats->rs_dedupe_launches += 1;
-        j.stats->rs_gather_recs += (passes > 0 ? passes : 1) * j.n_records;
-        j.stats->rs_gather_launches += passes > 0 ? passes : 1;
-        j.stats->rs_compact += 1;
-    }
-    // 4. ids back through the passes (as in the generic path)
-    const uint32_t *ids = ids_last.p;
-    DBuf<uint32_t> ids_mid;
-    if (b2 > 0) {
-        ids_mid.alloc(c, lvl1.length);
-        GatherArgs g{};
-        g.dest = dest2.p; g.perm = perm2.p; g.in = ids_last.p; g.out = ids_mid.p;
-        gather_pass(c, lvl1, 0, true, g);
-        ids = ids_mid.p;
-    }
-    GatherArgs g{};
-    g.dest = b1 > 0 ? dest1.p : nullptr; g.perm = perm1.p; g.in = ids;
-    g.out = reinterpret_cast<uint32_t *>(j.o_tgt); g.pos = j.pos; g.o_tgt = j.o_tgt; g.sortrec = j.sortrec; g.shift_t = j.shift_t;
-    gather_pass(c, lvl0, j.mode, true, g);
-    g_trace.end(c, h_all);
-    c.sync();
-    if (g_trace.on) g_trace.report(j.stats ? j.stats->ms : nullptr);
-    g_trace.on = g_trace.print;
-}
-
 }  // namespace
 
 int resolve_bits_needed(int64_t n_records_and_states) {
@@ -1155,14 +594,6 @@ void resolve_partitioned(Ctx &c, const ResolveJob &j) {
     if (j.key_bits + ib > 64) fail(FSTC_ERR_CAPACITY, "resolve: key (%d bits) + state id (%d bits) exceed 64 bits", j.key_bits, ib);
     if (j.n_records >= 0xFFFFFFFFll) fail(FSTC_ERR_CAPACITY, "resolve: more than 2^32 records");
     int bits = j.force_bits >= 0 ? j.force_bits : resolve_bits_needed(j.n_states_before + j.n_records);
-    if (!j.generic) {
-        // compact path (see above): the bins take enough bits of h(key) to leave at most RS_REM_BITS (and never more than
-        // 16) below them; more bins than the record count asks for only cost their bitmaps (~0.2 ms for 2^20 of them)
-        int cb = std::max(bits, j.key_bits - RS_REM_BITS);
-        cb = std::min(cb, std::min(20, j.key_bits));
-        if (j.force_bits >= 0) cb = std::min(j.force_bits, std::min(20, j.key_bits));
-        if (j.key_bits - cb <= 16 && j.key_bits - std::min(cb, 10) <= 32) { resolve_compact(c, j, cb); return; }
-    }
     g_trace.on = g_trace.print || j.profile;
     const int h_all = g_trace.begin(c, "RESOLVE TOTAL", j.n_records);
     for (;; ++bits) {

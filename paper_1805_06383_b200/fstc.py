@@ -66,7 +66,7 @@ class _Stats(ctypes.Structure):
         ("rs_scatter_recs", ctypes.c_int64), ("rs_scatter_dest_recs", ctypes.c_int64), ("rs_dedupe_arcs", ctypes.c_int64),
         ("rs_dedupe_states", ctypes.c_int64), ("rs_dedupe_new", ctypes.c_int64), ("rs_gather_recs", ctypes.c_int64),
         ("rs_scatter_launches", ctypes.c_int32), ("rs_dedupe_launches", ctypes.c_int32),
-        ("rs_gather_launches", ctypes.c_int32), ("rs_compact", ctypes.c_int32),
+        ("rs_gather_launches", ctypes.c_int32), ("pad2_", ctypes.c_int32),
         ("ms", ctypes.c_double * len(STAGES)), ("ms_total", ctypes.c_double),
         ("level_frontier", ctypes.c_int64 * MAX_LEVEL_STATS), ("level_raw", ctypes.c_int64 * MAX_LEVEL_STATS),
         ("level_new_states", ctypes.c_int64 * MAX_LEVEL_STATS),
@@ -275,7 +275,7 @@ def stats_dict(s: _Stats) -> dict:
         "n_resolve": int(s.n_resolve), "n_resolved_arcs": int(s.n_resolved_arcs),
         **{k: int(getattr(s, k)) for k in ("rs_scatter_recs", "rs_scatter_dest_recs", "rs_dedupe_arcs", "rs_dedupe_states",
                                            "rs_dedupe_new", "rs_gather_recs", "rs_scatter_launches", "rs_dedupe_launches",
-                                           "rs_gather_launches", "rs_compact")},
+                                           "rs_gather_launches")},
         "ms": {k: float(s.ms[i]) for i, k in enumerate(STAGES)}, "ms_total": float(s.ms_total),
         "level_frontier": [int(s.level_frontier[i]) for i in range(nl)],
         "level_raw": [int(s.level_raw[i]) for i in range(nl)],

@@ -15,21 +15,15 @@ from test_gpu_parity import SMALL, check_parity, fstc  # noqa: F401  (fixture)
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(params=["auto", "0", "3", "12", "generic-auto", "generic-3", "generic-12"])
+@pytest.fixture(params=["auto", "0", "3", "12"])
 def resolve_bits(request):
-    """Number of hash bits forced (zero, one, two scatter passes on small inputs); `generic-*` keeps the resolve off its
-    compact path (keys of <= 36 bits: 4- and 2-byte records, bitmap dedupe), which every small input would take."""
-    saved = {k: os.environ.pop(k, None) for k in ("FSTC_RESOLVE_BITS", "FSTC_RESOLVE_GENERIC")}
-    generic, _, bits = request.param.rpartition("-")
-    if bits != "auto":
-        os.environ["FSTC_RESOLVE_BITS"] = bits
-    if generic:
-        os.environ["FSTC_RESOLVE_GENERIC"] = "1"
+    old = os.environ.pop("FSTC_RESOLVE_BITS", None)
+    if request.param != "auto":
+        os.environ["FSTC_RESOLVE_BITS"] = request.param
     yield request.param
-    for k, v in saved.items():
-        os.environ.pop(k, None)
-        if v is not None:
-            os.environ[k] = v
+    os.environ.pop("FSTC_RESOLVE_BITS", None)
+    if old is not None:
+        os.environ["FSTC_RESOLVE_BITS"] = old
 
 
 @pytest.mark.parametrize("case", SMALL[:3] + SMALL[6:])
@@ -40,7 +34,6 @@ def test_small_random_machines_partitioned(fstc, case, merge_mode, resolve_bits)
     m2 = messy_random_fst(seed + 100, n2, gam, dlt, a2)
     res, _ = check_parity(fstc, m1, m2, merge_mode=merge_mode, resolve_mode=fstc.RESOLVE_PARTITIONED)
     assert res.stats["n_resolve"] > 0 and res.stats["table_capacity"] == 0
-    assert res.stats["rs_compact"] == 0 or not resolve_bits.startswith("generic")
 
 
 @pytest.mark.parametrize("merge_mode", [0, 1, 2])
