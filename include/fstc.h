@@ -97,6 +97,15 @@ enum {
   FSTC_RESOLVE_HASH = 3         /* always the open-addressing hash table, whatever |Q1||Q2|                    */
 };
 
+enum {
+  FSTC_SMALL_AUTO = 0,      /* default: the whole search first runs inside ONE thread block, with no host round trip
+                               per BFS level (small inputs are overhead-bound, :291-293); a problem that outgrows the
+                               block's capacities (4096 pairs or 65536 raw arcs in a level, 8192 states, 65536 arcs
+                               unless the capacity hints say more) is composed again by the level-synchronous path  */
+  FSTC_SMALL_OFF = 1,       /* never                                                                              */
+  FSTC_SMALL_ONLY = 2       /* FSTC_ERR_CAPACITY instead of the level-synchronous path (tests)                     */
+};
+
 /* Options; NULL or all-zero = defaults. */
 typedef struct fstc_opts_t {
   int32_t merge_mode;       /* FSTC_MERGE_*                                                           */
@@ -106,6 +115,8 @@ typedef struct fstc_opts_t {
   int64_t state_capacity_hint; /* expected number of output states (0 = none)                        */
   int32_t profile;          /* 1: time every stage with CUDA events on the stream (fills stats ms)    */
   int32_t resolve_mode;     /* FSTC_RESOLVE_*: how composed arcs find the ids of their target states          */
+  int32_t small_path;       /* FSTC_SMALL_*: the device-resident path for small problems                      */
+  int32_t reserved_;
 } fstc_opts_t;
 
 /* Rule T (the paper only notes that the result may not fit the device, :153).  BFS levels are
@@ -143,7 +154,8 @@ typedef struct fstc_stats_t {
   int64_t table_capacity;   /* final number of visited-table slots                                    */
   int32_t n_rehash, n_grow; /* table rebuilds, output regrow copies                                   */
   int32_t n_emit_launches, n_kernel_launches;
-  int32_t n_resolve, pad_;  /* emit launches whose target ids came from the partitioned resolve                */
+  int32_t n_resolve;        /* emit launches whose target ids came from the partitioned resolve                */
+  int32_t small_path;       /* 1: composed by the small path (one thread block, one launch)                    */
   int64_t n_resolved_arcs;  /* raw arcs of those launches                                                     */
   /* work of the partitioned resolve, for its roofline: records through the scatter passes without / with
    * the recorded permutation, arc keys and state records through the dedupe, ids through the gathers; launches    */
@@ -205,6 +217,15 @@ FSTC_API int fstc_packed_to_host(const fstc_packed_t *p, void *cuda_stream, uint
 /* M1∘M2 from packed operands (m1 packed with side 1, m2 with side 2; inner alphabets must agree, :45). */
 FSTC_API int fstc_compose_packed(const fstc_packed_t *m1, const fstc_packed_t *m2, const fstc_opts_t *opts,
                         void *cuda_stream, fstc_result_t **out, fstc_stats_t *stats /* nullable */);
+
+/* M1[k]∘M2 for k = 0..n-1 against ONE packed right operand, in one call: the paper's use case of many small lattices
+ * against one language model (:251-259).  Problems that fit a thread block are composed by one launch, a block each,
+ * with no host round trip (FSTC_SMALL_*); the others go through fstc_compose_packed's level-synchronous path one after
+ * the other.  m1: host array of n packed left operands (side 1); out: host array of n results (each released with
+ * fstc_result_free; results of one call may share a device block, which is released with the last of them);
+ * stats: NULL or a host array of n.  On error every out[k] is NULL and nothing is leaked. */
+FSTC_API int fstc_compose_batch(const fstc_packed_t *const *m1, int32_t n, const fstc_packed_t *m2, const fstc_opts_t *opts,
+                       void *cuda_stream, fstc_result_t **out, fstc_stats_t *stats /* nullable, [n] */);
 
 /* fst_compose(M1, M2) -> M1∘M2: packs both operands, composes, frees the packed forms. */
 FSTC_API int fstc_compose(const fstc_fst_t *m1, const fstc_fst_t *m2, const fstc_opts_t *opts, void *cuda_stream,

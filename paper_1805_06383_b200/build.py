@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libfstc.so")
-SOURCES = ["radix_sort.cu", "pack.cu", "resolve.cu", "compose.cu", "api.cu"]
+SOURCES = ["radix_sort.cu", "pack.cu", "resolve.cu", "compose.cu", "small.cu", "api.cu"]
 HEADERS = ["common.cuh", "scan.cuh", "internal.h", os.path.join("..", "..", "include", "fstc.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",

@@ -337,6 +337,32 @@ int fstc_compose_packed(const fstc_packed_t *m1, const fstc_packed_t *m2, const 
     });
 }
 
+int fstc_compose_batch(const fstc_packed_t *const *m1, int32_t n, const fstc_packed_t *m2, const fstc_opts_t *opts,
+                       void *cuda_stream, fstc_result_t **out, fstc_stats_t *stats) {
+    if (out) for (int32_t k = 0; k < n; ++k) out[k] = nullptr;
+    int rc = guarded([&] {
+        if (!m1 || !m2 || !out || n < 0) fail(FSTC_ERR_ARG, "null argument");
+        fstc_opts_t o = {};
+        if (opts) o = *opts;
+        if (o.small_path < 0 || o.small_path > 2) fail(FSTC_ERR_ARG, "bad options");
+        Ctx c = make_ctx(cuda_stream);
+        std::vector<char> ok(static_cast<size_t>(n), 0);
+        if (small_path_applies(o)) compose_small_batch(c, m1, n, *m2, o, out, stats, ok);
+        else if (o.small_path == FSTC_SMALL_ONLY) fail(FSTC_ERR_ARG, "the small path does not take these options");
+        fstc_opts_t big = o;
+        big.small_path = FSTC_SMALL_OFF;
+        for (int32_t k = 0; k < n; ++k) {                       // what did not fit a block: the level-synchronous path
+            if (ok[k]) continue;
+            if (!m1[k]) fail(FSTC_ERR_ARG, "null operand %d", k);
+            if (o.small_path == FSTC_SMALL_ONLY) fail(FSTC_ERR_CAPACITY, "problem %d does not fit the small path", k);
+            out[k] = compose_packed(c, *m1[k], *m2, big, stats ? stats + k : nullptr);
+        }
+    });
+    if (rc != FSTC_OK && out)
+        for (int32_t k = 0; k < n; ++k) { free_result(out[k]); out[k] = nullptr; }
+    return rc;
+}
+
 int fstc_compose(const fstc_fst_t *m1, const fstc_fst_t *m2, const fstc_opts_t *opts, void *cuda_stream,
                  fstc_result_t **out, fstc_stats_t *stats) {
     if (out) *out = nullptr;

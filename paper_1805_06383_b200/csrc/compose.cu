@@ -37,21 +37,6 @@ constexpr int64_t GROUP_MAX_RATIO = 8;     // class G while (groups of q1) x (gr
 
 __device__ __forceinline__ int64_t ceil_div_dev(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
-struct MachineView {
-    const uint4 *arcs;
-    const uint2 *segs;
-    const uint32_t *seg_ptr;
-    const uint8_t *flags;
-    const uint2 *garcs;          // grouped copy (internal.h): {inner, weight} sorted by (src, outer, tgt, inner)
-    const uint32_t *goff;
-    const uint2 *gkey;
-    const uint32_t *gptr;
-};
-
-inline MachineView view_of(const fstc_packed_t &p) {
-    return MachineView{p.arcs, p.segs, p.seg_ptr, p.flags, p.garcs, p.goff, p.gkey, p.gptr};
-}
-
 // ------------------------------------------------------------------------------------------ hash table
 // Open addressing over 32-byte BUCKETS of two 16-byte slots {key lo, key hi, id, unused}: a bucket is exactly
 // one DRAM sector, read with a single 256-bit load.  A key lives in the first free slot on its probe path
@@ -1058,10 +1043,6 @@ struct StageTimer {
     }
 };
 
-struct ResultImpl {           // owns the device arrays of a result
-    void *bufs[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-};
-
 struct Composer {
     Ctx &c;
     const fstc_packed_t &m1, &m2;
@@ -1733,21 +1714,20 @@ fstc_result_t *Composer::run() {
 
 fstc_result_t *compose_packed(Ctx &c, const fstc_packed_t &m1, const fstc_packed_t &m2, const fstc_opts_t &opts,
                               fstc_stats_t *stats) {
+    if (opts.small_path < 0 || opts.small_path > 2) fail(FSTC_ERR_ARG, "bad options");
+    if (small_path_applies(opts)) {
+        // small problems never leave the device (small.cu); one that outgrows the block's capacities comes back here
+        const fstc_packed_t *one = &m1;
+        fstc_result_t *r = nullptr;
+        std::vector<char> ok;
+        compose_small_batch(c, &one, 1, m2, opts, &r, stats, ok);
+        if (ok[0]) return r;
+        if (opts.small_path == FSTC_SMALL_ONLY) fail(FSTC_ERR_CAPACITY, "the problem does not fit the small path");
+    } else if (opts.small_path == FSTC_SMALL_ONLY) fail(FSTC_ERR_ARG, "the small path does not take these options");
     Composer k(c, m1, m2, opts);
     fstc_result_t *r = k.run();
     if (stats) *stats = k.st;
     return r;
-}
-
-void free_result(fstc_result_t *r) {
-    if (!r) return;
-    ResultImpl *impl = static_cast<ResultImpl *>(r->impl);
-    if (impl) {
-        for (void *p : impl->bufs)
-            if (p) persist_free(p, nullptr);
-        delete impl;
-    }
-    delete r;
 }
 
 }  // namespace fstc

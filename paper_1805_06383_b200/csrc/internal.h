@@ -52,13 +52,43 @@ struct fstc_packed_t {
 
 namespace fstc {
 
+// what the kernels read of a packed operand
+struct MachineView {
+    const uint4 *arcs;
+    const uint2 *segs;
+    const uint32_t *seg_ptr;
+    const uint8_t *flags;
+    const uint2 *garcs;          // grouped copy (internal.h): {inner, weight} sorted by (src, outer, tgt, inner)
+    const uint32_t *goff;
+    const uint2 *gkey;
+    const uint32_t *gptr;
+};
+
+inline MachineView view_of(const fstc_packed_t &p) {
+    return MachineView{p.arcs, p.segs, p.seg_ptr, p.flags, p.garcs, p.goff, p.gkey, p.gptr};
+}
+
 fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side);
 void free_packed(fstc_packed_t *p);
 
 // ---------------------------------------------------------------- composition (compose.cu)
 fstc_result_t *compose_packed(Ctx &c, const fstc_packed_t &m1, const fstc_packed_t &m2, const fstc_opts_t &opts,
                               fstc_stats_t *stats);
-void free_result(fstc_result_t *r);
+void free_result(fstc_result_t *r);            // small.cu
+
+struct SharedBlock {          // one device block that the results of a batch share
+    void *base;
+    int refs;
+};
+struct ResultImpl {           // owns the device arrays of a result
+    void *bufs[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    SharedBlock *shared = nullptr;   // set: the arrays are parts of a batch's block
+};
+
+// ---------------------------------------------------------------- small problems, one block each (small.cu)
+bool small_path_applies(const fstc_opts_t &o);
+void compose_small_batch(Ctx &c, const fstc_packed_t *const *m1, int n, const fstc_packed_t &m2, const fstc_opts_t &o,
+                         fstc_result_t **results, fstc_stats_t *stats, std::vector<char> &ok);
 
 // ---------------------------------------------------------------- partitioned target resolution (resolve.cu)
 // Finds or creates the state id of every composed arc of a big level without touching a table in DRAM at random:

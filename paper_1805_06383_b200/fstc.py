@@ -20,12 +20,14 @@ LIB_PATH = os.environ.get("FSTC_LIB") or os.path.join(_HERE, "libfstc.so")   # F
 FSTC_MEM_DEVICE, FSTC_MEM_HOST = 0, 1
 MERGE_AUTO, MERGE_OFF, MERGE_SORT_ALL = 0, 1, 2
 RESOLVE_AUTO, RESOLVE_TABLE, RESOLVE_PARTITIONED, RESOLVE_HASH = 0, 1, 2, 3
+SMALL_AUTO, SMALL_OFF, SMALL_ONLY = 0, 1, 2
+ERR_ARG, ERR_INPUT, ERR_OOM, ERR_CAPACITY, ERR_CUDA = -1, -2, -3, -4, -5
 MAX_LEVEL_STATS = 64
 STAGES = ("count", "scan", "match", "emit", "sort", "reduce", "table", "assemble", "rs_scatter", "rs_dedupe", "rs_gather")
 
 EXPORTS = (
     "fstc_pack", "fstc_packed_free", "fstc_packed_info", "fstc_packed_to_host", "fstc_compose_packed",
-    "fstc_compose", "fstc_result_to_host", "fstc_result_free", "fstc_trim_pool", "fstc_strerror",
+    "fstc_compose", "fstc_compose_batch", "fstc_result_to_host", "fstc_result_free", "fstc_trim_pool", "fstc_strerror",
     "fstc_last_error", "fstc_version",
 )
 
@@ -51,6 +53,7 @@ class _Opts(ctypes.Structure):
         ("merge_mode", ctypes.c_int32), ("max_levels", ctypes.c_int32), ("max_raw_arcs", ctypes.c_int64),
         ("arc_capacity_hint", ctypes.c_int64), ("state_capacity_hint", ctypes.c_int64),
         ("profile", ctypes.c_int32), ("resolve_mode", ctypes.c_int32),
+        ("small_path", ctypes.c_int32), ("reserved_", ctypes.c_int32),
     ]
 
 
@@ -62,7 +65,7 @@ class _Stats(ctypes.Structure):
         ("n_raw_sorted", ctypes.c_int64), ("n_raw_grouped", ctypes.c_int64), ("table_capacity", ctypes.c_int64),
         ("n_rehash", ctypes.c_int32), ("n_grow", ctypes.c_int32),
         ("n_emit_launches", ctypes.c_int32), ("n_kernel_launches", ctypes.c_int32),
-        ("n_resolve", ctypes.c_int32), ("n_resolve_arcs_pad", ctypes.c_int32), ("n_resolved_arcs", ctypes.c_int64),
+        ("n_resolve", ctypes.c_int32), ("small_path", ctypes.c_int32), ("n_resolved_arcs", ctypes.c_int64),
         ("rs_scatter_recs", ctypes.c_int64), ("rs_scatter_dest_recs", ctypes.c_int64), ("rs_dedupe_arcs", ctypes.c_int64),
         ("rs_dedupe_states", ctypes.c_int64), ("rs_dedupe_new", ctypes.c_int64), ("rs_gather_recs", ctypes.c_int64),
         ("rs_scatter_launches", ctypes.c_int32), ("rs_dedupe_launches", ctypes.c_int32),
@@ -108,6 +111,7 @@ def lib():
         L.fstc_packed_to_host.argtypes = [P, P, P, P, P, P, P]
         L.fstc_compose_packed.argtypes = [P, P, P, P, ctypes.POINTER(ctypes.POINTER(_Result)), P]
         L.fstc_compose.argtypes = [P, P, P, P, ctypes.POINTER(ctypes.POINTER(_Result)), P]
+        L.fstc_compose_batch.argtypes = [P, ctypes.c_int32, P, P, P, P, P]
         L.fstc_result_to_host.argtypes = [ctypes.POINTER(_Result), P, P]
         L.fstc_result_free.argtypes = [ctypes.POINTER(_Result)]
         L.fstc_result_free.restype = None
@@ -240,6 +244,14 @@ class ComposeResult:
         self.expanded = _tensor(r.expanded, (self.n_states,), "|u1", h)
         self.stats = stats_dict(stats) if stats is not None else None
 
+    def free(self):
+        """Releases the result now (fstc_result_free); the tensors of this object must no longer be used."""
+        self.pair = self.src = self.ilabel = self.olabel = self.tgt = self.weight = self.accept = self.expanded = None
+        h, self._h = self._h, None
+        if h is not None and h.ptr:
+            lib().fstc_result_free(h.ptr)
+            h.ptr = None
+
     def to_host(self, out: Optional[dict] = None, stream=None) -> dict:
         """Copies every array to host memory through fstc_result_to_host.  `out` may hold preallocated
         (pinned) torch CPU tensors named like the fields, each at least as long as needed."""
@@ -272,7 +284,7 @@ def stats_dict(s: _Stats) -> dict:
         "n_raw_sorted": int(s.n_raw_sorted), "n_raw_grouped": int(s.n_raw_grouped), "table_capacity": int(s.table_capacity),
         "n_rehash": int(s.n_rehash), "n_grow": int(s.n_grow), "n_emit_launches": int(s.n_emit_launches),
         "n_kernel_launches": int(s.n_kernel_launches),
-        "n_resolve": int(s.n_resolve), "n_resolved_arcs": int(s.n_resolved_arcs),
+        "n_resolve": int(s.n_resolve), "n_resolved_arcs": int(s.n_resolved_arcs), "small_path": int(s.small_path),
         **{k: int(getattr(s, k)) for k in ("rs_scatter_recs", "rs_scatter_dest_recs", "rs_dedupe_arcs", "rs_dedupe_states",
                                            "rs_dedupe_new", "rs_gather_recs", "rs_scatter_launches", "rs_dedupe_launches",
                                            "rs_gather_launches")},
@@ -284,9 +296,10 @@ def stats_dict(s: _Stats) -> dict:
 
 
 def _opts(merge_mode=MERGE_AUTO, max_raw_arcs=0, max_levels=0, arc_capacity_hint=0, state_capacity_hint=0,
-          profile=False, resolve_mode=0) -> _Opts:
+          profile=False, resolve_mode=0, small_path=0) -> _Opts:
     o = _Opts()
     o.resolve_mode = int(resolve_mode)
+    o.small_path = int(small_path)
     o.merge_mode, o.max_levels, o.max_raw_arcs = int(merge_mode), int(max_levels), int(max_raw_arcs)
     o.arc_capacity_hint, o.state_capacity_hint, o.profile = int(arc_capacity_hint), int(state_capacity_hint), int(bool(profile))
     return o
@@ -341,6 +354,26 @@ def fstc_compose_packed(p1: Packed, p2: Packed, *, stream=None, with_stats=True,
     _check(lib().fstc_compose_packed(p1.ptr, p2.ptr, ctypes.addressof(o), _stream_ptr(stream), ctypes.byref(out),
                                      ctypes.addressof(st) if st is not None else None))
     return ComposeResult(out, st)
+
+
+def fstc_compose_batch(p1s, p2: Packed, *, stream=None, with_stats=True, **opts) -> list:
+    """M1[k]∘M2 for every packed left operand of `p1s` against one packed right operand, in one call (the paper's
+    use case of many lattices against one language model)."""
+    n = len(p1s)
+    o = _opts(**opts)
+    ptrs = (ctypes.c_void_p * n)(*[p.ptr for p in p1s])
+    outs = (ctypes.POINTER(_Result) * n)()
+    sts = (_Stats * n)() if with_stats else None
+    _check(lib().fstc_compose_batch(ctypes.addressof(ptrs), n, p2.ptr, ctypes.addressof(o), _stream_ptr(stream),
+                                    ctypes.addressof(outs), ctypes.addressof(sts) if sts is not None else None))
+    res = []
+    for k in range(n):
+        st = None
+        if sts is not None:
+            st = _Stats()
+            ctypes.memmove(ctypes.addressof(st), ctypes.addressof(sts[k]), ctypes.sizeof(_Stats))
+        res.append(ComposeResult(outs[k], st))
+    return res
 
 
 def fstc_compose(m1, m2, *, stream=None, with_stats=True, **opts) -> ComposeResult:

@@ -33,12 +33,17 @@ def gpu_tables(res, n_q2):
     return keys, tab, w
 
 
-def check_parity(fstc, m1, m2, *, merge_mode=0, max_raw_arcs=0, max_levels=0, device_inputs=True, resolve_mode=0):
+def check_parity(fstc, m1, m2, *, merge_mode=0, max_raw_arcs=0, max_levels=0, device_inputs=True, resolve_mode=0, small_path=1,
+                 result=None):
+    """small_path: 1 (default here) = the level-synchronous path of compose.cu, so that small test inputs still exercise
+    it; tests/test_gpu_small.py passes 2 (one-block path only) and 0 (auto).  `result`: compare this result instead of
+    composing (batch tests)."""
     ref = oracle.compose(m1, m2, merge=True, max_raw_arcs=max_raw_arcs, max_levels=max_levels)
     a = fstc.DeviceFst.from_host(m1) if device_inputs else m1
     b = fstc.DeviceFst.from_host(m2) if device_inputs else m2
-    res = fstc.fstc_compose(a, b, merge_mode=merge_mode, max_raw_arcs=max_raw_arcs, max_levels=max_levels,
-                            resolve_mode=resolve_mode)
+    res = result if result is not None else fstc.fstc_compose(
+        a, b, merge_mode=merge_mode, max_raw_arcs=max_raw_arcs, max_levels=max_levels, resolve_mode=resolve_mode,
+        small_path=small_path)
     nq2 = m2.n_states
     keys, tab, w = gpu_tables(res, nq2)
     # --- states

@@ -98,8 +98,8 @@ def test_auto_goes_back_to_the_table_and_rebuilds_it(fstc):
     only through the cost model is not controllable from outside, so force both modes and compare them level by level."""
     m1, m2 = workloads.make_config("medium", scale=0.05)
     a, b = fstc.DeviceFst.from_host(m1), fstc.DeviceFst.from_host(m2)
-    r_t = fstc.fstc_compose(a, b, resolve_mode=fstc.RESOLVE_TABLE)
-    r_p = fstc.fstc_compose(a, b, resolve_mode=fstc.RESOLVE_PARTITIONED)
+    r_t = fstc.fstc_compose(a, b, small_path=1, resolve_mode=fstc.RESOLVE_TABLE)
+    r_p = fstc.fstc_compose(a, b, small_path=1, resolve_mode=fstc.RESOLVE_PARTITIONED)
     assert r_t.stats["level_new_states"] == r_p.stats["level_new_states"]
     assert r_t.stats["level_raw"] == r_p.stats["level_raw"]
     assert (r_t.n_states, r_t.n_arcs) == (r_p.n_states, r_p.n_arcs)
@@ -113,7 +113,7 @@ def test_workspace_is_reused_and_trimmed(fstc):
     a, b = fstc.DeviceFst.from_host(m1), fstc.DeviceFst.from_host(m2)
     first = None
     for it in range(4):
-        r = fstc.fstc_compose(a, b, max_raw_arcs=8_000_000, resolve_mode=fstc.RESOLVE_PARTITIONED)
+        r = fstc.fstc_compose(a, b, small_path=1, max_raw_arcs=8_000_000, resolve_mode=fstc.RESOLVE_PARTITIONED)
         # state ids differ from run to run (N6); sizes and the multiset of weights do not
         sig = (r.n_states, r.n_arcs, r.n_accept, float(r.weight.double().sum().item()))
         first = first or sig
@@ -131,7 +131,7 @@ def test_two_host_threads_compose_concurrently(fstc):
     import torch
     m1, m2 = workloads.make_config("medium", scale=0.03)
     a, b = fstc.DeviceFst.from_host(m1), fstc.DeviceFst.from_host(m2)
-    ref = fstc.fstc_compose(a, b)
+    ref = fstc.fstc_compose(a, b, small_path=1)
     want = (ref.n_states, ref.n_arcs, ref.n_raw_arcs)
     got, errs = [], []
 
@@ -140,7 +140,7 @@ def test_two_host_threads_compose_concurrently(fstc):
             s = torch.cuda.Stream()
             with torch.cuda.stream(s):
                 for _ in range(3):
-                    r = fstc.fstc_compose(a, b, stream=s, resolve_mode=mode)
+                    r = fstc.fstc_compose(a, b, small_path=1, stream=s, resolve_mode=mode)
                     got.append((r.n_states, r.n_arcs, r.n_raw_arcs))
                     del r
         except Exception as e:  # noqa: BLE001
@@ -182,6 +182,6 @@ def test_dense_table_is_rebuilt_after_partitioned_levels(fstc):
     partitioned resolve on the same input."""
     m1, m2 = workloads.make_config("medium", scale=0.05)
     a, b = fstc.DeviceFst.from_host(m1), fstc.DeviceFst.from_host(m2)
-    rs = [fstc.fstc_compose(a, b, resolve_mode=m) for m in (fstc.RESOLVE_TABLE, fstc.RESOLVE_HASH, fstc.RESOLVE_PARTITIONED)]
+    rs = [fstc.fstc_compose(a, b, small_path=1, resolve_mode=m) for m in (fstc.RESOLVE_TABLE, fstc.RESOLVE_HASH, fstc.RESOLVE_PARTITIONED)]
     assert len({(r.n_states, r.n_arcs, tuple(r.stats["level_new_states"])) for r in rs}) == 1
     assert rs[0].stats["table_capacity"] == m1.n_states * m2.n_states
