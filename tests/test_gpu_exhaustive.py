@@ -1,0 +1,149 @@
+"""Exhaustive parity at the TIMED size (SURVEY §8(c) "streaming verifier"): `large` and `skewed` at bench.py's budget
+of 1e9 raw arcs, every state and every arc compared with the oracle, no sampling.
+
+  * states, levels, expanded flags, accept set, counters: the oracle's own full run (Algorithm 1 + rule T, arcs not
+    kept) against the result, as sorted pair keys;
+  * arcs: every expanded source is expanded again by the oracle from the definition (`oracle.PairExpander`, fp64) and
+    compared with the source's arc group of the result in pair coordinates (structure exact, weights rtol 1e-5), the
+    sources sharded over the host cores (forked workers read the result's host copy, no pickling); unexpanded states
+    must carry no arc.
+
+About 10-25 minutes per config on a 16-core host, so it only runs when FSTC_EXHAUSTIVE=1 (`-m "gpu and slow"`); the
+one-line summaries of the last run are kept in profiles/.  The everyday full-size checks (exact parity under a small
+budget, sampled sources and invariants at the bench budget) are in test_gpu_fullsize.py."""
+from __future__ import annotations
+
+import json
+import multiprocessing as mp
+import os
+import time
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1805_06383_b200 import workloads
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow,
+              pytest.mark.skipif(os.environ.get("FSTC_EXHAUSTIVE") != "1", reason="set FSTC_EXHAUSTIVE=1 (10-25 min per config)")]
+RTOL = 1e-5
+_G = {}          # host copy of the result + inputs, inherited by the forked workers
+
+
+def _check_sources(bounds):
+    lo_id, hi_id = bounds
+    g = _G
+    x = oracle.PairExpander(g["m1"], g["m2"])
+    q1, q2, ptr, exp = g["q1"], g["q2"], g["ptr"], g["expanded"]
+    tgt, il, ol, w = g["tgt"], g["ilabel"], g["olabel"], g["weight"]
+    n_src = n_arc = n_raw = 0
+    worst = 0.0
+    deg = ptr[lo_id + 1:hi_id + 1] - ptr[lo_id:hi_id]
+    e = exp[lo_id:hi_id].astype(bool)
+    if (deg[~e] != 0).any():
+        return ("unexpanded state with arcs", lo_id + int(np.nonzero((deg != 0) & ~e)[0][0]))
+    for sid in (lo_id + np.nonzero(e)[0]).tolist():
+        a, b = int(ptr[sid]), int(ptr[sid + 1])
+        r1, r2, sa, sb, rw = x.expand(int(q1[sid]), int(q2[sid]), merge=True)
+        if b - a != len(rw):
+            return ("arc count", sid, b - a, len(rw))
+        n_raw += x.raw_count(int(q1[sid]), int(q2[sid]))
+        if b == a:
+            n_src += 1
+            continue
+        t = tgt[a:b]
+        g1, g2, ga, gb = q1[t], q2[t], il[a:b], ol[a:b]
+        o = np.lexsort((gb, ga, g2, g1))
+        if not ((g1[o] == r1).all() and (g2[o] == r2).all() and (ga[o] == sa).all() and (gb[o] == sb).all()):
+            return ("structure", sid)
+        rel = np.abs(w[a:b][o].astype(np.float64) - rw) / np.abs(rw)
+        m = float(rel.max())
+        if not m <= RTOL:
+            return ("weight", sid, m)
+        worst = max(worst, m)
+        n_src += 1
+        n_arc += b - a
+    x.close()
+    return ("ok", n_src, n_arc, n_raw, worst)
+
+
+def _exhaustive(name, budget):
+    import torch
+    from paper_1805_06383_b200 import fstc
+    fstc.lib()
+    t0 = time.time()
+    m1, m2 = workloads.make_config(name)
+    res = fstc.fstc_compose(fstc.DeviceFst.from_host(m1), fstc.DeviceFst.from_host(m2), max_raw_arcs=budget)
+    host = res.to_host()
+    stats = res.stats
+    ns, na = res.n_states, res.n_arcs
+    n_raw, n_levels, truncated, n_expanded = res.n_raw_arcs, res.n_levels, res.truncated, res.n_expanded
+    src = host["src"].numpy()
+    assert (np.diff(src) >= 0).all()
+    ptr = np.zeros(ns + 1, np.int64)
+    np.cumsum(np.bincount(src, minlength=ns), out=ptr[1:])
+    del src
+    pair = host["pair"].numpy()
+    _G.update(m1=m1, m2=m2, q1=np.ascontiguousarray(pair[:, 0]), q2=np.ascontiguousarray(pair[:, 1]), ptr=ptr,
+              expanded=host["expanded"].numpy(), tgt=host["tgt"].numpy(), ilabel=host["ilabel"].numpy(),
+              olabel=host["olabel"].numpy(), weight=host["weight"].numpy())
+    accept = host["accept"].numpy().astype(np.int64)
+    del res, host
+    torch.cuda.empty_cache()
+    t_gpu = time.time() - t0
+
+    # ---- arcs: every source, sharded over the host cores (shards of equal arc counts)
+    n_proc = max(1, (os.cpu_count() or 2) - 1)
+    n_shards = n_proc * 16
+    cuts = np.searchsorted(ptr, np.linspace(0, na, n_shards + 1)[1:-1]).tolist()
+    edges = sorted(set([0] + cuts + [ns]))
+    shards = list(zip(edges[:-1], edges[1:]))
+    t1 = time.time()
+    with mp.get_context("fork").Pool(n_proc) as pool:
+        out = pool.map(_check_sources, shards, chunksize=1)
+    t_arcs = time.time() - t1
+    bad = [o for o in out if o[0] != "ok"]
+    assert not bad, bad[:5]
+    n_src = sum(o[1] for o in out); n_arc = sum(o[2] for o in out); raw_sum = sum(o[3] for o in out)
+    worst = max(o[4] for o in out)
+    assert n_arc == na and n_src == n_expanded and raw_sum == n_raw
+
+    # ---- states, levels, flags, accept set, counters: the oracle's full run
+    t2 = time.time()
+    ref = oracle.compose(m1, m2, merge=True, max_raw_arcs=budget, keep_arcs=False)
+    t_oracle = time.time() - t2
+    assert (ns, n_raw, n_levels, truncated, n_expanded) == (ref.n_states, ref.n_raw_arcs, ref.n_levels, ref.truncated, ref.n_expanded)
+    assert na == ref.n_arcs
+    assert stats["level_raw"][:ref.n_levels] == [int(v) for v in ref.level_raw]
+    assert stats["level_frontier"][:ref.n_levels] == [int(v) for v in ref.level_size]
+    nq2 = m2.n_states
+    gk = _G["q1"].astype(np.int64) * nq2 + _G["q2"]
+    assert gk[0] == int(m1.start) * nq2 + int(m2.start)
+    go = np.argsort(gk, kind="stable")
+    rk = ref.state_keys()
+    ro = np.argsort(rk, kind="stable")
+    assert (gk[go] == rk[ro]).all()
+    assert (_G["expanded"][go] == ref.expanded[ro]).all()
+    assert (np.diff(accept) > 0).all()
+    assert (np.sort(gk[accept]) == np.sort(rk[ref.accept])).all()
+    summary = {"config": name, "max_raw_arcs": budget, "states": ns, "arcs": na, "raw_arcs": n_raw, "levels": n_levels,
+               "expanded_sources": n_expanded, "sources_compared": n_src, "arcs_compared": n_arc,
+               "worst_rel_weight_error": worst, "small_path": stats["small_path"], "n_resolve": stats["n_resolve"],
+               "host_cores": n_proc, "seconds": {"compose_and_copy": round(t_gpu, 1), "arcs": round(t_arcs, 1),
+                                                 "oracle_states": round(t_oracle, 1)}}
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open(os.path.join("gpurun_out", f"exhaustive_{name}.json"), "w") as f:
+        f.write(json.dumps(summary) + "\n")
+    print("EXHAUSTIVE", json.dumps(summary))
+    _G.clear()
+
+
+BUDGET = int(os.environ.get("FSTC_EXHAUSTIVE_BUDGET", 1_000_000_000))   # bench.py's budget; lower only to try the harness
+
+
+def test_large_every_state_and_arc_at_the_bench_budget():
+    _exhaustive("large", BUDGET)
+
+
+def test_skewed_every_state_and_arc_at_the_bench_budget():
+    _exhaustive("skewed", BUDGET)
