@@ -372,7 +372,7 @@ def main():
         "config": {"workload": WORKLOAD_DESC[args.workload], "name": args.workload, "seeds": [s1, s2],
                    "max_raw_arcs": budget, "merge_mode": args.merge_mode, "resolve_mode": args.resolve_mode, "parallelism": f"replicas x{world}",
                    "cache": "L2 flushed (256 MiB write) before every step; working set >> L2"},
-        "result": {"n_states": st["n_states"], "n_arcs": st["n_arcs"], "n_raw_arcs": st["n_raw_arcs"],
+        "result": {"small_path": st["small_path"], "n_states": st["n_states"], "n_arcs": st["n_arcs"], "n_raw_arcs": st["n_raw_arcs"],
                    "n_levels": st["n_levels"], "truncated": st["truncated"], "n_expanded": st["n_expanded"],
                    "merged_arcs_per_sec": st["n_arcs"] * world / (t_ms / args.steps * 1e-3)},
         "timing_ms": {"pack": pack_ms, "compose_packed": compose_ms, "stages": stage_ms,
@@ -412,27 +412,30 @@ def main():
             out[n] = torch.empty(na, dtype=torch.int32).pin_memory()
         out["weight"] = torch.empty(na, dtype=torch.float32).pin_memory()
         h2d = sum(int(getattr(h, n).numel()) * 4 for h in hs for n in ("src", "ilabel", "olabel", "tgt", "weight", "accept"))
-        e2e_ms, e2e_arcs, d2h = 0.0, 0, 0
+        e2e_ms, e2e_arcs, d2h, spill_saved = 0.0, 0, 0, 0
         n_e2e = max(1, min(args.e2e_steps, args.steps))
         for i in range(1 + n_e2e):
             flush.fill_(1)
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             barrier()
             a.record()
+            # host spill (fstc_spill_t): finished levels cross PCIe on a second stream while the next level runs, and the
+            # arcs are never held on the device beyond their level
             r = fstc.fstc_compose(hs[0], hs[1], merge_mode=args.merge_mode, max_raw_arcs=budget,
-                                  resolve_mode=args.resolve_mode)
-            r.to_host(out)
+                                  resolve_mode=args.resolve_mode, spill=out, spill_keep_device=False)
             b.record()
             torch.cuda.synchronize()
             if i > 0:
                 e2e_ms += a.elapsed_time(b)
                 e2e_arcs += r.n_raw_arcs
             d2h = 8 * r.n_states + r.n_states + 4 * r.n_accept + 20 * r.n_arcs
+            spill_saved = r.stats["spill_bytes_saved"]
             del r
         (e2e_ms,), (e2e_arcs,) = reduce_over_ranks(dist, world, [e2e_ms], [e2e_arcs], "cuda")
         line["e2e"] = {"value": e2e_arcs / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                        "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / n_e2e, "steps": n_e2e,
-                       "api": "fstc_compose(host arrays) + fstc_result_to_host(pinned buffers)"}
+                       "api": "fstc_compose(pinned host arrays in, fstc_spill_t pinned host arrays out)",
+                       "spill_bytes_saved_on_device": int(spill_saved)}
         del out
 
     # ---- the oracle, as it stands, on this box's host cores (rank 0, N = 1 only)

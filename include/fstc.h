@@ -55,7 +55,9 @@ enum {
   FSTC_ERR_INPUT = -2,    /* a state or symbol id out of range (found by a device validation pass)        */
   FSTC_ERR_OOM = -3,      /* device (or pinned host) allocation failed                                     */
   FSTC_ERR_CAPACITY = -4, /* an internal limit was exceeded (see fstc_opts_t and DESIGN.md "limits")       */
-  FSTC_ERR_CUDA = -5      /* any other CUDA runtime error                                                  */
+  FSTC_ERR_CUDA = -5,     /* any other CUDA runtime error                                                  */
+  FSTC_ERR_INTERNAL = -6, /* a consistency check of the library failed (a bug: please report the message)  */
+  FSTC_ERR_CALLBACK = -7  /* fstc_opts_t.resolve_cb returned non-zero                                        */
 };
 
 enum { FSTC_MEM_DEVICE = 0, FSTC_MEM_HOST = 1 };
@@ -83,8 +85,10 @@ typedef struct fstc_fst_t {
 enum {
   FSTC_MERGE_AUTO = 0,      /* default: identical (src,tgt,a,b) arcs are summed (:65).  Only the sources
                                that CAN hold duplicates (exact test, N10, replacing the lossy
-                               table H of :243) go through sort + reduce; their arcs come out sorted by
-                               (tgt,a,b), the other sources' arcs in generation order.                 */
+                               table H of :243) are merged: by construction from the (a,r1) x (b,r2) groups of the
+                               pair when that is cheaper (arcs in (a,r1,b,r2) order), else by sort + reduce (arcs
+                               sorted by (tgt,a,b)); the other sources' arcs come in generation order (inner
+                               symbol, e1, e2).  Arcs are always sorted by source id.                   */
   FSTC_MERGE_OFF = 1,       /* "without performing any reductions" (:289): one arc per (e1,e2) match */
   FSTC_MERGE_SORT_ALL = 2   /* every source goes through sort + reduce: arcs sorted by (src,tgt,a,b) */
 };
@@ -94,8 +98,40 @@ enum {
   FSTC_RESOLVE_TABLE = 1,       /* always a visited table (atomicCAS per arc, :237): the paper's dense table of one
                                    entry per pair when |Q1||Q2| <= 2^29, else the open-addressing hash table   */
   FSTC_RESOLVE_PARTITIONED = 2, /* always the streaming hash-partitioned resolve         */
-  FSTC_RESOLVE_HASH = 3         /* always the open-addressing hash table, whatever |Q1||Q2|                    */
+  FSTC_RESOLVE_HASH = 3,        /* always the open-addressing hash table, whatever |Q1||Q2|                    */
+  FSTC_RESOLVE_EXTERNAL = 4     /* the caller resolves target keys to state ids (fstc_opts_t.resolve_cb): one
+                                   composition sharded over several GPUs by ownership of the pair keys          */
 };
+
+/* FSTC_RESOLVE_EXTERNAL: every rank holds both operands and expands only the state pairs it OWNS; the target
+ * keys of its arcs go to resolve_cb, which exchanges them with the other ranks (one all-to-all per call), lets the owners
+ * find or create the states, and returns a GLOBAL state id per key.  Three calls per BFS level on every rank, whether or
+ * not the rank has arcs of that class: call 0 (arcs that go through sort + reduce), 1 (arcs merged by construction),
+ * 2 (all other arcs; sets *more = 1 if any rank created a state in this level, else the search ends everywhere).
+ * keys: device, [n_keys], (r1 << q2_bits) | r2.  ids_out: device, [n_keys].  *new_pairs: device [2 * *n_new], the pairs
+ * (q1, q2) this rank now owns in addition (local ids continue in that order); valid until the next call.  The callback
+ * must have finished its device work when it returns; a non-zero return aborts the composition (FSTC_ERR_CALLBACK).
+ * The result of a rank holds ITS states (pair, accept, expanded, local ids 0..n-1 in creation order) and their outgoing
+ * arcs: src is a local id, tgt a global id.  Not with max_raw_arcs, deterministic, spill or the small path. */
+typedef int (*fstc_resolve_fn)(void *ctx, int32_t level, int32_t call, int32_t q2_bits, const unsigned long long *keys,
+                               int64_t n_keys, int32_t *ids_out, const int32_t **new_pairs, int64_t *n_new, int32_t *more);
+
+/* Host spill (the paper streams its edge buffer to pinned host memory while the search goes on, :153-155,217,233).
+ * Caller-allocated PINNED host arrays that receive the result WHILE it is built: the arcs and state pairs of a BFS level are
+ * final once the level is placed, so their device->host copies run on a second stream under the next level's kernels;
+ * the call returns when the host copy is complete (accept list and expanded flags included).  keep_device = 0: the arcs
+ * then live on the host only — a level's device arrays are released as soon as its copy is done, the result's src /
+ * ilabel / olabel / tgt / weight are NULL and n_arcs tells how many the host arrays hold: 20 bytes of HBM per arc are
+ * never held beyond one level (stats.spill_bytes_saved).  keep_device = 1: the result keeps its device arrays as usual.
+ * A result that outgrows arc_capacity / state_capacity -> FSTC_ERR_CAPACITY. */
+struct fstc_host_result_t;
+typedef struct fstc_spill_t {
+  const struct fstc_host_result_t *host;  /* every array but `accept` / `expanded` may not be NULL              */
+  int64_t arc_capacity;     /* length of src, ilabel, olabel, tgt, weight                                     */
+  int64_t state_capacity;   /* length of pair / 2, accept, expanded                                           */
+  int32_t keep_device;
+  int32_t reserved_;
+} fstc_spill_t;
 
 enum {
   FSTC_SMALL_AUTO = 0,      /* default: the whole search first runs inside ONE thread block, with no host round trip
@@ -116,8 +152,29 @@ typedef struct fstc_opts_t {
   int32_t profile;          /* 1: time every stage with CUDA events on the stream (fills stats ms)    */
   int32_t resolve_mode;     /* FSTC_RESOLVE_*: how composed arcs find the ids of their target states          */
   int32_t small_path;       /* FSTC_SMALL_*: the device-resident path for small problems                      */
+  int32_t deterministic;    /* 1: state ids and arc order are identical from run to run (see below)           */
+  /* Allocator hooks: when `alloc` is set, EVERY device allocation of the call (temporaries and the arrays of the
+   * result / packed operand) goes through it instead of the library's own pool, so that e.g. PyTorch's caching allocator
+   * owns the memory.  alloc(bytes, stream, ctx) returns device memory usable by work queued on `stream` (NULL = out of
+   * memory -> FSTC_ERR_OOM); dealloc(ptr, stream, ctx) is called once per block: during the call for temporaries (on the
+   * call's stream, after the last kernel that uses them was queued), from fstc_result_free / fstc_packed_free for the
+   * arrays that left the library (stream = NULL).  Both must be set or both NULL. */
+  void *(*alloc)(size_t bytes, void *cuda_stream, void *ctx);
+  void (*dealloc)(void *ptr, void *cuda_stream, void *ctx);
+  void *alloc_ctx;
+  const fstc_spill_t *spill;/* NULL: the result stays on the device                                           */
+  fstc_resolve_fn resolve_cb;   /* FSTC_RESOLVE_EXTERNAL only                                                 */
+  void *resolve_ctx;
+  int32_t owns_start;       /* FSTC_RESOLVE_EXTERNAL: 1 on the rank that owns the start pair (its local state 0) */
   int32_t reserved_;
 } fstc_opts_t;
+
+/* deterministic = 1.  State ids are implementation-defined (:239 numbers states in discovery order, which is a race on
+ * a GPU).  With this flag the states a BFS level creates are numbered in ascending order of their pair key q1*|Q2|+q2
+ * (one sort of the new keys per level), and the arcs of a source come out in an order that only depends on the inputs
+ * (generation order, group order, or (tgt,a,b) order on the final ids): two runs give bit-identical pair, src, ilabel,
+ * olabel, tgt, accept and expanded arrays.  Weights of arcs merged by sort + reduce are summed with atomics and may differ
+ * in the last bit.  The small path is not used. */
 
 /* Rule T (the paper only notes that the result may not fit the device, :153).  BFS levels are
  * expanded whole while the running total of raw composed arcs stays <= max_raw_arcs.  The first
@@ -161,6 +218,7 @@ typedef struct fstc_stats_t {
    * the recorded permutation, arc keys and state records through the dedupe, ids through the gathers; launches    */
   int64_t rs_scatter_recs, rs_scatter_dest_recs, rs_dedupe_arcs, rs_dedupe_states, rs_dedupe_new, rs_gather_recs;
   int32_t rs_scatter_launches, rs_dedupe_launches, rs_gather_launches, pad2_;
+  int64_t spill_bytes, spill_bytes_saved;  /* bytes copied to the host while the search ran; device bytes never held (keep_device = 0) */
   double ms[FSTC_T_NSTAGES];/* device time per stage (CUDA events), only when opts.profile = 1       */
   double ms_total;          /* device time of the whole call (CUDA events), always                    */
   int64_t level_frontier[FSTC_MAX_LEVEL_STATS];  /* |F_l|                                             */
@@ -202,7 +260,8 @@ typedef struct fstc_host_result_t {
 typedef struct fstc_packed_t fstc_packed_t;
 
 /* side 1: the inner alphabet is the OUTPUT side (left operand M1); side 2: the INPUT side (M2). */
-FSTC_API int fstc_pack(const fstc_fst_t *m, int side, void *cuda_stream, fstc_packed_t **out);
+/* opts (nullable): only the allocator hooks are read. */
+FSTC_API int fstc_pack(const fstc_fst_t *m, int side, const fstc_opts_t *opts, void *cuda_stream, fstc_packed_t **out);
 FSTC_API void fstc_packed_free(fstc_packed_t *p);
 /* info[0..6] = n_states, n_arcs, n_segments (distinct (state, inner symbol)), n_inner, n_outer, side,
  *               kernel launches the pack took */
@@ -234,6 +293,8 @@ FSTC_API int fstc_compose(const fstc_fst_t *m1, const fstc_fst_t *m2, const fstc
 /* Copies the result arrays to caller-allocated host memory (pinned memory makes it asynchronous
  * until the final stream synchronisation, which this call performs). */
 FSTC_API int fstc_result_to_host(const fstc_result_t *r, void *cuda_stream, const fstc_host_result_t *dst);
+/* The caller must have finished every use of the result's device arrays (or ordered it before the legacy default
+ * stream) when it frees the result: the blocks are handed to the next composition that asks for their size. */
 FSTC_API void fstc_result_free(fstc_result_t *r);
 
 /* Releases the cached device memory back to the driver: the calling thread's workspace arena, the parked result /

@@ -234,24 +234,47 @@ void persist_release_all() {
     g_parked_bytes = 0;
 }
 
+// Out of memory: the workspace arena, the parked blocks and the pool's free list each hold memory the failing request
+// could use (and so could another allocator on the device, e.g. PyTorch's): everything idle goes back to the driver.
+void release_caches(cudaStream_t stream) {
+    (void)cudaStreamSynchronize(stream);
+    for (auto &ch : g_arena.chunks)                          // chunks of this thread that nobody uses
+        if (ch.base && ch.free_ranges.size() == 1 && ch.free_ranges.begin()->second == ch.size) {
+            (void)cudaFreeAsync(ch.base, stream);
+            ch.base = nullptr; ch.size = 0; ch.free_ranges.clear();
+        }
+    persist_release_all();
+    (void)cudaStreamSynchronize(stream);
+    (void)cudaStreamSynchronize(nullptr);
+    try { (void)cudaMemPoolTrimTo(device_pool(), 0); } catch (const Error &) {}
+    (void)cudaGetLastError();
+}
+
 namespace {
 
-Ctx make_ctx(void *stream) {
+Ctx make_ctx(void *stream, const fstc_opts_t *opts = nullptr) {
     Ctx c;
     c.stream = static_cast<cudaStream_t>(stream);
+    if (opts) {
+        if ((opts->alloc == nullptr) != (opts->dealloc == nullptr)) fail(FSTC_ERR_ARG, "alloc and dealloc must both be set or both be NULL");
+        c.hooks.alloc = opts->alloc; c.hooks.dealloc = opts->dealloc; c.hooks.ctx = opts->alloc_ctx;
+    }
     int dev = 0;
     FSTC_CUDA(cudaGetDevice(&dev));
     FSTC_CUDA(cudaDeviceGetAttribute(&c.n_sm, cudaDevAttrMultiProcessorCount, dev));
     return c;
 }
 
+// On an error the DBuf destructors have already handed their arena ranges back while kernels of the failed call may still
+// run: the stream is drained before the call returns, so that the next call cannot reuse a range that is still in use.
 template <typename F>
-int guarded(F &&body) {
+int guarded(F &&body, void *stream = nullptr, bool has_stream = false) {
     try {
         body();
         g_last_error.clear();
         return FSTC_OK;
     } catch (const Error &e) {
+        if (has_stream) { (void)cudaStreamSynchronize(static_cast<cudaStream_t>(stream)); (void)cudaGetLastError(); }
         g_last_error = e.msg;
         return e.code;
     } catch (const std::bad_alloc &) {
@@ -265,7 +288,7 @@ int guarded(F &&body) {
 
 template <typename T>
 void d2h(Ctx &c, T *dst, const T *src, int64_t n) {
-    if (dst && n > 0)
+    if (dst && src && n > 0)
         FSTC_CUDA(cudaMemcpyAsync(dst, src, sizeof(T) * static_cast<size_t>(n), cudaMemcpyDeviceToHost, c.stream));
 }
 
@@ -286,19 +309,21 @@ const char *fstc_strerror(int code) {
         case FSTC_ERR_OOM: return "out of memory";
         case FSTC_ERR_CAPACITY: return "internal capacity limit exceeded";
         case FSTC_ERR_CUDA: return "CUDA error";
+        case FSTC_ERR_INTERNAL: return "internal consistency check failed";
+        case FSTC_ERR_CALLBACK: return "the resolve callback failed";
         default: return "unknown error";
     }
 }
 
 const char *fstc_last_error(void) { return g_last_error.c_str(); }
 
-int fstc_pack(const fstc_fst_t *m, int side, void *cuda_stream, fstc_packed_t **out) {
+int fstc_pack(const fstc_fst_t *m, int side, const fstc_opts_t *opts, void *cuda_stream, fstc_packed_t **out) {
     if (out) *out = nullptr;
     return guarded([&] {
         if (!m || !out) fail(FSTC_ERR_ARG, "null argument");
-        Ctx c = make_ctx(cuda_stream);
+        Ctx c = make_ctx(cuda_stream, opts);
         *out = pack_fst(c, *m, side);
-    });
+    }, cuda_stream, true);
 }
 
 void fstc_packed_free(fstc_packed_t *p) { free_packed(p); }
@@ -332,9 +357,9 @@ int fstc_compose_packed(const fstc_packed_t *m1, const fstc_packed_t *m2, const 
         if (!m1 || !m2 || !out) fail(FSTC_ERR_ARG, "null argument");
         fstc_opts_t o = {};
         if (opts) o = *opts;
-        Ctx c = make_ctx(cuda_stream);
+        Ctx c = make_ctx(cuda_stream, &o);
         *out = compose_packed(c, *m1, *m2, o, stats);
-    });
+    }, cuda_stream, true);
 }
 
 int fstc_compose_batch(const fstc_packed_t *const *m1, int32_t n, const fstc_packed_t *m2, const fstc_opts_t *opts,
@@ -345,7 +370,7 @@ int fstc_compose_batch(const fstc_packed_t *const *m1, int32_t n, const fstc_pac
         fstc_opts_t o = {};
         if (opts) o = *opts;
         if (o.small_path < 0 || o.small_path > 2) fail(FSTC_ERR_ARG, "bad options");
-        Ctx c = make_ctx(cuda_stream);
+        Ctx c = make_ctx(cuda_stream, &o);
         std::vector<char> ok(static_cast<size_t>(n), 0);
         if (small_path_applies(o)) compose_small_batch(c, m1, n, *m2, o, out, stats, ok);
         else if (o.small_path == FSTC_SMALL_ONLY) fail(FSTC_ERR_ARG, "the small path does not take these options");
@@ -357,7 +382,7 @@ int fstc_compose_batch(const fstc_packed_t *const *m1, int32_t n, const fstc_pac
             if (o.small_path == FSTC_SMALL_ONLY) fail(FSTC_ERR_CAPACITY, "problem %d does not fit the small path", k);
             out[k] = compose_packed(c, *m1[k], *m2, big, stats ? stats + k : nullptr);
         }
-    });
+    }, cuda_stream, true);
     if (rc != FSTC_OK && out)
         for (int32_t k = 0; k < n; ++k) { free_result(out[k]); out[k] = nullptr; }
     return rc;
@@ -374,11 +399,11 @@ int fstc_compose(const fstc_fst_t *m1, const fstc_fst_t *m2, const fstc_opts_t *
                  m1->n_osyms, m2->n_isyms);
         fstc_opts_t o = {};
         if (opts) o = *opts;
-        Ctx c = make_ctx(cuda_stream);
+        Ctx c = make_ctx(cuda_stream, &o);
         p1 = pack_fst(c, *m1, 1);
         p2 = pack_fst(c, *m2, 2);
         *out = compose_packed(c, *p1, *p2, o, stats);
-    });
+    }, cuda_stream, true);
     free_packed(p1);
     free_packed(p2);
     return rc;

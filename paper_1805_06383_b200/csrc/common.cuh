@@ -53,11 +53,19 @@ void arena_release_all();
 void *persist_alloc(size_t bytes, cudaStream_t stream);   // null when device memory is out
 void persist_free(void *p, cudaStream_t stream);
 void persist_release_all();
+void release_caches(cudaStream_t stream);                 // out of memory: everything the library caches goes back to the driver
+
+struct AllocHooks {           // fstc_opts_t's allocator hooks (both set or both null)
+    void *(*alloc)(size_t, void *, void *) = nullptr;
+    void (*dealloc)(void *, void *, void *) = nullptr;
+    void *ctx = nullptr;
+};
 
 struct Ctx {
     cudaStream_t stream = nullptr;
     int n_sm = 148;
     int64_t n_launch = 0;
+    AllocHooks hooks;         // set: all device memory of the call comes from the caller
 
     // persistent: the block outlives the call (a result or packed array): a pool allocation of its own
     void *alloc_bytes(size_t bytes, bool persistent = false) {
@@ -67,7 +75,14 @@ struct Ctx {
         timespec t0, t1;
         if (trace) clock_gettime(CLOCK_MONOTONIC, &t0);
         cudaError_t e = cudaSuccess;
-        p = persistent ? persist_alloc(bytes, stream) : arena_alloc(bytes, stream);
+        if (hooks.alloc) p = hooks.alloc(bytes, stream, hooks.ctx);
+        else {
+            p = persistent ? persist_alloc(bytes, stream) : arena_alloc(bytes, stream);
+            if (!p) {             // the arena, the parked blocks and the pool each cache memory the other could use: all back, once
+                release_caches(stream);
+                p = persistent ? persist_alloc(bytes, stream) : arena_alloc(bytes, stream);
+            }
+        }
         if (!p) e = cudaErrorMemoryAllocation;
         if (trace && bytes >= (64u << 20)) {
             clock_gettime(CLOCK_MONOTONIC, &t1);
@@ -86,7 +101,8 @@ struct Ctx {
         static const bool trace = getenv("FSTC_ALLOC_TRACE") != nullptr;
         timespec t0, t1;
         if (trace) clock_gettime(CLOCK_MONOTONIC, &t0);
-        if (!arena_free(p)) persist_free(p, stream);
+        if (hooks.dealloc) hooks.dealloc(p, stream, hooks.ctx);
+        else if (!arena_free(p)) persist_free(p, stream);
         if (trace) {
             clock_gettime(CLOCK_MONOTONIC, &t1);
             const double ms = (t1.tv_sec - t0.tv_sec) * 1e3 + (t1.tv_nsec - t0.tv_nsec) * 1e-6;

@@ -22,6 +22,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <ctime>
+#include <mutex>
 
 #include "internal.h"
 #include "scan.cuh"
@@ -833,13 +834,15 @@ __global__ void k_place_grouped(const uint32_t *__restrict__ mab, const int32_t 
                                 const int64_t *__restrict__ foff, int64_t arc_base, int64_t f_lo,
                                 const uint32_t *__restrict__ sel, int bits_b, int32_t *__restrict__ o_src,
                                 int32_t *__restrict__ o_il, int32_t *__restrict__ o_ol, int32_t *__restrict__ o_tgt,
-                                float *__restrict__ o_w) {
+                                float *__restrict__ o_w, int64_t n0 = 0, int64_t n1 = 0, const uint32_t *__restrict__ rank = nullptr) {
     int64_t j = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (j >= n_merged) return;
     const uint32_t p = msrc[j], ab = mab[j];
     const int64_t q = arc_base + foff[p] + (j - mstart[p]);
     o_src[q] = static_cast<int>(f_lo + (sel ? sel[p] : p));
-    o_tgt[q] = mtgt[j];
+    int64_t t = mtgt[j];
+    if (rank && t >= n0 && t < n1) t = n0 + rank[t - n0];        // deterministic ids
+    o_tgt[q] = static_cast<int32_t>(t);
     o_il[q] = static_cast<int>(ab >> bits_b);
     o_ol[q] = static_cast<int>(ab & ((1u << bits_b) - 1u));
     o_w[q] = mw[j];
@@ -995,6 +998,66 @@ k_assemble_scatter(const int2 *__restrict__ pair, int64_t n, const uint32_t *__r
     }
 }
 
+// ------------------------------------------------------------------------------------------ deterministic ids
+// fstc_opts_t.deterministic: the states a level creates get their ids in ascending order of the pair key (the set a level
+// creates does not depend on thread scheduling, only the order the threads win their slots in does).  After the level: sort
+// the new keys, rank[old id - n0] = position, rewrite pair[], remap the target column of the level's arcs and the ids in
+// the visited table.  Arcs of sources that went through sort + reduce are sorted again on the new ids.
+__global__ void k_det_keys(const int2 *__restrict__ pair, int64_t n0, int64_t n, uint64_t nq2, uint4 *__restrict__ rec) {
+    const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int2 p = pair[n0 + i];
+    const uint64_t key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
+    rec[i] = make_uint4(static_cast<uint32_t>(key), static_cast<uint32_t>(key >> 32), 0u, static_cast<uint32_t>(i));
+}
+__global__ void k_det_apply(const uint4 *__restrict__ sorted, int64_t n0, int64_t n, uint64_t nq2, int2 *__restrict__ pair,
+                            uint32_t *__restrict__ rank) {
+    const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint4 r = sorted[i];
+    const uint64_t key = (static_cast<uint64_t>(r.y) << 32) | r.x;
+    const uint64_t q1 = key / nq2;
+    rank[r.w] = static_cast<uint32_t>(i);
+    pair[n0 + i] = make_int2(static_cast<int>(q1), static_cast<int>(key - q1 * nq2));
+}
+__global__ void k_det_remap(int32_t *__restrict__ tgt, int64_t n, int64_t n0, int64_t n1, const uint32_t *__restrict__ rank) {
+    const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int64_t t = tgt[i];
+    if (t >= n0 && t < n1) tgt[i] = static_cast<int32_t>(n0 + rank[t - n0]);
+}
+__global__ void k_det_table(const int2 *__restrict__ pair, int64_t n0, int64_t n, uint64_t nq2, uint32_t *__restrict__ dense,
+                            uint4 *__restrict__ table, uint64_t cap) {
+    const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int2 p = pair[n0 + i];
+    const unsigned long long key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
+    if (dense) { dense[key] = static_cast<uint32_t>(n0 + i) + 1u; return; }
+    uint64_t s = 2 * home_bucket(key, cap);                      // the key is in the table: walk its probe path
+    while (slot_key(table[s]) != key) s = (s + 1 == cap) ? 0 : s + 1;
+    reinterpret_cast<uint32_t *>(table + s)[2] = static_cast<uint32_t>(n0 + i);
+}
+// sort records of the merged class-F arcs with their NEW target ids: {key = tgt << shift_t | a << bits_b | b, pair index, weight}
+__global__ void k_det_frec(const unsigned long long *__restrict__ mkey, const uint32_t *__restrict__ msrc, const float *__restrict__ mw,
+                           int64_t n, int shift_t, int64_t n0, int64_t n1, const uint32_t *__restrict__ rank, uint4 *__restrict__ rec) {
+    const int64_t j = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    unsigned long long k = mkey[j];
+    int64_t t = static_cast<int64_t>(k >> shift_t);
+    if (t >= n0 && t < n1) t = n0 + rank[t - n0];
+    k = (static_cast<unsigned long long>(t) << shift_t) | (k & ((1ull << shift_t) - 1));
+    rec[j] = make_uint4(static_cast<uint32_t>(k), static_cast<uint32_t>(k >> 32), msrc[j], __float_as_uint(mw[j]));
+}
+__global__ void k_det_funpack(const uint4 *__restrict__ rec, int64_t n, unsigned long long *__restrict__ mkey, uint32_t *__restrict__ msrc,
+                              float *__restrict__ mw) {
+    const int64_t j = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const uint4 r = rec[j];
+    mkey[j] = (static_cast<unsigned long long>(r.y) << 32) | r.x;
+    msrc[j] = r.z;
+    mw[j] = __uint_as_float(r.w);
+}
+
 // Level compaction: when rule T will clearly cut the level, only the pairs below a key limit are worked on.
 __global__ void k_flag_below(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, uint64_t nq2, uint64_t key_limit,
                              uint8_t *__restrict__ flag) {
@@ -1053,6 +1116,84 @@ struct Composer {
     // growing outputs
     DBuf<int2> pair; int64_t pair_cap = 0;
     DBuf<int32_t> a_src, a_il, a_ol, a_tgt; DBuf<float> a_w; int64_t arc_cap = 0;
+    // what the kernels index with ABSOLUTE arc positions: the arrays above, or (host spill without a device copy) the
+    // arrays of the current level shifted back by the level's first position
+    int32_t *o_src = nullptr, *o_il = nullptr, *o_ol = nullptr, *o_tgt = nullptr; float *o_w = nullptr;
+    // ---- host spill (fstc_spill_t): finished levels go to pinned host memory on a second stream while the next level runs
+    const fstc_spill_t *sp = nullptr;
+    bool spill_only = false;             // keep_device = 0: the arcs of a level leave the device when their copy is done
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_main = nullptr;
+    struct LevelArcs { DBuf<int32_t> src, il, ol, tgt; DBuf<float> w; cudaEvent_t done = nullptr; };
+    std::vector<LevelArcs> inflight;     // level arrays whose copy may still run
+    LevelArcs cur;                       // spill_only: the arrays of the level being expanded
+    int64_t spilled_states = 0;
+
+    ~Composer() {
+        if (side) {                      // on every way out: no copy may still read a buffer the members are about to release
+            (void)cudaStreamSynchronize(side);
+            for (auto &l : inflight) if (l.done) (void)cudaEventDestroy(l.done);
+            if (ev_main) (void)cudaEventDestroy(ev_main);
+            (void)cudaStreamDestroy(side);
+        }
+    }
+    void spill_begin() {
+        sp = o.spill;
+        if (!sp) return;
+        const fstc_host_result_t *hr = sp->host;
+        if (!hr || !hr->pair || !hr->src || !hr->ilabel || !hr->olabel || !hr->tgt || !hr->weight || sp->arc_capacity < 0 || sp->state_capacity < 1)
+            fail(FSTC_ERR_ARG, "spill: host arrays missing");
+        spill_only = sp->keep_device == 0;
+        FSTC_CUDA(cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking));
+        FSTC_CUDA(cudaEventCreateWithFlags(&ev_main, cudaEventDisableTiming));
+    }
+    void spill_reap(bool all) {          // level arrays whose copy is complete go back to the workspace
+        for (size_t i = 0; i < inflight.size();) {
+            if (all) FSTC_CUDA(cudaEventSynchronize(inflight[i].done));
+            if (all || cudaEventQuery(inflight[i].done) == cudaSuccess) {
+                (void)cudaEventDestroy(inflight[i].done);
+                inflight.erase(inflight.begin() + i);
+            } else { (void)cudaGetLastError(); ++i; }
+        }
+    }
+    // spill_only: device arrays for the `r` arcs (at most) of the level that starts at arc position `base`
+    void spill_level_arrays(int64_t base, int64_t r) {
+        spill_reap(false);
+        const int64_t pad = base & 3, n = r + pad + 4;           // keeps the kernels' 16-byte stores aligned
+        cur = LevelArcs();
+        cur.src.alloc(c, n); cur.il.alloc(c, n); cur.ol.alloc(c, n); cur.tgt.alloc(c, n); cur.w.alloc(c, n);
+        o_src = cur.src.p + pad - base; o_il = cur.il.p + pad - base; o_ol = cur.ol.p + pad - base;
+        o_tgt = cur.tgt.p + pad - base; o_w = cur.w.p + pad - base;
+    }
+    // the level is placed: arcs [a0, a1) and states [s0, s1) are final
+    void spill_level(int64_t a0, int64_t a1, int64_t s1) {
+        if (!sp) return;
+        if (a1 > sp->arc_capacity || s1 > sp->state_capacity)
+            fail(FSTC_ERR_CAPACITY, "spill: the result (%lld arcs, %lld states so far) outgrows the host arrays", static_cast<long long>(a1), static_cast<long long>(s1));
+        FSTC_CUDA(cudaEventRecord(ev_main, c.stream));
+        FSTC_CUDA(cudaStreamWaitEvent(side, ev_main, 0));
+        const fstc_host_result_t *hr = sp->host;
+        const size_t nb = sizeof(int32_t) * static_cast<size_t>(a1 - a0);
+        if (a1 > a0) {
+            FSTC_CUDA(cudaMemcpyAsync(hr->src + a0, o_src + a0, nb, cudaMemcpyDeviceToHost, side));
+            FSTC_CUDA(cudaMemcpyAsync(hr->ilabel + a0, o_il + a0, nb, cudaMemcpyDeviceToHost, side));
+            FSTC_CUDA(cudaMemcpyAsync(hr->olabel + a0, o_ol + a0, nb, cudaMemcpyDeviceToHost, side));
+            FSTC_CUDA(cudaMemcpyAsync(hr->tgt + a0, o_tgt + a0, nb, cudaMemcpyDeviceToHost, side));
+            FSTC_CUDA(cudaMemcpyAsync(hr->weight + a0, o_w + a0, nb, cudaMemcpyDeviceToHost, side));
+        }
+        if (s1 > spilled_states)
+            FSTC_CUDA(cudaMemcpyAsync(hr->pair + 2 * spilled_states, pair.p + spilled_states, sizeof(int2) * static_cast<size_t>(s1 - spilled_states),
+                                      cudaMemcpyDeviceToHost, side));
+        st.spill_bytes += 5 * static_cast<int64_t>(nb) + 8 * (s1 - spilled_states);
+        spilled_states = s1;
+        if (spill_only) {
+            st.spill_bytes_saved += 5 * static_cast<int64_t>(nb);
+            FSTC_CUDA(cudaEventCreateWithFlags(&cur.done, cudaEventDisableTiming));
+            FSTC_CUDA(cudaEventRecord(cur.done, side));
+            inflight.push_back(std::move(cur));
+            cur = LevelArcs();
+        }
+    }
     int64_t n_arcs = 0, n_states = 0;
     // visited table
     DBuf<uint4> table; uint64_t cap = 0;
@@ -1060,9 +1201,17 @@ struct Composer {
     uint64_t n_pairs_all = 0;
     DBuf<unsigned long long> d_counters;   // [0] n_states, [1] seg visited, [2] match arcs, [3] n_selected, [4..259] hist
 
+    // test / debugging knobs from the environment, read once per call
+    int knob_resolve_bits = -1;          // FSTC_RESOLVE_BITS: hash bits of the partitioned resolve
+    bool knob_no_group = false;          // FSTC_NO_GROUP_MERGE: class G off
+    double knob_limit_margin = 1.5;      // FSTC_KEY_LIMIT_MARGIN: the guessed key limit of a level that will be cut
+
     Composer(Ctx &ctx, const fstc_packed_t &a, const fstc_packed_t &b, const fstc_opts_t &opts)
         : c(ctx), m1(a), m2(b), o(opts), tm(ctx, opts.profile != 0), nq2(static_cast<uint64_t>(b.n_states)) {
         std::memset(&st, 0, sizeof st);
+        if (const char *e = getenv("FSTC_RESOLVE_BITS")) knob_resolve_bits = atoi(e);
+        knob_no_group = getenv("FSTC_NO_GROUP_MERGE") != nullptr;
+        if (const char *e = getenv("FSTC_KEY_LIMIT_MARGIN")) knob_limit_margin = atof(e);
     }
 
     // Growable outputs and table.  `need` is what the coming launch requires; `want` >= need is a look-ahead
@@ -1079,9 +1228,11 @@ struct Composer {
     void ensure_pairs(int64_t need, int64_t want = 0) {
         if (need <= pair_cap) return;
         grow_to(need, std::max(want, pair_cap * 2), [&](int64_t nc) {
+            if (side) FSTC_CUDA(cudaStreamSynchronize(side));     // a copy to the host may still read the old block
             DBuf<int2> np(c, nc, true);
-            if (n_states > 0)
-                FSTC_CUDA(cudaMemcpyAsync(np.p, pair.p, sizeof(int2) * n_states, cudaMemcpyDeviceToDevice, c.stream));
+            const int64_t keep = std::max(n_states, n_states_live);  // (states appended inside the level, external resolve)
+            if (keep > 0 && pair.p)
+                FSTC_CUDA(cudaMemcpyAsync(np.p, pair.p, sizeof(int2) * keep, cudaMemcpyDeviceToDevice, c.stream));
             pair = std::move(np);
             pair_cap = nc;
         });
@@ -1089,7 +1240,9 @@ struct Composer {
     }
 
     void ensure_arcs(int64_t need, int64_t want = 0) {
+        if (spill_only) return;                                  // level arrays instead (spill_level_arrays)
         if (need <= arc_cap) return;
+        if (side) FSTC_CUDA(cudaStreamSynchronize(side));         // a copy to the host may still read the old arrays
         int h = tm.begin(FSTC_T_ASSEMBLE);
         grow_to(need, std::max(want, arc_cap + arc_cap / 2), [&](int64_t nc) {
             nc = (nc + 3) & ~int64_t(3);
@@ -1106,6 +1259,7 @@ struct Composer {
             a_src = std::move(n_src); a_il = std::move(n_il); a_ol = std::move(n_ol); a_tgt = std::move(n_tgt);
             a_w = std::move(n_w);
             arc_cap = nc;
+            o_src = a_src.p; o_il = a_il.p; o_ol = a_ol.p; o_tgt = a_tgt.p; o_w = a_w.p;
         });
         if (n_arcs > 0) st.n_grow += 1;
         tm.end(h);
@@ -1147,11 +1301,44 @@ struct Composer {
         tm.end(h);
     }
 
-    // several device scalars, one synchronisation
-    void read_scalars(std::initializer_list<std::pair<const int64_t *, int64_t *>> items) {
-        for (auto &it : items)
-            FSTC_CUDA(cudaMemcpyAsync(it.second, it.first, sizeof(int64_t), cudaMemcpyDeviceToHost, c.stream));
-        c.sync();
+    // ---- FSTC_RESOLVE_EXTERNAL: the caller's callback resolves target keys to global ids (one composition sharded by key
+    // ownership); pair[] holds the states this rank owns, in the order the callback announced them
+    bool external = false;
+    int cur_level = 0, ext_next_call = 0;
+    int32_t ext_more = 0;
+    int ext_q2_bits = 0;
+    void ext_call(const ResolveJob &j, int call) {
+        DBuf<int32_t> ids(c, j.n_records);
+        c.sync();                                                // the keys are complete; the callback works on its own stream
+        const int32_t *new_pairs = nullptr;
+        int64_t n_new = 0;
+        int32_t more = 0;
+        const int rc = o.resolve_cb(o.resolve_ctx, cur_level, call, ext_q2_bits, j.keys, j.n_records, ids.p, &new_pairs, &n_new, &more);
+        if (rc != 0) fail(FSTC_ERR_CALLBACK, "resolve_cb returned %d (level %d, call %d)", rc, cur_level, call);
+        if (n_new < 0 || (n_new > 0 && !new_pairs)) fail(FSTC_ERR_CALLBACK, "resolve_cb: bad new_pairs");
+        if (n_new > 0) {
+            if (n_states_live + n_new >= 0x7FFFFFFFll) fail(FSTC_ERR_CAPACITY, "more than 2^31-1 states");
+            ensure_pairs(n_states_live + n_new);
+            FSTC_CUDA(cudaMemcpyAsync(pair.p + n_states_live, new_pairs, sizeof(int2) * static_cast<size_t>(n_new), cudaMemcpyDeviceToDevice, c.stream));
+            c.sync();
+            n_states_live += n_new;
+        }
+        if (call == 2) ext_more = more;
+        resolve_apply_ids(c, j, reinterpret_cast<const uint32_t *>(ids.p));
+    }
+    // the ids of a list of target keys: the partitioned resolve, or the caller's (always calls 0, 1, 2 of a level in order)
+    void run_resolve(const ResolveJob &j, int call) {
+        if (external) {
+            for (; ext_next_call < call; ++ext_next_call) { ResolveJob e{}; ext_call(e, ext_next_call); }
+            ext_call(j, call);
+            ext_next_call = call + 1;
+        } else resolve_partitioned(c, j);
+        st.n_resolve += 1;
+        st.n_resolved_arcs += j.n_records;
+    }
+    void ext_finish_level() {
+        for (; ext_next_call < 3; ++ext_next_call) { ResolveJob e{}; ext_call(e, ext_next_call); }
+        ext_next_call = 0;
     }
 
     // partitioned = true: the level's target ids come from resolve_partitioned (no visited table)
@@ -1162,7 +1349,7 @@ struct Composer {
 
     void launch_emit(int mode, const MatchList &L, int64_t n_matches, int64_t R, int64_t pos_base, int64_t f_lo,
                      const int64_t *foff, const int64_t *roff, int64_t arc_base, uint4 *sortrec, int shift_t, int bits_b) {
-        if (R <= 0) return;
+        if (R <= 0) return;                                      // (external resolve: ext_finish_level makes the empty calls)
         const int64_t tile0 = (pos_base / EM_TILE) * EM_TILE;
         const int64_t n_tiles = ceil_div(pos_base + R - tile0, EM_TILE);
         DBuf<int64_t> tile_m(c, n_tiles + 1);
@@ -1174,7 +1361,7 @@ struct Composer {
         g.L = L; g.n_matches = n_matches; g.R = R; g.pos_base = pos_base; g.f_lo = f_lo; g.sel = cur_sel;
         g.foff = foff; g.roff = roff; g.arc_base = arc_base; g.nq2 = nq2;
         g.table = table.p; g.cap = cap; g.dense = dense.p; g.n_states = d_counters.p; g.pair = pair.p;
-        g.o_src = a_src.p; g.o_il = a_il.p; g.o_ol = a_ol.p; g.o_tgt = a_tgt.p; g.o_w = a_w.p;
+        g.o_src = o_src; g.o_il = o_il; g.o_ol = o_ol; g.o_tgt = o_tgt; g.o_w = o_w;
         g.sortrec = sortrec; g.shift_t = shift_t; g.bits_b = bits_b; g.tile_m = tile_m.p;
         g.keys = nullptr; g.posout = nullptr;
         g.q2_bits = bits_for(nq2 > 1 ? nq2 - 1 : 1);
@@ -1209,17 +1396,41 @@ struct Composer {
             j.n_states = d_counters.p;
             j.mode = mode == EMIT_DIRECT ? 0 : (mode == EMIT_INDIRECT ? 1 : 2);
             j.pos = posout.p;
-            j.o_tgt = mode == EMIT_SORTREC ? nullptr : a_tgt.p + (mode == EMIT_DIRECT ? pos_base : arc_base);
+            j.o_tgt = mode == EMIT_SORTREC ? nullptr : o_tgt + (mode == EMIT_DIRECT ? pos_base : arc_base);
             j.sortrec = mode == EMIT_SORTREC ? sortrec : nullptr;
             j.shift_t = shift_t;
-            j.force_bits = -1;
+            j.force_bits = knob_resolve_bits;
             j.stats = &st;
             j.profile = o.profile != 0;
-            if (const char *e = getenv("FSTC_RESOLVE_BITS")) j.force_bits = atoi(e);   // test knob: force multi-pass
-            resolve_partitioned(c, j);
-            st.n_resolve += 1;
-            st.n_resolved_arcs += R;
+            run_resolve(j, mode == EMIT_SORTREC ? 0 : 2);
         }
+    }
+
+    // deterministic ids (see k_det_keys): the states [n0, n1) the level created, renumbered by ascending key; the target
+    // column of the arcs [a0, a1) already written, and the table, follow.  Returns the rank array (old id - n0 -> position).
+    DBuf<uint32_t> det_renumber(int64_t n0, int64_t n1, int64_t a0, int64_t a1) {
+        const int64_t n = n1 - n0;
+        DBuf<uint32_t> rank(c, n);
+        if (n <= 0) return rank;
+        const int h = tm.begin(FSTC_T_TABLE);
+        DBuf<uint4> ra(c, n), rb(c, n);
+        k_det_keys<<<nblk(n), CT_THREADS, 0, c.stream>>>(pair.p, n0, n, nq2, ra.p);
+        FSTC_LAUNCH_CHECK();
+        uint4 *sorted = radix_sort_records(c, ra.p, rb.p, n, make_sort_passes(key_bits, 0));
+        k_det_apply<<<nblk(n), CT_THREADS, 0, c.stream>>>(sorted, n0, n, nq2, pair.p, rank.p);
+        FSTC_LAUNCH_CHECK();
+        if (a1 > a0) {
+            k_det_remap<<<nblk(a1 - a0), CT_THREADS, 0, c.stream>>>(o_tgt + a0, a1 - a0, n0, n1, rank.p);
+            FSTC_LAUNCH_CHECK();
+        }
+        if (!partitioned && (dense.p || table.p)) {
+            k_det_table<<<nblk(n), CT_THREADS, 0, c.stream>>>(pair.p, n0, n, nq2, dense.p, table.p, cap);
+            FSTC_LAUNCH_CHECK();
+        }
+        c.n_launch += 4;
+        tm.end(h);
+        c.sync();                                                // ra / rb go out of scope
+        return rank;
     }
 
     fstc_result_t *run();
@@ -1229,8 +1440,12 @@ fstc_result_t *Composer::run() {
     if (m1.side != 1 || m2.side != 2) fail(FSTC_ERR_ARG, "operands must be packed with side 1 (left) and side 2 (right)");
     if (m1.n_inner != m2.n_inner)
         fail(FSTC_ERR_ARG, "inner alphabets differ: |Γ| = %d vs %d (PAPER.md:45)", m1.n_inner, m2.n_inner);
-    if (o.merge_mode < 0 || o.merge_mode > 2 || o.max_levels < 0 || o.max_raw_arcs < 0 || o.resolve_mode < 0 || o.resolve_mode > 3)
+    if (o.merge_mode < 0 || o.merge_mode > 2 || o.max_levels < 0 || o.max_raw_arcs < 0 || o.resolve_mode < 0 || o.resolve_mode > 4)
         fail(FSTC_ERR_ARG, "bad options");
+    external = o.resolve_mode == FSTC_RESOLVE_EXTERNAL;
+    if (external && (!o.resolve_cb || o.max_raw_arcs != 0 || o.deterministic || o.spill))
+        fail(FSTC_ERR_ARG, "FSTC_RESOLVE_EXTERNAL needs resolve_cb and takes no max_raw_arcs, deterministic or spill");
+    ext_q2_bits = bits_for(nq2 > 1 ? nq2 - 1 : 1);
     const int bits_a = bits_for(m1.n_outer > 0 ? m1.n_outer - 1 : 0), bits_b = bits_for(m2.n_outer > 0 ? m2.n_outer - 1 : 0);
     const int shift_t = bits_a + bits_b;
     const uint64_t n_pairs_total = static_cast<uint64_t>(m1.n_states) * nq2;
@@ -1240,7 +1455,7 @@ fstc_result_t *Composer::run() {
                         (((m1.any_flags & FLAG_D) && (m2.any_flags & FLAG_D)) || (m1.any_flags & FLAG_X) || (m2.any_flags & FLAG_X)));
     key_bits = bits_for(n_pairs_total - 1);
     // class G (merge by construction) replaces sort + reduce for the pairs it suits; FSTC_MERGE_SORT_ALL keeps the sort
-    const bool has_G = has_F && o.merge_mode == FSTC_MERGE_AUTO && getenv("FSTC_NO_GROUP_MERGE") == nullptr;
+    const bool has_G = has_F && o.merge_mode == FSTC_MERGE_AUTO && !knob_no_group;
     n_pairs_all = n_pairs_total;
     use_dense = o.resolve_mode != FSTC_RESOLVE_HASH && n_pairs_total <= DENSE_MAX_PAIRS;
 
@@ -1257,13 +1472,18 @@ fstc_result_t *Composer::run() {
         if (ms - ht_last > 3.0) fprintf(stderr, "[fstc host] level %d %-12s at %8.2f ms (+%.2f)\n", level, what, ms, ms - ht_last);
         ht_last = ms;
     };
-    cudaEvent_t ev0, ev1;
-    FSTC_CUDA(cudaEventCreate(&ev0));
-    FSTC_CUDA(cudaEventCreate(&ev1));
+    struct EventPair {                                           // released on every way out, errors included
+        cudaEvent_t a = nullptr, b = nullptr;
+        ~EventPair() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); }
+    } evp;
+    FSTC_CUDA(cudaEventCreate(&evp.a));
+    FSTC_CUDA(cudaEventCreate(&evp.b));
+    const cudaEvent_t ev0 = evp.a, ev1 = evp.b;
     FSTC_CUDA(cudaEventRecord(ev0, c.stream));
 
     d_counters.alloc(c, 4 + 256);
     FSTC_CUDA(cudaMemsetAsync(d_counters.p, 0, sizeof(unsigned long long) * (4 + 256), c.stream));
+    spill_begin();
 
     // ---- init (Alg. 2 lines 1-3): state 0 = (s1, s2)
     ensure_pairs(std::max<int64_t>(o.state_capacity_hint, 1024));
@@ -1274,10 +1494,14 @@ fstc_result_t *Composer::run() {
         unsigned long long one = 1;
         FSTC_CUDA(cudaMemcpyAsync(d_counters.p, &one, sizeof one, cudaMemcpyHostToDevice, c.stream));
         n_states = 1;
-        ensure_table(std::max<int64_t>(o.state_capacity_hint, 1));
+        if (external) {                                          // no table; the start pair is local state 0 of its owner only
+            partitioned = true;
+            if (!o.owns_start) n_states = 0;
+            n_states_live = n_states;
+        } else ensure_table(std::max<int64_t>(o.state_capacity_hint, 1));
     }
 
-    int64_t f_lo = 0, f_hi = 1, cum_raw = 0;
+    int64_t f_lo = 0, f_hi = n_states, cum_raw = 0;
     int last_mode = 1;           // how the last frontier [f_lo, f_hi) was treated: 0 not expanded, 1 all, 2 cut
     uint64_t cut_key = 0;
     int64_t last_lo = 0, last_hi = 1;
@@ -1287,7 +1511,18 @@ fstc_result_t *Composer::run() {
 
     for (;; ++lvl) {
         const int64_t nf_all = f_hi - f_lo;                      // the frontier
-        if (nf_all == 0) break;
+        cur_level = lvl;
+        if (external) {
+            // the search ends when NO rank created a state; a rank without a frontier still takes part in the exchange
+            if (lvl > 0 && !ext_more) break;
+            if (o.max_levels > 0 && lvl == o.max_levels) { st.truncated = 1; last_lo = f_lo; last_hi = f_hi; last_mode = 0; break; }
+            if (nf_all == 0) {
+                ext_finish_level();
+                if (lvl < FSTC_MAX_LEVEL_STATS) { st.level_frontier[lvl] = 0; st.level_raw[lvl] = 0; st.level_new_states[lvl] = n_states_live - n_states; }
+                n_states = n_states_live; f_lo = f_hi; f_hi = n_states; st.n_levels = lvl + 1;
+                continue;
+            }
+        } else if (nf_all == 0) break;
         int64_t nf = nf_all;                                     // the pairs of it this level works on (see `sel`)
         last_lo = f_lo; last_hi = f_hi;
         if (o.max_levels > 0 && lvl == o.max_levels) { st.truncated = 1; last_mode = 0; break; }
@@ -1327,8 +1562,7 @@ fstc_result_t *Composer::run() {
             const double remaining = static_cast<double>(o.max_raw_arcs - cum_raw);
             const double predicted = static_cast<double>(nf) * last_fan;
             if (predicted > 4.0 * remaining) {
-                double margin = 1.5;                                 // test knob: a margin < 1 forces the widening path
-                if (const char *e = getenv("FSTC_KEY_LIMIT_MARGIN")) margin = atof(e);
+                const double margin = knob_limit_margin;             // test knob: a margin < 1 forces the widening path
                 key_limit = static_cast<uint64_t>(static_cast<double>(n_pairs_total) * (margin * remaining / predicted)) + 1;
             }
         }
@@ -1394,7 +1628,7 @@ fstc_result_t *Composer::run() {
                     if (before + hist[d] > remaining) break;
                     before += hist[d];
                 }
-                if (d == 256) fail(FSTC_ERR_CUDA, "internal: budget cut not found");
+                if (d == 256) fail(FSTC_ERR_INTERNAL, "budget cut not found (the level's counts changed under the search)");
                 prefix = (prefix << 8) | static_cast<uint64_t>(d);
             }
             cut_key = prefix;
@@ -1416,7 +1650,7 @@ fstc_result_t *Composer::run() {
         cur_sel = sel.p;
         // ---- capacities for this level
         const uint64_t remaining_pairs = n_pairs_total - static_cast<uint64_t>(n_states);
-        const int64_t new_bound = static_cast<int64_t>(std::min<uint64_t>(static_cast<uint64_t>(R), remaining_pairs));
+        const int64_t new_bound = external ? 0 : static_cast<int64_t>(std::min<uint64_t>(static_cast<uint64_t>(R), remaining_pairs));
         if (n_states + new_bound >= 0x7FFFFFFFll) fail(FSTC_ERR_CAPACITY, "more than 2^31-1 states");
         // ---- how this level resolves its target ids, decided per level from measured unit costs: the
         // visited table pays a random DRAM read per arc and a random write-back + publish per NEW state (and a rebuild
@@ -1425,6 +1659,11 @@ fstc_result_t *Composer::run() {
         auto prefer_partitioned = [&](int64_t r, int64_t bound, int64_t states_now, uint64_t slots_ready) {
             if (o.resolve_mode == FSTC_RESOLVE_TABLE || o.resolve_mode == FSTC_RESOLVE_HASH) return false;
             if (rkey_bits + bits_for(static_cast<uint64_t>(states_now + bound)) > 64) return false;  // state records: key << id_bits | id
+            if (!resolve_can_take(r, states_now)) {                  // u32 record indices, at most 2^20 bins
+                if (o.resolve_mode == FSTC_RESOLVE_PARTITIONED)
+                    fail(FSTC_ERR_CAPACITY, "a level of %lld arcs and %lld states is beyond the partitioned resolve", static_cast<long long>(r), static_cast<long long>(states_now));
+                return false;
+            }
             if (o.resolve_mode == FSTC_RESOLVE_PARTITIONED) return true;
             const uint64_t slots = use_dense ? n_pairs_all : slots_for(states_now + bound);
             const uint64_t table_bytes = slots * (use_dense ? sizeof(uint32_t) : sizeof(uint4));
@@ -1437,25 +1676,32 @@ fstc_result_t *Composer::run() {
             return t_part < 0.6 * t_table;
         };
         {
-            const bool want = prefer_partitioned(R, new_bound, n_states, use_dense ? (dense.p ? n_pairs_all : 0) : cap);
+            const bool want = external || prefer_partitioned(R, new_bound, n_states, use_dense ? (dense.p ? n_pairs_all : 0) : cap);
             if (want && !partitioned) { table = DBuf<uint4>(); cap = 0; dense = DBuf<uint32_t>(); }    // the table is dropped; ensure_table rebuilds it from pair[]
             partitioned = want;
         }
         // look-ahead: if the search goes on, the next level is about (new states) x (arcs per expanded pair)
         int64_t next_R = 0, next_S = 0;
         const bool must_grow = n_states + new_bound > pair_cap || (!partitioned && (use_dense ? dense.p == nullptr : slots_for(n_states + new_bound) > cap)) ||
-                               n_arcs + R > arc_cap;
+                               (!spill_only && n_arcs + R > arc_cap);
         if (must_grow && !stop_after && n_sel > 0 && R > 0) {
             const double fan = static_cast<double>(R) / static_cast<double>(n_sel);
             double pr = static_cast<double>(new_bound) * fan;
             if (o.max_raw_arcs > 0) pr = std::min(pr, static_cast<double>(o.max_raw_arcs - cum_raw - R));
             // what is free for us: the device's memory minus what our pool has handed out.  (cudaMemGetInfo would say it
             // exactly, but it goes to the driver and was seen to take 10-50 ms at times: the device size is read once.)
-            static size_t device_bytes = 0;
-            if (device_bytes == 0) {
-                size_t f = 0, t = 0;
-                (void)cudaMemGetInfo(&f, &t);
-                device_bytes = t > 0 ? t - t / 16 : size_t(64) << 30;            // leave 1/16 to others on the device
+            static std::mutex mu;
+            static size_t device_bytes_of[64] = {};
+            size_t device_bytes;
+            {
+                std::lock_guard<std::mutex> lk(mu);
+                size_t &slot = device_bytes_of[m1.device & 63];
+                if (slot == 0) {
+                    size_t f = 0, t = 0;
+                    (void)cudaMemGetInfo(&f, &t);
+                    slot = t > 0 ? t - t / 16 : size_t(64) << 30;                // leave 1/16 to others on the device
+                }
+                device_bytes = slot;
             }
             uint64_t pool_used = 0;
             (void)cudaMemPoolGetAttribute(device_pool(), cudaMemPoolAttrUsedMemCurrent, &pool_used);
@@ -1478,6 +1724,7 @@ fstc_result_t *Composer::run() {
             ensure_table(n_states + new_bound, next_partitioned ? 0 : n_states + new_bound + next_S);
         }
         ensure_arcs(n_arcs + R, n_arcs + R + next_R);
+        if (spill_only) spill_level_arrays(n_arcs, R);
         n_states_live = n_states;
         hostmark("ensure", lvl);
 
@@ -1503,6 +1750,7 @@ fstc_result_t *Composer::run() {
             // no source of this level can hold duplicates: arcs go straight to their final place
             launch_emit(EMIT_DIRECT, LU, MU, RU, arc_base, f_lo, nullptr, nullptr, 0, nullptr, 0, 0);
             n_arcs += RU;
+            if (o.deterministic) det_renumber(n_states, static_cast<int64_t>(read_scalar(c, d_counters.p)), arc_base, n_arcs);
         } else {
             if (shift_t > 32) fail(FSTC_ERR_CAPACITY, "bits(|Σ|)+bits(|Δ|) = %d > 32: merge key does not fit 64 bits", shift_t);
             // ---- class F: sort + reduce
@@ -1516,8 +1764,8 @@ fstc_result_t *Composer::run() {
                 sa.alloc(c, RF); sb.alloc(c, RF);
                 launch_emit(EMIT_SORTREC, LF, MF, RF, 0, f_lo, nullptr, nullptr, 0, sa.p, shift_t, bits_b);
                 // target ids are now known: n_states bounds them
-                const int64_t ns_now = static_cast<int64_t>(read_scalar(c, d_counters.p));
-                n_states_live = ns_now;
+                const int64_t ns_now = external ? 0x7FFFFFFFll : static_cast<int64_t>(read_scalar(c, d_counters.p));   // external: global ids
+                if (!external) n_states_live = ns_now;
                 const int tgt_bits = bits_for(static_cast<uint64_t>(ns_now - 1));
                 h = tm.begin(FSTC_T_SORT);
                 uint4 *sorted = radix_sort_records(c, sa.p, sb.p, RF, make_sort_passes(shift_t + tgt_bits, bits_for(static_cast<uint64_t>(nf - 1))));
@@ -1587,12 +1835,9 @@ fstc_result_t *Composer::run() {
                         j.key_bits = g.q2_bits + bits_for(static_cast<uint64_t>(m1.n_states > 1 ? m1.n_states - 1 : 1));
                         j.pair = pair.p; j.n_states_before = n_states_live; j.n_states = d_counters.p;
                         j.mode = 0; j.pos = nullptr; j.o_tgt = gtgt.p; j.sortrec = nullptr; j.shift_t = 0;
-                        j.force_bits = -1;
-                        if (const char *e = getenv("FSTC_RESOLVE_BITS")) j.force_bits = atoi(e);
+                        j.force_bits = knob_resolve_bits;
                         j.stats = &st; j.profile = o.profile != 0;
-                        resolve_partitioned(c, j);
-                        st.n_resolve += 1;
-                        st.n_resolved_arcs += MGm;
+                        run_resolve(j, 1);
                     } else {
                         h = tm.begin(FSTC_T_EMIT);
                         if (use_dense)
@@ -1605,7 +1850,7 @@ fstc_result_t *Composer::run() {
                         c.n_launch += 1;
                         tm.end(h);
                     }
-                    n_states_live = static_cast<int64_t>(read_scalar(c, d_counters.p));
+                    if (!external) n_states_live = static_cast<int64_t>(read_scalar(c, d_counters.p));
                 }
                 mstartG.alloc(c, nf + 1);
                 k_mstart<<<nblk(nf + 1), CT_THREADS, 0, c.stream>>>(gsrc.p, MGm, nf, mstartG.p);
@@ -1620,32 +1865,57 @@ fstc_result_t *Composer::run() {
             k_final_counts<<<nblk(nf), CT_THREADS, 0, c.stream>>>(rawU.p, mstartS.p, mstartG.p, nf, fc.p);
             FSTC_LAUNCH_CHECK();
             exclusive_scan<int64_t>(c, fc.p, nf, foff.p);
+            DBuf<uint32_t> rank;
+            int64_t det_n1 = 0;
+            if (o.deterministic) {
+                // every state of the level must exist before the ids can be ranked: the class-U arcs go out first; their
+                // targets (and only theirs: the other positions are not written yet) are remapped with the pair table
+                tm.end(h);
+                launch_emit(EMIT_INDIRECT, LU, MU, RU, 0, f_lo, foff.p, roffU.p, arc_base, nullptr, 0, 0);
+                det_n1 = static_cast<int64_t>(read_scalar(c, d_counters.p));
+                rank = det_renumber(n_states, det_n1, arc_base, arc_base + RU + M + MGm);
+                h = tm.begin(FSTC_T_REDUCE);
+                if (M > 0) {                                         // merged class-F arcs: sorted again, on the new ids
+                    DBuf<uint4> fa(c, M), fb(c, M);
+                    k_det_frec<<<nblk(M), CT_THREADS, 0, c.stream>>>(mkey.p, msrc.p, mw.p, M, shift_t, n_states, det_n1, rank.p, fa.p);
+                    FSTC_LAUNCH_CHECK();
+                    const int tgt_bits = bits_for(static_cast<uint64_t>(det_n1 > 1 ? det_n1 - 1 : 1));
+                    uint4 *fs = radix_sort_records(c, fa.p, fb.p, M, make_sort_passes(shift_t + tgt_bits, bits_for(static_cast<uint64_t>(nf - 1))));
+                    k_det_funpack<<<nblk(M), CT_THREADS, 0, c.stream>>>(fs, M, mkey.p, msrc.p, mw.p);
+                    FSTC_LAUNCH_CHECK();
+                    c.n_launch += 2;
+                    c.sync();
+                }
+            }
             if (M > 0) {
                 k_place_merged<<<nblk(M), CT_THREADS, 0, c.stream>>>(mkey.p, msrc.p, mw.p, M, mstartS.p, foff.p, arc_base, f_lo, sel.p,
-                                                                     shift_t, bits_b, a_src.p, a_il.p, a_ol.p, a_tgt.p, a_w.p);
+                                                                     shift_t, bits_b, o_src, o_il, o_ol, o_tgt, o_w);
                 FSTC_LAUNCH_CHECK();
             }
             if (MGm > 0) {
                 k_place_grouped<<<nblk(MGm), CT_THREADS, 0, c.stream>>>(gab.p, gtgt.p, gsrc.p, gw.p, MGm, mstartG.p, foff.p, arc_base,
-                                                                       f_lo, sel.p, bits_b, a_src.p, a_il.p, a_ol.p, a_tgt.p, a_w.p);
+                                                                       f_lo, sel.p, bits_b, o_src, o_il, o_ol, o_tgt, o_w,
+                                                                       n_states, det_n1, o.deterministic ? rank.p : nullptr);
                 FSTC_LAUNCH_CHECK();
             }
             c.n_launch += 3;
             tm.end(h);
-            launch_emit(EMIT_INDIRECT, LU, MU, RU, 0, f_lo, foff.p, roffU.p, arc_base, nullptr, 0, 0);
+            if (!o.deterministic) launch_emit(EMIT_INDIRECT, LU, MU, RU, 0, f_lo, foff.p, roffU.p, arc_base, nullptr, 0, 0);
             n_arcs += RU + M + MGm;
             st.n_raw_sorted += RF;
             c.sync();   // the level's temporaries go out of scope below
         }
 
         hostmark("emit+resolve", lvl);
-        const int64_t ns_after = static_cast<int64_t>(read_scalar(c, d_counters.p));
+        if (external) ext_finish_level();
+        const int64_t ns_after = external ? n_states_live : static_cast<int64_t>(read_scalar(c, d_counters.p));
         hostmark("ns read", lvl);
         if (lvl < FSTC_MAX_LEVEL_STATS) {
             st.level_frontier[lvl] = nf_all;
             st.level_raw[lvl] = R;
             st.level_new_states[lvl] = ns_after - n_states;
         }
+        spill_level(arc_base, n_arcs, ns_after);
         if (partitioned) st.rs_dedupe_new += ns_after - n_states;
         st.n_matches += MU + MF;
         st.n_expanded += n_sel;
@@ -1679,14 +1949,25 @@ fstc_result_t *Composer::run() {
     c.n_launch += 2;
     tm.end(h);
 
+    if (sp) {
+        if (n_states > sp->state_capacity) fail(FSTC_ERR_CAPACITY, "spill: %lld states outgrow the host arrays", static_cast<long long>(n_states));
+        if (n_states > spilled_states)                            // (a search that stopped before its first level)
+            FSTC_CUDA(cudaMemcpyAsync(sp->host->pair + 2 * spilled_states, pair.p + spilled_states, sizeof(int2) * static_cast<size_t>(n_states - spilled_states),
+                                      cudaMemcpyDeviceToHost, c.stream));
+        if (sp->host->accept && n_accept > 0)
+            FSTC_CUDA(cudaMemcpyAsync(sp->host->accept, accept.p, sizeof(int32_t) * static_cast<size_t>(n_accept), cudaMemcpyDeviceToHost, c.stream));
+        if (sp->host->expanded)
+            FSTC_CUDA(cudaMemcpyAsync(sp->host->expanded, expanded.p, static_cast<size_t>(n_states), cudaMemcpyDeviceToHost, c.stream));
+        st.spill_bytes += 8 * (n_states - spilled_states) + 4 * n_accept + n_states;
+        FSTC_CUDA(cudaStreamSynchronize(side));
+        spill_reap(true);
+    }
     unsigned long long cnt[3];
     FSTC_CUDA(cudaMemcpyAsync(cnt, d_counters.p, sizeof cnt, cudaMemcpyDeviceToHost, c.stream));
     FSTC_CUDA(cudaEventRecord(ev1, c.stream));
     c.sync();
     float ms = 0.f;
     cudaEventElapsedTime(&ms, ev0, ev1);
-    cudaEventDestroy(ev0);
-    cudaEventDestroy(ev1);
     tm.collect(st.ms);
     hostmark("assembled", lvl);
 
@@ -1699,11 +1980,15 @@ fstc_result_t *Composer::run() {
 
     fstc_result_t *r = new fstc_result_t();
     ResultImpl *impl = new ResultImpl();
+    impl->hooks = c.hooks;
     r->n_states = n_states; r->n_arcs = n_arcs; r->n_raw_arcs = cum_raw; r->n_accept = n_accept;
     r->n_expanded = st.n_expanded; r->n_levels = st.n_levels; r->truncated = st.truncated;
     r->pair = reinterpret_cast<int32_t *>(pair.take());
-    r->src = a_src.take(); r->ilabel = a_il.take(); r->olabel = a_ol.take(); r->tgt = a_tgt.take();
-    r->weight = a_w.take(); r->accept = accept.take(); r->expanded = expanded.take();
+    if (!spill_only) {
+        r->src = a_src.take(); r->ilabel = a_il.take(); r->olabel = a_ol.take(); r->tgt = a_tgt.take();
+        r->weight = a_w.take();
+    }
+    r->accept = accept.take(); r->expanded = expanded.take();
     impl->bufs[0] = r->pair; impl->bufs[1] = r->src; impl->bufs[2] = r->ilabel; impl->bufs[3] = r->olabel;
     impl->bufs[4] = r->tgt; impl->bufs[5] = r->weight; impl->bufs[6] = r->accept; impl->bufs[7] = r->expanded;
     r->impl = impl;
@@ -1714,7 +1999,11 @@ fstc_result_t *Composer::run() {
 
 fstc_result_t *compose_packed(Ctx &c, const fstc_packed_t &m1, const fstc_packed_t &m2, const fstc_opts_t &opts,
                               fstc_stats_t *stats) {
-    if (opts.small_path < 0 || opts.small_path > 2) fail(FSTC_ERR_ARG, "bad options");
+    if (opts.small_path < 0 || opts.small_path > 2 || opts.deterministic < 0 || opts.deterministic > 1) fail(FSTC_ERR_ARG, "bad options");
+    int dev = 0;
+    FSTC_CUDA(cudaGetDevice(&dev));
+    if (m1.device != dev || m2.device != dev)
+        fail(FSTC_ERR_ARG, "operands were packed on device %d / %d, the current device is %d", m1.device, m2.device, dev);
     if (small_path_applies(opts)) {
         // small problems never leave the device (small.cu); one that outgrows the block's capacities comes back here
         const fstc_packed_t *one = &m1;

@@ -48,6 +48,7 @@ struct fstc_packed_t {
     uint32_t *goff = nullptr;     // [n_groups+1] first arc of each group; goff[n_groups] = n_arcs
     uint2 *gkey = nullptr;        // [n_groups]   {outer symbol, target}
     uint32_t *gptr = nullptr;     // [n_states+1] first group of each state
+    fstc::AllocHooks hooks;       // who owns the arrays (set: the caller's allocator)
 };
 
 namespace fstc {
@@ -79,11 +80,17 @@ void free_result(fstc_result_t *r);            // small.cu
 struct SharedBlock {          // one device block that the results of a batch share
     void *base;
     int refs;
+    AllocHooks hooks;
 };
 struct ResultImpl {           // owns the device arrays of a result
     void *bufs[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     SharedBlock *shared = nullptr;   // set: the arrays are parts of a batch's block
+    AllocHooks hooks;                // who owns the arrays (set: the caller's allocator)
 };
+inline void release_block(void *p, const AllocHooks &h) {      // an array that left the library comes back
+    if (!p) return;
+    if (h.dealloc) h.dealloc(p, nullptr, h.ctx); else persist_free(p, nullptr);
+}
 
 // ---------------------------------------------------------------- small problems, one block each (small.cu)
 bool small_path_applies(const fstc_opts_t &o);
@@ -112,6 +119,8 @@ struct ResolveJob {
     bool profile;
 };
 int resolve_bits_needed(int64_t n_records_and_states);
+bool resolve_can_take(int64_t n_records, int64_t n_states);   // within the u32 record indices and the 2^20 bins of resolve.cu
 void resolve_partitioned(Ctx &c, const ResolveJob &j);
+void resolve_apply_ids(Ctx &c, const ResolveJob &j, const uint32_t *ids);   // ids known (external resolve): deliver them
 
 }  // namespace fstc

@@ -179,15 +179,15 @@ const T *stage(Ctx &c, const T *p, int64_t n, int mem, DBuf<T> &hold) {
 void free_packed(fstc_packed_t *p) {
     if (!p) return;
     // freed stream-ordered on the legacy stream: safe after any stream of ours has been synchronised
-    if (p->arcs) persist_free(p->arcs, nullptr);
-    if (p->segs) persist_free(p->segs, nullptr);
-    if (p->seg_ptr) persist_free(p->seg_ptr, nullptr);
-    if (p->flags) persist_free(p->flags, nullptr);
-    if (p->accept_bits) persist_free(p->accept_bits, nullptr);
-    if (p->garcs) persist_free(p->garcs, nullptr);
-    if (p->goff) persist_free(p->goff, nullptr);
-    if (p->gkey) persist_free(p->gkey, nullptr);
-    if (p->gptr) persist_free(p->gptr, nullptr);
+    release_block(p->arcs, p->hooks);
+    release_block(p->segs, p->hooks);
+    release_block(p->seg_ptr, p->hooks);
+    release_block(p->flags, p->hooks);
+    release_block(p->accept_bits, p->hooks);
+    release_block(p->garcs, p->hooks);
+    release_block(p->goff, p->hooks);
+    release_block(p->gkey, p->hooks);
+    release_block(p->gptr, p->hooks);
     delete p;
 }
 
@@ -313,6 +313,7 @@ fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side) {
     p->side = side;
     p->n_states = m.n_states; p->n_inner = n_inner; p->n_outer = n_outer; p->start = m.start;
     p->n_arcs = n; p->n_segs = n_segs;
+    p->hooks = c.hooks;
     p->arcs = arcs.take(); p->segs = segs.take(); p->seg_ptr = seg_ptr.take();
     p->flags = flags.take(); p->accept_bits = accept_bits.take();
     p->n_groups = n_groups;

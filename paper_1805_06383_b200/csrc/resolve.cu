@@ -544,7 +544,7 @@ SegSet scatter_pass(Ctx &c, const SegSet &in, int shift, int hshift, int nbins, 
         FSTC_LAUNCH_CHECK();
         c.n_launch += 4;
         if (!read_scalar(c, flag.p)) break;
-        if (attempt == 1) fail(FSTC_ERR_CUDA, "internal: resolve scatter overflowed with exact capacities");
+        if (attempt == 1) fail(FSTC_ERR_INTERNAL, "resolve scatter overflowed with exact capacities");
     }
     out.cnt.alloc(c, nb);
     rs_compact_counts<<<rs_blocks(nb), 256, 0, c.stream>>>(cursor.p, cur_stride, nb, out.cnt.p);
@@ -588,7 +588,38 @@ int resolve_bits_needed(int64_t n_records_and_states) {
     return b;
 }
 
+// the ids of the job's keys are known (ids[r], in rank order): deliver them the way the job asks for (target column,
+// indirect positions, or into the sort records)
+void resolve_apply_ids(Ctx &c, const ResolveJob &j, const uint32_t *ids) {
+    if (j.n_records <= 0) return;
+    SegSet lvl0 = single_segment(c, j.keys, j.n_records);
+    GatherArgs g{};
+    g.dest = nullptr; g.perm = nullptr; g.in = ids;
+    g.out = reinterpret_cast<uint32_t *>(j.o_tgt); g.pos = j.pos; g.o_tgt = j.o_tgt; g.sortrec = j.sortrec; g.shift_t = j.shift_t;
+    gather_pass(c, lvl0, j.mode, true, g);
+    c.sync();
+}
+
+bool resolve_can_take(int64_t n_records, int64_t n_states) {
+    // a scatter pass holds up to 17/16 n + 192 per bin records, indexed by u32; 2^20 bins of DD_TARGET keys at most
+    return n_records < 0xE0000000ll && ((n_records + n_states) >> 20) <= DD_TARGET;
+}
+
+namespace { void resolve_partitioned_impl(Ctx &c, const ResolveJob &j); }
+
 void resolve_partitioned(Ctx &c, const ResolveJob &j) {
+    try {
+        resolve_partitioned_impl(c, j);
+    } catch (...) {                                              // a failed call leaves no stage spans behind for the next one
+        for (auto &s : g_trace.spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
+        g_trace.spans.clear();
+        g_trace.on = g_trace.print;
+        throw;
+    }
+}
+
+namespace {
+void resolve_partitioned_impl(Ctx &c, const ResolveJob &j) {
     FSTC_CUDA(cudaFuncSetAttribute(rs_dedupe, cudaFuncAttributeMaxDynamicSharedMemorySize, DD_SLOTS * 12));   // per device
     const int ib = bits_for(static_cast<uint64_t>(j.n_states_before > 1 ? j.n_states_before - 1 : 1));
     if (j.key_bits + ib > 64) fail(FSTC_ERR_CAPACITY, "resolve: key (%d bits) + state id (%d bits) exceed 64 bits", j.key_bits, ib);
@@ -667,5 +698,6 @@ void resolve_partitioned(Ctx &c, const ResolveJob &j) {
         return;
     }
 }
+}  // namespace
 
 }  // namespace fstc

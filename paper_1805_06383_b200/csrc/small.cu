@@ -434,10 +434,9 @@ void free_result(fstc_result_t *r) {
         if (impl->shared) {                                    // a result of a batch: the block goes when its last result goes
             bool last;
             { std::lock_guard<std::mutex> lk(g_shared_mu); last = --impl->shared->refs == 0; }
-            if (last) { persist_free(impl->shared->base, nullptr); delete impl->shared; }
+            if (last) { release_block(impl->shared->base, impl->shared->hooks); delete impl->shared; }
         } else {
-            for (void *p : impl->bufs)
-                if (p) persist_free(p, nullptr);
+            for (void *p : impl->bufs) release_block(p, impl->hooks);
         }
         delete impl;
     }
@@ -445,7 +444,7 @@ void free_result(fstc_result_t *r) {
 }
 
 bool small_path_applies(const fstc_opts_t &o) {
-    return o.small_path != FSTC_SMALL_OFF && o.merge_mode != FSTC_MERGE_SORT_ALL &&
+    return o.small_path != FSTC_SMALL_OFF && o.merge_mode != FSTC_MERGE_SORT_ALL && !o.spill && !o.deterministic && o.resolve_mode != FSTC_RESOLVE_EXTERNAL &&
            o.state_capacity_hint <= (1 << 20) && o.arc_capacity_hint <= (1 << 22);
 }
 
@@ -523,7 +522,7 @@ void compose_small_batch(Ctx &c, const fstc_packed_t *const *m1, int n, const fs
     for (int k = 0; k < n; ++k) {
         const SmallOut &so = h[k];
         if (so.status != SP_OK) continue;
-        if (!shared) shared = new SharedBlock{block.take(), 0};
+        if (!shared) shared = new SharedBlock{block.take(), 0, c.hooks};
         const SmallProb &p = prob[k];
         fstc_result_t *r = new fstc_result_t();
         ResultImpl *impl = new ResultImpl();

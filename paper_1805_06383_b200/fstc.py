@@ -19,9 +19,9 @@ LIB_PATH = os.environ.get("FSTC_LIB") or os.path.join(_HERE, "libfstc.so")   # F
 
 FSTC_MEM_DEVICE, FSTC_MEM_HOST = 0, 1
 MERGE_AUTO, MERGE_OFF, MERGE_SORT_ALL = 0, 1, 2
-RESOLVE_AUTO, RESOLVE_TABLE, RESOLVE_PARTITIONED, RESOLVE_HASH = 0, 1, 2, 3
+RESOLVE_AUTO, RESOLVE_TABLE, RESOLVE_PARTITIONED, RESOLVE_HASH, RESOLVE_EXTERNAL = 0, 1, 2, 3, 4
 SMALL_AUTO, SMALL_OFF, SMALL_ONLY = 0, 1, 2
-ERR_ARG, ERR_INPUT, ERR_OOM, ERR_CAPACITY, ERR_CUDA = -1, -2, -3, -4, -5
+ERR_ARG, ERR_INPUT, ERR_OOM, ERR_CAPACITY, ERR_CUDA, ERR_INTERNAL, ERR_CALLBACK = -1, -2, -3, -4, -5, -6, -7
 MAX_LEVEL_STATS = 64
 STAGES = ("count", "scan", "match", "emit", "sort", "reduce", "table", "assemble", "rs_scatter", "rs_dedupe", "rs_gather")
 
@@ -53,8 +53,17 @@ class _Opts(ctypes.Structure):
         ("merge_mode", ctypes.c_int32), ("max_levels", ctypes.c_int32), ("max_raw_arcs", ctypes.c_int64),
         ("arc_capacity_hint", ctypes.c_int64), ("state_capacity_hint", ctypes.c_int64),
         ("profile", ctypes.c_int32), ("resolve_mode", ctypes.c_int32),
-        ("small_path", ctypes.c_int32), ("reserved_", ctypes.c_int32),
+        ("small_path", ctypes.c_int32), ("deterministic", ctypes.c_int32),
+        ("alloc", ctypes.c_void_p), ("dealloc", ctypes.c_void_p), ("alloc_ctx", ctypes.c_void_p),
+        ("spill", ctypes.c_void_p),
+        ("resolve_cb", ctypes.c_void_p), ("resolve_ctx", ctypes.c_void_p), ("owns_start", ctypes.c_int32),
+        ("reserved_", ctypes.c_int32),
     ]
+
+
+class _Spill(ctypes.Structure):
+    _fields_ = [("host", ctypes.c_void_p), ("arc_capacity", ctypes.c_int64), ("state_capacity", ctypes.c_int64),
+                ("keep_device", ctypes.c_int32), ("reserved_", ctypes.c_int32)]
 
 
 class _Stats(ctypes.Structure):
@@ -70,6 +79,7 @@ class _Stats(ctypes.Structure):
         ("rs_dedupe_states", ctypes.c_int64), ("rs_dedupe_new", ctypes.c_int64), ("rs_gather_recs", ctypes.c_int64),
         ("rs_scatter_launches", ctypes.c_int32), ("rs_dedupe_launches", ctypes.c_int32),
         ("rs_gather_launches", ctypes.c_int32), ("pad2_", ctypes.c_int32),
+        ("spill_bytes", ctypes.c_int64), ("spill_bytes_saved", ctypes.c_int64),
         ("ms", ctypes.c_double * len(STAGES)), ("ms_total", ctypes.c_double),
         ("level_frontier", ctypes.c_int64 * MAX_LEVEL_STATS), ("level_raw", ctypes.c_int64 * MAX_LEVEL_STATS),
         ("level_new_states", ctypes.c_int64 * MAX_LEVEL_STATS),
@@ -104,7 +114,7 @@ def lib():
                               "(there is no CPU fallback)")
         L = ctypes.CDLL(LIB_PATH)
         P, I = ctypes.c_void_p, ctypes.c_int
-        L.fstc_pack.argtypes = [P, I, P, ctypes.POINTER(P)]
+        L.fstc_pack.argtypes = [P, I, P, P, ctypes.POINTER(P)]
         L.fstc_packed_free.argtypes = [P]
         L.fstc_packed_free.restype = None
         L.fstc_packed_info.argtypes = [P, P]
@@ -205,7 +215,9 @@ def _tensor(ptr, shape, typestr, owner):
     import torch
     n = int(np.prod(shape))
     dt = {"<i4": torch.int32, "<f4": torch.float32, "|u1": torch.uint8}[typestr]
-    if n == 0 or not ptr:
+    if n > 0 and not ptr:
+        return None                 # the array is not on the device (host spill without a device copy)
+    if n == 0:
         return torch.empty(tuple(shape), dtype=dt, device="cuda")
     return torch.as_tensor(_DevView(ptr, shape, typestr, owner), device="cuda")
 
@@ -285,6 +297,7 @@ def stats_dict(s: _Stats) -> dict:
         "n_rehash": int(s.n_rehash), "n_grow": int(s.n_grow), "n_emit_launches": int(s.n_emit_launches),
         "n_kernel_launches": int(s.n_kernel_launches),
         "n_resolve": int(s.n_resolve), "n_resolved_arcs": int(s.n_resolved_arcs), "small_path": int(s.small_path),
+        "spill_bytes": int(s.spill_bytes), "spill_bytes_saved": int(s.spill_bytes_saved),
         **{k: int(getattr(s, k)) for k in ("rs_scatter_recs", "rs_scatter_dest_recs", "rs_dedupe_arcs", "rs_dedupe_states",
                                            "rs_dedupe_new", "rs_gather_recs", "rs_scatter_launches", "rs_dedupe_launches",
                                            "rs_gather_launches")},
@@ -296,13 +309,70 @@ def stats_dict(s: _Stats) -> dict:
 
 
 def _opts(merge_mode=MERGE_AUTO, max_raw_arcs=0, max_levels=0, arc_capacity_hint=0, state_capacity_hint=0,
-          profile=False, resolve_mode=0, small_path=0) -> _Opts:
+          profile=False, resolve_mode=0, small_path=0, deterministic=False, allocator=None, spill=None,
+          spill_keep_device=False) -> _Opts:
+    """allocator: None (the library's pool) or "torch": every device allocation of the call goes through PyTorch's caching
+    allocator (fstc_opts_t.alloc / dealloc)."""
     o = _Opts()
+    o.deterministic = int(bool(deterministic))
+    if spill is not None:
+        # spill: dict of PINNED torch CPU tensors named like the result's fields (pair [S,2] int32, src/ilabel/olabel/tgt
+        # int32 [A], weight float32 [A], accept int32 [S], expanded uint8 [S]); they receive the result while it is built
+        hr = _HostResult()
+        for name in ("pair", "src", "ilabel", "olabel", "tgt", "weight", "accept", "expanded"):
+            t = spill.get(name)
+            if t is not None:
+                assert t.is_contiguous() and t.device.type == "cpu"
+                setattr(hr, name, t.data_ptr())
+        sp = _Spill()
+        sp.host = ctypes.addressof(hr)
+        sp.arc_capacity = min(int(spill[k].numel()) for k in ("src", "ilabel", "olabel", "tgt", "weight"))
+        sp.state_capacity = int(spill["pair"].numel()) // 2
+        for k in ("accept", "expanded"):
+            if spill.get(k) is not None:
+                sp.state_capacity = min(sp.state_capacity, int(spill[k].numel()))
+        sp.keep_device = int(bool(spill_keep_device))
+        o.spill = ctypes.addressof(sp)
+        o._keep = (hr, sp, spill)
+    if allocator == "torch":
+        a, d = _torch_allocator()
+        o.alloc, o.dealloc = ctypes.cast(a, ctypes.c_void_p), ctypes.cast(d, ctypes.c_void_p)
+    elif allocator is not None:
+        raise ValueError("allocator must be None or 'torch'")
     o.resolve_mode = int(resolve_mode)
     o.small_path = int(small_path)
     o.merge_mode, o.max_levels, o.max_raw_arcs = int(merge_mode), int(max_levels), int(max_raw_arcs)
     o.arc_capacity_hint, o.state_capacity_hint, o.profile = int(arc_capacity_hint), int(state_capacity_hint), int(bool(profile))
     return o
+
+
+_ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p, ctypes.c_void_p)
+_DEALLOC_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p)
+_torch_hooks = None
+ALLOC_LOG = {"alloc": 0, "dealloc": 0, "bytes": 0}      # calls that went through the torch hooks (tests)
+
+
+def _torch_allocator():
+    """ctypes callbacks over torch.cuda.caching_allocator_alloc / _delete (kept alive for the life of the process)."""
+    global _torch_hooks
+    if _torch_hooks is None:
+        import torch
+
+        def alloc(nbytes, stream, _ctx):
+            try:
+                p = torch.cuda.caching_allocator_alloc(int(nbytes), stream=int(stream or 0))
+            except Exception:
+                return None
+            ALLOC_LOG["alloc"] += 1
+            ALLOC_LOG["bytes"] += int(nbytes)
+            return p
+
+        def dealloc(ptr, _stream, _ctx):
+            ALLOC_LOG["dealloc"] += 1
+            torch.cuda.caching_allocator_delete(int(ptr))
+
+        _torch_hooks = (_ALLOC_FN(alloc), _DEALLOC_FN(dealloc))
+    return _torch_hooks
 
 
 class Packed:
@@ -339,10 +409,11 @@ class Packed:
             pass
 
 
-def fstc_pack(m, side: int, stream=None) -> Packed:
+def fstc_pack(m, side: int, stream=None, allocator=None) -> Packed:
     s, keep = _marshal(m)
     out = ctypes.c_void_p()
-    _check(lib().fstc_pack(ctypes.addressof(s), int(side), _stream_ptr(stream), ctypes.byref(out)))
+    o = _opts(allocator=allocator)
+    _check(lib().fstc_pack(ctypes.addressof(s), int(side), ctypes.addressof(o), _stream_ptr(stream), ctypes.byref(out)))
     del keep
     return Packed(out)
 

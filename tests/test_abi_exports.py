@@ -63,8 +63,9 @@ def test_ctypes_struct_layout_matches_the_c_compiler(tmp_path):
     src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "fstc.h"\nint main(void){\n'
                    'printf("%zu %zu %zu %zu %zu\\n", sizeof(fstc_fst_t), sizeof(fstc_opts_t), sizeof(fstc_stats_t),'
                    ' sizeof(fstc_result_t), sizeof(fstc_host_result_t));\n'
-                   'printf("%zu %zu %zu %zu\\n", offsetof(fstc_fst_t, mem), offsetof(fstc_opts_t, profile),'
-                   ' offsetof(fstc_stats_t, ms_total), offsetof(fstc_result_t, expanded));\nreturn 0;}\n')
+                   'printf("%zu %zu %zu %zu %zu %zu\\n", offsetof(fstc_fst_t, mem), offsetof(fstc_opts_t, profile),'
+                   ' offsetof(fstc_stats_t, ms_total), offsetof(fstc_result_t, expanded), offsetof(fstc_opts_t, alloc_ctx),'
+                   ' offsetof(fstc_stats_t, small_path));\nreturn 0;}\n')
     exe = tmp_path / "sz"
     subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)])
     a, b = subprocess.check_output([str(exe)], text=True).strip().split("\n")
@@ -73,7 +74,7 @@ def test_ctypes_struct_layout_matches_the_c_compiler(tmp_path):
     assert sizes == [ctypes.sizeof(fstc._Fst), ctypes.sizeof(fstc._Opts), ctypes.sizeof(fstc._Stats),
                      ctypes.sizeof(fstc._Result), ctypes.sizeof(fstc._HostResult)]
     assert offs == [fstc._Fst.mem.offset, fstc._Opts.profile.offset, fstc._Stats.ms_total.offset,
-                    fstc._Result.expanded.offset]
+                    fstc._Result.expanded.offset, fstc._Opts.alloc_ctx.offset, fstc._Stats.small_path.offset]
 
 
 def test_no_product_path_touches_the_oracle():
