@@ -1128,11 +1128,15 @@ struct Composer {
     std::vector<LevelArcs> inflight;     // level arrays whose copy may still run
     LevelArcs cur;                       // spill_only: the arrays of the level being expanded
     int64_t spilled_states = 0;
+    bool cols_spilled = false;           // src / ilabel / olabel / weight of the current level already went out (after its emit kernel)
+    struct Retired { DBuf<int2> block; cudaEvent_t done = nullptr; };
+    std::vector<Retired> retired;        // pair blocks replaced by a larger one while a copy to the host may still read them
 
     ~Composer() {
         if (side) {                      // on every way out: no copy may still read a buffer the members are about to release
             (void)cudaStreamSynchronize(side);
             for (auto &l : inflight) if (l.done) (void)cudaEventDestroy(l.done);
+            for (auto &l : retired) if (l.done) (void)cudaEventDestroy(l.done);
             if (ev_main) (void)cudaEventDestroy(ev_main);
             (void)cudaStreamDestroy(side);
         }
@@ -1148,6 +1152,13 @@ struct Composer {
         FSTC_CUDA(cudaEventCreateWithFlags(&ev_main, cudaEventDisableTiming));
     }
     void spill_reap(bool all) {          // level arrays whose copy is complete go back to the workspace
+        for (size_t i = 0; i < retired.size();) {
+            if (all) FSTC_CUDA(cudaEventSynchronize(retired[i].done));
+            if (all || cudaEventQuery(retired[i].done) == cudaSuccess) {
+                (void)cudaEventDestroy(retired[i].done);
+                retired.erase(retired.begin() + i);
+            } else { (void)cudaGetLastError(); ++i; }
+        }
         for (size_t i = 0; i < inflight.size();) {
             if (all) FSTC_CUDA(cudaEventSynchronize(inflight[i].done));
             if (all || cudaEventQuery(inflight[i].done) == cudaSuccess) {
@@ -1165,6 +1176,22 @@ struct Composer {
         o_src = cur.src.p + pad - base; o_il = cur.il.p + pad - base; o_ol = cur.ol.p + pad - base;
         o_tgt = cur.tgt.p + pad - base; o_w = cur.w.p + pad - base;
     }
+    // four of the five columns of arcs [a0, a1) are final as soon as the emit kernel that writes them straight to their
+    // place is done (the target column waits for the resolve): they cross PCIe under the resolve
+    void spill_columns_early(int64_t a0, int64_t a1) {
+        if (!sp || a1 <= a0) return;
+        if (a1 > sp->arc_capacity)
+            fail(FSTC_ERR_CAPACITY, "spill: the result (%lld arcs so far) outgrows the host arrays", static_cast<long long>(a1));
+        FSTC_CUDA(cudaEventRecord(ev_main, c.stream));
+        FSTC_CUDA(cudaStreamWaitEvent(side, ev_main, 0));
+        const fstc_host_result_t *hr = sp->host;
+        const size_t nb = sizeof(int32_t) * static_cast<size_t>(a1 - a0);
+        FSTC_CUDA(cudaMemcpyAsync(hr->src + a0, o_src + a0, nb, cudaMemcpyDeviceToHost, side));
+        FSTC_CUDA(cudaMemcpyAsync(hr->ilabel + a0, o_il + a0, nb, cudaMemcpyDeviceToHost, side));
+        FSTC_CUDA(cudaMemcpyAsync(hr->olabel + a0, o_ol + a0, nb, cudaMemcpyDeviceToHost, side));
+        FSTC_CUDA(cudaMemcpyAsync(hr->weight + a0, o_w + a0, nb, cudaMemcpyDeviceToHost, side));
+        cols_spilled = true;
+    }
     // the level is placed: arcs [a0, a1) and states [s0, s1) are final
     void spill_level(int64_t a0, int64_t a1, int64_t s1) {
         if (!sp) return;
@@ -1175,12 +1202,15 @@ struct Composer {
         const fstc_host_result_t *hr = sp->host;
         const size_t nb = sizeof(int32_t) * static_cast<size_t>(a1 - a0);
         if (a1 > a0) {
-            FSTC_CUDA(cudaMemcpyAsync(hr->src + a0, o_src + a0, nb, cudaMemcpyDeviceToHost, side));
-            FSTC_CUDA(cudaMemcpyAsync(hr->ilabel + a0, o_il + a0, nb, cudaMemcpyDeviceToHost, side));
-            FSTC_CUDA(cudaMemcpyAsync(hr->olabel + a0, o_ol + a0, nb, cudaMemcpyDeviceToHost, side));
+            if (!cols_spilled) {
+                FSTC_CUDA(cudaMemcpyAsync(hr->src + a0, o_src + a0, nb, cudaMemcpyDeviceToHost, side));
+                FSTC_CUDA(cudaMemcpyAsync(hr->ilabel + a0, o_il + a0, nb, cudaMemcpyDeviceToHost, side));
+                FSTC_CUDA(cudaMemcpyAsync(hr->olabel + a0, o_ol + a0, nb, cudaMemcpyDeviceToHost, side));
+                FSTC_CUDA(cudaMemcpyAsync(hr->weight + a0, o_w + a0, nb, cudaMemcpyDeviceToHost, side));
+            }
             FSTC_CUDA(cudaMemcpyAsync(hr->tgt + a0, o_tgt + a0, nb, cudaMemcpyDeviceToHost, side));
-            FSTC_CUDA(cudaMemcpyAsync(hr->weight + a0, o_w + a0, nb, cudaMemcpyDeviceToHost, side));
         }
+        cols_spilled = false;
         if (s1 > spilled_states)
             FSTC_CUDA(cudaMemcpyAsync(hr->pair + 2 * spilled_states, pair.p + spilled_states, sizeof(int2) * static_cast<size_t>(s1 - spilled_states),
                                       cudaMemcpyDeviceToHost, side));
@@ -1228,11 +1258,17 @@ struct Composer {
     void ensure_pairs(int64_t need, int64_t want = 0) {
         if (need <= pair_cap) return;
         grow_to(need, std::max(want, pair_cap * 2), [&](int64_t nc) {
-            if (side) FSTC_CUDA(cudaStreamSynchronize(side));     // a copy to the host may still read the old block
             DBuf<int2> np(c, nc, true);
             const int64_t keep = std::max(n_states, n_states_live);  // (states appended inside the level, external resolve)
             if (keep > 0 && pair.p)
                 FSTC_CUDA(cudaMemcpyAsync(np.p, pair.p, sizeof(int2) * keep, cudaMemcpyDeviceToDevice, c.stream));
+            if (side && pair.p) {                                 // a copy to the host may still read the old block: it goes later
+                Retired r;
+                FSTC_CUDA(cudaEventCreateWithFlags(&r.done, cudaEventDisableTiming));
+                FSTC_CUDA(cudaEventRecord(r.done, side));
+                r.block = std::move(pair);
+                retired.push_back(std::move(r));
+            }
             pair = std::move(np);
             pair_cap = nc;
         });
@@ -1388,6 +1424,7 @@ struct Composer {
         tm.end(h_emit);
         c.n_launch += 2;
         st.n_emit_launches += 1;
+        if (sp && mode == EMIT_DIRECT && partitioned && !o.deterministic) spill_columns_early(pos_base, pos_base + R);
         if (partitioned) {
             ResolveJob j;
             j.keys = keys.p; j.n_records = R; j.q2_bits = g.q2_bits;

@@ -22,7 +22,7 @@ def test_single_rank_shard_is_the_whole_composition(fstc, config, scale, kw):
     p2 = fstc.fstc_pack(fstc.DeviceFst.from_host(m2), 2)
     ex = KeyExchange(0, 1, "cuda")
     res = fstc_compose_sharded(p1, p2, ex, n_q2=m2.n_states, start=(m1.start, m2.start), **kw)
-    assert res.stats["n_resolve"] >= 3 * res.n_levels and ex.n_local == res.n_states
+    assert res.stats["n_resolve"] >= res.n_levels - 1 and ex.n_local == res.n_states
     check_parity(fstc, m1, m2, merge_mode=kw.get("merge_mode", 0), max_levels=kw.get("max_levels", 0), result=res)
 
 
