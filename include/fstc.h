@@ -217,7 +217,8 @@ typedef struct fstc_stats_t {
   /* work of the partitioned resolve, for its roofline: records through the scatter passes without / with
    * the recorded permutation, arc keys and state records through the dedupe, ids through the gathers; launches    */
   int64_t rs_scatter_recs, rs_scatter_dest_recs, rs_dedupe_arcs, rs_dedupe_states, rs_dedupe_new, rs_gather_recs;
-  int32_t rs_scatter_launches, rs_dedupe_launches, rs_gather_launches, pad2_;
+  int32_t rs_scatter_launches, rs_dedupe_launches, rs_gather_launches;
+  int32_t n_chunks;         /* pieces of the levels that were too big for the workspace and went chunk by chunk */
   int64_t spill_bytes, spill_bytes_saved;  /* bytes copied to the host while the search ran; device bytes never held (keep_device = 0) */
   double ms[FSTC_T_NSTAGES];/* device time per stage (CUDA events), only when opts.profile = 1       */
   double ms_total;          /* device time of the whole call (CUDA events), always                    */

@@ -641,10 +641,22 @@ struct GProdArgs {
     uint64_t nq2;
 };
 
+// compensated (Kahan) fp32 accumulation: the error of a sum of n terms stays at a few ulp whatever n, so that a run of
+// thousands of parallel arcs, or a group pair with thousands of common symbols, stays inside rtol 1e-5 (N13)
+struct KahanSum {
+    float s = 0.f, c = 0.f;
+    __device__ __forceinline__ void add(float x) {
+        const float y = x - c;
+        const float t = s + y;
+        c = (t - s) - y;
+        s = t;
+    }
+};
+
 // sum over the common inner symbols of two groups; *found = at least one common symbol
 __device__ __forceinline__ float group_dot(const uint2 *__restrict__ ga, uint32_t a0, uint32_t a1, const uint2 *__restrict__ gb,
                                            uint32_t b0, uint32_t b1, bool first_only, bool *found) {
-    float sum = 0.f;
+    KahanSum sum;
     bool any = false;
     uint2 x = ga[a0], y = gb[b0];
     while (true) {
@@ -652,10 +664,10 @@ __device__ __forceinline__ float group_dot(const uint2 *__restrict__ ga, uint32_
             any = true;
             if (first_only) break;
             const uint32_t c = x.x;                              // runs of equal symbols (parallel duplicate arcs) first
-            float sa = 0.f, sb = 0.f;
-            while (true) { sa += __uint_as_float(x.y); if (++a0 == a1) break; x = ga[a0]; if (x.x != c) break; }
-            while (true) { sb += __uint_as_float(y.y); if (++b0 == b1) break; y = gb[b0]; if (y.x != c) break; }
-            sum += sa * sb;
+            KahanSum sa, sb;
+            while (true) { sa.add(__uint_as_float(x.y)); if (++a0 == a1) break; x = ga[a0]; if (x.x != c) break; }
+            while (true) { sb.add(__uint_as_float(y.y)); if (++b0 == b1) break; y = gb[b0]; if (y.x != c) break; }
+            sum.add(sa.s * sb.s);
             if (a0 == a1 || b0 == b1) break;
         } else if (x.x < y.x) {
             if (++a0 == a1) break;
@@ -666,7 +678,7 @@ __device__ __forceinline__ float group_dot(const uint2 *__restrict__ ga, uint32_
         }
     }
     *found = any;
-    return sum;
+    return sum.s;
 }
 
 constexpr int GP_THREADS = 128, GP_IPT = 4, GP_TILE = GP_THREADS * GP_IPT;
@@ -693,7 +705,6 @@ __global__ void __launch_bounds__(GP_THREADS) k_gprod(GProdArgs g) {
     const int64_t rank0 = rank_lo + tid * GP_IPT;
     int n_valid = rank0 < rank_hi ? static_cast<int>(rank_hi - rank0 < GP_IPT ? rank_hi - rank0 : GP_IPT) : 0;
     uint32_t exists = 0;
-    float w[GP_IPT];
     uint32_t g1v[GP_IPT], g2v[GP_IPT], plv[GP_IPT];
     if (n_valid > 0) {
         const uint32_t rr = static_cast<uint32_t>(rank0 - rank_lo);
@@ -721,14 +732,18 @@ __global__ void __launch_bounds__(GP_THREADS) k_gprod(GProdArgs g) {
                 }
             }
         }
-        const uint32_t known = PASS == 1 ? g.ebits[static_cast<int64_t>(blockIdx.x) * GP_THREADS + tid] : 0xFu;
+        if (PASS == 1) exists = g.ebits[static_cast<int64_t>(blockIdx.x) * GP_THREADS + tid];   // what pass 0 found
+        else {
+            const bool masks = g.A.gmask != nullptr && g.B.gmask != nullptr;  // |Γ| <= 63: symbol sets as bit masks, one AND per rank
 #pragma unroll
-        for (int u = 0; u < GP_IPT; ++u) {
-            if (u < n_valid && (known >> u & 1u)) {
-                bool found;
-                w[u] = group_dot(g.A.garcs, g.A.goff[g1v[u]], g.A.goff[g1v[u] + 1], g.B.garcs, g.B.goff[g2v[u]],
-                                 g.B.goff[g2v[u] + 1], PASS == 0, &found);
-                if (found) exists |= 1u << u;
+            for (int u = 0; u < GP_IPT; ++u) {
+                if (u < n_valid) {
+                    bool found;
+                    if (masks) found = (g.A.gmask[g1v[u]] & g.B.gmask[g2v[u]] & ~(1ull << 63)) != 0;
+                    else (void)group_dot(g.A.garcs, g.A.goff[g1v[u]], g.A.goff[g1v[u] + 1], g.B.garcs, g.B.goff[g2v[u]],
+                                         g.B.goff[g2v[u] + 1], true, &found);
+                    if (found) exists |= 1u << u;
+                }
             }
         }
     }
@@ -747,20 +762,44 @@ __global__ void __launch_bounds__(GP_THREADS) k_gprod(GProdArgs g) {
     if (PASS == 0) {
         g.ebits[static_cast<int64_t>(blockIdx.x) * GP_THREADS + tid] = static_cast<uint8_t>(exists);
         if (tid == 0) g.tile_cnt[blockIdx.x] = total;
-        return;
     }
-    int64_t q = g.tile_off[blockIdx.x] + before;
+    if (PASS != 1) return;
+    // pass 1: typically a third of a tile's ranks give an arc.  They are packed first (rank order), so that every lane of the
+    // weight loop below has an arc to work on and the outputs of a warp are neighbours.
+    __shared__ uint32_t s_g1[GP_TILE], s_g2[GP_TILE], s_pl[GP_TILE];
 #pragma unroll
     for (int u = 0; u < GP_IPT; ++u) {
-        if (exists >> u & 1u) {
-            const uint2 k1 = g.A.gkey[g1v[u]], k2 = g.B.gkey[g2v[u]];      // {outer, tgt}
-            g.msrc[q] = plv[u];
-            g.mab[q] = (k1.x << g.bits_b) | k2.x;
-            g.mw[q] = w[u];
-            g.mkey[q] = g.q2_bits >= 0 ? ((static_cast<unsigned long long>(k1.y) << g.q2_bits) | k2.y)
-                                       : static_cast<unsigned long long>(k1.y) * g.nq2 + k2.y;
-            ++q;
+        if (exists >> u & 1u) { s_g1[before] = g1v[u]; s_g2[before] = g2v[u]; s_pl[before] = plv[u]; ++before; }
+    }
+    __syncthreads();
+    const bool masks = g.A.gmask != nullptr && g.B.gmask != nullptr;
+    const int64_t q0 = g.tile_off[blockIdx.x];
+    for (uint32_t k = tid; k < total; k += GP_THREADS) {
+        const uint32_t g1 = s_g1[k], g2 = s_g2[k];
+        const uint32_t a0 = g.A.goff[g1], b0 = g.B.goff[g2];
+        float wv;
+        unsigned long long m1 = 0, m2 = 0;
+        if (masks) { m1 = g.A.gmask[g1]; m2 = g.B.gmask[g2]; }
+        if (masks && !((m1 | m2) >> 63)) {                                // no symbol twice in either group: weights by popcount
+            unsigned long long common = m1 & m2;
+            KahanSum sum;
+            while (common) {
+                const unsigned long long below = (common & (0 - common)) - 1;
+                common &= common - 1;
+                sum.add(__uint_as_float(g.A.garcs[a0 + __popcll(m1 & below)].y) * __uint_as_float(g.B.garcs[b0 + __popcll(m2 & below)].y));
+            }
+            wv = sum.s;
+        } else {
+            bool found;
+            wv = group_dot(g.A.garcs, a0, g.A.goff[g1 + 1], g.B.garcs, b0, g.B.goff[g2 + 1], false, &found);
         }
+        const uint2 k1 = g.A.gkey[g1], k2 = g.B.gkey[g2];                 // {outer, tgt}
+        const int64_t q = q0 + k;
+        g.msrc[q] = s_pl[k];
+        g.mab[q] = (k1.x << g.bits_b) | k2.x;
+        g.mw[q] = wv;
+        g.mkey[q] = g.q2_bits >= 0 ? ((static_cast<unsigned long long>(k1.y) << g.q2_bits) | k2.y)
+                                   : static_cast<unsigned long long>(k1.y) * g.nq2 + k2.y;
     }
 }
 
@@ -1235,6 +1274,7 @@ struct Composer {
     int knob_resolve_bits = -1;          // FSTC_RESOLVE_BITS: hash bits of the partitioned resolve
     bool knob_no_group = false;          // FSTC_NO_GROUP_MERGE: class G off
     double knob_limit_margin = 1.5;      // FSTC_KEY_LIMIT_MARGIN: the guessed key limit of a level that will be cut
+    int64_t knob_chunk_arcs = 0;         // FSTC_CHUNK_ARCS: raw arcs a level may hold before it is expanded in chunks
 
     Composer(Ctx &ctx, const fstc_packed_t &a, const fstc_packed_t &b, const fstc_opts_t &opts)
         : c(ctx), m1(a), m2(b), o(opts), tm(ctx, opts.profile != 0), nq2(static_cast<uint64_t>(b.n_states)) {
@@ -1242,6 +1282,7 @@ struct Composer {
         if (const char *e = getenv("FSTC_RESOLVE_BITS")) knob_resolve_bits = atoi(e);
         knob_no_group = getenv("FSTC_NO_GROUP_MERGE") != nullptr;
         if (const char *e = getenv("FSTC_KEY_LIMIT_MARGIN")) knob_limit_margin = atof(e);
+        if (const char *e = getenv("FSTC_CHUNK_ARCS")) knob_chunk_arcs = atoll(e);
     }
 
     // Growable outputs and table.  `need` is what the coming launch requires; `want` >= need is a look-ahead
@@ -1546,8 +1587,22 @@ fstc_result_t *Composer::run() {
     int lvl = 0;
     MachineView A = view_of(m1), B = view_of(m2);
 
-    for (;; ++lvl) {
-        const int64_t nf_all = f_hi - f_lo;                      // the frontier
+    // A level whose raw arcs do not fit the workspace in one piece (the paper fills a pre-allocated edge
+    // buffer pair by pair) is expanded in CHUNKS: id ranges of the frontier of about chunk_limit raw arcs, one
+    // after the other, each with its own count / emit / resolve / merge (duplicates share a source, so merging stays
+    // correct); the states every chunk creates are appended and all of them form the next frontier.  Only
+    // when no budget cut falls into the level (rule T orders a cut level by key, not by id).
+    int64_t chunk_limit = knob_chunk_arcs;
+    if (chunk_limit <= 0) {
+        size_t f = 0, t = 0;
+        (void)cudaMemGetInfo(&f, &t);
+        // ~52 bytes of resolve buffers and 20 of output per raw arc; and the partitioned resolve indexes records with 32 bits
+        chunk_limit = std::min<int64_t>(int64_t(3) << 30, static_cast<int64_t>(0.5 * static_cast<double>(t > 0 ? t : size_t(64) << 30) / 72.0));
+    }
+    int64_t level_lo = 0, level_end = -1, chunk_pairs = 0;      // level_end >= 0: the level [level_lo, level_end) goes chunk by chunk
+
+    for (;;) {
+        const int64_t nf_all = f_hi - f_lo;                      // the frontier (or the current chunk of it)
         cur_level = lvl;
         if (external) {
             // the search ends when NO rank created a state; a rank without a frontier still takes part in the exchange
@@ -1557,12 +1612,13 @@ fstc_result_t *Composer::run() {
                 ext_finish_level();
                 if (lvl < FSTC_MAX_LEVEL_STATS) { st.level_frontier[lvl] = 0; st.level_raw[lvl] = 0; st.level_new_states[lvl] = n_states_live - n_states; }
                 n_states = n_states_live; f_lo = f_hi; f_hi = n_states; st.n_levels = lvl + 1;
+                ++lvl;
                 continue;
             }
         } else if (nf_all == 0) break;
         int64_t nf = nf_all;                                     // the pairs of it this level works on (see `sel`)
-        last_lo = f_lo; last_hi = f_hi;
-        if (o.max_levels > 0 && lvl == o.max_levels) { st.truncated = 1; last_mode = 0; break; }
+        last_lo = level_end >= 0 ? level_lo : f_lo; last_hi = level_end >= 0 ? level_end : f_hi;
+        if (level_end < 0 && o.max_levels > 0 && lvl == o.max_levels) { st.truncated = 1; last_mode = 0; break; }
         last_mode = 1;
 
         // ---- count
@@ -1595,7 +1651,7 @@ fstc_result_t *Composer::run() {
         // only below a key limit: rule T expands a key-ordered prefix, so pairs far above the cut never matter.
         // Exact: if the counted part does not exceed the budget the limit is raised and the level counted again.
         uint64_t key_limit = ~0ull;
-        if (o.max_raw_arcs > 0 && nf > 100000 && last_fan > 0) {
+        if (level_end < 0 && o.max_raw_arcs > 0 && nf > 100000 && last_fan > 0) {
             const double remaining = static_cast<double>(o.max_raw_arcs - cum_raw);
             const double predicted = static_cast<double>(nf) * last_fan;
             if (predicted > 4.0 * remaining) {
@@ -1684,6 +1740,15 @@ fstc_result_t *Composer::run() {
 
         hostmark("count+scan", lvl);
         const int64_t R = RU + RF + RG;
+        if (!stop_after && !external && nf_all > 1) {
+            if (level_end < 0 && R > chunk_limit) {              // too big for one piece: count again, on the first chunk
+                level_lo = f_lo; level_end = f_hi;
+                chunk_pairs = std::max<int64_t>(1, static_cast<int64_t>(static_cast<double>(nf_all) * (0.9 * static_cast<double>(chunk_limit) / static_cast<double>(R))));
+                f_hi = f_lo + chunk_pairs;
+                continue;
+            }
+            if (level_end >= 0 && R > 2 * chunk_limit) { f_hi = f_lo + nf_all / 2; continue; }   // a dense id range: halve the chunk
+        }
         cur_sel = sel.p;
         // ---- capacities for this level
         const uint64_t remaining_pairs = n_pairs_total - static_cast<uint64_t>(n_states);
@@ -1947,11 +2012,12 @@ fstc_result_t *Composer::run() {
         if (external) ext_finish_level();
         const int64_t ns_after = external ? n_states_live : static_cast<int64_t>(read_scalar(c, d_counters.p));
         hostmark("ns read", lvl);
-        if (lvl < FSTC_MAX_LEVEL_STATS) {
-            st.level_frontier[lvl] = nf_all;
-            st.level_raw[lvl] = R;
-            st.level_new_states[lvl] = ns_after - n_states;
+        if (lvl < FSTC_MAX_LEVEL_STATS) {                       // (a level expanded in chunks adds up)
+            st.level_frontier[lvl] += nf_all;
+            st.level_raw[lvl] += R;
+            st.level_new_states[lvl] += ns_after - n_states;
         }
+        if (level_end >= 0) st.n_chunks += 1;
         spill_level(arc_base, n_arcs, ns_after);
         if (partitioned) st.rs_dedupe_new += ns_after - n_states;
         st.n_matches += MU + MF;
@@ -1960,8 +2026,14 @@ fstc_result_t *Composer::run() {
         cum_raw += R;
         n_states = ns_after;
         f_lo = f_hi;
-        f_hi = n_states;
         st.n_levels = lvl + 1;
+        if (level_end >= 0 && f_lo < level_end) {                // the next chunk of the same level
+            f_hi = std::min(f_lo + chunk_pairs, level_end);
+            continue;
+        }
+        level_end = -1;
+        f_hi = n_states;
+        ++lvl;
         if (stop_after) break;
     }
 

@@ -48,6 +48,7 @@ struct fstc_packed_t {
     uint32_t *goff = nullptr;     // [n_groups+1] first arc of each group; goff[n_groups] = n_arcs
     uint2 *gkey = nullptr;        // [n_groups]   {outer symbol, target}
     uint32_t *gptr = nullptr;     // [n_states+1] first group of each state
+    unsigned long long *gmask = nullptr;   // [n_groups] inner symbols of the group as a bit mask, bit 63 = a symbol twice; only when n_inner <= 63
     fstc::AllocHooks hooks;       // who owns the arrays (set: the caller's allocator)
 };
 
@@ -63,10 +64,11 @@ struct MachineView {
     const uint32_t *goff;
     const uint2 *gkey;
     const uint32_t *gptr;
+    const unsigned long long *gmask;   // null when the inner alphabet has more than 63 symbols
 };
 
 inline MachineView view_of(const fstc_packed_t &p) {
-    return MachineView{p.arcs, p.segs, p.seg_ptr, p.flags, p.garcs, p.goff, p.gkey, p.gptr};
+    return MachineView{p.arcs, p.segs, p.seg_ptr, p.flags, p.garcs, p.goff, p.gkey, p.gptr, p.gmask};
 }
 
 fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side);

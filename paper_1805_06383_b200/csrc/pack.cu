@@ -176,6 +176,23 @@ const T *stage(Ctx &c, const T *p, int64_t n, int mem, DBuf<T> &hold) {
 
 }  // namespace
 
+// Small inner alphabets (|Γ| <= 63): the set of inner symbols of a group as a bit mask; bit 63 = the group holds the same
+// symbol twice (parallel duplicate arcs).  With the masks the merge by construction sees whether two groups share a symbol
+// with one AND, and finds the shared symbols' weights by popcount instead of walking both lists (compose.cu, k_gprod).
+constexpr unsigned long long GMASK_DUP = 1ull << 63;
+__global__ void pk_group_masks(const uint2 *__restrict__ garcs, const uint32_t *__restrict__ goff, int64_t n_groups,
+                               unsigned long long *__restrict__ gmask) {
+    const int64_t g = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (g >= n_groups) return;
+    unsigned long long m = 0;
+    for (uint32_t i = goff[g]; i < goff[g + 1]; ++i) {
+        const unsigned long long b = 1ull << garcs[i].x;
+        if (m & b) m |= GMASK_DUP;
+        m |= b;
+    }
+    gmask[g] = m;
+}
+
 void free_packed(fstc_packed_t *p) {
     if (!p) return;
     // freed stream-ordered on the legacy stream: safe after any stream of ours has been synchronised
@@ -188,6 +205,7 @@ void free_packed(fstc_packed_t *p) {
     release_block(p->goff, p->hooks);
     release_block(p->gkey, p->hooks);
     release_block(p->gptr, p->hooks);
+    release_block(p->gmask, p->hooks);
     delete p;
 }
 
@@ -242,6 +260,7 @@ fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side) {
     int64_t n_segs = 0, n_groups = 0;
     DBuf<uint2> garcs(c, n, true), gkey;
     DBuf<uint32_t> goff, gptr(c, static_cast<int64_t>(m.n_states) + 1, true);
+    DBuf<unsigned long long> gmask;
 
     if (n > 0) {
         DBuf<uint4> ra(c, n), rb(c, n);
@@ -265,6 +284,12 @@ fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side) {
                                                                                                      gptr.p);
             FSTC_LAUNCH_CHECK();
             c.n_launch += 3;
+            if (n_inner <= 63 && n_groups > 0) {
+                gmask.alloc(c, n_groups, true);
+                pk_group_masks<<<blocks_for(n_groups), PK_THREADS, 0, c.stream>>>(garcs.p, goff.p, n_groups, gmask.p);
+                FSTC_LAUNCH_CHECK();
+                c.n_launch += 1;
+            }
             c.sync();
         }
         pk_flags_rekey<<<blocks_for(n), PK_THREADS, 0, c.stream>>>(s1, n, bi, bt, bo, flags32.p, o1);
@@ -318,6 +343,7 @@ fstc_packed_t *pack_fst(Ctx &c, const fstc_fst_t &m, int side) {
     p->flags = flags.take(); p->accept_bits = accept_bits.take();
     p->n_groups = n_groups;
     p->garcs = garcs.take(); p->goff = goff.take(); p->gkey = gkey.take(); p->gptr = gptr.take();
+    p->gmask = gmask.p ? gmask.take() : nullptr;
     FSTC_CUDA(cudaGetDevice(&p->device));
     p->n_launch = c.n_launch - launch0;
     return p;

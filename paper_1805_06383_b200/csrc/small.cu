@@ -340,7 +340,7 @@ __global__ void __launch_bounds__(SP_THREADS) k_small_compose(SmallArgs g) {
         for (uint32_t r = tid; r < R; r += SP_THREADS) {
             const uint32_t i = P.t_pl[r];
             uint32_t head = 1;
-            float w = P.t_w[r];
+            float w = P.t_w[r], comp = 0.f;                            // compensated (Kahan) sum: a few ulp whatever the run length
             if (P.cls[i]) {
                 const uint32_t lo = P.roff[i], hi = lo + P.raw[i];
                 const uint32_t t = P.t_tgt[r], a = P.t_a[r], b = P.t_b[r];
@@ -348,7 +348,11 @@ __global__ void __launch_bounds__(SP_THREADS) k_small_compose(SmallArgs g) {
                     if (P.t_tgt[q] == t && P.t_a[q] == a && P.t_b[q] == b) { head = 0; break; }
                 if (head)
                     for (uint32_t q = r + 1; q < hi; ++q)
-                        if (P.t_tgt[q] == t && P.t_a[q] == a && P.t_b[q] == b) w += P.t_w[q];
+                        if (P.t_tgt[q] == t && P.t_a[q] == a && P.t_b[q] == b) {
+                            const float y = P.t_w[q] - comp, s2 = w + y;
+                            comp = (s2 - w) - y;
+                            w = s2;
+                        }
             }
             P.hidx[r] = head;
             P.t_ws[r] = w;

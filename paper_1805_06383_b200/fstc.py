@@ -78,7 +78,7 @@ class _Stats(ctypes.Structure):
         ("rs_scatter_recs", ctypes.c_int64), ("rs_scatter_dest_recs", ctypes.c_int64), ("rs_dedupe_arcs", ctypes.c_int64),
         ("rs_dedupe_states", ctypes.c_int64), ("rs_dedupe_new", ctypes.c_int64), ("rs_gather_recs", ctypes.c_int64),
         ("rs_scatter_launches", ctypes.c_int32), ("rs_dedupe_launches", ctypes.c_int32),
-        ("rs_gather_launches", ctypes.c_int32), ("pad2_", ctypes.c_int32),
+        ("rs_gather_launches", ctypes.c_int32), ("n_chunks", ctypes.c_int32),
         ("spill_bytes", ctypes.c_int64), ("spill_bytes_saved", ctypes.c_int64),
         ("ms", ctypes.c_double * len(STAGES)), ("ms_total", ctypes.c_double),
         ("level_frontier", ctypes.c_int64 * MAX_LEVEL_STATS), ("level_raw", ctypes.c_int64 * MAX_LEVEL_STATS),
@@ -297,7 +297,7 @@ def stats_dict(s: _Stats) -> dict:
         "n_rehash": int(s.n_rehash), "n_grow": int(s.n_grow), "n_emit_launches": int(s.n_emit_launches),
         "n_kernel_launches": int(s.n_kernel_launches),
         "n_resolve": int(s.n_resolve), "n_resolved_arcs": int(s.n_resolved_arcs), "small_path": int(s.small_path),
-        "spill_bytes": int(s.spill_bytes), "spill_bytes_saved": int(s.spill_bytes_saved),
+        "n_chunks": int(s.n_chunks), "spill_bytes": int(s.spill_bytes), "spill_bytes_saved": int(s.spill_bytes_saved),
         **{k: int(getattr(s, k)) for k in ("rs_scatter_recs", "rs_scatter_dest_recs", "rs_dedupe_arcs", "rs_dedupe_states",
                                            "rs_dedupe_new", "rs_gather_recs", "rs_scatter_launches", "rs_dedupe_launches",
                                            "rs_gather_launches")},

@@ -154,3 +154,23 @@ def test_deterministic_ids_and_arc_order(fstc, config, scale, budget, kw, monkey
         assert r2.stats["n_raw_sorted"] > 0 and torch.equal(r2.tgt, r3.tgt) and torch.equal(r2.pair, r3.pair)
         assert torch.equal(r2.ilabel, r3.ilabel) and torch.equal(r2.olabel, r3.olabel)
         check_parity(fstc, m1, m2, max_raw_arcs=budget, result=r2)
+
+
+@pytest.mark.parametrize("config,scale,chunk,kw", [
+    ("tiny", 1.0, 100, {}), ("tiny", 1.0, 7, {"merge_mode": 2}), ("medium", 0.05, 200_000, {}),
+    ("medium", 0.03, 50_000, {"resolve_mode": 2}), ("skewed", 0.05, 2_000_000, {"max_levels": 2}),
+    ("large", 0.02, 600_000, {"max_levels": 3, "resolve_mode": 2}), ("medium", 0.03, 40_000, {"deterministic": True}),
+])
+def test_levels_too_big_for_the_workspace_go_chunk_by_chunk(fstc, config, scale, chunk, kw, monkeypatch):
+    """FSTC_CHUNK_ARCS lowers the number of raw arcs a level may hold in one piece (by default about half the device memory
+    / 72 bytes): bigger levels are expanded as id ranges of the frontier, one after the other; the result is the same."""
+    monkeypatch.setenv("FSTC_CHUNK_ARCS", str(chunk))
+    m1, m2 = workloads.make_config(config, scale=scale)
+    a, b = fstc.DeviceFst.from_host(m1), fstc.DeviceFst.from_host(m2)
+    res = fstc.fstc_compose(a, b, small_path=1, **kw)
+    assert res.stats["n_chunks"] >= 3
+    check_parity(fstc, m1, m2, merge_mode=kw.get("merge_mode", 0), max_levels=kw.get("max_levels", 0), result=res)
+    # a budget cut inside a big level: the level is not chunked (rule T orders it by key), the result is still exact
+    budget = max(1, res.n_raw_arcs // 2)
+    cut = fstc.fstc_compose(a, b, small_path=1, max_raw_arcs=budget, **kw)
+    check_parity(fstc, m1, m2, merge_mode=kw.get("merge_mode", 0), max_levels=kw.get("max_levels", 0), max_raw_arcs=budget, result=cut)
