@@ -245,6 +245,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--fixed-warmup", action="store_true", help="exactly --warmup untimed steps (profiler runs), no settling loop")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -307,12 +308,12 @@ def main():
     # warm-up: at least W (>= 3) untimed steps; then, while the machine is still settling (memory pools filling, clocks
     # ramping), up to 30 more until three steps in a row agree within 2 % of the fastest step seen
     n_warm, recent, best = 0, [], float("inf")
-    while n_warm < max(args.warmup, 3) + 30:
+    while n_warm < (max(args.warmup, 3) + 30 if not args.fixed_warmup else args.warmup):
         ms, st, _ = step()
         n_warm += 1
         best = min(best, ms)
         recent = (recent + [ms])[-3:]
-        if n_warm >= max(args.warmup, 3) and len(recent) == 3 and max(recent) <= 1.02 * best:
+        if not args.fixed_warmup and n_warm >= max(args.warmup, 3) and len(recent) == 3 and max(recent) <= 1.02 * best:
             break
     barrier()
     sampler = ClockSampler(local_rank)
