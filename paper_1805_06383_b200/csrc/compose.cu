@@ -964,45 +964,51 @@ __global__ void k_place_merged(const unsigned long long *__restrict__ mkey, cons
 }
 
 // ------------------------------------------------------------------------------------------ assembly
-// Accept list (ascending ids with q1 in F1 and q2 in F2) and expanded flags in two passes over the
-// pair table: pass 1 counts accepting states per 2048-state tile and writes `expanded`; after a scan of the tile
-// counts, pass 2 recomputes the flags and compacts each tile in order.
+// Accept list (ascending ids with q1 in F1 and q2 in F2) in two passes over the pair table: pass 1 counts
+// accepting states per 2048-state tile; after a scan of the tile counts, pass 2 recomputes the flags of the tiles that have
+// any and compacts each in order.  Expanded flags: ones before the last frontier, zeros after it, a kernel for the frontier.
 constexpr int AS_THREADS = 256;
 constexpr int AS_ITEMS = 8;
 constexpr int AS_TILE = AS_THREADS * AS_ITEMS;
 
 __device__ __forceinline__ uint32_t is_accept(int2 p, const uint32_t *acc1, const uint32_t *acc2) {
-    return ((acc1[p.x >> 5] >> (p.x & 31)) & 1u) & ((acc2[p.y >> 5] >> (p.y & 31)) & 1u);
+    // F1 is small (1 % of Q1 in the BASELINE configs): the second bitmap is only read for the pairs that pass the first
+    if (!((__ldg(acc1 + (p.x >> 5)) >> (p.x & 31)) & 1u)) return 0u;
+    return (__ldg(acc2 + (p.y >> 5)) >> (p.y & 31)) & 1u;
 }
 
-// expanded[i] = 1 for every state before the last frontier [last_lo, last_hi); inside it, 1 iff it was selected;
-// states created while expanding the frontier that stopped the search are never expanded.
+// expanded[i] for the LAST frontier [lo, hi): 1 iff it was expanded whole (mode 1) or the pair lies below the cut (mode 2).
+// (Every state before it is expanded, every state after it is not: two memsets.)
+__global__ void k_expanded_last(const int2 *__restrict__ pair, int64_t lo, int64_t hi, int mode, uint64_t nq2, uint64_t cut,
+                                uint8_t *__restrict__ expanded) {
+    const int64_t i = lo + static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= hi) return;
+    uint8_t e = mode == 1;
+    if (mode == 2) {
+        const int2 p = pair[i];
+        e = (static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y)) < cut;
+    }
+    expanded[i] = e;
+}
+
+// accepting states per 2048-state tile
 __global__ void __launch_bounds__(AS_THREADS)
 k_assemble_count(const int2 *__restrict__ pair, int64_t n, const uint32_t *__restrict__ acc1,
-                 const uint32_t *__restrict__ acc2, int64_t last_lo, int64_t last_hi,
-                 int last_mode /*0 none, 1 all, 2 cut*/, uint64_t nq2, uint64_t cut, uint8_t *__restrict__ expanded,
-                 uint32_t *__restrict__ tile_count) {
+                 const uint32_t *__restrict__ acc2, uint32_t *__restrict__ tile_count) {
     __shared__ uint32_t s_cnt;
     if (threadIdx.x == 0) s_cnt = 0;
     __syncthreads();
     const int64_t base = static_cast<int64_t>(blockIdx.x) * AS_TILE;
+    int2 p[AS_ITEMS];
+#pragma unroll
+    for (int r = 0; r < AS_ITEMS; ++r) {                      // all loads of the thread in flight together
+        const int64_t i = base + r * AS_THREADS + threadIdx.x;
+        p[r] = i < n ? __ldcs(pair + i) : make_int2(-1, -1);
+    }
     uint32_t cnt = 0;
 #pragma unroll
-    for (int r = 0; r < AS_ITEMS; ++r) {
-        const int64_t i = base + r * AS_THREADS + threadIdx.x;
-        if (i < n) {
-            const int2 p = pair[i];
-            cnt += is_accept(p, acc1, acc2);
-            uint8_t e = 1;
-            if (i >= last_hi) e = 0;
-            else if (i >= last_lo) {
-                if (last_mode == 0) e = 0;
-                else if (last_mode == 2)
-                    e = (static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y)) < cut;
-            }
-            expanded[i] = e;
-        }
-    }
+    for (int r = 0; r < AS_ITEMS; ++r)
+        if (p[r].x >= 0) cnt += is_accept(p[r], acc1, acc2);
     cnt = __reduce_add_sync(0xffffffffu, cnt);
     if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(&s_cnt, cnt);
     __syncthreads();
@@ -1144,6 +1150,21 @@ struct StageTimer {
         }
     }
 };
+
+// Total memory of a device, asked once per process: cudaMemGetInfo goes to the driver and was seen to take 10-50 ms at times
+// (the source of the 60-150 ms step-time outliers of round 1, and of +25 ms per call when it came back in round 2).
+size_t device_total_bytes(int dev) {
+    static std::mutex mu;
+    static size_t total_of[64] = {};
+    std::lock_guard<std::mutex> lk(mu);
+    size_t &slot = total_of[dev & 63];
+    if (slot == 0) {
+        size_t f = 0, t = 0;
+        (void)cudaMemGetInfo(&f, &t);
+        slot = t > 0 ? t : size_t(64) << 30;
+    }
+    return slot;
+}
 
 struct Composer {
     Ctx &c;
@@ -1593,12 +1614,8 @@ fstc_result_t *Composer::run() {
     // correct); the states every chunk creates are appended and all of them form the next frontier.  Only
     // when no budget cut falls into the level (rule T orders a cut level by key, not by id).
     int64_t chunk_limit = knob_chunk_arcs;
-    if (chunk_limit <= 0) {
-        size_t f = 0, t = 0;
-        (void)cudaMemGetInfo(&f, &t);
-        // ~52 bytes of resolve buffers and 20 of output per raw arc; and the partitioned resolve indexes records with 32 bits
-        chunk_limit = std::min<int64_t>(int64_t(3) << 30, static_cast<int64_t>(0.5 * static_cast<double>(t > 0 ? t : size_t(64) << 30) / 72.0));
-    }
+    if (chunk_limit <= 0)   // ~52 bytes of resolve buffers and 20 of output per raw arc; and the partitioned resolve indexes records with 32 bits
+        chunk_limit = std::min<int64_t>(int64_t(3) << 30, static_cast<int64_t>(0.5 * static_cast<double>(device_total_bytes(m1.device)) / 72.0));
     int64_t level_lo = 0, level_end = -1, chunk_pairs = 0;      // level_end >= 0: the level [level_lo, level_end) goes chunk by chunk
 
     for (;;) {
@@ -1792,19 +1809,7 @@ fstc_result_t *Composer::run() {
             if (o.max_raw_arcs > 0) pr = std::min(pr, static_cast<double>(o.max_raw_arcs - cum_raw - R));
             // what is free for us: the device's memory minus what our pool has handed out.  (cudaMemGetInfo would say it
             // exactly, but it goes to the driver and was seen to take 10-50 ms at times: the device size is read once.)
-            static std::mutex mu;
-            static size_t device_bytes_of[64] = {};
-            size_t device_bytes;
-            {
-                std::lock_guard<std::mutex> lk(mu);
-                size_t &slot = device_bytes_of[m1.device & 63];
-                if (slot == 0) {
-                    size_t f = 0, t = 0;
-                    (void)cudaMemGetInfo(&f, &t);
-                    slot = t > 0 ? t - t / 16 : size_t(64) << 30;                // leave 1/16 to others on the device
-                }
-                device_bytes = slot;
-            }
+            const size_t device_bytes = device_total_bytes(m1.device) - device_total_bytes(m1.device) / 16;   // leave 1/16 to others on the device
             uint64_t pool_used = 0;
             (void)cudaMemPoolGetAttribute(device_pool(), cudaMemPoolAttrUsedMemCurrent, &pool_used);
             const size_t free_b = device_bytes > pool_used ? device_bytes - pool_used : 0;
@@ -2044,8 +2049,13 @@ fstc_result_t *Composer::run() {
     const int64_t as_tiles = ceil_div(n_states, AS_TILE);
     DBuf<uint32_t> tile_count(c, as_tiles);
     DBuf<int64_t> tile_off(c, as_tiles + 1);
-    k_assemble_count<<<static_cast<unsigned>(as_tiles), AS_THREADS, 0, c.stream>>>(
-        pair.p, n_states, m1.accept_bits, m2.accept_bits, last_lo, last_hi, last_mode, nq2, cut_key, expanded.p, tile_count.p);
+    if (last_lo > 0) FSTC_CUDA(cudaMemsetAsync(expanded.p, 1, static_cast<size_t>(last_lo), c.stream));
+    if (n_states > last_hi) FSTC_CUDA(cudaMemsetAsync(expanded.p + last_hi, 0, static_cast<size_t>(n_states - last_hi), c.stream));
+    if (last_hi > last_lo) {
+        k_expanded_last<<<nblk(last_hi - last_lo), CT_THREADS, 0, c.stream>>>(pair.p, last_lo, last_hi, last_mode, nq2, cut_key, expanded.p);
+        FSTC_LAUNCH_CHECK();
+    }
+    k_assemble_count<<<static_cast<unsigned>(as_tiles), AS_THREADS, 0, c.stream>>>(pair.p, n_states, m1.accept_bits, m2.accept_bits, tile_count.p);
     FSTC_LAUNCH_CHECK();
     exclusive_scan<uint32_t>(c, tile_count.p, as_tiles, tile_off.p);
     const int64_t n_accept = read_scalar(c, tile_off.p + as_tiles);
@@ -2055,7 +2065,7 @@ fstc_result_t *Composer::run() {
             pair.p, n_states, m1.accept_bits, m2.accept_bits, tile_count.p, tile_off.p, accept.p);
         FSTC_LAUNCH_CHECK();
     }
-    c.n_launch += 2;
+    c.n_launch += 3;
     tm.end(h);
 
     if (sp) {
