@@ -87,6 +87,69 @@ __global__ void tb_dense_insert_ids(const int2 *__restrict__ pair, int64_t n, ui
     dense[static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y)] = static_cast<uint32_t>(i) + 1u;
 }
 
+// ------------------------------------------------------------------------------------------ find or insert, one key per thread
+// The visited-set step of PAPER.md:237-239 for one key per thread of a block (all threads call it, `valid` or not): the
+// dense table (entry = id + 1, 0 = not visited) or the open-addressing hash table; the new ids of the block come from one
+// atomicAdd, the winner of a key publishes the id and writes pair[id], a thread that met a pending entry waits for it.
+// Same protocol as inside k_emit.  s_warp: [THREADS / 32] shared words, s_base: one shared 64-bit word.
+template <bool DENSE, int THREADS>
+__device__ __forceinline__ uint32_t block_find_or_insert(unsigned long long key, bool valid, int2 tgt_pair, uint32_t *dense, uint4 *table,
+                                                         uint64_t cap, unsigned long long *n_states, int2 *pair, uint32_t *s_warp,
+                                                         unsigned long long *s_base) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    uint32_t id = 0;
+    bool won = false;
+    uint32_t *slotp = nullptr;                                   // where the id is (or will be) published
+    if (valid) {
+        if (DENSE) {
+            slotp = dense + key;
+            uint32_t v = __ldcg(slotp);
+            if (v == 0u) v = atomicCAS(slotp, 0u, PENDING_ID);
+            if (v == 0u) won = true; else id = v == PENDING_ID ? PENDING_ID : v - 1u;
+        } else {
+            const uint64_t n_buckets = cap >> 1;
+            uint64_t b = home_bucket(key, cap);
+            while (true) {
+                Bucket v = ld_bucket(table, b);
+                const unsigned long long k0 = slot_key(v.s0), k1 = slot_key(v.s1);
+                int cas = -1;
+                if (k0 == key) { id = v.s0.z; slotp = reinterpret_cast<uint32_t *>(table + 2 * b) + 2; break; }
+                else if (k0 == EMPTY_KEY) cas = 0;
+                else if (k1 == key) { id = v.s1.z; slotp = reinterpret_cast<uint32_t *>(table + 2 * b + 1) + 2; break; }
+                else if (k1 == EMPTY_KEY) cas = 1;
+                if (cas < 0) { b = (b + 1 == n_buckets) ? 0 : b + 1; continue; }
+                const unsigned long long old = atomicCAS(reinterpret_cast<unsigned long long *>(table + 2 * b + cas), EMPTY_KEY, key);
+                if (old == EMPTY_KEY || old == key) {
+                    slotp = reinterpret_cast<uint32_t *>(table + 2 * b + cas) + 2;
+                    if (old == EMPTY_KEY) won = true; else id = PENDING_ID;
+                    break;
+                }                                                // another key took the slot: look at the bucket again
+            }
+        }
+    }
+    const uint32_t bal = __ballot_sync(0xffffffffu, won);
+    if (lane == 0) s_warp[warp] = __popc(bal);
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t tot = 0;
+#pragma unroll
+        for (int wv = 0; wv < THREADS / 32; ++wv) { uint32_t cnt = s_warp[wv]; s_warp[wv] = tot; tot += cnt; }
+        *s_base = tot ? atomicAdd(n_states, static_cast<unsigned long long>(tot)) : 0ull;
+    }
+    __syncthreads();
+    if (won) {
+        id = static_cast<uint32_t>(*s_base) + s_warp[warp] + __popc(bal & ((1u << lane) - 1u));
+        __stcg(slotp, DENSE ? id + 1u : id);
+        pair[id] = tgt_pair;
+    } else if (valid && id == PENDING_ID) {
+        uint32_t v;
+        while ((v = __ldcg(slotp)) == PENDING_ID) __nanosleep(20);
+        id = DENSE ? v - 1u : v;
+    }
+    __syncthreads();                                             // s_warp / s_base may be reused by the next call
+    return id;
+}
+
 // ------------------------------------------------------------------------------------------ count / match
 // Intersection of the two states' sorted inner-symbol lists.  F is called for every shared symbol with
 // (first arc of q1's segment, n1, first arc of q2's segment, n2).
@@ -639,6 +702,14 @@ struct GProdArgs {
     unsigned long long *mkey;    //   target key (table: r1 * |Q2| + r2; partitioned resolve: (r1 << q2_bits) | r2)
     int bits_b, q2_bits;         // q2_bits < 0: table key
     uint64_t nq2;
+    uint16_t *eprefix;           // [tiles * GP_THREADS] arcs of the tile before the thread's ranks (pass 0 -> k_gcount, pass 2)
+    // pass 2 (fused: weights, visited table, final place in one kernel; table levels only)
+    uint32_t *dense; uint4 *table; uint64_t cap;
+    unsigned long long *n_states; int2 *pair;
+    const int64_t *mstart, *foff;    // per pair of the level: first merged class-G arc, first final arc
+    int64_t arc_base, f_lo;
+    const uint32_t *sel;
+    int32_t *o_src, *o_il, *o_ol, *o_tgt; float *o_w;
 };
 
 // compensated (Kahan) fp32 accumulation: the error of a sum of n terms stays at a few ulp whatever n, so that a run of
@@ -684,7 +755,7 @@ __device__ __forceinline__ float group_dot(const uint2 *__restrict__ ga, uint32_
 constexpr int GP_THREADS = 128, GP_IPT = 4, GP_TILE = GP_THREADS * GP_IPT;
 static_assert(GP_TILE == EM_TILE, "k_partition places tiles of EM_TILE ranks");
 
-template <int PASS>
+template <int PASS, bool DENSE>
 __global__ void __launch_bounds__(GP_THREADS) k_gprod(GProdArgs g) {
     __shared__ uint32_t relcum[GP_TILE + 1];
     __shared__ int64_t s_first_cum;
@@ -761,9 +832,10 @@ __global__ void __launch_bounds__(GP_THREADS) k_gprod(GProdArgs g) {
     for (int wv = 0; wv < GP_THREADS / 32; ++wv) { if (wv < warp) before += s_warp[wv]; total += s_warp[wv]; }
     if (PASS == 0) {
         g.ebits[static_cast<int64_t>(blockIdx.x) * GP_THREADS + tid] = static_cast<uint8_t>(exists);
+        g.eprefix[static_cast<int64_t>(blockIdx.x) * GP_THREADS + tid] = static_cast<uint16_t>(before);
         if (tid == 0) g.tile_cnt[blockIdx.x] = total;
     }
-    if (PASS != 1) return;
+    if constexpr (PASS != 0) {
     // pass 1: typically a third of a tile's ranks give an arc.  They are packed first (rank order), so that every lane of the
     // weight loop below has an arc to work on and the outputs of a warp are neighbours.
     __shared__ uint32_t s_g1[GP_TILE], s_g2[GP_TILE], s_pl[GP_TILE];
@@ -774,8 +846,12 @@ __global__ void __launch_bounds__(GP_THREADS) k_gprod(GProdArgs g) {
     __syncthreads();
     const bool masks = g.A.gmask != nullptr && g.B.gmask != nullptr;
     const int64_t q0 = g.tile_off[blockIdx.x];
-    for (uint32_t k = tid; k < total; k += GP_THREADS) {
-        const uint32_t g1 = s_g1[k], g2 = s_g2[k];
+    __shared__ unsigned long long s_base;
+    for (uint32_t kb = 0; kb < total; kb += GP_THREADS) {          // (uniform trip count: pass 2 has block barriers inside)
+        const uint32_t k = kb + tid;
+        const bool valid = k < total;
+        if (PASS == 1 && !valid) continue;
+        const uint32_t g1 = valid ? s_g1[k] : s_g1[0], g2 = valid ? s_g2[k] : s_g2[0];
         const uint32_t a0 = g.A.goff[g1], b0 = g.B.goff[g2];
         float wv;
         unsigned long long m1 = 0, m2 = 0;
@@ -794,13 +870,42 @@ __global__ void __launch_bounds__(GP_THREADS) k_gprod(GProdArgs g) {
             wv = group_dot(g.A.garcs, a0, g.A.goff[g1 + 1], g.B.garcs, b0, g.B.goff[g2 + 1], false, &found);
         }
         const uint2 k1 = g.A.gkey[g1], k2 = g.B.gkey[g2];                 // {outer, tgt}
-        const int64_t q = q0 + k;
-        g.msrc[q] = s_pl[k];
-        g.mab[q] = (k1.x << g.bits_b) | k2.x;
-        g.mw[q] = wv;
-        g.mkey[q] = g.q2_bits >= 0 ? ((static_cast<unsigned long long>(k1.y) << g.q2_bits) | k2.y)
-                                   : static_cast<unsigned long long>(k1.y) * g.nq2 + k2.y;
+        if (PASS == 1) {
+            const int64_t q = q0 + k;
+            g.msrc[q] = s_pl[k];
+            g.mab[q] = (k1.x << g.bits_b) | k2.x;
+            g.mw[q] = wv;
+            g.mkey[q] = g.q2_bits >= 0 ? ((static_cast<unsigned long long>(k1.y) << g.q2_bits) | k2.y)
+                                       : static_cast<unsigned long long>(k1.y) * g.nq2 + k2.y;
+        } else {
+            // fused: the target's id from the visited table, and the arc straight to its final place behind the pair's offset
+            const unsigned long long key = static_cast<unsigned long long>(k1.y) * g.nq2 + k2.y;
+            const uint32_t id = DENSE ? block_find_or_insert<true, GP_THREADS>(key, valid, make_int2(static_cast<int>(k1.y), static_cast<int>(k2.y)), g.dense, g.table, g.cap, g.n_states, g.pair, s_warp, &s_base)
+                                      : block_find_or_insert<false, GP_THREADS>(key, valid, make_int2(static_cast<int>(k1.y), static_cast<int>(k2.y)), g.dense, g.table, g.cap, g.n_states, g.pair, s_warp, &s_base);
+            if (valid) {
+                const uint32_t p = s_pl[k];
+                const int64_t q = g.arc_base + g.foff[p] + (q0 + k - g.mstart[p]);
+                g.o_src[q] = static_cast<int>(g.f_lo + (g.sel ? g.sel[p] : p));
+                g.o_il[q] = static_cast<int>(k1.x); g.o_ol[q] = static_cast<int>(k2.x);
+                g.o_tgt[q] = static_cast<int>(id); g.o_w[q] = wv;
+            }
+        }
     }
+}   // PASS != 0
+}
+
+// Merged class-G arcs per pair of the level, from what pass 0 left (ebits, eprefix, tile_off): cntG[pair] = arcs among the
+// pair's ranks [cum[m], cum[m+1]).  (One match per class-G pair; the other pairs keep 0.)
+__device__ __forceinline__ int64_t g_arcs_before(const GProdArgs &g, int64_t r) {      // existing ranks < r
+    const int64_t t = r / GP_TILE;
+    const int64_t th = t * GP_THREADS + (r % GP_TILE) / GP_IPT;
+    if (r >= g.W) return g.tile_off[(g.W + GP_TILE - 1) / GP_TILE];
+    return g.tile_off[t] + g.eprefix[th] + __popc(g.ebits[th] & ((1u << (r % GP_IPT)) - 1u));
+}
+__global__ void k_gcount(GProdArgs g, int64_t *__restrict__ cntG) {
+    const int64_t m = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (m >= g.n_matches) return;
+    cntG[g.L.pl[m]] = g_arcs_before(g, g.L.cum[m + 1]) - g_arcs_before(g, g.L.cum[m]);
 }
 
 // Ids of a list of target keys through the visited table (dense or hash), outside the emit kernel: one key per thread,
@@ -811,60 +916,12 @@ k_resolve_keys(const unsigned long long *__restrict__ keys, int64_t n, uint32_t 
                unsigned long long *n_states, int2 *pair, int32_t *__restrict__ ids) {
     __shared__ uint32_t s_warp[CT_THREADS / 32];
     __shared__ unsigned long long s_base;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + tid;
+    const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     const bool valid = i < n;
-    unsigned long long key = valid ? keys[i] : 0ull;
-    uint32_t id = 0;
-    bool won = false;
-    uint32_t *slotp = nullptr;                                   // where the id is (or will be) published
-    if (valid) {
-        if (DENSE) {
-            slotp = dense + key;
-            uint32_t v = __ldcg(slotp);
-            if (v == 0u) v = atomicCAS(slotp, 0u, PENDING_ID);
-            if (v == 0u) won = true; else id = v == PENDING_ID ? PENDING_ID : v - 1u;
-        } else {
-            const uint64_t n_buckets = cap >> 1;
-            uint64_t b = home_bucket(key, cap);
-            while (true) {
-                Bucket v = ld_bucket(table, b);
-                const unsigned long long k0 = slot_key(v.s0), k1 = slot_key(v.s1);
-                int cas = -1;
-                if (k0 == key) { id = v.s0.z; slotp = reinterpret_cast<uint32_t *>(table + 2 * b) + 2; break; }
-                else if (k0 == EMPTY_KEY) cas = 0;
-                else if (k1 == key) { id = v.s1.z; slotp = reinterpret_cast<uint32_t *>(table + 2 * b + 1) + 2; break; }
-                else if (k1 == EMPTY_KEY) cas = 1;
-                if (cas < 0) { b = (b + 1 == n_buckets) ? 0 : b + 1; continue; }
-                const unsigned long long old = atomicCAS(reinterpret_cast<unsigned long long *>(table + 2 * b + cas), EMPTY_KEY, key);
-                if (old == EMPTY_KEY || old == key) {
-                    slotp = reinterpret_cast<uint32_t *>(table + 2 * b + cas) + 2;
-                    if (old == EMPTY_KEY) won = true; else id = PENDING_ID;
-                    break;
-                }                                                // another key took the slot: look at the bucket again
-            }
-        }
-    }
-    const uint32_t bal = __ballot_sync(0xffffffffu, won);
-    if (lane == 0) s_warp[warp] = __popc(bal);
-    __syncthreads();
-    if (tid == 0) {
-        uint32_t tot = 0;
-#pragma unroll
-        for (int wv = 0; wv < CT_THREADS / 32; ++wv) { uint32_t cnt = s_warp[wv]; s_warp[wv] = tot; tot += cnt; }
-        s_base = tot ? atomicAdd(n_states, static_cast<unsigned long long>(tot)) : 0ull;
-    }
-    __syncthreads();
-    if (won) {
-        id = static_cast<uint32_t>(s_base) + s_warp[warp] + __popc(bal & ((1u << lane) - 1u));
-        __stcg(slotp, DENSE ? id + 1u : id);
-        const unsigned long long q1 = key / nq2;
-        pair[id] = make_int2(static_cast<int>(q1), static_cast<int>(key - q1 * nq2));
-    } else if (valid && id == PENDING_ID) {
-        uint32_t v;
-        while ((v = __ldcg(slotp)) == PENDING_ID) __nanosleep(20);
-        id = DENSE ? v - 1u : v;
-    }
+    const unsigned long long key = valid ? keys[i] : 0ull;
+    const unsigned long long q1 = key / nq2;
+    const uint32_t id = block_find_or_insert<DENSE, CT_THREADS>(key, valid, make_int2(static_cast<int>(q1), static_cast<int>(key - q1 * nq2)),
+                                                                dense, table, cap, n_states, pair, s_warp, &s_base);
     if (valid) ids[i] = static_cast<int32_t>(id);
 }
 
@@ -1902,6 +1959,8 @@ fstc_result_t *Composer::run() {
             DBuf<float> gw;
             DBuf<int32_t> gtgt;
             DBuf<int64_t> mstartG;
+            DBuf<int64_t> fc, foff;                                  // final arcs per pair of the level, and their offsets
+            bool g_placed = false;                                   // the class-G arcs are already in their final place (fused pass)
             if (RG > 0) {
                 h = tm.begin(FSTC_T_REDUCE);
                 DBuf<int64_t> cumG(c, MG + 1);
@@ -1915,22 +1974,51 @@ fstc_result_t *Composer::run() {
                 DBuf<int64_t> tile_m(c, n_tiles + 1), tile_off(c, n_tiles + 1);
                 DBuf<uint32_t> tile_cnt(c, n_tiles);
                 DBuf<uint8_t> ebits(c, n_tiles * GP_THREADS);
+                DBuf<uint16_t> eprefix(c, n_tiles * GP_THREADS);
                 k_partition<<<nblk(n_tiles + 1), CT_THREADS, 0, c.stream>>>(cumG.p, MG, WG, 0, n_tiles, tile_m.p);
                 FSTC_LAUNCH_CHECK();
                 GProdArgs g;
                 g.A = A; g.B = B; g.L = LG; g.n_matches = MG; g.W = WG; g.tile_m = tile_m.p;
-                g.tile_cnt = tile_cnt.p; g.tile_off = nullptr; g.ebits = ebits.p;
+                g.tile_cnt = tile_cnt.p; g.tile_off = nullptr; g.ebits = ebits.p; g.eprefix = eprefix.p;
                 g.msrc = nullptr; g.mab = nullptr; g.mw = nullptr; g.mkey = nullptr;
+                g.dense = dense.p; g.table = table.p; g.cap = cap; g.n_states = d_counters.p; g.pair = pair.p;
+                g.mstart = nullptr; g.foff = nullptr; g.arc_base = arc_base; g.f_lo = f_lo; g.sel = sel.p;
+                g.o_src = o_src; g.o_il = o_il; g.o_ol = o_ol; g.o_tgt = o_tgt; g.o_w = o_w;
                 g.bits_b = bits_b; g.nq2 = nq2;
                 g.q2_bits = partitioned ? bits_for(nq2 > 1 ? nq2 - 1 : 1) : -1;
-                k_gprod<0><<<static_cast<unsigned>(n_tiles), GP_THREADS, 0, c.stream>>>(g);
+                k_gprod<0, false><<<static_cast<unsigned>(n_tiles), GP_THREADS, 0, c.stream>>>(g);
                 FSTC_LAUNCH_CHECK();
                 exclusive_scan<uint32_t>(c, tile_cnt.p, n_tiles, tile_off.p);
                 MGm = read_scalar(c, tile_off.p + n_tiles);
+                g.tile_off = tile_off.p;
+                if (!partitioned && !o.deterministic && MGm > 0) {
+                    // table level: ONE more kernel computes the weights, resolves the targets in the visited table and writes
+                    // the arcs to their final place; for that the per-pair counts come from what pass 0 left behind
+                    DBuf<int64_t> cntG(c, nf);
+                    FSTC_CUDA(cudaMemsetAsync(cntG.p, 0, sizeof(int64_t) * nf, c.stream));
+                    k_gcount<<<nblk(MG), CT_THREADS, 0, c.stream>>>(g, cntG.p);
+                    FSTC_LAUNCH_CHECK();
+                    mstartG.alloc(c, nf + 1);
+                    exclusive_scan<int64_t>(c, cntG.p, nf, mstartG.p);
+                    fc.alloc(c, nf); foff.alloc(c, nf + 1);
+                    k_final_counts<<<nblk(nf), CT_THREADS, 0, c.stream>>>(rawU.p, mstartS.p, mstartG.p, nf, fc.p);
+                    FSTC_LAUNCH_CHECK();
+                    exclusive_scan<int64_t>(c, fc.p, nf, foff.p);
+                    g.mstart = mstartG.p; g.foff = foff.p;
+                    if (use_dense) k_gprod<2, true><<<static_cast<unsigned>(n_tiles), GP_THREADS, 0, c.stream>>>(g);
+                    else k_gprod<2, false><<<static_cast<unsigned>(n_tiles), GP_THREADS, 0, c.stream>>>(g);
+                    FSTC_LAUNCH_CHECK();
+                    c.n_launch += 6;
+                    tm.end(h);
+                    n_states_live = static_cast<int64_t>(read_scalar(c, d_counters.p));
+                    g_placed = true;
+                    st.n_raw_grouped += RG;
+                    c.sync();
+                } else {
                 gsrc.alloc(c, MGm); gab.alloc(c, MGm); gw.alloc(c, MGm); gtgt.alloc(c, MGm);
                 DBuf<unsigned long long> gkeys(c, MGm + 2);
                 g.tile_off = tile_off.p; g.msrc = gsrc.p; g.mab = gab.p; g.mw = gw.p; g.mkey = gkeys.p;
-                k_gprod<1><<<static_cast<unsigned>(n_tiles), GP_THREADS, 0, c.stream>>>(g);
+                k_gprod<1, false><<<static_cast<unsigned>(n_tiles), GP_THREADS, 0, c.stream>>>(g);
                 FSTC_LAUNCH_CHECK();
                 c.n_launch += 4;
                 tm.end(h);
@@ -1965,13 +2053,16 @@ fstc_result_t *Composer::run() {
                 c.n_launch += 1;
                 st.n_raw_grouped += RG;
                 c.sync();
+                }
             }
             // ---- final place of every arc of the level
             h = tm.begin(FSTC_T_REDUCE);
-            DBuf<int64_t> fc(c, nf), foff(c, nf + 1);
-            k_final_counts<<<nblk(nf), CT_THREADS, 0, c.stream>>>(rawU.p, mstartS.p, mstartG.p, nf, fc.p);
-            FSTC_LAUNCH_CHECK();
-            exclusive_scan<int64_t>(c, fc.p, nf, foff.p);
+            if (!g_placed) {
+                fc.alloc(c, nf); foff.alloc(c, nf + 1);
+                k_final_counts<<<nblk(nf), CT_THREADS, 0, c.stream>>>(rawU.p, mstartS.p, mstartG.p, nf, fc.p);
+                FSTC_LAUNCH_CHECK();
+                exclusive_scan<int64_t>(c, fc.p, nf, foff.p);
+            }
             DBuf<uint32_t> rank;
             int64_t det_n1 = 0;
             if (o.deterministic) {
@@ -1999,7 +2090,7 @@ fstc_result_t *Composer::run() {
                                                                      shift_t, bits_b, o_src, o_il, o_ol, o_tgt, o_w);
                 FSTC_LAUNCH_CHECK();
             }
-            if (MGm > 0) {
+            if (MGm > 0 && !g_placed) {
                 k_place_grouped<<<nblk(MGm), CT_THREADS, 0, c.stream>>>(gab.p, gtgt.p, gsrc.p, gw.p, MGm, mstartG.p, foff.p, arc_base,
                                                                        f_lo, sel.p, bits_b, o_src, o_il, o_ol, o_tgt, o_w,
                                                                        n_states, det_n1, o.deterministic ? rank.p : nullptr);
