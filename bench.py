@@ -242,6 +242,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--merge-mode", type=int, default=0)
     ap.add_argument("--resolve-mode", type=int, default=0, help="0 auto, 1 visited table only, 2 partitioned resolve only")
+    ap.add_argument("--deterministic", action="store_true", help="fstc_opts_t.deterministic: ids in key order inside every level")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -290,7 +291,7 @@ def main():
         t2 = time.perf_counter()
         e1.record()
         r = fstc.fstc_compose_packed(p1, p2, merge_mode=args.merge_mode, max_raw_arcs=budget, profile=profile,
-                                     resolve_mode=args.resolve_mode)
+                                     resolve_mode=args.resolve_mode, deterministic=args.deterministic)
         t3 = time.perf_counter()
         e2.record()
         torch.cuda.synchronize()
@@ -371,7 +372,7 @@ def main():
         "warmup": n_warm, "ms_per_step": t_ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": WORKLOAD_DESC[args.workload], "name": args.workload, "seeds": [s1, s2],
-                   "max_raw_arcs": budget, "merge_mode": args.merge_mode, "resolve_mode": args.resolve_mode, "parallelism": f"replicas x{world}",
+                   "max_raw_arcs": budget, "merge_mode": args.merge_mode, "resolve_mode": args.resolve_mode, "deterministic": bool(args.deterministic), "parallelism": f"replicas x{world}",
                    "cache": "L2 flushed (256 MiB write) before every step; working set >> L2"},
         "result": {"small_path": st["small_path"], "n_states": st["n_states"], "n_arcs": st["n_arcs"], "n_raw_arcs": st["n_raw_arcs"],
                    "n_levels": st["n_levels"], "truncated": st["truncated"], "n_expanded": st["n_expanded"],

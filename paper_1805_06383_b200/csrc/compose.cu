@@ -353,6 +353,7 @@ __device__ __forceinline__ uint4 ld_keep(const uint4 *ptr, uint64_t policy) {
 constexpr int64_t RESOLVE_MIN_ARCS = FSTC_RESOLVE_MIN_ARCS;          // smaller levels always use the table
 constexpr uint64_t DENSE_MAX_PAIRS = 1ull << 29;                     // dense visited table (4 B per pair) up to 2 GB
 constexpr uint64_t RESOLVE_TABLE_BYTES = 96ull << 20;               // a table beyond this no longer lives in L2
+constexpr int64_t DORD_MIN_ARCS = int64_t(1) << 20;                  // smaller levels are not worth a scan of the dense table
 // unit costs measured on a B200, in picoseconds
 constexpr double COST_PROBE_PS = 21.0;            // random 32-byte sector read: one probe
 constexpr double COST_INSERT_PS = 75.0;           // CAS write-back + id publish of a new state
@@ -413,10 +414,13 @@ __global__ void k_partition(const int64_t *__restrict__ cum, int64_t n_matches, 
 // table, or, when |Q1||Q2| is small enough, the paper's dense table of one entry per pair (entry =
 // id + 1, 0 = not visited).  RES_KEYS: the kernel leaves the target column open and writes the target key of every
 // arc for resolve_partitioned.
-enum { RES_HASH = 0, RES_KEYS = 1, RES_DENSE = 2 };
+// RES_DORD: dense table, ids in KEY ORDER: the kernel only marks the targets it meets for the first time (entry 0 -> PENDING)
+// and leaves ~key in the target column of arcs to unnumbered states; k_dord_* number the marked entries in a scan of the table
+// (ascending key) and k_dord_fix completes the target column.
+enum { RES_HASH = 0, RES_KEYS = 1, RES_DENSE = 2, RES_DORD = 3 };
 template <int MODE, int RES>
 __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
-    constexpr bool KEYS = RES == RES_KEYS, DENSE = RES == RES_DENSE;
+    constexpr bool KEYS = RES == RES_KEYS, DENSE = RES == RES_DENSE, DORD = RES == RES_DORD;
     __shared__ uint32_t relcum[EM_TILE + 1];
     __shared__ int64_t s_first_cum;
     __shared__ uint32_t s_warp[EM_THREADS / 32];
@@ -522,6 +526,16 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
                 if (u >= skip && u < skip + n_valid)
                     g.posout[rank0 + u] = static_cast<uint32_t>(g.foff[pl[u]] + (rank0 + u - g.roff[pl[u]]));
         }
+    } else if (DORD) {
+        uint32_t v[EM_IPT];
+#pragma unroll
+        for (int u = 0; u < EM_IPT; ++u) v[u] = (todo >> u & 1u) ? __ldcg(g.dense + key[u]) : 1u;
+#pragma unroll
+        for (int u = 0; u < EM_IPT; ++u)
+            if ((todo >> u & 1u) && v[u] == 0u) v[u] = atomicCAS(g.dense + key[u], 0u, PENDING_ID);
+#pragma unroll
+        for (int u = 0; u < EM_IPT; ++u)
+            id[u] = (v[u] == 0u || v[u] == PENDING_ID) ? ~static_cast<uint32_t>(key[u]) : v[u] - 1u;   // (keys < 2^29: ~key < 0 as int32)
     } else {
     // ---- visited set: find or insert.  Rounds of: all pending bucket reads in flight
     // together, then all pending CAS in flight together; a rank leaves when it finds its key or wins a slot.
@@ -1160,6 +1174,62 @@ __global__ void k_det_funpack(const uint4 *__restrict__ rec, int64_t n, unsigned
     mw[j] = __uint_as_float(r.w);
 }
 
+// ------------------------------------------------------------------------------------------ dense table, ids in key order
+// After k_emit<DIRECT, RES_DORD>: the entries of the dense table that hold PENDING are the states this level created.  A scan
+// of the table numbers them in ascending key order (count per tile of DO_TILE entries, scan, assign) and writes pair[]; the
+// arcs whose target column holds ~key get their id from the table.  The ids do not depend on thread scheduling, and the
+// next level's frontier is sorted by (q1, q2): consecutive pairs share q1's arcs and the table rows of their targets, which
+// is worth more than the scan costs when the table is far larger than L2 (`medium`: emit 27 -> 19 ms).
+constexpr int DO_THREADS = 256, DO_ITEMS = 8, DO_TILE = DO_THREADS * DO_ITEMS;
+__global__ void __launch_bounds__(DO_THREADS) k_dord_count(const uint32_t *__restrict__ dense, uint64_t n, uint32_t *__restrict__ tile_cnt) {
+    __shared__ uint32_t s_cnt;
+    if (threadIdx.x == 0) s_cnt = 0;
+    __syncthreads();
+    const uint64_t base = static_cast<uint64_t>(blockIdx.x) * DO_TILE;
+    uint32_t c = 0;
+#pragma unroll
+    for (int r = 0; r < DO_ITEMS; ++r) {
+        const uint64_t i = base + static_cast<uint64_t>(r) * DO_THREADS + threadIdx.x;
+        if (i < n && __ldcs(dense + i) == PENDING_ID) ++c;
+    }
+    c = __reduce_add_sync(0xffffffffu, c);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(&s_cnt, c);
+    __syncthreads();
+    if (threadIdx.x == 0) tile_cnt[blockIdx.x] = s_cnt;
+}
+__global__ void __launch_bounds__(DO_THREADS) k_dord_assign(uint32_t *__restrict__ dense, uint64_t n, uint64_t nq2, const uint32_t *__restrict__ tile_cnt,
+                                                             const int64_t *__restrict__ tile_off, int64_t n0, int2 *__restrict__ pair) {
+    if (tile_cnt[blockIdx.x] == 0) return;
+    __shared__ uint32_t s_warp[DO_THREADS / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint64_t base = static_cast<uint64_t>(blockIdx.x) * DO_TILE;
+    int64_t off = n0 + tile_off[blockIdx.x];
+    for (int r = 0; r < DO_ITEMS; ++r) {                        // rows of 256 consecutive keys, in order
+        const uint64_t i = base + static_cast<uint64_t>(r) * DO_THREADS + threadIdx.x;
+        const bool f = i < n && dense[i] == PENDING_ID;
+        const uint32_t b = __ballot_sync(0xffffffffu, f);
+        if (lane == 0) s_warp[warp] = __popc(b);
+        __syncthreads();
+        uint32_t before = 0, total = 0;
+#pragma unroll
+        for (int wv = 0; wv < DO_THREADS / 32; ++wv) { const uint32_t c = s_warp[wv]; if (wv < warp) before += c; total += c; }
+        if (f) {
+            const int64_t id = off + before + __popc(b & ((1u << lane) - 1u));
+            dense[i] = static_cast<uint32_t>(id) + 1u;
+            const uint64_t q1 = i / nq2;
+            pair[id] = make_int2(static_cast<int>(q1), static_cast<int>(i - q1 * nq2));
+        }
+        off += total;
+        __syncthreads();
+    }
+}
+__global__ void k_dord_fix(int32_t *__restrict__ tgt, int64_t n, const uint32_t *__restrict__ dense) {
+    const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int32_t t = __ldcs(tgt + i);
+    if (t < 0) tgt[i] = static_cast<int32_t>(__ldcg(dense + static_cast<uint32_t>(~t)) - 1u);
+}
+
 // Level compaction: when rule T will clearly cut the level, only the pairs below a key limit are worked on.
 __global__ void k_flag_below(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, uint64_t nq2, uint64_t key_limit,
                              uint8_t *__restrict__ flag) {
@@ -1353,6 +1423,7 @@ struct Composer {
     bool knob_no_group = false;          // FSTC_NO_GROUP_MERGE: class G off
     double knob_limit_margin = 1.5;      // FSTC_KEY_LIMIT_MARGIN: the guessed key limit of a level that will be cut
     int64_t knob_chunk_arcs = 0;         // FSTC_CHUNK_ARCS: raw arcs a level may hold before it is expanded in chunks
+    bool knob_no_dord = false;           // FSTC_NO_KEY_ORDER: dense-table levels never number their states in key order
 
     Composer(Ctx &ctx, const fstc_packed_t &a, const fstc_packed_t &b, const fstc_opts_t &opts)
         : c(ctx), m1(a), m2(b), o(opts), tm(ctx, opts.profile != 0), nq2(static_cast<uint64_t>(b.n_states)) {
@@ -1361,6 +1432,7 @@ struct Composer {
         knob_no_group = getenv("FSTC_NO_GROUP_MERGE") != nullptr;
         if (const char *e = getenv("FSTC_KEY_LIMIT_MARGIN")) knob_limit_margin = atof(e);
         if (const char *e = getenv("FSTC_CHUNK_ARCS")) knob_chunk_arcs = atoll(e);
+        knob_no_dord = getenv("FSTC_NO_KEY_ORDER") != nullptr;
     }
 
     // Growable outputs and table.  `need` is what the coming launch requires; `want` >= need is a look-ahead
@@ -1498,6 +1570,32 @@ struct Composer {
 
     // partitioned = true: the level's target ids come from resolve_partitioned (no visited table)
     bool partitioned = false;
+    bool dense_ordered = false;          // this level numbers its new states in key order (RES_DORD; dense table levels without merges)
+    // numbers the PENDING entries of the dense table in ascending key order (ids from n0), completes the target column of the
+    // arcs [a0, a1); returns the number of states after it
+    int64_t dense_number_pending(int64_t n0, int64_t a0, int64_t a1) {
+        const int h = tm.begin(FSTC_T_TABLE);
+        const int64_t tiles = ceil_div(static_cast<int64_t>(n_pairs_all), DO_TILE);
+        DBuf<uint32_t> tile_cnt(c, tiles);
+        DBuf<int64_t> tile_off(c, tiles + 1);
+        k_dord_count<<<static_cast<unsigned>(tiles), DO_THREADS, 0, c.stream>>>(dense.p, n_pairs_all, tile_cnt.p);
+        FSTC_LAUNCH_CHECK();
+        exclusive_scan<uint32_t>(c, tile_cnt.p, tiles, tile_off.p);
+        const int64_t n_new = read_scalar(c, tile_off.p + tiles);
+        if (n0 + n_new > pair_cap) fail(FSTC_ERR_INTERNAL, "dense_number_pending: %lld new states exceed the reserved pair table", static_cast<long long>(n_new));
+        k_dord_assign<<<static_cast<unsigned>(tiles), DO_THREADS, 0, c.stream>>>(dense.p, n_pairs_all, nq2, tile_cnt.p, tile_off.p, n0, pair.p);
+        FSTC_LAUNCH_CHECK();
+        if (a1 > a0) {
+            k_dord_fix<<<nblk(a1 - a0), CT_THREADS, 0, c.stream>>>(o_tgt + a0, a1 - a0, dense.p);
+            FSTC_LAUNCH_CHECK();
+        }
+        const unsigned long long ns = static_cast<unsigned long long>(n0 + n_new);
+        FSTC_CUDA(cudaMemcpyAsync(d_counters.p, &ns, sizeof ns, cudaMemcpyHostToDevice, c.stream));
+        c.n_launch += 3;
+        tm.end(h);
+        c.sync();
+        return n0 + n_new;
+    }
     int key_bits = 0;
     const uint32_t *cur_sel = nullptr;  // compaction of the level being expanded (null: none)
     int64_t n_states_live = 1;         // states created so far, including those of the launches of this level
@@ -1531,7 +1629,8 @@ struct Composer {
             else if (mode == EMIT_INDIRECT) k_emit<EMIT_INDIRECT, RES_KEYS><<<grid, EM_THREADS, 0, c.stream>>>(g);
             else k_emit<EMIT_SORTREC, RES_KEYS><<<grid, EM_THREADS, 0, c.stream>>>(g);
         } else if (use_dense) {
-            if (mode == EMIT_DIRECT) k_emit<EMIT_DIRECT, RES_DENSE><<<grid, EM_THREADS, 0, c.stream>>>(g);
+            if (mode == EMIT_DIRECT && dense_ordered) k_emit<EMIT_DIRECT, RES_DORD><<<grid, EM_THREADS, 0, c.stream>>>(g);
+            else if (mode == EMIT_DIRECT) k_emit<EMIT_DIRECT, RES_DENSE><<<grid, EM_THREADS, 0, c.stream>>>(g);
             else if (mode == EMIT_INDIRECT) k_emit<EMIT_INDIRECT, RES_DENSE><<<grid, EM_THREADS, 0, c.stream>>>(g);
             else k_emit<EMIT_SORTREC, RES_DENSE><<<grid, EM_THREADS, 0, c.stream>>>(g);
         } else {
@@ -1912,9 +2011,15 @@ fstc_result_t *Composer::run() {
         const int64_t arc_base = n_arcs;
         if (RF == 0 && RG == 0) {
             // no source of this level can hold duplicates: arcs go straight to their final place
+            // a big level on a dense table that is far larger than L2: ids in key order (see k_dord_count)
+            dense_ordered = use_dense && !partitioned && !external && !knob_no_dord && RU >= DORD_MIN_ARCS &&
+                            n_pairs_all * sizeof(uint32_t) > RESOLVE_TABLE_BYTES;
             launch_emit(EMIT_DIRECT, LU, MU, RU, arc_base, f_lo, nullptr, nullptr, 0, nullptr, 0, 0);
             n_arcs += RU;
-            if (o.deterministic) det_renumber(n_states, static_cast<int64_t>(read_scalar(c, d_counters.p)), arc_base, n_arcs);
+            if (dense_ordered) {
+                n_states_live = dense_number_pending(n_states, arc_base, n_arcs);
+                dense_ordered = false;
+            } else if (o.deterministic) det_renumber(n_states, static_cast<int64_t>(read_scalar(c, d_counters.p)), arc_base, n_arcs);
         } else {
             if (shift_t > 32) fail(FSTC_ERR_CAPACITY, "bits(|Σ|)+bits(|Δ|) = %d > 32: merge key does not fit 64 bits", shift_t);
             // ---- class F: sort + reduce
