@@ -174,7 +174,8 @@ typedef struct fstc_opts_t {
  * (one sort of the new keys per level), and the arcs of a source come out in an order that only depends on the inputs
  * (generation order, group order, or (tgt,a,b) order on the final ids): two runs give bit-identical pair, src, ilabel,
  * olabel, tgt, accept and expanded arrays.  Weights of arcs merged by sort + reduce are summed with atomics and may differ
- * in the last bit.  The small path is not used. */
+ * in the last bit.  The small path is not used.  (Big levels on the dense table number their states in key order in any
+ * case: DESIGN.md §6h.) */
 
 /* Rule T (the paper only notes that the result may not fit the device, :153).  BFS levels are
  * expanded whole while the running total of raw composed arcs stays <= max_raw_arcs.  The first
