@@ -79,12 +79,13 @@ __global__ void rs_bin_caps(SegView in, int nbins, int slack_div, uint32_t slack
                             int cur_stride, int exact, uint32_t *__restrict__ cap) {
     const int64_t g = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (g >= static_cast<int64_t>(in.n_seg) * nbins) return;
-    if (exact) { cap[g] = cursor[static_cast<size_t>(g) * cur_stride]; return; }
+    // capacities are multiples of 8 records: every bin then starts 16-byte aligned in the record, dest and perm arrays (bulk copies)
+    if (exact) { cap[g] = (cursor[static_cast<size_t>(g) * cur_stride] + 7u) & ~7u; return; }
     const uint32_t n = in.cnt[g / nbins];
     const uint64_t mean = (static_cast<uint64_t>(n) + nbins - 1) / nbins;
     uint64_t c = mean + mean / slack_div + slack_add;
     if (c > n) c = n;                                           // a bin never holds more than its whole segment
-    cap[g] = static_cast<uint32_t>(c);
+    cap[g] = (static_cast<uint32_t>(c) + 7u) & ~7u;
 }
 
 __global__ void rs_check_overflow(const uint32_t *__restrict__ cursor, int cur_stride, const uint32_t *__restrict__ cap,
@@ -129,6 +130,30 @@ struct ScatterArgs {
 #ifndef FSTC_SC_MINB
 #define FSTC_SC_MINB 3
 #endif
+// FSTC_SC_TMA=1 (default): a whole, 16-byte aligned tile is brought into shared memory with ONE 1-D bulk copy (cp.async.bulk +
+// mbarrier, SASS UBLKCP) instead of 8-16 global loads per thread: rs_scatter 16.7 -> 15.1 ms on `large` (the LSU is what this
+// kernel is short of: its shared-memory atomics go through it too).
+#ifndef FSTC_SC_TMA
+#define FSTC_SC_TMA 1
+#endif
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src),
+                 "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, uint32_t parity) {
+    asm volatile("{\n.reg .pred P1;\nLAB_WAIT:\nmbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n@P1 bra DONE;\nbra LAB_WAIT;\nDONE:\n}" ::"r"(smem_u32(bar)),
+                 "r"(parity)
+                 : "memory");
+}
 template <bool DEST, int SC_TILE>
 __global__ void __launch_bounds__(SC_THREADS, SC_TILE == SC_TILE_BIG ? 2 : FSTC_SC_MINB) rs_scatter(ScatterArgs a) {
     constexpr int SC_IPT = SC_TILE / SC_THREADS;
@@ -155,6 +180,18 @@ __global__ void __launch_bounds__(SC_THREADS, SC_TILE == SC_TILE_BIG ? 2 : FSTC_
 
     unsigned long long rec[SC_IPT];
     uint32_t br[SC_IPT];                                        // bin << 16 | rank inside the bin (tile-local)
+#if FSTC_SC_TMA
+    __shared__ unsigned long long s_bar;
+    const bool bulk = n == SC_TILE && (in_base & 1) == 0;       // whole tile, 16-byte aligned: one bulk copy into `sorted`
+    if (bulk) {
+        if (tid == 0) mbar_init(&s_bar, 1);
+        __syncthreads();
+        if (tid == 0) { mbar_expect_tx(&s_bar, SC_TILE * 8u); bulk_g2s(sorted, src, SC_TILE * 8u, &s_bar); }
+        mbar_wait(&s_bar, 0);
+#pragma unroll
+        for (int u = 0; u < SC_IPT; ++u) rec[u] = sorted[u * SC_THREADS + tid];
+    } else
+#endif
 #pragma unroll
     for (int u = 0; u < SC_IPT; ++u) {
         const int i = u * SC_THREADS + tid;
@@ -217,8 +254,8 @@ __global__ void __launch_bounds__(SC_THREADS, SC_TILE == SC_TILE_BIG ? 2 : FSTC_
         const long long dst = gdelta[p] + i;
         if (fits) a.out[dst] = sorted[i];                       // a full bin drops the record; the host retries
         if (DEST) {                                             // the way back: sorted slot -> output index, input index
-            a.dest[in_base + i] = fits ? static_cast<uint32_t>(dst) : 0xFFFFFFFFu;
-            a.perm[in_base + i] = static_cast<uint16_t>(m >> 16);
+            a.dest[in_base + i] = fits ? static_cast<uint32_t>(dst) : 0xFFFFFFFFu;   // (a bulk store of the tile's dest[] from shared
+            a.perm[in_base + i] = static_cast<uint16_t>(m >> 16);                    //  memory was tried: 15.0 -> 15.7 ms)
         }
     }
 }
@@ -247,6 +284,7 @@ constexpr int DD_SLOTS = FSTC_DD_SLOTS;        // keys 8 B + ids 4 B per slot, i
 constexpr int DD_SLOT_BITS = DD_SLOTS == 2048 ? 11 : (DD_SLOTS == 4096 ? 12 : (DD_SLOTS == 8192 ? 13 : -1));
 static_assert(DD_SLOT_BITS > 0, "DD_SLOTS must be 2048, 4096 or 8192");
 constexpr int DD_TARGET = FSTC_DD_TARGET;      // aimed maximum of the mean number of distinct keys per bin
+constexpr int DD_SMEM = DD_SLOTS * 12;         // (a bulk copy of a round's keys was tried: 9.2 -> 10.0 ms, a bin is one short round)
 
 struct DedupeArgs {
     SegView st;                // state records  key << ib | id
@@ -374,8 +412,11 @@ struct GatherArgs {
 template <int MODE, int SC_TILE>
 __global__ void __launch_bounds__(GA_THREADS) rs_gather_ids(GatherArgs a) {
     constexpr int GA_IPT = SC_TILE / GA_THREADS;
-    __shared__ uint32_t s_id[SC_TILE];
+    extern __shared__ __align__(16) unsigned char ga_raw[];
+    uint32_t *s_id = reinterpret_cast<uint32_t *>(ga_raw);                    // [SC_TILE] ids in input order (first: the tile of dest)
+    uint16_t *s_perm = reinterpret_cast<uint16_t *>(ga_raw + 4 * SC_TILE);    // [SC_TILE] the tile of perm (bulk copy)
     __shared__ int s_seg;
+    __shared__ unsigned long long s_bar;
     const int tid = threadIdx.x;
     if (tid == 0) s_seg = rs_find_segment(a.tile_first, a.seg.n_seg);
     __syncthreads();
@@ -386,11 +427,27 @@ __global__ void __launch_bounds__(GA_THREADS) rs_gather_ids(GatherArgs a) {
     const int64_t base = a.seg.start[s] + lo;
     if (a.dest) {
         uint32_t d[GA_IPT], li[GA_IPT];
+        // a whole, 16-byte aligned tile: dest and perm come in with two bulk copies (segments start at multiples of 8 records)
+        const bool bulk = FSTC_SC_TMA && n == SC_TILE && (base & 7) == 0;
+        if (bulk) {
+            if (tid == 0) mbar_init(&s_bar, 1);
+            __syncthreads();
+            if (tid == 0) {
+                mbar_expect_tx(&s_bar, SC_TILE * 6u);
+                bulk_g2s(s_id, a.dest + base, SC_TILE * 4u, &s_bar);
+                bulk_g2s(s_perm, a.perm + base, SC_TILE * 2u, &s_bar);
+            }
+            mbar_wait(&s_bar, 0);
 #pragma unroll
-        for (int u = 0; u < GA_IPT; ++u) {
-            const int i = u * GA_THREADS + tid;
-            d[u] = i < n ? __ldcs(a.dest + base + i) : 0xFFFFFFFFu;
-            li[u] = i < n ? __ldcs(a.perm + base + i) : 0u;
+            for (int u = 0; u < GA_IPT; ++u) { d[u] = s_id[u * GA_THREADS + tid]; li[u] = s_perm[u * GA_THREADS + tid]; }
+            __syncthreads();                                   // every thread holds its part of dest before s_id is overwritten
+        } else {
+#pragma unroll
+            for (int u = 0; u < GA_IPT; ++u) {
+                const int i = u * GA_THREADS + tid;
+                d[u] = i < n ? __ldcs(a.dest + base + i) : 0xFFFFFFFFu;
+                li[u] = i < n ? __ldcs(a.perm + base + i) : 0u;
+            }
         }
         uint32_t v[GA_IPT];
 #pragma unroll
@@ -553,6 +610,13 @@ SegSet scatter_pass(Ctx &c, const SegSet &in, int shift, int hshift, int nbins, 
     return out;
 }
 
+template <int MODE, int TILE>
+void launch_gather(Ctx &c, unsigned grid, const GatherArgs &a) {
+    constexpr int smem = 6 * TILE;
+    FSTC_CUDA(cudaFuncSetAttribute(rs_gather_ids<MODE, TILE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    rs_gather_ids<MODE, TILE><<<grid, GA_THREADS, smem, c.stream>>>(a);
+}
+
 // undoes one scatter pass (or, with dest = null, just delivers the ids): see rs_gather_ids
 void gather_pass(Ctx &c, const SegSet &seg, int mode, bool big_tile, GatherArgs a) {
     const int SC_TILE = big_tile ? SC_TILE_BIG : SC_TILE_SMALL;
@@ -566,13 +630,13 @@ void gather_pass(Ctx &c, const SegSet &seg, int mode, bool big_tile, GatherArgs 
         const int h = g_trace.begin(c, mode == 0 && a.dest ? "gather" : "apply", tiles * SC_TILE, FSTC_T_RS_GATHER);
         const unsigned grid = static_cast<unsigned>(tiles);
         if (big_tile) {
-            if (mode == 0) rs_gather_ids<0, SC_TILE_BIG><<<grid, GA_THREADS, 0, c.stream>>>(a);
-            else if (mode == 1) rs_gather_ids<1, SC_TILE_BIG><<<grid, GA_THREADS, 0, c.stream>>>(a);
-            else rs_gather_ids<2, SC_TILE_BIG><<<grid, GA_THREADS, 0, c.stream>>>(a);
+            if (mode == 0) launch_gather<0, SC_TILE_BIG>(c, grid, a);
+            else if (mode == 1) launch_gather<1, SC_TILE_BIG>(c, grid, a);
+            else launch_gather<2, SC_TILE_BIG>(c, grid, a);
         } else {
-            if (mode == 0) rs_gather_ids<0, SC_TILE_SMALL><<<grid, GA_THREADS, 0, c.stream>>>(a);
-            else if (mode == 1) rs_gather_ids<1, SC_TILE_SMALL><<<grid, GA_THREADS, 0, c.stream>>>(a);
-            else rs_gather_ids<2, SC_TILE_SMALL><<<grid, GA_THREADS, 0, c.stream>>>(a);
+            if (mode == 0) launch_gather<0, SC_TILE_SMALL>(c, grid, a);
+            else if (mode == 1) launch_gather<1, SC_TILE_SMALL>(c, grid, a);
+            else launch_gather<2, SC_TILE_SMALL>(c, grid, a);
         }
         FSTC_LAUNCH_CHECK();
         g_trace.end(c, h);
@@ -620,7 +684,7 @@ void resolve_partitioned(Ctx &c, const ResolveJob &j) {
 
 namespace {
 void resolve_partitioned_impl(Ctx &c, const ResolveJob &j) {
-    FSTC_CUDA(cudaFuncSetAttribute(rs_dedupe, cudaFuncAttributeMaxDynamicSharedMemorySize, DD_SLOTS * 12));   // per device
+    FSTC_CUDA(cudaFuncSetAttribute(rs_dedupe, cudaFuncAttributeMaxDynamicSharedMemorySize, DD_SMEM));   // per device
     const int ib = bits_for(static_cast<uint64_t>(j.n_states_before > 1 ? j.n_states_before - 1 : 1));
     if (j.key_bits + ib > 64) fail(FSTC_ERR_CAPACITY, "resolve: key (%d bits) + state id (%d bits) exceed 64 bits", j.key_bits, ib);
     if (j.n_records >= 0xFFFFFFFFll) fail(FSTC_ERR_CAPACITY, "resolve: more than 2^32 records");
@@ -659,7 +723,7 @@ void resolve_partitioned_impl(Ctx &c, const ResolveJob &j) {
         FSTC_CUDA(cudaMemcpyAsync(j.n_states, &n_before, sizeof n_before, cudaMemcpyHostToDevice, c.stream));
         DedupeArgs d{st.view(), arcs.view(), ib, ids_last.p, j.q2_bits, j.n_states, j.pair, err.p};
         const int hd = g_trace.begin(c, "dedupe", nb, FSTC_T_RS_DEDUPE);
-        rs_dedupe<<<static_cast<unsigned>(nb), DD_THREADS, DD_SLOTS * 12, c.stream>>>(d);
+        rs_dedupe<<<static_cast<unsigned>(nb), DD_THREADS, DD_SMEM, c.stream>>>(d);
         FSTC_LAUNCH_CHECK();
         g_trace.end(c, hd);
         c.n_launch += 1;
