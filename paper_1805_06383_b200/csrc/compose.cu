@@ -422,6 +422,8 @@ template <int MODE, int RES>
 __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
     constexpr bool KEYS = RES == RES_KEYS, DENSE = RES == RES_DENSE, DORD = RES == RES_DORD;
     __shared__ uint32_t relcum[EM_TILE + 1];
+    __shared__ uint4 s_rec[EM_TILE + 1];                      // the tile's matches, staged with coalesced loads: rank -> match -> arcs
+    __shared__ uint32_t s_pl[EM_TILE + 1];                    // then waits on ONE dependent global load (the arcs), not two
     __shared__ int64_t s_first_cum;
     __shared__ uint32_t s_warp[EM_THREADS / 32];
     __shared__ unsigned long long s_base;
@@ -441,6 +443,8 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
     for (int j = tid; j < nm; j += EM_THREADS) {
         int64_t c = g.L.cum[m_lo + j] - rank_lo;
         relcum[j] = c < 0 ? 0u : static_cast<uint32_t>(c > EM_TILE ? EM_TILE : c);
+        s_rec[j] = g.L.rec[m_lo + j];
+        s_pl[j] = g.L.pl[m_lo + j];
     }
     if (tid == 0) s_first_cum = g.L.cum[m_lo];
     __syncthreads();
@@ -467,8 +471,8 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
         int j = lo - 1;
         int64_t m = m_lo + j;
         uint64_t r = (j == 0) ? static_cast<uint64_t>(first - s_first_cum) : static_cast<uint64_t>(rr - relcum[j]);
-        uint4 rec = g.L.rec[m];
-        uint32_t p = g.L.pl[m];
+        uint4 rec = s_rec[j];
+        uint32_t p = s_pl[j];
         uint32_t i1, i2;
         if (r < 0xFFFFFFFFull) { i1 = static_cast<uint32_t>(r) / rec.w; i2 = static_cast<uint32_t>(r) - i1 * rec.w; }
         else { i1 = static_cast<uint32_t>(r / rec.w); i2 = static_cast<uint32_t>(r - static_cast<uint64_t>(i1) * rec.w); }
@@ -479,8 +483,8 @@ __global__ void __launch_bounds__(EM_THREADS, FSTC_EM_MINB) k_emit(EmitArgs g) {
                 if (++i2 == rec.w) {
                     i2 = 0;
                     if (++i1 == rec.z) {
-                        i1 = 0; ++m;
-                        if (m <= m_hi) { rec = g.L.rec[m]; p = g.L.pl[m]; }
+                        i1 = 0; ++m; ++j;
+                        if (m <= m_hi) { rec = s_rec[j]; p = s_pl[j]; }
                     }
                 }
             }
