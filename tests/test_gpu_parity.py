@@ -244,8 +244,8 @@ def test_result_to_host_roundtrip(fstc):
 
 def test_merge_by_construction_and_sort_merge_agree(fstc):
     """Class G (group products, no sort) and class F (radix sort + segmented sum) are two ways to the same merged arcs:
-    both against the oracle, on an input where nearly every source can hold duplicates; the packed operand's grouped
-    copy is checked against a host grouping on the way."""
+    both against the oracle, on an input where nearly every source can hold duplicates.  (The packed operand's grouped
+    copy and its inner-symbol masks are not exported: they are checked end to end, through these results.)"""
     import os
     m1, m2 = workloads.make_config("skewed", scale=0.05)
     res_g, ref = check_parity(fstc, m1, m2, max_raw_arcs=2_000_000)
@@ -263,3 +263,25 @@ def test_merge_by_construction_and_sort_merge_agree(fstc):
         a = messy_random_fst(seed, n1, sig, gam, a1)
         b = messy_random_fst(seed + 100, n2, gam, dlt, a2)
         check_parity(fstc, a, b)
+
+
+@pytest.mark.parametrize("small_path", [1, 2])
+@pytest.mark.parametrize("no_group", [False, True])
+def test_long_runs_of_parallel_arcs_stay_within_tolerance(fstc, small_path, no_group, monkeypatch):
+    """3 000 parallel duplicates of one arc on each side, weights spread over three decades: the merged arc is a sum of 9e6
+    products (class G: 3 000 x 3 000 by group sums; class F and the small path: sums of up to 3 000 x 3 000 / merged terms).
+    A plain sequential fp32 sum of that many terms can leave rtol 1e-5; the merges use compensated sums /
+    trees.  Both merge classes and the one-block path against the oracle's fp64 sums."""
+    if no_group:
+        monkeypatch.setenv("FSTC_NO_GROUP_MERGE", "1")
+    rng = np.random.default_rng(12)
+    n = 3000 if small_path == 1 else 80                      # the one-block path caps a duplicate-prone source at 8192 raw arcs
+    w1 = 10.0 ** rng.uniform(-3, 0, n)
+    w2 = 10.0 ** rng.uniform(-3, 0, n)
+    arcs1 = [(0, 1, 2, 1, float(w)) for w in w1] + [(1, 0, 1, 0, 0.5), (0, 2, 0, 1, 0.25)]
+    arcs2 = [(0, 2, 3, 1, float(w)) for w in w2] + [(1, 1, 0, 0, 0.125), (0, 0, 1, 1, 2.0)]
+    m1 = fst_from_arcs(2, 3, 3, arcs1, accept=[1])
+    m2 = fst_from_arcs(2, 3, 4, arcs2, accept=[0])
+    res, ref = check_parity(fstc, m1, m2, small_path=small_path)
+    assert ref.n_raw_arcs > n * n and ref.n_arcs < 20
+    assert res.stats["small_path"] == (1 if small_path == 2 else 0)
