@@ -19,13 +19,16 @@
  * Memory spaces.  Every array pointer inside fstc_fst_t lives in the space named by its
  * `mem` field: FSTC_MEM_DEVICE (CUDA device memory of the current device) or FSTC_MEM_HOST
  * (ordinary or pinned host memory; the library stages it to the device itself).  All arrays of
- * fstc_result_t are DEVICE memory owned by the library.  Struct pointers themselves
+ * fstc_result_t are DEVICE memory owned by the library (allocated through fstc_opts_t.alloc when the
+ * caller set allocator hooks; the arc arrays are NULL when the result was spilled to the host without
+ * a device copy, fstc_spill_t).  Struct pointers themselves
  * (fstc_fst_t*, fstc_opts_t*, fstc_stats_t*, fstc_host_result_t*) are host pointers.
  *
  * Threading / streams.  All work of a call is enqueued on `cuda_stream` (a cudaStream_t; NULL =
  * the legacy default stream).  Calls synchronise that stream internally where a size has to be
- * known on the host (once or twice per BFS level) and before returning.  Inputs are never
- * modified and may be released as soon as the call returns.
+ * known on the host (a few times per BFS level; not at all inside the one-block path for small
+ * problems) and before returning.  Inputs are never modified and may be released as soon as the
+ * call returns.
  *
  * Errors.  Every int-returning call returns FSTC_OK (0) or a negative FSTC_ERR_* code; on error
  * the output pointer is set to NULL, nothing is leaked, and fstc_last_error() (thread-local)
@@ -41,7 +44,7 @@
 extern "C" {
 #endif
 
-#define FSTC_VERSION 1
+#define FSTC_VERSION 2      /* 2: fstc_pack takes options; fstc_compose_batch; hooks, spill, deterministic, external resolve */
 
 #if defined(__GNUC__)
 #define FSTC_API __attribute__((visibility("default")))
