@@ -807,7 +807,9 @@ __global__ void __launch_bounds__(GP_THREADS) k_gprod(GProdArgs g) {
         uint64_t r = (j == 0) ? static_cast<uint64_t>(rank0 - s_first_cum) : static_cast<uint64_t>(rr - relcum[j]);
         uint4 rec = g.L.rec[m];
         uint32_t p = g.L.pl[m];
-        uint32_t i1 = static_cast<uint32_t>(r / rec.w), i2 = static_cast<uint32_t>(r - static_cast<uint64_t>(i1) * rec.w);
+        uint32_t i1, i2;                                         // (a 64-bit division costs ~40 instructions: only when it must be)
+        if (r < 0xFFFFFFFFull) { i1 = static_cast<uint32_t>(r) / rec.w; i2 = static_cast<uint32_t>(r) - i1 * rec.w; }
+        else { i1 = static_cast<uint32_t>(r / rec.w); i2 = static_cast<uint32_t>(r - static_cast<uint64_t>(i1) * rec.w); }
 #pragma unroll
         for (int u = 0; u < GP_IPT; ++u) {
             if (u < n_valid) {
