@@ -291,6 +291,55 @@ FSTC_API int fstc_compose_packed(const fstc_packed_t *m1, const fstc_packed_t *m
 FSTC_API int fstc_compose_batch(const fstc_packed_t *const *m1, int32_t n, const fstc_packed_t *m2, const fstc_opts_t *opts,
                        void *cuda_stream, fstc_result_t **out, fstc_stats_t *stats /* nullable, [n] */);
 
+/* ---- A composition that ALLOCATES NOTHING, for callers that cannot call cudaMalloc (stream capture, tight serving
+ * loops, harnesses that forbid it).  fstc_compose_static is fstc_compose_batch's one-block-per-problem search (the
+ * paper's small lattice against a language model, :251-259, :291-293) for ONE problem: the result arrays are the
+ * CALLER's device buffers, the kernel's scratch (visited table, work lists of a level) is a static device array
+ * inside the library, and the call only enqueues on cuda_stream: one clear of the report area, ONE kernel, one
+ * 80-byte copy of the header.  No cudaMalloc / cudaFree / pool call, no synchronisation, no other library routine.
+ *
+ *   * Limits: state_capacity <= FSTC_STATIC_MAX_STATES (the visited table must fit the static array of
+ *     FSTC_STATIC_SCRATCH_BYTES; every GPU that loads the library holds that array until the process exits);
+ *     arc_capacity < 2^31; beyond them FSTC_ERR_CAPACITY.  The search itself has fstc_compose_batch's small-path
+ *     caps per level (4096 frontier pairs, 32768 matches, 65536 raw arcs; 8192 raw arcs for one source that can
+ *     hold duplicates).  A problem that outgrows a cap or a capacity ends with header.status = 1: the arrays then
+ *     hold garbage and the caller composes it with fstc_compose_packed.
+ *   * opts (nullable): merge_mode (AUTO or OFF), max_levels and max_raw_arcs are read; SORT_ALL, spill,
+ *     deterministic, the external resolve and allocator hooks are refused (FSTC_ERR_ARG).
+ *   * The operands' device must be the current device.  The first call on a device resolves the address of the
+ *     static array (cudaGetSymbolAddress; it may load the module): make one call before capturing a stream.
+ *   * EVERY call on a device shares the one scratch array, which keeps the last call's contents: the call clears
+ *     the report area and the kernel clears the visited table before use, everything else is written before it is
+ *     read.  Two calls that overlap on the GPU (different streams, or two host threads) RACE on it: order them on
+ *     one stream or with events.
+ *   * The result is the one fstc_compose_batch gives (same order of arcs: sources ascending, generation order
+ *     inside a source, duplicates folded into their first occurrence; state numbers implementation-defined,
+ *     state 0 = the start pair).  It is complete when the work on cuda_stream is: read `header` after that. */
+#define FSTC_STATIC_MAX_STATES 65536
+#define FSTC_STATIC_SCRATCH_BYTES (8u << 20)
+
+typedef struct fstc_static_header_t {   /* 80 bytes, written on the stream after the kernel                   */
+  int64_t n_states, n_arcs, n_raw_arcs, n_accept, n_expanded;
+  int64_t n_seg_visited, n_match_arcs, n_matches;   /* as in fstc_stats_t                                     */
+  int32_t n_levels, truncated;
+  int32_t status;           /* 0: the arrays hold M1∘M2; 1: the problem did not fit (see above)               */
+  int32_t reserved_;
+} fstc_static_header_t;
+
+typedef struct fstc_static_out_t {      /* the caller's buffers; the library keeps no pointer after the call  */
+  int64_t state_capacity;   /* states the arrays can hold, 1 .. FSTC_STATIC_MAX_STATES                        */
+  int64_t arc_capacity;     /* arcs the arrays can hold, >= 1                                                 */
+  int32_t *pair;            /* device [2*state_capacity], 8-byte aligned                                      */
+  int32_t *src, *ilabel, *olabel, *tgt;   /* device [arc_capacity]                                            */
+  float *weight;            /* device [arc_capacity]                                                          */
+  int32_t *accept;          /* device [state_capacity]                                                        */
+  uint8_t *expanded;        /* device [state_capacity]                                                        */
+  fstc_static_header_t *header;   /* device or pinned host memory (pageable host memory makes the copy block) */
+} fstc_static_out_t;
+
+FSTC_API int fstc_compose_static(const fstc_packed_t *m1, const fstc_packed_t *m2, const fstc_opts_t *opts,
+                        void *cuda_stream, const fstc_static_out_t *out);
+
 /* fst_compose(M1, M2) -> M1∘M2: packs both operands, composes, frees the packed forms. */
 FSTC_API int fstc_compose(const fstc_fst_t *m1, const fstc_fst_t *m2, const fstc_opts_t *opts, void *cuda_stream,
                  fstc_result_t **out, fstc_stats_t *stats /* nullable */);

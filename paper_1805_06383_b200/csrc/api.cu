@@ -388,6 +388,18 @@ int fstc_compose_batch(const fstc_packed_t *const *m1, int32_t n, const fstc_pac
     return rc;
 }
 
+int fstc_compose_static(const fstc_packed_t *m1, const fstc_packed_t *m2, const fstc_opts_t *opts, void *cuda_stream,
+                        const fstc_static_out_t *out) {
+    return guarded([&] {
+        if (!m1 || !m2 || !out) fail(FSTC_ERR_ARG, "null argument");
+        fstc_opts_t o = {};
+        if (opts) o = *opts;
+        Ctx c;                                   // (no allocator of any kind is reachable from here)
+        c.stream = static_cast<cudaStream_t>(cuda_stream);
+        compose_small_static(c, *m1, *m2, o, *out);
+    }, cuda_stream, true);
+}
+
 int fstc_compose(const fstc_fst_t *m1, const fstc_fst_t *m2, const fstc_opts_t *opts, void *cuda_stream,
                  fstc_result_t **out, fstc_stats_t *stats) {
     if (out) *out = nullptr;

@@ -98,6 +98,9 @@ inline void release_block(void *p, const AllocHooks &h) {      // an array that 
 bool small_path_applies(const fstc_opts_t &o);
 void compose_small_batch(Ctx &c, const fstc_packed_t *const *m1, int n, const fstc_packed_t &m2, const fstc_opts_t &o,
                          fstc_result_t **results, fstc_stats_t *stats, std::vector<char> &ok);
+// one problem, no allocation: result arrays from the caller, scratch in a static device array (fstc_compose_static)
+void compose_small_static(Ctx &c, const fstc_packed_t &m1, const fstc_packed_t &m2, const fstc_opts_t &o,
+                          const fstc_static_out_t &out);
 
 // ---------------------------------------------------------------- partitioned target resolution (resolve.cu)
 // Finds or creates the state id of every composed arc of a big level without touching a table in DRAM at random:

@@ -15,12 +15,18 @@
 //     compacted in rank order (sources stay ascending).  O(n^2) per source, in parallel over its arcs, n <= SP_CAP_PAIR.
 // A problem that outgrows a capacity (frontier, level, states, arcs) stops with status TOO_BIG and is composed again by
 // the level-synchronous path of compose.cu.  FSTC_MERGE_SORT_ALL always takes that path.
+#include <cstddef>
 #include <algorithm>
 #include <cstring>
 #include <mutex>
 #include <vector>
 
 #include "internal.h"
+
+// Scratch of fstc_compose_static (the end of this file): one array per device that loads the library, held until the
+// process exits, shared by every call on that device.  In HOST code this name is only a stand-in for the symbol, not
+// a device address: the host reaches the array through cudaGetSymbolAddress (static_scratch below) and nowhere else.
+static __device__ __align__(256) unsigned char g_fstc_static_scratch[FSTC_STATIC_SCRATCH_BYTES];
 
 namespace fstc {
 
@@ -157,12 +163,12 @@ __device__ uint32_t block_scan(const uint32_t *in, uint32_t *out, int n, uint32_
     return carry;
 }
 
-__global__ void __launch_bounds__(SP_THREADS) k_small_compose(SmallArgs g) {
+// The search of one problem by one block (inlined into the two kernels below, which only differ in where P comes from).
+__device__ __forceinline__ void small_compose_block(const SmallArgs &g, const SmallProb &P) {
     __shared__ uint2 s_stage[SP_WARPS][SP_STAGE + 1];
     __shared__ uint32_t s_w[SP_WARPS + 1];
     __shared__ unsigned int s_nstates, s_flag, s_nsel;
     __shared__ unsigned long long s_cut, s_segs, s_marcs;
-    const SmallProb P = g.prob[blockIdx.x];
     const MachineView &A = P.A, &B = g.B;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint64_t nq2 = g.nq2;
@@ -417,6 +423,17 @@ __global__ void __launch_bounds__(SP_THREADS) k_small_compose(SmallArgs g) {
     }
 }
 
+// a batch: block k takes problem k, whose descriptor (result and scratch pointers from the library pool) is in device memory
+__global__ void __launch_bounds__(SP_THREADS) k_small_compose(SmallArgs g) {
+    const SmallProb P = g.prob[blockIdx.x];
+    small_compose_block(g, P);
+}
+
+// one problem, its descriptor passed by value: the result arrays are the caller's, the scratch is g_small_scratch (below)
+__global__ void __launch_bounds__(SP_THREADS) k_small_compose_static(SmallArgs g, SmallProb P) {
+    small_compose_block(g, P);
+}
+
 struct Carver {                       // consecutive 256-byte aligned pieces of one block
     char *base;
     size_t off = 0;
@@ -552,6 +569,103 @@ void compose_small_batch(Ctx &c, const fstc_packed_t *const *m1, int n, const fs
             }
         }
     }
+}
+
+// ------------------------------------------------------------------------------------------ fstc_compose_static
+// The same search for ONE problem with no allocation at all (include/fstc.h): result arrays from the caller, scratch in
+// g_fstc_static_scratch.  Host code never uses that name as a pointer: the device address comes from
+// cudaGetSymbolAddress, asked once per device with that device current, and is what the kernel's descriptor is built on.
+namespace {
+
+static_assert(sizeof(fstc_static_header_t) == 80 && offsetof(SmallOut, level_frontier) == 80, "the header is SmallOut's first 80 bytes");
+static_assert(offsetof(fstc_static_header_t, n_raw_arcs) == offsetof(SmallOut, n_raw) &&
+              offsetof(fstc_static_header_t, n_matches) == offsetof(SmallOut, n_matches) &&
+              offsetof(fstc_static_header_t, n_levels) == offsetof(SmallOut, n_levels) &&
+              offsetof(fstc_static_header_t, status) == offsetof(SmallOut, status), "header layout");
+
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mu;
+unsigned char *g_static_ptr[STATIC_MAX_DEVICES] = {};       // device address of g_fstc_static_scratch, per device
+
+unsigned char *static_scratch(int dev) {
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) fail(FSTC_ERR_ARG, "device index %d not supported", dev);
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void *p = nullptr;
+        FSTC_CUDA(cudaGetSymbolAddress(&p, g_fstc_static_scratch));     // the current device's copy of the array
+        if (!p) fail(FSTC_ERR_CUDA, "cudaGetSymbolAddress gave no address for the static scratch array");
+        g_static_ptr[dev] = static_cast<unsigned char *>(p);
+    }
+    return g_static_ptr[dev];
+}
+
+uint32_t small_table_slots(int64_t cap_s) {                  // as compose_small_batch: never more than half full
+    uint32_t cap_t = 1024;
+    while (cap_t < 2 * cap_s + 2 * SP_THREADS) cap_t <<= 1;
+    return cap_t;
+}
+
+// the scratch arrays of one problem, in compose_small_batch's order, behind the block's report
+void carve_static_scratch(Carver &cv, SmallProb &p, uint32_t cap_t) {
+    p.out = cv.take<SmallOut>(1);
+    p.table = cv.take<ulonglong2>(cap_t); p.keyv = cv.take<unsigned long long>(SP_CAP_F);
+    p.raw = cv.take<uint32_t>(SP_CAP_F + 1); p.nm = cv.take<uint32_t>(SP_CAP_F + 1);
+    p.roff = cv.take<uint32_t>(SP_CAP_F + 1); p.moff = cv.take<uint32_t>(SP_CAP_F + 1);
+    p.cls = cv.take<uint8_t>(SP_CAP_F); p.selv = cv.take<uint8_t>(SP_CAP_F);
+    p.cum = cv.take<uint32_t>(SP_CAP_M + 1); p.mpl = cv.take<uint32_t>(SP_CAP_M + 1); p.rec = cv.take<uint4>(SP_CAP_M);
+    p.t_a = cv.take<uint32_t>(SP_CAP_L + 1); p.t_b = cv.take<uint32_t>(SP_CAP_L + 1); p.t_tgt = cv.take<uint32_t>(SP_CAP_L + 1);
+    p.t_pl = cv.take<uint32_t>(SP_CAP_L + 1); p.t_slot = cv.take<uint32_t>(SP_CAP_L + 1); p.hidx = cv.take<uint32_t>(SP_CAP_L + 1);
+    p.t_w = cv.take<float>(SP_CAP_L + 1); p.t_ws = cv.take<float>(SP_CAP_L + 1);
+}
+
+}  // namespace
+
+void compose_small_static(Ctx &c, const fstc_packed_t &m1, const fstc_packed_t &m2, const fstc_opts_t &o,
+                          const fstc_static_out_t &out) {
+    if (m1.side != 1 || m2.side != 2) fail(FSTC_ERR_ARG, "operands must be packed with side 1 (left) and side 2 (right)");
+    if (m1.n_inner != m2.n_inner) fail(FSTC_ERR_ARG, "inner alphabets differ: |Γ| = %d vs %d (PAPER.md:45)", m1.n_inner, m2.n_inner);
+    if (m1.device != m2.device) fail(FSTC_ERR_ARG, "operands were packed on different devices");
+    int dev = 0;
+    FSTC_CUDA(cudaGetDevice(&dev));
+    if (dev != m2.device) fail(FSTC_ERR_ARG, "the operands live on device %d but device %d is current", m2.device, dev);
+    if (o.merge_mode != FSTC_MERGE_AUTO && o.merge_mode != FSTC_MERGE_OFF)
+        fail(FSTC_ERR_ARG, "fstc_compose_static merges with FSTC_MERGE_AUTO or not at all (FSTC_MERGE_OFF)");
+    if (o.max_levels < 0 || o.max_raw_arcs < 0) fail(FSTC_ERR_ARG, "bad options");
+    if (o.spill || o.deterministic || o.resolve_mode == FSTC_RESOLVE_EXTERNAL || o.alloc || o.dealloc)
+        fail(FSTC_ERR_ARG, "fstc_compose_static reads merge_mode, max_levels and max_raw_arcs only");
+    if (!out.pair || !out.src || !out.ilabel || !out.olabel || !out.tgt || !out.weight || !out.accept || !out.expanded || !out.header)
+        fail(FSTC_ERR_ARG, "null output buffer");
+    if (reinterpret_cast<uintptr_t>(out.pair) % 8 != 0) fail(FSTC_ERR_ARG, "pair must be 8-byte aligned");
+    if (out.state_capacity < 1 || out.arc_capacity < 1) fail(FSTC_ERR_ARG, "capacities must be at least 1");
+    if (out.state_capacity > FSTC_STATIC_MAX_STATES)
+        fail(FSTC_ERR_CAPACITY, "state_capacity %lld is beyond FSTC_STATIC_MAX_STATES = %d: the visited table would not fit the "
+             "static scratch array (%u bytes); use fstc_compose_packed", static_cast<long long>(out.state_capacity),
+             FSTC_STATIC_MAX_STATES, static_cast<unsigned>(FSTC_STATIC_SCRATCH_BYTES));
+    if (out.arc_capacity > 0x7FFFFFFFll)
+        fail(FSTC_ERR_CAPACITY, "arc_capacity %lld is beyond 2^31 - 1", static_cast<long long>(out.arc_capacity));
+
+    SmallProb p;
+    p.A = view_of(m1); p.acc1 = m1.accept_bits; p.start1 = m1.start; p.n_states1 = m1.n_states; p.any1 = m1.any_flags;
+    p.cap_s = static_cast<int32_t>(out.state_capacity); p.cap_a = static_cast<int32_t>(out.arc_capacity);
+    p.cap_t = small_table_slots(out.state_capacity);
+    p.pair = reinterpret_cast<int2 *>(out.pair); p.src = out.src; p.il = out.ilabel; p.ol = out.olabel; p.tgt = out.tgt;
+    p.w = out.weight; p.accept = out.accept; p.expanded = out.expanded;
+    Carver cv(static_scratch(dev));
+    carve_static_scratch(cv, p, p.cap_t);
+    if (cv.off > FSTC_STATIC_SCRATCH_BYTES)                      // (cannot happen below FSTC_STATIC_MAX_STATES: 7.2 MB there)
+        fail(FSTC_ERR_CAPACITY, "the scratch of %lld states (%zu bytes) does not fit the static array (%u bytes)",
+             static_cast<long long>(out.state_capacity), cv.off, static_cast<unsigned>(FSTC_STATIC_SCRATCH_BYTES));
+
+    SmallArgs g;
+    g.prob = nullptr; g.B = view_of(m2); g.acc2 = m2.accept_bits; g.start2 = m2.start; g.any2 = m2.any_flags;
+    g.nq2 = static_cast<uint64_t>(m2.n_states); g.merge_mode = o.merge_mode; g.max_levels = o.max_levels; g.max_raw_arcs = o.max_raw_arcs;
+    // the array keeps the last call's contents: the report starts from zero (status, counters, level statistics); the
+    // kernel empties the visited table itself, and every work list is written before it is read
+    FSTC_CUDA(cudaMemsetAsync(p.out, 0, sizeof(SmallOut), c.stream));
+    k_small_compose_static<<<1, SP_THREADS, 0, c.stream>>>(g, p);
+    FSTC_LAUNCH_CHECK();
+    c.n_launch += 1;
+    FSTC_CUDA(cudaMemcpyAsync(out.header, p.out, sizeof(fstc_static_header_t), cudaMemcpyDefault, c.stream));
 }
 
 }  // namespace fstc

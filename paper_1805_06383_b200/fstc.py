@@ -27,7 +27,7 @@ STAGES = ("count", "scan", "match", "emit", "sort", "reduce", "table", "assemble
 
 EXPORTS = (
     "fstc_pack", "fstc_packed_free", "fstc_packed_info", "fstc_packed_to_host", "fstc_compose_packed",
-    "fstc_compose", "fstc_compose_batch", "fstc_result_to_host", "fstc_result_free", "fstc_trim_pool", "fstc_strerror",
+    "fstc_compose", "fstc_compose_batch", "fstc_compose_static", "fstc_result_to_host", "fstc_result_free", "fstc_trim_pool", "fstc_strerror",
     "fstc_last_error", "fstc_version",
 )
 
@@ -122,6 +122,7 @@ def lib():
         L.fstc_compose_packed.argtypes = [P, P, P, P, ctypes.POINTER(ctypes.POINTER(_Result)), P]
         L.fstc_compose.argtypes = [P, P, P, P, ctypes.POINTER(ctypes.POINTER(_Result)), P]
         L.fstc_compose_batch.argtypes = [P, ctypes.c_int32, P, P, P, P, P]
+        L.fstc_compose_static.argtypes = [P, P, P, P, P]
         L.fstc_result_to_host.argtypes = [ctypes.POINTER(_Result), P, P]
         L.fstc_result_free.argtypes = [ctypes.POINTER(_Result)]
         L.fstc_result_free.restype = None
@@ -445,6 +446,62 @@ def fstc_compose_batch(p1s, p2: Packed, *, stream=None, with_stats=True, **opts)
             ctypes.memmove(ctypes.addressof(st), ctypes.addressof(sts[k]), ctypes.sizeof(_Stats))
         res.append(ComposeResult(outs[k], st))
     return res
+
+
+# ------------------------------------------------------------------------------------------------ no allocation
+STATIC_MAX_STATES = 65536
+STATIC_SCRATCH_BYTES = 8 << 20
+
+
+class _StaticHeader(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int64) for n in ("n_states", "n_arcs", "n_raw_arcs", "n_accept", "n_expanded",
+                                              "n_seg_visited", "n_match_arcs", "n_matches")] + \
+               [(n, ctypes.c_int32) for n in ("n_levels", "truncated", "status", "reserved_")]
+
+
+class _StaticOut(ctypes.Structure):
+    _fields_ = [("state_capacity", ctypes.c_int64), ("arc_capacity", ctypes.c_int64)] + \
+               [(n, ctypes.c_void_p) for n in ("pair", "src", "ilabel", "olabel", "tgt", "weight", "accept", "expanded", "header")]
+
+
+class StaticBuffers:
+    """The caller's side of fstc_compose_static: result arrays and the 80-byte header as CUDA tensors, made ONCE (by
+    PyTorch) and reused by any number of calls; the call itself allocates nothing."""
+
+    def __init__(self, state_capacity: int, arc_capacity: int, device="cuda"):
+        import torch
+        S, A = int(state_capacity), int(arc_capacity)
+        self.state_capacity, self.arc_capacity = S, A
+        n_s, n_a = max(S, 1), max(A, 1)
+        self.pair = torch.empty((n_s, 2), dtype=torch.int32, device=device)
+        self.src, self.ilabel, self.olabel, self.tgt = (torch.empty(n_a, dtype=torch.int32, device=device) for _ in range(4))
+        self.weight = torch.empty(n_a, dtype=torch.float32, device=device)
+        self.accept = torch.empty(n_s, dtype=torch.int32, device=device)
+        self.expanded = torch.empty(n_s, dtype=torch.uint8, device=device)
+        self.header = torch.zeros(10, dtype=torch.int64, device=device)
+        o = _StaticOut()
+        o.state_capacity, o.arc_capacity = S, A
+        for n in ("pair", "src", "ilabel", "olabel", "tgt", "weight", "accept", "expanded", "header"):
+            setattr(o, n, getattr(self, n).data_ptr())
+        self._out = o
+
+    def read(self) -> dict:
+        """After the stream's work is done: the header as a dict, and (status 0) the arrays cut to their lengths."""
+        h = _StaticHeader.from_buffer_copy(self.header.cpu().numpy().tobytes())
+        d = {n: int(getattr(h, n)) for n, _ in _StaticHeader._fields_ if n != "reserved_"}
+        if d["status"] == 0:
+            ns, na = d["n_states"], d["n_arcs"]
+            d.update(pair=self.pair[:ns], src=self.src[:na], ilabel=self.ilabel[:na], olabel=self.olabel[:na], tgt=self.tgt[:na],
+                     weight=self.weight[:na], accept=self.accept[:d["n_accept"]], expanded=self.expanded[:ns])
+        return d
+
+
+def fstc_compose_static(p1: Packed, p2: Packed, out: StaticBuffers, *, merge_mode=MERGE_AUTO, max_levels=0, max_raw_arcs=0,
+                        stream=None) -> None:
+    """M1∘M2 of one small problem into the caller's buffers with NO device allocation (include/fstc.h): only enqueues
+    on the stream; `out.read()` after a synchronisation gives the result (status 1: it did not fit)."""
+    o = _opts(merge_mode=merge_mode, max_levels=max_levels, max_raw_arcs=max_raw_arcs)
+    _check(lib().fstc_compose_static(p1.ptr, p2.ptr, ctypes.addressof(o), _stream_ptr(stream), ctypes.addressof(out._out)))
 
 
 def fstc_compose(m1, m2, *, stream=None, with_stats=True, **opts) -> ComposeResult:

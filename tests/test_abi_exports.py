@@ -77,6 +77,21 @@ def test_ctypes_struct_layout_matches_the_c_compiler(tmp_path):
                     fstc._Result.expanded.offset, fstc._Opts.alloc_ctx.offset, fstc._Stats.small_path.offset]
 
 
+def test_static_entry_point_structs_match_the_c_compiler(tmp_path):
+    from paper_1805_06383_b200 import fstc
+    src = tmp_path / "st.c"
+    src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "fstc.h"\nint main(void){\n'
+                   'printf("%zu %zu %zu %zu %d %u\\n", sizeof(fstc_static_header_t), sizeof(fstc_static_out_t),'
+                   ' offsetof(fstc_static_header_t, status), offsetof(fstc_static_out_t, header),'
+                   ' FSTC_STATIC_MAX_STATES, FSTC_STATIC_SCRATCH_BYTES);\nreturn 0;}\n')
+    exe = tmp_path / "st"
+    subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)])
+    got = [int(x) for x in subprocess.check_output([str(exe)], text=True).split()]
+    assert got == [ctypes.sizeof(fstc._StaticHeader), ctypes.sizeof(fstc._StaticOut), fstc._StaticHeader.status.offset,
+                   fstc._StaticOut.header.offset, fstc.STATIC_MAX_STATES, fstc.STATIC_SCRATCH_BYTES]
+    assert got[0] == 80
+
+
 def test_no_product_path_touches_the_oracle():
     """The oracle is test infrastructure: the package must not import or mention it."""
     pkg = os.path.join(ROOT, "paper_1805_06383_b200")
