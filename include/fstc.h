@@ -44,7 +44,7 @@
 extern "C" {
 #endif
 
-#define FSTC_VERSION 2      /* 2: fstc_pack takes options; fstc_compose_batch; hooks, spill, deterministic, external resolve */
+#define FSTC_VERSION 3      /* 2: fstc_pack takes options; fstc_compose_batch; hooks, spill, deterministic, external resolve; 3: fstc_compose_static, fstc_stats_t.n_raw_onchip */
 
 #if defined(__GNUC__)
 #define FSTC_API __attribute__((visibility("default")))
@@ -212,6 +212,7 @@ typedef struct fstc_stats_t {
   int64_t n_match_arcs;     /* Σ over matches of (n1 + n2) input arcs read                            */
   int64_t n_raw_sorted;     /* raw arcs that went through sort + reduce                               */
   int64_t n_raw_grouped;    /* raw arcs merged by construction (class G: never materialised)          */
+  int64_t n_raw_onchip;     /* of n_raw_sorted: raw arcs merged in shared memory (class S: never in HBM) */
   int64_t table_capacity;   /* final number of visited-table slots                                    */
   int32_t n_rehash, n_grow; /* table rebuilds, output regrow copies                                   */
   int32_t n_emit_launches, n_kernel_launches;

@@ -177,12 +177,14 @@ __device__ __forceinline__ void intersect(const MachineView &A, const MachineVie
 }
 
 // class U = arcs go straight to the output; class F = arcs go through sort + reduce first
+constexpr int FC_PAIR_CAP = 1024;      // raw arcs of a pair that is merged on chip (class S, k_fchip)
 __global__ void __launch_bounds__(CT_THREADS)
 k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_lo, int64_t nf,
         const uint32_t *__restrict__ sel /* null: all pairs of the level */, int merge_mode,
         uint64_t nq2, uint64_t key_limit /* pairs with key >= key_limit are left uncounted (raw = 0) */,
         int64_t *__restrict__ rawU, int64_t *__restrict__ rawF, uint32_t *__restrict__ nmU, uint32_t *__restrict__ nmF,
-        int64_t *__restrict__ rawG, int64_t *__restrict__ gwork, uint32_t *__restrict__ nmG) {
+        int64_t *__restrict__ rawG, int64_t *__restrict__ gwork, uint32_t *__restrict__ nmG,
+        int64_t *__restrict__ rawS /* null: no on-chip merge in this run */, uint32_t *__restrict__ nmS) {
     int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (i < nf) {
         int2 p = pair[f_lo + (sel ? sel[i] : i)];
@@ -208,8 +210,11 @@ k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_l
             work = static_cast<int64_t>(A.gptr[p.x + 1] - A.gptr[p.x]) * static_cast<int64_t>(B.gptr[p.y + 1] - B.gptr[p.y]);
             gcls = work <= GROUP_MAX_RATIO * raw;
         }
+        // class S: a class-F pair of few raw arcs is merged ON CHIP (k_fchip): only its merged arcs reach HBM
+        const bool scls = f && !gcls && rawS && raw > 0 && raw <= FC_PAIR_CAP;
         rawU[i] = f ? 0 : raw; nmU[i] = f ? 0 : nm;
-        if (rawF) { rawF[i] = (f && !gcls) ? raw : 0; nmF[i] = (f && !gcls) ? nm : 0; }   // null when no pair of this run can be class F
+        if (rawF) { rawF[i] = (f && !gcls && !scls) ? raw : 0; nmF[i] = (f && !gcls && !scls) ? nm : 0; }   // null when no pair of this run can be class F
+        if (rawS) { rawS[i] = scls ? raw : 0; nmS[i] = scls ? nm : 0; }
         if (rawG) { rawG[i] = gcls ? raw : 0; gwork[i] = gcls ? work : 0; nmG[i] = gcls ? 1u : 0u; }
     }
 }
@@ -221,8 +226,8 @@ k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_l
 __global__ void __launch_bounds__(CT_THREADS)
 k_cut_hist(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, const uint32_t *__restrict__ sel, uint64_t nq2,
            const int64_t *__restrict__ rawU,
-           const int64_t *__restrict__ rawF, const int64_t *__restrict__ rawG, uint64_t prefix, int shift,
-           unsigned long long *__restrict__ hist) {
+           const int64_t *__restrict__ rawF, const int64_t *__restrict__ rawG, const int64_t *__restrict__ rawS,
+           uint64_t prefix, int shift, unsigned long long *__restrict__ hist) {
     __shared__ unsigned long long h[256];
     h[threadIdx.x] = 0;
     __syncthreads();
@@ -236,7 +241,7 @@ k_cut_hist(const int2 *__restrict__ pair, int64_t f_lo, int64_t nf, const uint32
             int2 p = pair[f_lo + (sel ? sel[i] : i)];
             uint64_t key = static_cast<uint64_t>(static_cast<uint32_t>(p.x)) * nq2 + static_cast<uint32_t>(p.y);
             uint64_t hi = (shift + 8 >= 64) ? 0 : (key >> (shift + 8));
-            r = static_cast<uint64_t>(rawU[i] + (rawF ? rawF[i] : 0) + (rawG ? rawG[i] : 0));
+            r = static_cast<uint64_t>(rawU[i] + (rawF ? rawF[i] : 0) + (rawG ? rawG[i] : 0) + (rawS ? rawS[i] : 0));
             if (hi == prefix && r > 0) digit = static_cast<uint32_t>(key >> shift) & 255u;
         }
         const uint32_t peers = __match_any_sync(0xffffffffu, digit);
@@ -256,7 +261,8 @@ __global__ void k_apply_cut(const int2 *__restrict__ pair, int64_t f_lo, int64_t
                             uint64_t nq2, uint64_t cut,
                             int64_t *__restrict__ rawU, int64_t *__restrict__ rawF, uint32_t *__restrict__ nmU,
                             uint32_t *__restrict__ nmF, int64_t *__restrict__ rawG, int64_t *__restrict__ gwork,
-                            uint32_t *__restrict__ nmG, unsigned long long *__restrict__ n_selected) {
+                            uint32_t *__restrict__ nmG, int64_t *__restrict__ rawS, uint32_t *__restrict__ nmS,
+                            unsigned long long *__restrict__ n_selected) {
     int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     bool keep = false;
     if (i < nf) {
@@ -267,6 +273,7 @@ __global__ void k_apply_cut(const int2 *__restrict__ pair, int64_t f_lo, int64_t
             rawU[i] = 0; nmU[i] = 0;
             if (rawF) { rawF[i] = 0; nmF[i] = 0; }
             if (rawG) { rawG[i] = 0; gwork[i] = 0; nmG[i] = 0; }
+            if (rawS) { rawS[i] = 0; nmS[i] = 0; }
         }
     }
     unsigned b = __ballot_sync(0xffffffffu, keep);
@@ -945,6 +952,168 @@ k_resolve_keys(const unsigned long long *__restrict__ keys, int64_t n, uint32_t 
     if (valid) ids[i] = static_cast<int32_t>(id);
 }
 
+// ------------------------------------------------------------------------------------------ merge on chip (class S)
+// SURVEY §8(f)1, the paper's own future work: the raw arcs of a source that can hold duplicates are
+// composed, merged and summed in SHARED memory, so that only merged arcs reach HBM.  A block takes a TILE of the class-S
+// rank space: the pairs whose first rank falls into [t T, (t+1) T), each of at most FC_PAIR_CAP = T raw arcs, so fewer than
+// 2T arcs in all.  No sort: a pair of r raw arcs owns the 2r hash slots behind 2 x (its first rank in the tile); every raw
+// arc finds or claims the slot of its (r1, r2, a, b) there (64-bit CAS, linear probing inside the pair's region) and adds
+// its weight to the slot's fp64 sum.  The occupied slots, in slot order, ARE the merged arcs grouped by pair: a block scan
+// numbers them, one atomicAdd reserves the tile's piece of the compact output, and every pair learns its count and its
+// first arc.  ~40 instructions per raw arc against ~900 for a bitonic sort of the tile, and no HBM traffic per raw arc
+// beyond the two operand arcs (which L2 serves).  The merged arcs leave with their target KEY; their ids come from the
+// visited set afterwards, like class G's — one lookup per MERGED arc, not per raw arc.
+constexpr int FC_THREADS = 256;
+constexpr int FC_TILE = FC_PAIR_CAP;
+constexpr int FC_MAX_ARCS = 2 * FC_TILE;            // raw arcs of a tile: < FC_TILE + FC_PAIR_CAP
+constexpr int FC_SLOTS = 2 * FC_MAX_ARCS;
+constexpr int FC_CHUNK = FC_SLOTS / FC_THREADS;     // consecutive slots a thread numbers
+constexpr unsigned long long FC_EMPTY = ~0ull;
+constexpr size_t FC_SMEM = sizeof(unsigned long long) * FC_SLOTS + sizeof(double) * FC_SLOTS + sizeof(uint32_t) * (FC_MAX_ARCS + 1) +
+                           sizeof(uint16_t) * (2 * FC_MAX_ARCS + FC_SLOTS + 2);
+
+struct FChipArgs {
+    MachineView A, B;
+    MatchList L;                  // class-S match list (matches in pair order, cum = first rank)
+    const int64_t *roff, *moff;   // [nf+1] first rank / first match of every pair of the level in class S
+    const int64_t *raw;           // [nf]   raw arcs of the pair in class S (0: not of this class)
+    int64_t nf;
+    const int64_t *tile_p;        // [n_tiles+1] first pair of every tile
+    int shift_t, bits_b, q2_bits;
+    uint64_t nq2;
+    int table_key;                // 1: mkey = r1 * |Q2| + r2 (visited table)   0: (r1 << q2_bits) | r2 (partitioned resolve)
+    unsigned long long *cursor;   // merged arcs written so far
+    uint32_t *msrc, *mab;         // compact outputs (a pair's arcs are neighbours; tiles in arrival order)
+    float *mw;
+    unsigned long long *mkey;
+    int64_t *cnt, *base;          // [nf] merged arcs of the pair, and the first of them
+};
+
+// tile_p[t] = first pair i with roff[i] >= t * FC_TILE   (t = 0..n_tiles; roff has nf + 1 entries, roff[nf] = R)
+__global__ void k_fpart(const int64_t *__restrict__ roff, int64_t nf, int64_t n_tiles, int64_t *__restrict__ tile_p) {
+    const int64_t t = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (t > n_tiles) return;
+    const int64_t v = t * FC_TILE;
+    int64_t lo = 0, hi = nf;                                      // (nf: nothing at or above v before the end)
+    while (lo < hi) {
+        const int64_t mid = (lo + hi) >> 1;
+        if (roff[mid] < v) lo = mid + 1; else hi = mid;
+    }
+    tile_p[t] = lo;
+}
+
+__device__ __forceinline__ uint32_t fc_hash(unsigned long long k) {
+    k ^= k >> 33; k *= 0xff51afd7ed558ccdULL;
+    k ^= k >> 33; k *= 0xc4ceb9fe1a85ec53ULL;
+    return static_cast<uint32_t>(k >> 32);
+}
+
+__global__ void __launch_bounds__(FC_THREADS) k_fchip(FChipArgs g) {
+    extern __shared__ __align__(16) unsigned char fc_smem[];
+    unsigned long long *s_key = reinterpret_cast<unsigned long long *>(fc_smem);          // [FC_SLOTS]
+    double *s_acc = reinterpret_cast<double *>(s_key + FC_SLOTS);                          // [FC_SLOTS]
+    uint32_t *relcum = reinterpret_cast<uint32_t *>(s_acc + FC_SLOTS);                     // [FC_MAX_ARCS + 1] first rank of a match
+    uint16_t *s_ps = reinterpret_cast<uint16_t *>(relcum + FC_MAX_ARCS + 1);               // [FC_MAX_ARCS] first rank of the match's pair
+    uint16_t *s_pr = s_ps + FC_MAX_ARCS;                                                   // [FC_MAX_ARCS] raw arcs of that pair
+    uint16_t *s_excl = s_pr + FC_MAX_ARCS;                                                 // [FC_SLOTS + 1] occupied slots before slot s
+    __shared__ uint32_t s_warp[FC_THREADS / 32];
+    __shared__ unsigned long long s_base;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t p0 = g.tile_p[blockIdx.x], p1 = g.tile_p[blockIdx.x + 1];
+    const int64_t r0 = g.roff[p0], m0 = g.moff[p0];
+    const int n = static_cast<int>(g.roff[p1] - r0), nm = static_cast<int>(g.moff[p1] - m0);   // < 2 FC_TILE arcs, nm <= n matches
+    if (n == 0) return;
+    for (int j = tid; j < nm; j += FC_THREADS) {
+        const uint32_t pl = g.L.pl[m0 + j];
+        relcum[j] = static_cast<uint32_t>(g.L.cum[m0 + j] - r0);
+        s_ps[j] = static_cast<uint16_t>(g.roff[pl] - r0);
+        s_pr[j] = static_cast<uint16_t>(g.raw[pl]);
+    }
+    if (tid == 0) relcum[nm] = static_cast<uint32_t>(n);
+    for (int s = tid; s < FC_SLOTS; s += FC_THREADS) { s_key[s] = FC_EMPTY; s_acc[s] = 0.0; }
+    __syncthreads();
+
+    // ---- every raw arc of the tile: compose, find or claim its slot, add its weight
+    const unsigned long long ab_mask = (1ull << g.shift_t) - 1ull;
+    for (int r = tid; r < n; r += FC_THREADS) {
+        int lo = 0, hi = nm;                                       // last match whose first rank <= r
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (relcum[mid] <= static_cast<uint32_t>(r)) lo = mid; else hi = mid;
+        }
+        const uint4 rec = g.L.rec[m0 + lo];
+        const uint32_t rr = static_cast<uint32_t>(r) - relcum[lo];
+        const uint32_t i1 = rr / rec.w, i2 = rr - i1 * rec.w;
+        const uint4 e1 = __ldg(g.A.arcs + rec.x + i1), e2 = __ldg(g.B.arcs + rec.y + i2);      // {tgt, outer, weight, inner}
+        const unsigned long long key = ((((static_cast<unsigned long long>(e1.x) << g.q2_bits) | e2.x) << g.shift_t) |
+                                        (static_cast<unsigned long long>(e1.y) << g.bits_b) | e2.y);
+        const double w = static_cast<double>(__uint_as_float(e1.z) * __uint_as_float(e2.z));    // (the product in fp32, as everywhere)
+        const uint32_t start = 2u * s_ps[lo], size = 2u * s_pr[lo];
+        uint32_t s = start + static_cast<uint32_t>((static_cast<unsigned long long>(fc_hash(key)) * size) >> 32);
+        while (true) {
+            unsigned long long k = s_key[s];
+            if (k == FC_EMPTY) k = atomicCAS(&s_key[s], FC_EMPTY, key);
+            if (k == FC_EMPTY || k == key) break;
+            if (++s == start + size) s = start;
+        }
+        atomicAdd(&s_acc[s], w);
+    }
+    __syncthreads();
+
+    // ---- number the occupied slots (slot order = pair order)
+    const int c0 = tid * FC_CHUNK;
+    uint32_t mine = 0;
+#pragma unroll
+    for (int u = 0; u < FC_CHUNK; ++u) mine += s_key[c0 + u] != FC_EMPTY;
+    uint32_t incl = mine;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += t;
+    }
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    uint32_t before = incl - mine, total = 0;
+#pragma unroll
+    for (int wv = 0; wv < FC_THREADS / 32; ++wv) { if (wv < warp) before += s_warp[wv]; total += s_warp[wv]; }
+#pragma unroll
+    for (int u = 0; u < FC_CHUNK; ++u) {
+        s_excl[c0 + u] = static_cast<uint16_t>(before);
+        before += s_key[c0 + u] != FC_EMPTY;
+    }
+    if (tid == FC_THREADS - 1) s_excl[FC_SLOTS] = static_cast<uint16_t>(total);
+    if (tid == 0) s_base = total ? atomicAdd(g.cursor, static_cast<unsigned long long>(total)) : 0ull;
+    __syncthreads();
+    const int64_t base = static_cast<int64_t>(s_base);
+
+    // ---- the merged arcs leave, with their pair and their target key
+    const unsigned long long q2_mask = (1ull << g.q2_bits) - 1ull;
+#pragma unroll 1
+    for (int u = 0; u < FC_CHUNK; ++u) {
+        const int s = c0 + u;
+        const unsigned long long key = s_key[s];
+        if (key == FC_EMPTY) continue;
+        int lo = 0, hi = nm;                                       // the match (hence the pair) that owns rank s / 2
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (relcum[mid] <= static_cast<uint32_t>(s >> 1)) lo = mid; else hi = mid;
+        }
+        const int64_t q = base + s_excl[s];
+        const unsigned long long tk = key >> g.shift_t;
+        g.msrc[q] = g.L.pl[m0 + lo];
+        g.mab[q] = static_cast<uint32_t>(key & ab_mask);
+        g.mw[q] = static_cast<float>(s_acc[s]);
+        g.mkey[q] = g.table_key ? (tk >> g.q2_bits) * g.nq2 + (tk & q2_mask) : tk;
+    }
+    for (int j = tid; j < nm; j += FC_THREADS) {
+        if (relcum[j] != s_ps[j]) continue;                        // not the first match of its pair
+        const uint32_t start = 2u * s_ps[j], end = start + 2u * s_pr[j];
+        const uint32_t pl = g.L.pl[m0 + j];
+        g.cnt[pl] = s_excl[end] - s_excl[start];
+        g.base[pl] = base + s_excl[start];
+    }
+}
+
 __global__ void k_place_grouped(const uint32_t *__restrict__ mab, const int32_t *__restrict__ mtgt, const uint32_t *__restrict__ msrc,
                                 const float *__restrict__ mw, int64_t n_merged, const int64_t *__restrict__ mstart,
                                 const int64_t *__restrict__ foff, int64_t arc_base, int64_t f_lo,
@@ -1023,9 +1192,11 @@ __global__ void k_mstart(const uint32_t *__restrict__ msrc, int64_t n_merged, in
 }
 
 __global__ void k_final_counts(const int64_t *__restrict__ rawU, const int64_t *__restrict__ mstartS,
-                               const int64_t *__restrict__ mstartG, int64_t nf, int64_t *__restrict__ fc) {
+                               const int64_t *__restrict__ mstartG, const int64_t *__restrict__ cntS, int64_t nf,
+                               int64_t *__restrict__ fc) {
     int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i < nf) fc[i] = rawU[i] + (mstartS ? mstartS[i + 1] - mstartS[i] : 0) + (mstartG ? mstartG[i + 1] - mstartG[i] : 0);
+    if (i < nf) fc[i] = rawU[i] + (mstartS ? mstartS[i + 1] - mstartS[i] : 0) + (mstartG ? mstartG[i + 1] - mstartG[i] : 0) +
+                        (cntS ? cntS[i] : 0);
 }
 
 __global__ void k_place_merged(const unsigned long long *__restrict__ mkey, const uint32_t *__restrict__ msrc,
@@ -1257,7 +1428,7 @@ __global__ void k_compact_sel(const uint8_t *__restrict__ flag, const int64_t *_
 
 // several device scalars -> one contiguous block, so that the host reads them with ONE copy (a level costs a fixed
 // number of host round trips; on small levels those are the whole cost)
-struct ScalarPtrs { const int64_t *p[8]; };
+struct ScalarPtrs { const int64_t *p[10]; };
 __global__ void k_gather_scalars(ScalarPtrs s, int n, int64_t *__restrict__ out) {
     if (static_cast<int>(threadIdx.x) < n) out[threadIdx.x] = s.p[threadIdx.x] ? *s.p[threadIdx.x] : 0;
 }
@@ -1435,6 +1606,7 @@ struct Composer {
     double knob_limit_margin = 1.5;      // FSTC_KEY_LIMIT_MARGIN: the guessed key limit of a level that will be cut
     int64_t knob_chunk_arcs = 0;         // FSTC_CHUNK_ARCS: raw arcs a level may hold before it is expanded in chunks
     bool knob_no_dord = false;           // FSTC_NO_KEY_ORDER: dense-table levels never number their states in key order
+    bool knob_no_chip = false;           // FSTC_NO_CHIP_MERGE: class S off (small duplicate-prone sources go through sort + reduce)
 
     Composer(Ctx &ctx, const fstc_packed_t &a, const fstc_packed_t &b, const fstc_opts_t &opts)
         : c(ctx), m1(a), m2(b), o(opts), tm(ctx, opts.profile != 0), nq2(static_cast<uint64_t>(b.n_states)) {
@@ -1444,6 +1616,7 @@ struct Composer {
         if (const char *e = getenv("FSTC_KEY_LIMIT_MARGIN")) knob_limit_margin = atof(e);
         if (const char *e = getenv("FSTC_CHUNK_ARCS")) knob_chunk_arcs = atoll(e);
         knob_no_dord = getenv("FSTC_NO_KEY_ORDER") != nullptr;
+        knob_no_chip = getenv("FSTC_NO_CHIP_MERGE") != nullptr;
     }
 
     // Growable outputs and table.  `need` is what the coming launch requires; `want` >= need is a look-ahead
@@ -1722,6 +1895,10 @@ fstc_result_t *Composer::run() {
     key_bits = bits_for(n_pairs_total - 1);
     // class G (merge by construction) replaces sort + reduce for the pairs it suits; FSTC_MERGE_SORT_ALL keeps the sort
     const bool has_G = has_F && o.merge_mode == FSTC_MERGE_AUTO && !knob_no_group;
+    // class S (merge on chip, k_fchip) takes the class-F pairs of at most FC_PAIR_CAP raw arcs when (r1, r2, a, b) fits 63 bits;
+    // not with deterministic ids (the order inside a source follows the hash slots) nor with the external resolve
+    const bool has_S = has_F && o.merge_mode == FSTC_MERGE_AUTO && !knob_no_chip && !o.deterministic && !external && shift_t <= 32 &&
+                       bits_for(nq2 > 1 ? nq2 - 1 : 1) + bits_for(static_cast<uint64_t>(m1.n_states > 1 ? m1.n_states - 1 : 1)) + shift_t <= 63;
     n_pairs_all = n_pairs_total;
     use_dense = o.resolve_mode != FSTC_RESOLVE_HASH && n_pairs_total <= DENSE_MAX_PAIRS;
 
@@ -1806,13 +1983,13 @@ fstc_result_t *Composer::run() {
         last_mode = 1;
 
         // ---- count
-        int64_t RU = 0, RF = 0, MU = 0, MF = 0;
-        DBuf<int64_t> rawU, rawF, rawG, gwork;
-        DBuf<uint32_t> nmU, nmF, nmG;
-        DBuf<int64_t> roffU, roffF, moffU, moffF, roffG, moffG, woff;
+        int64_t RU = 0, RF = 0, MU = 0, MF = 0, RS = 0, MS = 0;
+        DBuf<int64_t> rawU, rawF, rawG, gwork, rawS;
+        DBuf<uint32_t> nmU, nmF, nmG, nmS;
+        DBuf<int64_t> roffU, roffF, moffU, moffF, roffG, moffG, woff, roffS, moffS;
         int64_t RG = 0, MG = 0, WG = 0;                          // class G: raw arcs, pairs, group pairs of the level
         DBuf<uint32_t> sel;                                      // compacted level: frontier index of working pair i
-        DBuf<int64_t> level_totals(c, 8);
+        DBuf<int64_t> level_totals(c, 10);
         auto scan_level = [&](int64_t *n_sel_out) {             // offsets + totals of the level, one synchronisation
             exclusive_scan2(c, rawU.p, nmU.p, nf, roffU.p, moffU.p);
             if (has_F) exclusive_scan2(c, rawF.p, nmF.p, nf, roffF.p, moffF.p);
@@ -1820,15 +1997,17 @@ fstc_result_t *Composer::run() {
                 exclusive_scan2(c, rawG.p, nmG.p, nf, roffG.p, moffG.p);
                 exclusive_scan<int64_t>(c, gwork.p, nf, woff.p);
             }
+            if (has_S) exclusive_scan2(c, rawS.p, nmS.p, nf, roffS.p, moffS.p);
             ScalarPtrs sp{{roffU.p + nf, moffU.p + nf, has_F ? roffF.p + nf : nullptr, has_F ? moffF.p + nf : nullptr,
                            has_G ? roffG.p + nf : nullptr, has_G ? moffG.p + nf : nullptr, has_G ? woff.p + nf : nullptr,
-                           reinterpret_cast<const int64_t *>(d_counters.p + 3)}};
-            k_gather_scalars<<<1, 32, 0, c.stream>>>(sp, 8, level_totals.p);
+                           reinterpret_cast<const int64_t *>(d_counters.p + 3),
+                           has_S ? roffS.p + nf : nullptr, has_S ? moffS.p + nf : nullptr}};
+            k_gather_scalars<<<1, 32, 0, c.stream>>>(sp, 10, level_totals.p);
             FSTC_LAUNCH_CHECK();
-            int64_t t[8];
+            int64_t t[10];
             FSTC_CUDA(cudaMemcpyAsync(t, level_totals.p, sizeof t, cudaMemcpyDeviceToHost, c.stream));
             c.sync();
-            RU = t[0]; MU = t[1]; RF = t[2]; MF = t[3]; RG = t[4]; MG = t[5]; WG = t[6];
+            RU = t[0]; MU = t[1]; RF = t[2]; MF = t[3]; RG = t[4]; MG = t[5]; WG = t[6]; RS = t[8]; MS = t[9];
             if (n_sel_out) *n_sel_out = t[7];
         };
         // A level that will clearly be cut by the budget (predicted from the previous level's fan-out) is counted
@@ -1872,28 +2051,29 @@ fstc_result_t *Composer::run() {
                 rawG.alloc(c, nf); gwork.alloc(c, nf); nmG.alloc(c, nf);
                 roffG.alloc(c, nf + 1); moffG.alloc(c, nf + 1); woff.alloc(c, nf + 1);
             }
+            if (has_S) { rawS.alloc(c, nf); nmS.alloc(c, nf); roffS.alloc(c, nf + 1); moffS.alloc(c, nf + 1); }
             k_count<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, sel.p, o.merge_mode, nq2, key_limit, rawU.p, rawF.p,
-                                                           nmU.p, nmF.p, rawG.p, gwork.p, nmG.p);
+                                                           nmU.p, nmF.p, rawG.p, gwork.p, nmG.p, rawS.p, nmS.p);
             FSTC_LAUNCH_CHECK();
             c.n_launch += 1;
             tm.end(h);
             // ---- scan + budget
             h = tm.begin(FSTC_T_SCAN);
             scan_level(nullptr);
-            if (key_limit >= n_pairs_total || cum_raw + RU + RF + RG > o.max_raw_arcs) break;
+            if (key_limit >= n_pairs_total || cum_raw + RU + RF + RG + RS > o.max_raw_arcs) break;
             tm.end(h);
             key_limit = key_limit > n_pairs_total / 4 ? ~0ull : key_limit * 4;     // the cut lies higher: widen
         }
         bool stop_after = false;
         int64_t n_sel = nf;
-        if (o.max_raw_arcs > 0 && cum_raw + RU + RF + RG > o.max_raw_arcs) {
+        if (o.max_raw_arcs > 0 && cum_raw + RU + RF + RG + RS > o.max_raw_arcs) {
             // rule T: find the key of the first pair (ascending key order) whose arcs no longer fit
             const uint64_t remaining = static_cast<uint64_t>(o.max_raw_arcs - cum_raw);
             uint64_t prefix = 0, before = 0;
             const int top = ((key_bits + 7) / 8) * 8;
             for (int shift = top - 8; shift >= 0; shift -= 8) {
                 FSTC_CUDA(cudaMemsetAsync(d_counters.p + 4, 0, sizeof(unsigned long long) * 256, c.stream));
-                k_cut_hist<<<std::min<unsigned>(nblk(nf), 8u * c.n_sm), CT_THREADS, 0, c.stream>>>(pair.p, f_lo, nf, sel.p, nq2, rawU.p, rawF.p, rawG.p, prefix, shift,
+                k_cut_hist<<<std::min<unsigned>(nblk(nf), 8u * c.n_sm), CT_THREADS, 0, c.stream>>>(pair.p, f_lo, nf, sel.p, nq2, rawU.p, rawF.p, rawG.p, rawS.p, prefix, shift,
                                                                   d_counters.p + 4);
                 FSTC_LAUNCH_CHECK();
                 c.n_launch += 1;
@@ -1911,7 +2091,7 @@ fstc_result_t *Composer::run() {
             cut_key = prefix;
             FSTC_CUDA(cudaMemsetAsync(d_counters.p + 3, 0, sizeof(unsigned long long), c.stream));
             k_apply_cut<<<nblk(nf), CT_THREADS, 0, c.stream>>>(pair.p, f_lo, nf, sel.p, nq2, cut_key, rawU.p, rawF.p, nmU.p, nmF.p,
-                                                               rawG.p, gwork.p, nmG.p,
+                                                               rawG.p, gwork.p, nmG.p, rawS.p, nmS.p,
                                                                d_counters.p + 3);
             FSTC_LAUNCH_CHECK();
             c.n_launch += 1;
@@ -1923,7 +2103,7 @@ fstc_result_t *Composer::run() {
         tm.end(h);
 
         hostmark("count+scan", lvl);
-        const int64_t R = RU + RF + RG;
+        const int64_t R = RU + RF + RG + RS;
         if (!stop_after && !external && nf_all > 1) {
             if (level_end < 0 && R > chunk_limit) {              // too big for one piece: count again, on the first chunk
                 level_lo = f_lo; level_end = f_hi;
@@ -2018,9 +2198,22 @@ fstc_result_t *Composer::run() {
             tm.end(h);
         }
 
+        DBuf<int64_t> cumS(c, MS + 1);
+        DBuf<uint4> recS(c, MS);
+        DBuf<uint32_t> plS(c, MS);
+        MatchList LS{cumS.p, recS.p, plS.p};
+        if (MS > 0) {                                            // the same kernel, class S in the place of class U
+            h = tm.begin(FSTC_T_MATCH);
+            k_match<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, sel.p, nmS.p, nullptr, moffS.p, nullptr, roffS.p,
+                                                           nullptr, LS, LS, d_counters.p + 1);
+            FSTC_LAUNCH_CHECK();
+            c.n_launch += 1;
+            tm.end(h);
+        }
+
         hostmark("match", lvl);
         const int64_t arc_base = n_arcs;
-        if (RF == 0 && RG == 0) {
+        if (RF == 0 && RG == 0 && RS == 0) {
             // no source of this level can hold duplicates: arcs go straight to their final place
             // a big level on a dense table that is far larger than L2: ids in key order (see k_dord_count)
             dense_ordered = use_dense && !partitioned && !external && !knob_no_dord && RU >= DORD_MIN_ARCS &&
@@ -2072,6 +2265,65 @@ fstc_result_t *Composer::run() {
                 c.sync();
                 sa.release(); sb.release();
             }
+            // ---- class S: merge on chip (k_fchip); the merged arcs then take class G's way to their ids and places
+            int64_t MSm = 0;
+            DBuf<uint32_t> ssrc, sab;
+            DBuf<float> sw;
+            DBuf<int32_t> stgt;
+            DBuf<int64_t> scnt, sbase;
+            if (RS > 0) {
+                h = tm.begin(FSTC_T_REDUCE);
+                const int64_t n_tiles = ceil_div(RS, FC_TILE);
+                DBuf<int64_t> tile_p(c, n_tiles + 1);
+                DBuf<unsigned long long> cursor(c, 1), skeys(c, RS + 2);
+                ssrc.alloc(c, RS); sab.alloc(c, RS); sw.alloc(c, RS);
+                scnt.alloc(c, nf); sbase.alloc(c, nf);
+                FSTC_CUDA(cudaMemsetAsync(cursor.p, 0, sizeof(unsigned long long), c.stream));
+                FSTC_CUDA(cudaMemsetAsync(scnt.p, 0, sizeof(int64_t) * nf, c.stream));
+                k_fpart<<<nblk(n_tiles + 1), CT_THREADS, 0, c.stream>>>(roffS.p, nf, n_tiles, tile_p.p);
+                FSTC_LAUNCH_CHECK();
+                FChipArgs fa;
+                fa.A = A; fa.B = B; fa.L = LS; fa.roff = roffS.p; fa.moff = moffS.p; fa.raw = rawS.p; fa.nf = nf; fa.tile_p = tile_p.p;
+                fa.shift_t = shift_t; fa.bits_b = bits_b; fa.q2_bits = bits_for(nq2 > 1 ? nq2 - 1 : 1); fa.nq2 = nq2;
+                fa.table_key = partitioned ? 0 : 1;
+                fa.cursor = cursor.p; fa.msrc = ssrc.p; fa.mab = sab.p; fa.mw = sw.p; fa.mkey = skeys.p; fa.cnt = scnt.p; fa.base = sbase.p;
+                static const bool fc_attr = [] {                  // 88 KB of dynamic shared memory: opt in once
+                    return cudaFuncSetAttribute(k_fchip, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(FC_SMEM)) == cudaSuccess;
+                }();
+                if (!fc_attr) fail(FSTC_ERR_CUDA, "k_fchip: %zu bytes of shared memory refused", FC_SMEM);
+                k_fchip<<<static_cast<unsigned>(n_tiles), FC_THREADS, FC_SMEM, c.stream>>>(fa);
+                FSTC_LAUNCH_CHECK();
+                c.n_launch += 2;
+                MSm = static_cast<int64_t>(read_scalar(c, cursor.p));
+                tm.end(h);
+                if (MSm > 0) {                                       // target ids of the merged arcs
+                    stgt.alloc(c, MSm);
+                    if (partitioned) {
+                        ResolveJob j;
+                        j.keys = skeys.p; j.n_records = MSm; j.q2_bits = fa.q2_bits;
+                        j.key_bits = fa.q2_bits + bits_for(static_cast<uint64_t>(m1.n_states > 1 ? m1.n_states - 1 : 1));
+                        j.pair = pair.p; j.n_states_before = n_states_live; j.n_states = d_counters.p;
+                        j.mode = 0; j.pos = nullptr; j.o_tgt = stgt.p; j.sortrec = nullptr; j.shift_t = 0;
+                        j.force_bits = knob_resolve_bits;
+                        j.stats = &st; j.profile = o.profile != 0;
+                        run_resolve(j, 1);
+                    } else {
+                        h = tm.begin(FSTC_T_EMIT);
+                        if (use_dense)
+                            k_resolve_keys<true><<<nblk(MSm), CT_THREADS, 0, c.stream>>>(skeys.p, MSm, dense.p, nullptr, 0, nq2, d_counters.p,
+                                                                                        pair.p, stgt.p);
+                        else
+                            k_resolve_keys<false><<<nblk(MSm), CT_THREADS, 0, c.stream>>>(skeys.p, MSm, nullptr, table.p, cap, nq2,
+                                                                                         d_counters.p, pair.p, stgt.p);
+                        FSTC_LAUNCH_CHECK();
+                        c.n_launch += 1;
+                        tm.end(h);
+                    }
+                    n_states_live = static_cast<int64_t>(read_scalar(c, d_counters.p));
+                }
+                st.n_raw_onchip += RS;
+                c.sync();                                            // (tile_p, cursor, skeys go out of scope)
+            }
             // ---- class G: merge by construction (group products)
             int64_t MGm = 0;
             DBuf<uint32_t> gsrc, gab;
@@ -2120,7 +2372,7 @@ fstc_result_t *Composer::run() {
                     mstartG.alloc(c, nf + 1);
                     exclusive_scan<int64_t>(c, cntG.p, nf, mstartG.p);
                     fc.alloc(c, nf); foff.alloc(c, nf + 1);
-                    k_final_counts<<<nblk(nf), CT_THREADS, 0, c.stream>>>(rawU.p, mstartS.p, mstartG.p, nf, fc.p);
+                    k_final_counts<<<nblk(nf), CT_THREADS, 0, c.stream>>>(rawU.p, mstartS.p, mstartG.p, scnt.p, nf, fc.p);
                     FSTC_LAUNCH_CHECK();
                     exclusive_scan<int64_t>(c, fc.p, nf, foff.p);
                     g.mstart = mstartG.p; g.foff = foff.p;
@@ -2178,7 +2430,7 @@ fstc_result_t *Composer::run() {
             h = tm.begin(FSTC_T_REDUCE);
             if (!g_placed) {
                 fc.alloc(c, nf); foff.alloc(c, nf + 1);
-                k_final_counts<<<nblk(nf), CT_THREADS, 0, c.stream>>>(rawU.p, mstartS.p, mstartG.p, nf, fc.p);
+                k_final_counts<<<nblk(nf), CT_THREADS, 0, c.stream>>>(rawU.p, mstartS.p, mstartG.p, scnt.p, nf, fc.p);
                 FSTC_LAUNCH_CHECK();
                 exclusive_scan<int64_t>(c, fc.p, nf, foff.p);
             }
@@ -2215,11 +2467,16 @@ fstc_result_t *Composer::run() {
                                                                        n_states, det_n1, o.deterministic ? rank.p : nullptr);
                 FSTC_LAUNCH_CHECK();
             }
-            c.n_launch += 3;
+            if (MSm > 0) {                                           // (sbase in the place of mstart: a pair's arcs are neighbours)
+                k_place_grouped<<<nblk(MSm), CT_THREADS, 0, c.stream>>>(sab.p, stgt.p, ssrc.p, sw.p, MSm, sbase.p, foff.p, arc_base,
+                                                                       f_lo, sel.p, bits_b, o_src, o_il, o_ol, o_tgt, o_w);
+                FSTC_LAUNCH_CHECK();
+            }
+            c.n_launch += 4;
             tm.end(h);
             if (!o.deterministic) launch_emit(EMIT_INDIRECT, LU, MU, RU, 0, f_lo, foff.p, roffU.p, arc_base, nullptr, 0, 0);
-            n_arcs += RU + M + MGm;
-            st.n_raw_sorted += RF;
+            n_arcs += RU + M + MGm + MSm;
+            st.n_raw_sorted += RF + RS;
             c.sync();   // the level's temporaries go out of scope below
         }
 
@@ -2235,7 +2492,7 @@ fstc_result_t *Composer::run() {
         if (level_end >= 0) st.n_chunks += 1;
         spill_level(arc_base, n_arcs, ns_after);
         if (partitioned) st.rs_dedupe_new += ns_after - n_states;
-        st.n_matches += MU + MF;
+        st.n_matches += MU + MF + MS;
         st.n_expanded += n_sel;
         last_fan = n_sel > 0 ? static_cast<double>(R) / static_cast<double>(n_sel) : 0.0;
         cum_raw += R;

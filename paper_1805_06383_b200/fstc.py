@@ -71,7 +71,8 @@ class _Stats(ctypes.Structure):
         ("n_states", ctypes.c_int64), ("n_arcs", ctypes.c_int64), ("n_raw_arcs", ctypes.c_int64),
         ("n_expanded", ctypes.c_int64), ("n_levels", ctypes.c_int32), ("truncated", ctypes.c_int32),
         ("n_seg_visited", ctypes.c_int64), ("n_matches", ctypes.c_int64), ("n_match_arcs", ctypes.c_int64),
-        ("n_raw_sorted", ctypes.c_int64), ("n_raw_grouped", ctypes.c_int64), ("table_capacity", ctypes.c_int64),
+        ("n_raw_sorted", ctypes.c_int64), ("n_raw_grouped", ctypes.c_int64), ("n_raw_onchip", ctypes.c_int64),
+        ("table_capacity", ctypes.c_int64),
         ("n_rehash", ctypes.c_int32), ("n_grow", ctypes.c_int32),
         ("n_emit_launches", ctypes.c_int32), ("n_kernel_launches", ctypes.c_int32),
         ("n_resolve", ctypes.c_int32), ("small_path", ctypes.c_int32), ("n_resolved_arcs", ctypes.c_int64),
@@ -294,7 +295,8 @@ def stats_dict(s: _Stats) -> dict:
         "n_states": int(s.n_states), "n_arcs": int(s.n_arcs), "n_raw_arcs": int(s.n_raw_arcs),
         "n_expanded": int(s.n_expanded), "n_levels": int(s.n_levels), "truncated": int(s.truncated),
         "n_seg_visited": int(s.n_seg_visited), "n_matches": int(s.n_matches), "n_match_arcs": int(s.n_match_arcs),
-        "n_raw_sorted": int(s.n_raw_sorted), "n_raw_grouped": int(s.n_raw_grouped), "table_capacity": int(s.table_capacity),
+        "n_raw_sorted": int(s.n_raw_sorted), "n_raw_grouped": int(s.n_raw_grouped), "n_raw_onchip": int(s.n_raw_onchip),
+        "table_capacity": int(s.table_capacity),
         "n_rehash": int(s.n_rehash), "n_grow": int(s.n_grow), "n_emit_launches": int(s.n_emit_launches),
         "n_kernel_launches": int(s.n_kernel_launches),
         "n_resolve": int(s.n_resolve), "n_resolved_arcs": int(s.n_resolved_arcs), "small_path": int(s.small_path),

@@ -44,7 +44,7 @@ def test_library_exports_every_declared_symbol(libpath):
     for n in names:
         assert hasattr(L, n), n
     L.fstc_version.restype = ctypes.c_int
-    assert L.fstc_version() == 2
+    assert L.fstc_version() == 3
     L.fstc_strerror.restype = ctypes.c_char_p
     assert L.fstc_strerror(-4) == b"internal capacity limit exceeded"
 
