@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """Benchmark of the composition hot path (pack -> compose) on BASELINE.json's workloads.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload large|medium|skewed|nlp|tiny]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload large|medium|skewed|nlp|tiny|dups]
                     [--impl ours|reference] [--no-e2e] [--no-cpu-baseline]
 
 One "step" = one pass of the whole hot path over one pair of synthetic transducers: pack(M1),
@@ -39,7 +39,7 @@ if ROOT not in sys.path:
 METRIC = "composed_raw_arcs_per_sec"
 UNIT = "arcs/s"
 # bounded oracle samples (raw-arc budget) sized for roughly 10-30 s of one host core
-ORACLE_SAMPLE_BUDGET = {"large": 20_000_000, "medium": 60_000_000, "skewed": 60_000_000, "nlp": 0, "tiny": 0}
+ORACLE_SAMPLE_BUDGET = {"large": 20_000_000, "medium": 60_000_000, "skewed": 60_000_000, "nlp": 0, "tiny": 0, "dups": 40_000_000}
 WORKLOAD_DESC = {
     "large": "large random (BASELINE.json configs[3]): |Q1|=|Q2|=1e5, |Σ|=|Δ|=2e4, |Γ|=5e3 Zipf 1.1, 5e6 arcs each, "
              "max_raw_arcs=1e9 (rule T)",
@@ -48,6 +48,8 @@ WORKLOAD_DESC = {
               "max_raw_arcs=1e9",
     "nlp": "NLP-shaped (configs[2]): 50x8 lattice ∘ 30k-state bigram (3e6 arcs), complete",
     "tiny": "tiny random (configs[0])",
+    "dups": "medium random + 10 % parallel duplicate arcs (NOT a BASELINE config: the workload of the merge on chip, SURVEY §8(f)1): "
+            "|Q1|=|Q2|=1e4, |Γ|=1e3 Zipf 1.0, 2.2e5 arcs each, every source duplicate-prone, complete",
 }
 
 

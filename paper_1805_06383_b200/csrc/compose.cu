@@ -177,7 +177,13 @@ __device__ __forceinline__ void intersect(const MachineView &A, const MachineVie
 }
 
 // class U = arcs go straight to the output; class F = arcs go through sort + reduce first
-constexpr int FC_PAIR_CAP = 1024;      // raw arcs of a pair that is merged on chip (class S, k_fchip)
+#ifndef FSTC_FC_PAIR_CAP
+#define FSTC_FC_PAIR_CAP 512
+#endif
+#ifndef FSTC_FC_THREADS
+#define FSTC_FC_THREADS 512
+#endif
+constexpr int FC_PAIR_CAP = FSTC_FC_PAIR_CAP;      // raw arcs of a pair that is merged on chip (class S, k_fchip)
 __global__ void __launch_bounds__(CT_THREADS)
 k_count(MachineView A, MachineView B, const int2 *__restrict__ pair, int64_t f_lo, int64_t nf,
         const uint32_t *__restrict__ sel /* null: all pairs of the level */, int merge_mode,
@@ -960,17 +966,20 @@ k_resolve_keys(const unsigned long long *__restrict__ keys, int64_t n, uint32_t 
 // arc finds or claims the slot of its (r1, r2, a, b) there (64-bit CAS, linear probing inside the pair's region) and adds
 // its weight to the slot's fp64 sum.  The occupied slots, in slot order, ARE the merged arcs grouped by pair: a block scan
 // numbers them, one atomicAdd reserves the tile's piece of the compact output, and every pair learns its count and its
-// first arc.  ~40 instructions per raw arc against ~900 for a bitonic sort of the tile, and no HBM traffic per raw arc
-// beyond the two operand arcs (which L2 serves).  The merged arcs leave with their target KEY; their ids come from the
+// first arc.  ~250 instructions per raw arc against ~900 for a bitonic sort of the tile, and no HBM traffic per raw arc
+// beyond the two operand arcs (which L2 serves) and its match record.  T = 512 with one thread per rank of the tile
+// (measured on the `dups` workload, reduce stage: T/threads 512/256 63.5 ms, 512/512 54.8, 256/256 51.6, 128/128 50.8,
+// 256/512 76.5, 128/256 71.5; the match records staged in shared memory: 73.2 — occupancy).  The merged arcs leave with their target KEY; their ids come from the
 // visited set afterwards, like class G's — one lookup per MERGED arc, not per raw arc.
-constexpr int FC_THREADS = 256;
+constexpr int FC_THREADS = FSTC_FC_THREADS;
 constexpr int FC_TILE = FC_PAIR_CAP;
 constexpr int FC_MAX_ARCS = 2 * FC_TILE;            // raw arcs of a tile: < FC_TILE + FC_PAIR_CAP
 constexpr int FC_SLOTS = 2 * FC_MAX_ARCS;
-constexpr int FC_CHUNK = FC_SLOTS / FC_THREADS;     // consecutive slots a thread numbers
+constexpr int FC_CHUNK = FC_SLOTS / FC_THREADS;     // rounds of 32 slots a warp numbers
 constexpr unsigned long long FC_EMPTY = ~0ull;
 constexpr size_t FC_SMEM = sizeof(unsigned long long) * FC_SLOTS + sizeof(double) * FC_SLOTS + sizeof(uint32_t) * (FC_MAX_ARCS + 1) +
-                           sizeof(uint16_t) * (2 * FC_MAX_ARCS + FC_SLOTS + 2);
+                           sizeof(uint16_t) * (3 * FC_MAX_ARCS + FC_SLOTS + 2);
+static_assert(FC_SLOTS % (FC_THREADS) == 0 && FC_MAX_ARCS < 65536, "slot rounds of a warp; uint16 indices");
 
 struct FChipArgs {
     MachineView A, B;
@@ -1015,7 +1024,8 @@ __global__ void __launch_bounds__(FC_THREADS) k_fchip(FChipArgs g) {
     uint32_t *relcum = reinterpret_cast<uint32_t *>(s_acc + FC_SLOTS);                     // [FC_MAX_ARCS + 1] first rank of a match
     uint16_t *s_ps = reinterpret_cast<uint16_t *>(relcum + FC_MAX_ARCS + 1);               // [FC_MAX_ARCS] first rank of the match's pair
     uint16_t *s_pr = s_ps + FC_MAX_ARCS;                                                   // [FC_MAX_ARCS] raw arcs of that pair
-    uint16_t *s_excl = s_pr + FC_MAX_ARCS;                                                 // [FC_SLOTS + 1] occupied slots before slot s
+    uint16_t *s_mi = s_pr + FC_MAX_ARCS;                                                   // [FC_MAX_ARCS] rank -> match of the tile
+    uint16_t *s_excl = s_mi + FC_MAX_ARCS;                                                 // [FC_SLOTS + 1] occupied slots before slot s
     __shared__ uint32_t s_warp[FC_THREADS / 32];
     __shared__ unsigned long long s_base;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -1032,23 +1042,26 @@ __global__ void __launch_bounds__(FC_THREADS) k_fchip(FChipArgs g) {
     if (tid == 0) relcum[nm] = static_cast<uint32_t>(n);
     for (int s = tid; s < FC_SLOTS; s += FC_THREADS) { s_key[s] = FC_EMPTY; s_acc[s] = 0.0; }
     __syncthreads();
+    // rank -> match, written match by match (the matches of such sources are short): the arc loop and the way out both
+    // find their match, hence their pair, with one load instead of a binary search
+    for (int j = tid; j < nm; j += FC_THREADS) {
+        const uint32_t e = relcum[j + 1];
+        for (uint32_t r = relcum[j]; r < e; ++r) s_mi[r] = static_cast<uint16_t>(j);
+    }
+    __syncthreads();
 
     // ---- every raw arc of the tile: compose, find or claim its slot, add its weight
     const unsigned long long ab_mask = (1ull << g.shift_t) - 1ull;
     for (int r = tid; r < n; r += FC_THREADS) {
-        int lo = 0, hi = nm;                                       // last match whose first rank <= r
-        while (hi - lo > 1) {
-            const int mid = (lo + hi) >> 1;
-            if (relcum[mid] <= static_cast<uint32_t>(r)) lo = mid; else hi = mid;
-        }
-        const uint4 rec = g.L.rec[m0 + lo];
-        const uint32_t rr = static_cast<uint32_t>(r) - relcum[lo];
+        const int j = s_mi[r];
+        const uint4 rec = g.L.rec[m0 + j];
+        const uint32_t rr = static_cast<uint32_t>(r) - relcum[j];
         const uint32_t i1 = rr / rec.w, i2 = rr - i1 * rec.w;
         const uint4 e1 = __ldg(g.A.arcs + rec.x + i1), e2 = __ldg(g.B.arcs + rec.y + i2);      // {tgt, outer, weight, inner}
         const unsigned long long key = ((((static_cast<unsigned long long>(e1.x) << g.q2_bits) | e2.x) << g.shift_t) |
                                         (static_cast<unsigned long long>(e1.y) << g.bits_b) | e2.y);
         const double w = static_cast<double>(__uint_as_float(e1.z) * __uint_as_float(e2.z));    // (the product in fp32, as everywhere)
-        const uint32_t start = 2u * s_ps[lo], size = 2u * s_pr[lo];
+        const uint32_t start = 2u * s_ps[j], size = 2u * s_pr[j];
         uint32_t s = start + static_cast<uint32_t>((static_cast<unsigned long long>(fc_hash(key)) * size) >> 32);
         while (true) {
             unsigned long long k = s_key[s];
@@ -1060,29 +1073,25 @@ __global__ void __launch_bounds__(FC_THREADS) k_fchip(FChipArgs g) {
     }
     __syncthreads();
 
-    // ---- number the occupied slots (slot order = pair order)
-    const int c0 = tid * FC_CHUNK;
+    // ---- number the occupied slots (slot order = pair order).  A warp owns FC_CHUNK x 32 consecutive slots and takes them
+    // 32 at a time (neighbouring lanes, neighbouring slots: no bank conflict, and the way out writes neighbouring arcs).
+    const int w0 = warp * (FC_CHUNK * 32);
     uint32_t mine = 0;
 #pragma unroll
-    for (int u = 0; u < FC_CHUNK; ++u) mine += s_key[c0 + u] != FC_EMPTY;
-    uint32_t incl = mine;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
-        if (lane >= d) incl += t;
-    }
-    if (lane == 31) s_warp[warp] = incl;
+    for (int u = 0; u < FC_CHUNK; ++u) mine += __popc(__ballot_sync(0xffffffffu, s_key[w0 + u * 32 + lane] != FC_EMPTY));
+    if (lane == 0) s_warp[warp] = mine;
     __syncthreads();
-    uint32_t before = incl - mine, total = 0;
+    uint32_t before = 0, total = 0;
 #pragma unroll
     for (int wv = 0; wv < FC_THREADS / 32; ++wv) { if (wv < warp) before += s_warp[wv]; total += s_warp[wv]; }
+    if (tid == 0) s_base = total ? atomicAdd(g.cursor, static_cast<unsigned long long>(total)) : 0ull;
 #pragma unroll
     for (int u = 0; u < FC_CHUNK; ++u) {
-        s_excl[c0 + u] = static_cast<uint16_t>(before);
-        before += s_key[c0 + u] != FC_EMPTY;
+        const uint32_t bal = __ballot_sync(0xffffffffu, s_key[w0 + u * 32 + lane] != FC_EMPTY);
+        s_excl[w0 + u * 32 + lane] = static_cast<uint16_t>(before + __popc(bal & ((1u << lane) - 1u)));
+        before += __popc(bal);
     }
     if (tid == FC_THREADS - 1) s_excl[FC_SLOTS] = static_cast<uint16_t>(total);
-    if (tid == 0) s_base = total ? atomicAdd(g.cursor, static_cast<unsigned long long>(total)) : 0ull;
     __syncthreads();
     const int64_t base = static_cast<int64_t>(s_base);
 
@@ -1090,17 +1099,13 @@ __global__ void __launch_bounds__(FC_THREADS) k_fchip(FChipArgs g) {
     const unsigned long long q2_mask = (1ull << g.q2_bits) - 1ull;
 #pragma unroll 1
     for (int u = 0; u < FC_CHUNK; ++u) {
-        const int s = c0 + u;
+        const int s = w0 + u * 32 + lane;
+        if ((s >> 1) >= n) break;                                  // (uniform per warp but for the last round: nothing behind the tile's arcs)
         const unsigned long long key = s_key[s];
         if (key == FC_EMPTY) continue;
-        int lo = 0, hi = nm;                                       // the match (hence the pair) that owns rank s / 2
-        while (hi - lo > 1) {
-            const int mid = (lo + hi) >> 1;
-            if (relcum[mid] <= static_cast<uint32_t>(s >> 1)) lo = mid; else hi = mid;
-        }
         const int64_t q = base + s_excl[s];
         const unsigned long long tk = key >> g.shift_t;
-        g.msrc[q] = g.L.pl[m0 + lo];
+        g.msrc[q] = g.L.pl[m0 + s_mi[s >> 1]];                     // (rank s / 2 lies in the ranks of the pair that owns slot s)
         g.mab[q] = static_cast<uint32_t>(key & ab_mask);
         g.mw[q] = static_cast<float>(s_acc[s]);
         g.mkey[q] = g.table_key ? (tk >> g.q2_bits) * g.nq2 + (tk & q2_mask) : tk;

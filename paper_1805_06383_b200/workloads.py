@@ -208,12 +208,25 @@ def _nlp_bigram(seed: int, vocab: int, n_succ: int, s: float) -> Fst:
 
 
 # name -> (description, default seeds, default max_raw_arcs budget [0 = unlimited])
+def _with_parallel_arcs(m: Fst, seed: int, frac: float) -> Fst:
+    """m plus round(frac * arcs) copies of randomly chosen arcs (same source, labels, target; a new weight)."""
+    rng = np.random.default_rng(seed + 20_000)
+    pick = rng.integers(0, m.n_arcs, size=int(round(frac * m.n_arcs)))
+    cat = lambda a: np.concatenate([a, a[pick]])          # noqa: E731
+    out = Fst(m.n_states, m.n_isyms, m.n_osyms, m.start, cat(m.src), cat(m.ilabel), cat(m.olabel), cat(m.tgt),
+              np.concatenate([m.weight, _weights(rng, len(pick))]), m.accept)
+    out.check()
+    return out
+
+
 CONFIGS: Dict[str, Dict[str, object]] = {
     "tiny":   {"index": 0, "seeds": (102, 103), "max_raw_arcs": 0},
     "medium": {"index": 1, "seeds": (201, 202), "max_raw_arcs": 0},
     "nlp":    {"index": 2, "seeds": (301, 302), "max_raw_arcs": 0},
     "large":  {"index": 3, "seeds": (401, 402), "max_raw_arcs": 1_000_000_000},
     "skewed": {"index": 4, "seeds": (501, 502), "max_raw_arcs": 1_000_000_000},
+    # not a BASELINE.json config: `medium` with parallel duplicate arcs, the workload of the merge on chip (SURVEY §8(f)1)
+    "dups":   {"index": 5, "seeds": (601, 602), "max_raw_arcs": 0},
 }
 
 
@@ -245,6 +258,12 @@ def make_config(name: str, seeds: Tuple[int, int] | None = None, scale: float = 
         q, sig, gam, arcs = sc(100_000), sc(20_000), sc(5_000), sc(5_000_000)
         m1 = random_fst(s1, q, sig, gam, arcs, inner_side="out", inner_zipf=1.1, n_accept=max(1, q // 100))
         m2 = random_fst(s2, q, gam, sig, arcs, inner_side="in", inner_zipf=1.1, n_accept=max(1, q // 100))
+    elif name == "dups":
+        # every state can hold duplicates (10 % of the arcs are repeated with a new weight: same source, labels and
+        # target), while two states seldom share an inner symbol: many small sources whose raw arcs must be merged
+        q, sig, gam, arcs = sc(10_000), sc(1_000), sc(1_000), sc(200_000)
+        m1 = _with_parallel_arcs(random_fst(s1, q, sig, gam, arcs, inner_side="out", inner_zipf=1.0, n_accept=max(1, q // 100)), s1, 0.1)
+        m2 = _with_parallel_arcs(random_fst(s2, q, gam, sig, arcs, inner_side="in", inner_zipf=1.0, n_accept=max(1, q // 100)), s2, 0.1)
     else:  # skewed
         q, arcs = sc(2_000), sc(1_000_000)
         r1 = np.random.default_rng(s1 + 10_000)

@@ -1,5 +1,5 @@
 """Class S, the merge ON CHIP (compose.cu `k_fchip`, SURVEY §8(f)1 / PAPER.md:321): sources that can hold duplicates and
-have at most 1 024 raw arcs are composed, merged and summed in shared memory; only their merged arcs reach HBM.  Parity
+have at most 512 raw arcs are composed, merged and summed in shared memory; only their merged arcs reach HBM.  Parity
 with the oracle element by element like test_gpu_parity.py, on inputs that put raw arcs on every merge route at once
 (S on chip, F through the HBM sort, G by construction), on every way to the target ids (dense table, hash table,
 partitioned resolve), under a budget cut, in chunks, and with long runs of parallel arcs.  `-m gpu`."""
@@ -71,7 +71,7 @@ def test_every_merge_mode_on_the_same_input(fstc, merge_mode):
 @pytest.mark.parametrize("case", SMALL)
 def test_messy_machines_without_class_g(fstc, case, monkeypatch):
     """Zero weights, parallel duplicates, states without arcs (messy_random_fst), class G off: every duplicate-prone
-    source of at most 1 024 raw arcs goes on chip, the heavier ones through the sort."""
+    source of at most 512 raw arcs goes on chip, the heavier ones through the sort."""
     monkeypatch.setenv("FSTC_NO_GROUP_MERGE", "1")
     seed, n1, sig, gam, a1, n2, dlt, a2 = case
     m1 = messy_random_fst(seed, n1, sig, gam, a1)
@@ -115,11 +115,11 @@ def test_on_chip_merge_in_chunks(fstc, monkeypatch):
 
 
 def test_long_runs_of_parallel_arcs_on_chip(fstc, monkeypatch):
-    """31 x 31 = 961 products into ONE merged arc (a source just under the cap of class S), weights over three decades, next to
+    """22 x 22 = 484 products into ONE merged arc (a source just under the cap of class S), weights over three decades, next to
     sources of a handful of arcs: the fp64 slot sums keep rtol 1e-5 (check_parity) whatever the order of arrival."""
     monkeypatch.setenv("FSTC_NO_GROUP_MERGE", "1")
     rng = np.random.default_rng(7)
-    n = 31
+    n = 22
     w1, w2 = 10.0 ** rng.uniform(-3, 0, n), 10.0 ** rng.uniform(-3, 0, n)
     arcs1 = [(0, 1, 2, 1, float(w)) for w in w1] + [(1, 0, 1, 0, 0.5), (1, 0, 1, 0, 0.25), (0, 2, 0, 1, 0.25)]
     arcs2 = [(0, 2, 3, 1, float(w)) for w in w2] + [(1, 1, 0, 0, 0.125), (1, 1, 0, 0, 0.5), (0, 0, 1, 1, 2.0)]
