@@ -89,9 +89,10 @@ enum {
   FSTC_MERGE_AUTO = 0,      /* default: identical (src,tgt,a,b) arcs are summed (:65).  Only the sources
                                that CAN hold duplicates (exact test, N10, replacing the lossy
                                table H of :243) are merged: by construction from the (a,r1) x (b,r2) groups of the
-                               pair when that is cheaper (arcs in (a,r1,b,r2) order), else by sort + reduce (arcs
-                               sorted by (tgt,a,b)); the other sources' arcs come in generation order (inner
-                               symbol, e1, e2).  Arcs are always sorted by source id.                   */
+                               pair when that is cheaper (arcs in (a,r1,b,r2) order), else in shared memory when
+                               the source has at most 512 raw arcs (arcs in no particular order), else by sort +
+                               reduce (arcs sorted by (tgt,a,b)); the other sources' arcs come in generation order
+                               (inner symbol, e1, e2).  Arcs are always sorted by source id.            */
   FSTC_MERGE_OFF = 1,       /* "without performing any reductions" (:289): one arc per (e1,e2) match */
   FSTC_MERGE_SORT_ALL = 2   /* every source goes through sort + reduce: arcs sorted by (src,tgt,a,b) */
 };
