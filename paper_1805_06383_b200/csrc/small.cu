@@ -32,7 +32,7 @@ namespace fstc {
 
 namespace {
 
-constexpr int SP_THREADS = 512, SP_WARPS = SP_THREADS / 32;
+constexpr int SP_THREADS = 512;       // the widest block (the narrower ones: k_small_compose<T>)
 constexpr int SP_CAP_F = 4096;        // frontier pairs of a level
 constexpr int SP_CAP_M = 32768;       // matches of a level
 constexpr int SP_CAP_L = 65536;       // raw arcs of a level
@@ -137,10 +137,11 @@ __device__ __forceinline__ void warp_intersect(const MachineView &A, const Machi
 }
 
 // out[i] = sum of in[j], j < i (i = 0..n; out[n] = total), n <= 65536, by the whole block; returns the total.  in == out is fine.
-__device__ uint32_t block_scan(const uint32_t *in, uint32_t *out, int n, uint32_t *s_w /* [SP_WARPS + 1] */) {
+template <int T>
+__device__ uint32_t block_scan(const uint32_t *in, uint32_t *out, int n, uint32_t *s_w /* [(T / 32) + 1] */) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     uint32_t carry = 0;
-    for (int base = 0; base < n; base += SP_THREADS) {
+    for (int base = 0; base < n; base += T) {
         const int i = base + tid;
         const uint32_t v = i < n ? in[i] : 0u;
         uint32_t incl = v;
@@ -153,7 +154,7 @@ __device__ uint32_t block_scan(const uint32_t *in, uint32_t *out, int n, uint32_
         __syncthreads();
         uint32_t before = 0, total = 0;
 #pragma unroll
-        for (int w = 0; w < SP_WARPS; ++w) { const uint32_t c = s_w[w]; if (w < warp) before += c; total += c; }
+        for (int w = 0; w < (T / 32); ++w) { const uint32_t c = s_w[w]; if (w < warp) before += c; total += c; }
         if (i < n) out[i] = carry + before + incl - v;
         carry += total;
         __syncthreads();
@@ -163,10 +164,12 @@ __device__ uint32_t block_scan(const uint32_t *in, uint32_t *out, int n, uint32_
     return carry;
 }
 
-// The search of one problem by one block (inlined into the two kernels below, which only differ in where P comes from).
+// The search of one problem by one block of T threads (inlined into the kernels below, which only differ in where P comes
+// from and in T).
+template <int T>
 __device__ __forceinline__ void small_compose_block(const SmallArgs &g, const SmallProb &P) {
-    __shared__ uint2 s_stage[SP_WARPS][SP_STAGE + 1];
-    __shared__ uint32_t s_w[SP_WARPS + 1];
+    __shared__ uint2 s_stage[(T / 32)][SP_STAGE + 1];
+    __shared__ uint32_t s_w[(T / 32) + 1];
     __shared__ unsigned int s_nstates, s_flag, s_nsel;
     __shared__ unsigned long long s_cut, s_segs, s_marcs;
     const MachineView &A = P.A, &B = g.B;
@@ -176,7 +179,7 @@ __device__ __forceinline__ void small_compose_block(const SmallArgs &g, const Sm
                            (((P.any1 & FLAG_D) && (g.any2 & FLAG_D)) || (P.any1 & FLAG_X) || (g.any2 & FLAG_X));
 
     // ---- init (Alg. 2 lines 1-3): empty table, state 0 = (s1, s2)
-    for (uint32_t s = tid; s < P.cap_t; s += SP_THREADS) P.table[s] = make_ulonglong2(SP_EMPTY, 0ull);
+    for (uint32_t s = tid; s < P.cap_t; s += T) P.table[s] = make_ulonglong2(SP_EMPTY, 0ull);
     if (tid == 0) {
         s_nstates = 1; s_flag = 0; s_segs = 0; s_marcs = 0;
         P.pair[0] = make_int2(P.start1, g.start2);
@@ -203,7 +206,7 @@ __device__ __forceinline__ void small_compose_block(const SmallArgs &g, const Sm
         if (nf > SP_CAP_F) { status = SP_TOO_BIG; break; }
 
         // ---- count: a warp per pair
-        for (int i = warp; i < nf; i += SP_WARPS) {
+        for (int i = warp; i < nf; i += (T / 32)) {
             const int2 p = P.pair[f_lo + i];
             unsigned long long raw = 0;
             uint32_t nm = 0;
@@ -233,7 +236,7 @@ __device__ __forceinline__ void small_compose_block(const SmallArgs &g, const Sm
 
         // ---- scan + budget (rule T)
         unsigned long long R64 = 0;
-        for (int i = tid; i < nf; i += SP_THREADS) R64 += P.raw[i];
+        for (int i = tid; i < nf; i += T) R64 += P.raw[i];
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) R64 += __shfl_xor_sync(0xffffffffu, R64, d);
         if (tid == 0) s_cut = 0;
@@ -249,7 +252,7 @@ __device__ __forceinline__ void small_compose_block(const SmallArgs &g, const Sm
             const unsigned long long remaining = static_cast<unsigned long long>(g.max_raw_arcs - cum_raw);
             if (tid == 0) { s_cut = ~0ull; s_nsel = 0; }
             __syncthreads();
-            for (int i = tid; i < nf; i += SP_THREADS) {
+            for (int i = tid; i < nf; i += T) {
                 const unsigned long long ki = P.keyv[i];
                 unsigned long long pre = 0;
                 for (int j = 0; j < nf; ++j) if (P.keyv[j] <= ki) pre += P.raw[j];
@@ -258,18 +261,18 @@ __device__ __forceinline__ void small_compose_block(const SmallArgs &g, const Sm
                 if (sel) atomicAdd(&s_nsel, 1u); else atomicMin(&s_cut, ki);
             }
             __syncthreads();
-            for (int i = tid; i < nf; i += SP_THREADS) if (!P.selv[i]) { P.raw[i] = 0; P.nm[i] = 0; }
+            for (int i = tid; i < nf; i += T) if (!P.selv[i]) { P.raw[i] = 0; P.nm[i] = 0; }
             cut_key = s_cut;
             n_sel = static_cast<int>(s_nsel);
             truncated = 1; stop_after = true; last_mode = 2;
             __syncthreads();
         } else if (R64 > SP_CAP_L) { status = SP_TOO_BIG; break; }
-        const uint32_t R = block_scan(P.raw, P.roff, nf, s_w);
-        const uint32_t M = block_scan(P.nm, P.moff, nf, s_w);
+        const uint32_t R = block_scan<T>(P.raw, P.roff, nf, s_w);
+        const uint32_t M = block_scan<T>(P.nm, P.moff, nf, s_w);
         if (M > SP_CAP_M || R > SP_CAP_L || n_arcs + R > P.cap_a) { status = SP_TOO_BIG; break; }
 
         // ---- match work-list: second walk, records in (pair, symbol) order with the running arc rank
-        for (int i = warp; i < nf; i += SP_WARPS) {
+        for (int i = warp; i < nf; i += (T / 32)) {
             if (P.nm[i] == 0) continue;
             const int2 p = P.pair[f_lo + i];
             uint32_t m = P.moff[i], run = P.roff[i];
@@ -305,7 +308,7 @@ __device__ __forceinline__ void small_compose_block(const SmallArgs &g, const Sm
 
         // ---- emit: a thread per output rank (rank -> match -> (i,j)), find-or-insert of the target pair
         const uint32_t ns_before = s_nstates;
-        for (uint32_t r = tid; r < R; r += SP_THREADS) {
+        for (uint32_t r = tid; r < R; r += T) {
             if (*reinterpret_cast<volatile unsigned int *>(&s_flag)) break;   // out of state ids: no more inserts (the table keeps free slots)
             uint32_t lo = 0, hi = M;                                          // last match whose first rank <= r
             while (hi - lo > 1) {
@@ -339,11 +342,11 @@ __device__ __forceinline__ void small_compose_block(const SmallArgs &g, const Sm
         }
         __syncthreads();
         if (s_flag) { status = SP_TOO_BIG; break; }
-        for (uint32_t r = tid; r < R; r += SP_THREADS) P.t_tgt[r] = static_cast<uint32_t>(P.table[P.t_slot[r]].y);   // ids are all published now
+        for (uint32_t r = tid; r < R; r += T) P.t_tgt[r] = static_cast<uint32_t>(P.table[P.t_slot[r]].y);   // ids are all published now
         __syncthreads();
 
         // ---- merge: heads of equal (tgt, a, b) inside a source that can hold duplicates
-        for (uint32_t r = tid; r < R; r += SP_THREADS) {
+        for (uint32_t r = tid; r < R; r += T) {
             const uint32_t i = P.t_pl[r];
             uint32_t head = 1;
             float w = P.t_w[r], comp = 0.f;                            // compensated (Kahan) sum: a few ulp whatever the run length
@@ -364,10 +367,10 @@ __device__ __forceinline__ void small_compose_block(const SmallArgs &g, const Sm
             P.t_ws[r] = w;
         }
         __syncthreads();
-        for (uint32_t r = tid; r < R; r += SP_THREADS) P.t_slot[r] = P.hidx[r];      // keep the flags: the scan overwrites them
+        for (uint32_t r = tid; r < R; r += T) P.t_slot[r] = P.hidx[r];      // keep the flags: the scan overwrites them
         __syncthreads();
-        const uint32_t Mg = block_scan(P.hidx, P.hidx, static_cast<int>(R), s_w);
-        for (uint32_t r = tid; r < R; r += SP_THREADS) {
+        const uint32_t Mg = block_scan<T>(P.hidx, P.hidx, static_cast<int>(R), s_w);
+        for (uint32_t r = tid; r < R; r += T) {
             if (!P.t_slot[r]) continue;
             const int64_t q = n_arcs + P.hidx[r];
             P.src[q] = f_lo + static_cast<int>(P.t_pl[r]);
@@ -390,7 +393,7 @@ __device__ __forceinline__ void small_compose_block(const SmallArgs &g, const Sm
     const int n_states = static_cast<int>(s_nstates);
     uint32_t n_accept = 0;
     if (status == SP_OK) {
-        for (int base = 0; base < n_states; base += SP_THREADS) {
+        for (int base = 0; base < n_states; base += T) {
             const int i = base + tid;
             uint32_t acc = 0;
             if (i < n_states) {
@@ -409,7 +412,7 @@ __device__ __forceinline__ void small_compose_block(const SmallArgs &g, const Sm
             __syncthreads();
             uint32_t before = 0, total = 0;
 #pragma unroll
-            for (int w = 0; w < SP_WARPS; ++w) { const uint32_t c = s_w[w]; if (w < warp) before += c; total += c; }
+            for (int w = 0; w < (T / 32); ++w) { const uint32_t c = s_w[w]; if (w < warp) before += c; total += c; }
             if (acc) P.accept[n_accept + before + __popc(bal & ((1u << lane) - 1u))] = i;
             n_accept += total;
             __syncthreads();
@@ -424,14 +427,17 @@ __device__ __forceinline__ void small_compose_block(const SmallArgs &g, const Sm
 }
 
 // a batch: block k takes problem k, whose descriptor (result and scratch pointers from the library pool) is in device memory
-__global__ void __launch_bounds__(SP_THREADS) k_small_compose(SmallArgs g) {
+// T = 512 for a few problems (latency: every step of a level spreads over 16 warps); big batches take narrower blocks, 256 or
+// 128 threads, so that 2 or 4 problems are resident per SM (108 registers per thread: a block of 512 fills an SM's file)
+template <int T>
+__global__ void __launch_bounds__(T) k_small_compose(SmallArgs g) {
     const SmallProb P = g.prob[blockIdx.x];
-    small_compose_block(g, P);
+    small_compose_block<T>(g, P);
 }
 
 // one problem, its descriptor passed by value: the result arrays are the caller's, the scratch is g_small_scratch (below)
 __global__ void __launch_bounds__(SP_THREADS) k_small_compose_static(SmallArgs g, SmallProb P) {
-    small_compose_block(g, P);
+    small_compose_block<SP_THREADS>(g, P);
 }
 
 struct Carver {                       // consecutive 256-byte aligned pieces of one block
@@ -529,7 +535,9 @@ void compose_small_batch(Ctx &c, const fstc_packed_t *const *m1, int n, const fs
     SmallArgs g;
     g.prob = d_prob.p; g.B = view_of(m2); g.acc2 = m2.accept_bits; g.start2 = m2.start; g.any2 = m2.any_flags;
     g.nq2 = static_cast<uint64_t>(m2.n_states); g.merge_mode = o.merge_mode; g.max_levels = o.max_levels; g.max_raw_arcs = o.max_raw_arcs;
-    k_small_compose<<<static_cast<unsigned>(n), SP_THREADS, 0, c.stream>>>(g);
+    if (n >= 4 * c.n_sm) k_small_compose<128><<<static_cast<unsigned>(n), 128, 0, c.stream>>>(g);
+    else if (n >= 2 * c.n_sm) k_small_compose<256><<<static_cast<unsigned>(n), 256, 0, c.stream>>>(g);
+    else k_small_compose<SP_THREADS><<<static_cast<unsigned>(n), SP_THREADS, 0, c.stream>>>(g);
     FSTC_LAUNCH_CHECK();
     c.n_launch += 1;
     std::vector<SmallOut> h(n);

@@ -9,6 +9,7 @@ from __future__ import annotations
 
 import ctypes
 import os
+import struct
 from dataclasses import dataclass
 from typing import Optional
 
@@ -124,8 +125,8 @@ def lib():
         L.fstc_compose.argtypes = [P, P, P, P, ctypes.POINTER(ctypes.POINTER(_Result)), P]
         L.fstc_compose_batch.argtypes = [P, ctypes.c_int32, P, P, P, P, P]
         L.fstc_compose_static.argtypes = [P, P, P, P, P]
-        L.fstc_result_to_host.argtypes = [ctypes.POINTER(_Result), P, P]
-        L.fstc_result_free.argtypes = [ctypes.POINTER(_Result)]
+        L.fstc_result_to_host.argtypes = [P, P, P]
+        L.fstc_result_free.argtypes = [P]
         L.fstc_result_free.restype = None
         L.fstc_trim_pool.argtypes = []
         L.fstc_strerror.argtypes = [I]
@@ -239,28 +240,48 @@ class _ResultHandle:
 
 class ComposeResult:
     """M1∘M2 on the device.  State i is the pair (pair[i,0], pair[i,1]) = (q1,q2); state 0 = (s1,s2).
-    Arcs are sorted by source id; tensors are views of library memory kept alive by this object."""
+    Arcs are sorted by source id; tensors are views of library memory kept alive by this object.  The views and the stats
+    dict are made on first use: a batch of thousands of results costs the C call, not thousands of wrappers."""
 
-    def __init__(self, rptr, stats: Optional[_Stats]):
-        self._h = _ResultHandle(rptr)
-        r = rptr.contents
-        self.n_states, self.n_arcs, self.n_raw_arcs = int(r.n_states), int(r.n_arcs), int(r.n_raw_arcs)
-        self.n_accept, self.n_expanded = int(r.n_accept), int(r.n_expanded)
-        self.n_levels, self.truncated = int(r.n_levels), int(r.truncated)
-        h = self._h
-        self.pair = _tensor(r.pair, (self.n_states, 2), "<i4", h)
-        self.src = _tensor(r.src, (self.n_arcs,), "<i4", h)
-        self.ilabel = _tensor(r.ilabel, (self.n_arcs,), "<i4", h)
-        self.olabel = _tensor(r.olabel, (self.n_arcs,), "<i4", h)
-        self.tgt = _tensor(r.tgt, (self.n_arcs,), "<i4", h)
-        self.weight = _tensor(r.weight, (self.n_arcs,), "<f4", h)
-        self.accept = _tensor(r.accept, (self.n_accept,), "<i4", h)
-        self.expanded = _tensor(r.expanded, (self.n_states,), "|u1", h)
-        self.stats = stats_dict(stats) if stats is not None else None
+    _ORDER = ("pair", "src", "ilabel", "olabel", "tgt", "weight", "accept", "expanded")
+    _FIELDS = {"pair": ("n_states", 2, "<i4"), "src": ("n_arcs", 0, "<i4"), "ilabel": ("n_arcs", 0, "<i4"),
+               "olabel": ("n_arcs", 0, "<i4"), "tgt": ("n_arcs", 0, "<i4"), "weight": ("n_arcs", 0, "<f4"),
+               "accept": ("n_accept", 0, "<i4"), "expanded": ("n_states", 0, "|u1")}
+
+    _HEAD = struct.Struct("5q2i8P")                   # fstc_result_t up to `impl`, read in one go
+
+    def __init__(self, rptr, stats):
+        """rptr: a POINTER(_Result) or the address of a fstc_result_t.  stats: None, a _Stats, or (array of _Stats, index)."""
+        addr = rptr if isinstance(rptr, int) else ctypes.cast(rptr, ctypes.c_void_p).value
+        self._h = _ResultHandle(addr)
+        v = self._HEAD.unpack(ctypes.string_at(addr, self._HEAD.size))
+        (self.n_states, self.n_arcs, self.n_raw_arcs, self.n_accept, self.n_expanded, self.n_levels, self.truncated) = v[:7]
+        self._ptrs = v[7:]
+        self._views = {}
+        self._stats = stats
+
+    def __getattr__(self, name):                      # only reached for names that are not set yet: the lazy views
+        if name in ComposeResult._FIELDS and "_views" in self.__dict__:
+            v = self._views
+            if name not in v:
+                if self._h is None:
+                    return None
+                length, inner, typestr = self._FIELDS[name]
+                n = getattr(self, length)
+                v[name] = _tensor(self._ptrs[self._ORDER.index(name)], (n, inner) if inner else (n,), typestr, self._h)
+            return v[name]
+        if name == "stats" and "_stats" in self.__dict__:
+            st = self._stats
+            if isinstance(st, tuple):
+                st = st[0][st[1]]
+            if st is not None and not isinstance(st, dict):
+                st = self._stats = stats_dict(st)
+            return st
+        raise AttributeError(name)
 
     def free(self):
         """Releases the result now (fstc_result_free); the tensors of this object must no longer be used."""
-        self.pair = self.src = self.ilabel = self.olabel = self.tgt = self.weight = self.accept = self.expanded = None
+        self._views = {k: None for k in self._FIELDS}
         h, self._h = self._h, None
         if h is not None and h.ptr:
             lib().fstc_result_free(h.ptr)
@@ -440,14 +461,8 @@ def fstc_compose_batch(p1s, p2: Packed, *, stream=None, with_stats=True, **opts)
     sts = (_Stats * n)() if with_stats else None
     _check(lib().fstc_compose_batch(ctypes.addressof(ptrs), n, p2.ptr, ctypes.addressof(o), _stream_ptr(stream),
                                     ctypes.addressof(outs), ctypes.addressof(sts) if sts is not None else None))
-    res = []
-    for k in range(n):
-        st = None
-        if sts is not None:
-            st = _Stats()
-            ctypes.memmove(ctypes.addressof(st), ctypes.addressof(sts[k]), ctypes.sizeof(_Stats))
-        res.append(ComposeResult(outs[k], st))
-    return res
+    addrs = struct.unpack(f"{n}P", ctypes.string_at(ctypes.addressof(outs), 8 * n)) if n else ()
+    return [ComposeResult(a, (sts, k) if sts is not None else None) for k, a in enumerate(addrs)]
 
 
 # ------------------------------------------------------------------------------------------------ no allocation

@@ -22,7 +22,7 @@ from typing import Dict, Tuple
 
 import numpy as np
 
-__all__ = ["Fst", "CONFIGS", "make_config", "random_fst", "zipf_symbols"]
+__all__ = ["Fst", "CONFIGS", "make_config", "make_lattices", "random_fst", "zipf_symbols"]
 
 
 @dataclass
@@ -228,6 +228,13 @@ CONFIGS: Dict[str, Dict[str, object]] = {
     # not a BASELINE.json config: `medium` with parallel duplicate arcs, the workload of the merge on chip
     "dups":   {"index": 5, "seeds": (601, 602), "max_raw_arcs": 0},
 }
+
+
+def make_lattices(n: int, seed0: int = 301, scale: float = 1.0) -> list:
+    """n seeded word lattices of config `nlp`'s shape (50 positions x 8 alternatives over the same vocabulary): the many
+    left operands of ONE language model, the paper's translation use case."""
+    vocab = max(200, int(round(30_000 * scale)))
+    return [_nlp_lattice(seed0 + 1000 * (k + 1), 50, 8, vocab, 1.1) for k in range(n)]
 
 
 def make_config(name: str, seeds: Tuple[int, int] | None = None, scale: float = 1.0) -> Tuple[Fst, Fst]:

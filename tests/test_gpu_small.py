@@ -137,6 +137,33 @@ def test_batch_of_lattices_against_one_language_model(fstc):
         check_parity(fstc, m, lm, max_levels=4, result=r)
 
 
+@pytest.mark.parametrize("n", [300, 640])
+def test_big_batches_take_narrower_blocks(fstc, n):
+    """From 2 x and 4 x (number of SMs) problems on, a batch runs in blocks of 256 and 128 threads (several problems
+    resident per SM): same results.  Lattices with merges (parallel arcs) and `tiny`-like random machines among them, so
+    that the narrower blocks run every step (cut, merge, several matches per pair), each against the oracle."""
+    import torch
+    assert n >= (4 if n > 600 else 2) * torch.cuda.get_device_properties(0).multi_processor_count
+    vocab = 500
+    lm = workloads._nlp_bigram(9500, vocab, 40, 1.1)
+    lats = []
+    for k in range(n):
+        m = workloads._nlp_lattice(9600 + k, 4 + k % 7, 2 + k % 4, vocab, 1.1)
+        if k % 3 == 0:                                     # parallel duplicate arcs: duplicate-prone sources, merged in the block
+            m = workloads._with_parallel_arcs(m, k, 0.5)
+        lats.append(m)
+    p2 = fstc.fstc_pack(fstc.DeviceFst.from_host(lm), 2)
+    p1s = [fstc.fstc_pack(fstc.DeviceFst.from_host(m), 1) for m in lats]
+    for opts in ({}, {"max_raw_arcs": 40}):
+        results = fstc.fstc_compose_batch(p1s, p2, **opts)
+        assert all(r.stats["small_path"] == 1 and r.stats["n_kernel_launches"] == 1 for r in results)
+        merged = 0
+        for m, r in zip(lats, results):
+            _, ref = check_parity(fstc, m, lm, result=r, **opts)
+            merged += ref.n_arcs < ref.n_raw_arcs
+        assert merged > n // 10
+
+
 def test_batch_hands_over_what_does_not_fit(fstc):
     m1, m2 = workloads.make_config("medium", scale=0.03)
     t1, _ = workloads.make_config("tiny")
