@@ -1050,7 +1050,8 @@ __global__ void __launch_bounds__(FC_THREADS) k_fchip(FChipArgs g) {
     }
     __syncthreads();
 
-    // ---- every raw arc of the tile: compose, find or claim its slot, add its weight
+    // ---- every raw arc of the tile: compose, find or claim its slot, add its weight.  (Two ranks per thread with the loads
+    // of both in flight lost to this loop, 54.8 -> 63.5 ms on `dups`: 44 registers, or 32 and spills.)
     const unsigned long long ab_mask = (1ull << g.shift_t) - 1ull;
     for (int r = tid; r < n; r += FC_THREADS) {
         const int j = s_mi[r];
@@ -2194,20 +2195,26 @@ fstc_result_t *Composer::run() {
         DBuf<uint32_t> plU(c, MU), plF(c, MF);
         LU = MatchList{cumU.p, recU.p, plU.p};
         LF = MatchList{cumF.p, recF.p, plF.p};
-        if (MU + MF > 0) {
-            h = tm.begin(FSTC_T_MATCH);
-            k_match<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, sel.p, nmU.p, nmF.p, moffU.p, moffF.p, roffU.p,
-                                                           roffF.p, LU, LF, d_counters.p + 1);
-            FSTC_LAUNCH_CHECK();
-            c.n_launch += 1;
-            tm.end(h);
-        }
-
         DBuf<int64_t> cumS(c, MS + 1);
         DBuf<uint4> recS(c, MS);
         DBuf<uint32_t> plS(c, MS);
         MatchList LS{cumS.p, recS.p, plS.p};
-        if (MS > 0) {                                            // the same kernel, class S in the place of class U
+        // one walk writes two classes' lists: U and F, or — the usual case of a level with class S, which has no class F —
+        // U and S; only a level with all three walks a second time
+        const bool s_with_u = MS > 0 && MF == 0;
+        if (MU + MF > 0 || s_with_u) {
+            h = tm.begin(FSTC_T_MATCH);
+            if (s_with_u)
+                k_match<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, sel.p, nmU.p, nmS.p, moffU.p, moffS.p, roffU.p,
+                                                               roffS.p, LU, LS, d_counters.p + 1);
+            else
+                k_match<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, sel.p, nmU.p, nmF.p, moffU.p, moffF.p, roffU.p,
+                                                               roffF.p, LU, LF, d_counters.p + 1);
+            FSTC_LAUNCH_CHECK();
+            c.n_launch += 1;
+            tm.end(h);
+        }
+        if (MS > 0 && !s_with_u) {                               // class S in the place of class U
             h = tm.begin(FSTC_T_MATCH);
             k_match<<<nblk(nf), CT_THREADS, 0, c.stream>>>(A, B, pair.p, f_lo, nf, sel.p, nmS.p, nullptr, moffS.p, nullptr, roffS.p,
                                                            nullptr, LS, LS, d_counters.p + 1);

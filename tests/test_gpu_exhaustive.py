@@ -1,5 +1,5 @@
 """Exhaustive parity at the TIMED size (SURVEY §8(c) "streaming verifier"): `large` and `skewed` at bench.py's budget
-of 1e9 raw arcs, every state and every arc compared with the oracle, no sampling.
+of 1e9 raw arcs (and the complete `dups`), every state and every arc compared with the oracle, no sampling.
 
   * states, levels, expanded flags, accept set, counters: the oracle's own full run (Algorithm 1 + rule T, arcs not
     kept) against the result, as sorted pair keys;
@@ -147,3 +147,9 @@ def test_large_every_state_and_arc_at_the_bench_budget():
 
 def test_skewed_every_state_and_arc_at_the_bench_budget():
     _exhaustive("skewed", BUDGET)
+
+
+def test_dups_every_state_and_arc_complete():
+    """`dups` (not a BASELINE config: the workload of the merge on chip), complete: 1.42e9 raw arcs, nearly
+    all of them merged in shared memory by k_fchip, every merged arc compared."""
+    _exhaustive("dups", 0)
