@@ -966,11 +966,12 @@ k_resolve_keys(const unsigned long long *__restrict__ keys, int64_t n, uint32_t 
 // arc finds or claims the slot of its (r1, r2, a, b) there (64-bit CAS, linear probing inside the pair's region) and adds
 // its weight to the slot's fp64 sum.  The occupied slots, in slot order, ARE the merged arcs grouped by pair: a block scan
 // numbers them, one atomicAdd reserves the tile's piece of the compact output, and every pair learns its count and its
-// first arc.  ~250 instructions per raw arc against ~900 for a bitonic sort of the tile, and no HBM traffic per raw arc
-// beyond the two operand arcs (which L2 serves) and its match record.  T = 512 with one thread per rank of the tile
-// (measured on the `dups` workload, reduce stage: T/threads 512/256 63.5 ms, 512/512 54.8, 256/256 51.6, 128/128 50.8,
-// 256/512 76.5, 128/256 71.5; the match records staged in shared memory: 73.2 — occupancy).  The merged arcs leave with their target KEY; their ids come from the
-// visited set afterwards, like class G's — one lookup per MERGED arc, not per raw arc.
+// first arc.  ~600 thread-instructions per raw arc (ncu: 19 warp-instructions) against several thousand for a bitonic sort
+// of the tile, and no HBM traffic per raw arc beyond its match record and the two operand arcs (which L2 serves).
+// T = 512 with one thread per rank of the tile (`dups`, reduce stage, T / threads: 512/256 63.5 ms, 512/512 54.8,
+// 256/256 51.6, 128/128 50.8, 256/512 76.5, 128/256 71.5; match records staged in shared memory 73.2: occupancy).
+// The merged arcs leave with their target KEY; their ids come from the visited set afterwards, like class G's — one
+// lookup per MERGED arc, not per raw arc.
 constexpr int FC_THREADS = FSTC_FC_THREADS;
 constexpr int FC_TILE = FC_PAIR_CAP;
 constexpr int FC_MAX_ARCS = 2 * FC_TILE;            // raw arcs of a tile: < FC_TILE + FC_PAIR_CAP
