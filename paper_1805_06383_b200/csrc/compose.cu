@@ -1121,6 +1121,33 @@ __global__ void __launch_bounds__(FC_THREADS) k_fchip(FChipArgs g) {
     }
 }
 
+// Class S on a table level: the ids of the merged arcs' targets (as k_resolve_keys) and the arcs straight to their final
+// place behind the pair's offset (as k_place_grouped), in one kernel: the target column is written once and never read.
+template <bool DENSE>
+__global__ void __launch_bounds__(CT_THREADS)
+k_resolve_place(const unsigned long long *__restrict__ keys, const uint32_t *__restrict__ msrc, const uint32_t *__restrict__ mab,
+                const float *__restrict__ mw, int64_t n, const int64_t *__restrict__ mbase, const int64_t *__restrict__ foff,
+                int64_t arc_base, int64_t f_lo, const uint32_t *__restrict__ sel, int bits_b, uint32_t *dense, uint4 *table,
+                uint64_t cap, uint64_t nq2, unsigned long long *n_states, int2 *pair, int32_t *__restrict__ o_src,
+                int32_t *__restrict__ o_il, int32_t *__restrict__ o_ol, int32_t *__restrict__ o_tgt, float *__restrict__ o_w) {
+    __shared__ uint32_t s_warp[CT_THREADS / 32];
+    __shared__ unsigned long long s_base;
+    const int64_t j = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    const bool valid = j < n;
+    const unsigned long long key = valid ? keys[j] : 0ull;
+    const unsigned long long q1 = key / nq2;
+    const uint32_t id = block_find_or_insert<DENSE, CT_THREADS>(key, valid, make_int2(static_cast<int>(q1), static_cast<int>(key - q1 * nq2)),
+                                                                dense, table, cap, n_states, pair, s_warp, &s_base);
+    if (!valid) return;
+    const uint32_t p = msrc[j], ab = mab[j];
+    const int64_t q = arc_base + foff[p] + (j - mbase[p]);
+    o_src[q] = static_cast<int>(f_lo + (sel ? sel[p] : p));
+    o_tgt[q] = static_cast<int32_t>(id);
+    o_il[q] = static_cast<int>(ab >> bits_b);
+    o_ol[q] = static_cast<int>(ab & ((1u << bits_b) - 1u));
+    o_w[q] = mw[j];
+}
+
 __global__ void k_place_grouped(const uint32_t *__restrict__ mab, const int32_t *__restrict__ mtgt, const uint32_t *__restrict__ msrc,
                                 const float *__restrict__ mw, int64_t n_merged, const int64_t *__restrict__ mstart,
                                 const int64_t *__restrict__ foff, int64_t arc_base, int64_t f_lo,
@@ -2284,11 +2311,13 @@ fstc_result_t *Composer::run() {
             DBuf<float> sw;
             DBuf<int32_t> stgt;
             DBuf<int64_t> scnt, sbase;
+            DBuf<unsigned long long> skeys;                          // target keys of the merged arcs (table level: resolved at placement)
             if (RS > 0) {
                 h = tm.begin(FSTC_T_REDUCE);
                 const int64_t n_tiles = ceil_div(RS, FC_TILE);
                 DBuf<int64_t> tile_p(c, n_tiles + 1);
-                DBuf<unsigned long long> cursor(c, 1), skeys(c, RS + 2);
+                DBuf<unsigned long long> cursor(c, 1);
+                skeys.alloc(c, RS + 2);
                 ssrc.alloc(c, RS); sab.alloc(c, RS); sw.alloc(c, RS);
                 scnt.alloc(c, nf); sbase.alloc(c, nf);
                 FSTC_CUDA(cudaMemsetAsync(cursor.p, 0, sizeof(unsigned long long), c.stream));
@@ -2309,9 +2338,9 @@ fstc_result_t *Composer::run() {
                 c.n_launch += 2;
                 MSm = static_cast<int64_t>(read_scalar(c, cursor.p));
                 tm.end(h);
-                if (MSm > 0) {                                       // target ids of the merged arcs
+                if (MSm > 0 && partitioned) {                        // target ids of the merged arcs (a table level: at placement)
                     stgt.alloc(c, MSm);
-                    if (partitioned) {
+                    {
                         ResolveJob j;
                         j.keys = skeys.p; j.n_records = MSm; j.q2_bits = fa.q2_bits;
                         j.key_bits = fa.q2_bits + bits_for(static_cast<uint64_t>(m1.n_states > 1 ? m1.n_states - 1 : 1));
@@ -2320,22 +2349,11 @@ fstc_result_t *Composer::run() {
                         j.force_bits = knob_resolve_bits;
                         j.stats = &st; j.profile = o.profile != 0;
                         run_resolve(j, 1);
-                    } else {
-                        h = tm.begin(FSTC_T_EMIT);
-                        if (use_dense)
-                            k_resolve_keys<true><<<nblk(MSm), CT_THREADS, 0, c.stream>>>(skeys.p, MSm, dense.p, nullptr, 0, nq2, d_counters.p,
-                                                                                        pair.p, stgt.p);
-                        else
-                            k_resolve_keys<false><<<nblk(MSm), CT_THREADS, 0, c.stream>>>(skeys.p, MSm, nullptr, table.p, cap, nq2,
-                                                                                         d_counters.p, pair.p, stgt.p);
-                        FSTC_LAUNCH_CHECK();
-                        c.n_launch += 1;
-                        tm.end(h);
                     }
                     n_states_live = static_cast<int64_t>(read_scalar(c, d_counters.p));
                 }
                 st.n_raw_onchip += RS;
-                c.sync();                                            // (tile_p, cursor, skeys go out of scope)
+                c.sync();                                            // (tile_p, cursor go out of scope)
             }
             // ---- class G: merge by construction (group products)
             int64_t MGm = 0;
@@ -2480,10 +2498,24 @@ fstc_result_t *Composer::run() {
                                                                        n_states, det_n1, o.deterministic ? rank.p : nullptr);
                 FSTC_LAUNCH_CHECK();
             }
-            if (MSm > 0) {                                           // (sbase in the place of mstart: a pair's arcs are neighbours)
+            if (MSm > 0 && partitioned) {                            // (sbase in the place of mstart: a pair's arcs are neighbours)
                 k_place_grouped<<<nblk(MSm), CT_THREADS, 0, c.stream>>>(sab.p, stgt.p, ssrc.p, sw.p, MSm, sbase.p, foff.p, arc_base,
                                                                        f_lo, sel.p, bits_b, o_src, o_il, o_ol, o_tgt, o_w);
                 FSTC_LAUNCH_CHECK();
+            } else if (MSm > 0) {                                    // table level: ids and placement in one kernel
+                tm.end(h);
+                h = tm.begin(FSTC_T_EMIT);
+                if (use_dense)
+                    k_resolve_place<true><<<nblk(MSm), CT_THREADS, 0, c.stream>>>(skeys.p, ssrc.p, sab.p, sw.p, MSm, sbase.p, foff.p, arc_base, f_lo,
+                                                                                 sel.p, bits_b, dense.p, nullptr, 0, nq2, d_counters.p, pair.p,
+                                                                                 o_src, o_il, o_ol, o_tgt, o_w);
+                else
+                    k_resolve_place<false><<<nblk(MSm), CT_THREADS, 0, c.stream>>>(skeys.p, ssrc.p, sab.p, sw.p, MSm, sbase.p, foff.p, arc_base, f_lo,
+                                                                                  sel.p, bits_b, nullptr, table.p, cap, nq2, d_counters.p, pair.p,
+                                                                                  o_src, o_il, o_ol, o_tgt, o_w);
+                FSTC_LAUNCH_CHECK();
+                tm.end(h);
+                h = tm.begin(FSTC_T_REDUCE);
             }
             c.n_launch += 4;
             tm.end(h);
