@@ -1414,7 +1414,8 @@ __global__ void __launch_bounds__(DO_THREADS) k_dord_count(const uint32_t *__res
     if (threadIdx.x == 0) tile_cnt[blockIdx.x] = s_cnt;
 }
 __global__ void __launch_bounds__(DO_THREADS) k_dord_assign(uint32_t *__restrict__ dense, uint64_t n, uint64_t nq2, const uint32_t *__restrict__ tile_cnt,
-                                                             const int64_t *__restrict__ tile_off, int64_t n0, int2 *__restrict__ pair) {
+                                                             const int64_t *__restrict__ tile_off, int64_t n0, int2 *__restrict__ pair,
+                                                             uint2 *__restrict__ rankdir) {
     if (tile_cnt[blockIdx.x] == 0) return;
     __shared__ uint32_t s_warp[DO_THREADS / 32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -1429,6 +1430,9 @@ __global__ void __launch_bounds__(DO_THREADS) k_dord_assign(uint32_t *__restrict
         uint32_t before = 0, total = 0;
 #pragma unroll
         for (int wv = 0; wv < DO_THREADS / 32; ++wv) { const uint32_t c = s_warp[wv]; if (wv < warp) before += c; total += c; }
+        // the rank directory: {which of these 32 keys were numbered now, id of the first of them}: 8 bytes per 32 keys, small
+        // enough to stay in L2, so that k_dord_fix does not go back to the table (far larger than L2) for every arc
+        if (lane == 0 && i < n) rankdir[i >> 5] = make_uint2(b, static_cast<uint32_t>(off + before));
         if (f) {
             const int64_t id = off + before + __popc(b & ((1u << lane) - 1u));
             dense[i] = static_cast<uint32_t>(id) + 1u;
@@ -1439,11 +1443,23 @@ __global__ void __launch_bounds__(DO_THREADS) k_dord_assign(uint32_t *__restrict
         __syncthreads();
     }
 }
-__global__ void k_dord_fix(int32_t *__restrict__ tgt, int64_t n, const uint32_t *__restrict__ dense) {
-    const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const int32_t t = __ldcs(tgt + i);
-    if (t < 0) tgt[i] = static_cast<int32_t>(__ldcg(dense + static_cast<uint32_t>(~t)) - 1u);
+// tgt: the whole target column (16-byte aligned); the arcs [a0, a1) of it are completed, four per thread
+__global__ void k_dord_fix(int32_t *__restrict__ tgt, int64_t a0, int64_t a1, const uint2 *__restrict__ rankdir) {
+    const int64_t q = (a0 / 4 + static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x) * 4;
+    if (q >= a1) return;
+    auto fix = [&](int32_t t) {                                  // ~key of a state this level created: its id from the directory
+        if (t >= 0) return t;
+        const uint32_t key = static_cast<uint32_t>(~t);
+        const uint2 d = __ldg(rankdir + (key >> 5));
+        return static_cast<int32_t>(d.y + __popc(d.x & ((1u << (key & 31u)) - 1u)));
+    };
+    if (q >= a0 && q + 4 <= a1) {
+        int4 v = __ldcs(reinterpret_cast<const int4 *>(tgt + q));
+        v.x = fix(v.x); v.y = fix(v.y); v.z = fix(v.z); v.w = fix(v.w);
+        __stcs(reinterpret_cast<int4 *>(tgt + q), v);
+    } else {
+        for (int64_t i = q < a0 ? a0 : q; i < q + 4 && i < a1; ++i) tgt[i] = fix(tgt[i]);
+    }
 }
 
 // Level compaction: when rule T will clearly cut the level, only the pairs below a key limit are worked on.
@@ -1801,10 +1817,12 @@ struct Composer {
         exclusive_scan<uint32_t>(c, tile_cnt.p, tiles, tile_off.p);
         const int64_t n_new = read_scalar(c, tile_off.p + tiles);
         if (n0 + n_new > pair_cap) fail(FSTC_ERR_INTERNAL, "dense_number_pending: %lld new states exceed the reserved pair table", static_cast<long long>(n_new));
-        k_dord_assign<<<static_cast<unsigned>(tiles), DO_THREADS, 0, c.stream>>>(dense.p, n_pairs_all, nq2, tile_cnt.p, tile_off.p, n0, pair.p);
+        DBuf<uint2> rankdir(c, ceil_div(static_cast<int64_t>(n_pairs_all), 32));
+        k_dord_assign<<<static_cast<unsigned>(tiles), DO_THREADS, 0, c.stream>>>(dense.p, n_pairs_all, nq2, tile_cnt.p, tile_off.p, n0, pair.p,
+                                                                                 rankdir.p);
         FSTC_LAUNCH_CHECK();
         if (a1 > a0) {
-            k_dord_fix<<<nblk(a1 - a0), CT_THREADS, 0, c.stream>>>(o_tgt + a0, a1 - a0, dense.p);
+            k_dord_fix<<<nblk(a1 / 4 - a0 / 4 + 1), CT_THREADS, 0, c.stream>>>(o_tgt, a0, a1, rankdir.p);
             FSTC_LAUNCH_CHECK();
         }
         const unsigned long long ns = static_cast<unsigned long long>(n0 + n_new);
