@@ -1,5 +1,5 @@
 """Exhaustive parity at the TIMED size (SURVEY §8(c) "streaming verifier"): `large` and `skewed` at bench.py's budget
-of 1e9 raw arcs (and the complete `dups`), every state and every arc compared with the oracle, no sampling.
+of 1e9 raw arcs (and the complete `medium` and `dups`), every state and every arc compared with the oracle, no sampling.
 
   * states, levels, expanded flags, accept set, counters: the oracle's own full run (Algorithm 1 + rule T, arcs not
     kept) against the result, as sorted pair keys;
@@ -147,6 +147,12 @@ def test_large_every_state_and_arc_at_the_bench_budget():
 
 def test_skewed_every_state_and_arc_at_the_bench_budget():
     _exhaustive("skewed", BUDGET)
+
+
+def test_medium_every_state_and_arc_complete():
+    """`medium` (BASELINE.json configs[1]), complete: 1.16e9 arcs, the levels that number their states in key order on the
+    dense table (k_emit<RES_DORD>, the rank directory of k_dord_assign / k_dord_fix)."""
+    _exhaustive("medium", 0)
 
 
 def test_dups_every_state_and_arc_complete():
