@@ -1419,28 +1419,38 @@ __global__ void __launch_bounds__(DO_THREADS) k_dord_assign(uint32_t *__restrict
     if (tile_cnt[blockIdx.x] == 0) return;
     __shared__ uint32_t s_warp[DO_THREADS / 32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const uint64_t base = static_cast<uint64_t>(blockIdx.x) * DO_TILE;
-    int64_t off = n0 + tile_off[blockIdx.x];
-    for (int r = 0; r < DO_ITEMS; ++r) {                        // rows of 256 consecutive keys, in order
-        const uint64_t i = base + static_cast<uint64_t>(r) * DO_THREADS + threadIdx.x;
-        const bool f = i < n && dense[i] == PENDING_ID;
-        const uint32_t b = __ballot_sync(0xffffffffu, f);
-        if (lane == 0) s_warp[warp] = __popc(b);
-        __syncthreads();
-        uint32_t before = 0, total = 0;
+    // a warp owns DO_ITEMS x 32 consecutive keys of the tile: all its loads in flight together, one block barrier per tile
+    const uint64_t base = static_cast<uint64_t>(blockIdx.x) * DO_TILE + static_cast<uint64_t>(warp) * (DO_ITEMS * 32);
+    uint32_t bal[DO_ITEMS], cnt = 0;
+    uint32_t v[DO_ITEMS];
 #pragma unroll
-        for (int wv = 0; wv < DO_THREADS / 32; ++wv) { const uint32_t c = s_warp[wv]; if (wv < warp) before += c; total += c; }
+    for (int r = 0; r < DO_ITEMS; ++r) {
+        const uint64_t i = base + static_cast<uint64_t>(r) * 32 + lane;
+        v[r] = i < n ? dense[i] : 0u;
+    }
+#pragma unroll
+    for (int r = 0; r < DO_ITEMS; ++r) {
+        bal[r] = __ballot_sync(0xffffffffu, v[r] == PENDING_ID);
+        cnt += __popc(bal[r]);
+    }
+    if (lane == 0) s_warp[warp] = cnt;
+    __syncthreads();
+    int64_t off = n0 + tile_off[blockIdx.x];
+#pragma unroll
+    for (int wv = 0; wv < DO_THREADS / 32; ++wv) if (wv < warp) off += s_warp[wv];
+#pragma unroll
+    for (int r = 0; r < DO_ITEMS; ++r) {                         // rows of 32 consecutive keys, in order
+        const uint64_t i = base + static_cast<uint64_t>(r) * 32 + lane;
         // the rank directory: {which of these 32 keys were numbered now, id of the first of them}: 8 bytes per 32 keys, small
         // enough to stay in L2, so that k_dord_fix does not go back to the table (far larger than L2) for every arc
-        if (lane == 0 && i < n) rankdir[i >> 5] = make_uint2(b, static_cast<uint32_t>(off + before));
-        if (f) {
-            const int64_t id = off + before + __popc(b & ((1u << lane) - 1u));
+        if (lane == 0 && i < n) rankdir[i >> 5] = make_uint2(bal[r], static_cast<uint32_t>(off));
+        if (bal[r] >> lane & 1u) {
+            const int64_t id = off + __popc(bal[r] & ((1u << lane) - 1u));
             dense[i] = static_cast<uint32_t>(id) + 1u;
             const uint64_t q1 = i / nq2;
             pair[id] = make_int2(static_cast<int>(q1), static_cast<int>(i - q1 * nq2));
         }
-        off += total;
-        __syncthreads();
+        off += __popc(bal[r]);
     }
 }
 // tgt: the whole target column (16-byte aligned); the arcs [a0, a1) of it are completed, four per thread
